@@ -1,0 +1,192 @@
+"""ORACLE — TEST INFRASTRUCTURE ONLY.
+
+ctypes binding of the plain single-threaded C++ oracle in this directory (see orc.hpp for
+what it is and what pins it). Only tests/, __graft_entry__.smoke() and the cpu_baseline /
+--impl reference legs of bench.py may import this package. It imports nothing from the
+CUDA product (paper_2510_13965_b200) and the product imports nothing from here.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SOURCES = ["orc_stencil.cpp", "orc_eos.cpp", "orc_c2p.cpp", "orc_ccz4.cpp", "orc_grmhd.cpp",
+            "orc_rk.cpp", "orc_capi.cpp"]
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+NSTATE, NPRIM = 32, 10
+# field indices (mirror orc.hpp)
+GXX, AXX, CHI, KHAT, THETA, GAMX, ALPHA, BETAX = 0, 6, 12, 13, 14, 15, 18, 19
+DBAR, DYEBAR, TAUBAR, SXBAR, BXBAR, PHIBAR = 22, 23, 24, 25, 28, 31
+RHO, YE, EPS, PRESS, VX, WLOR, TEMP, CS2 = 0, 1, 2, 3, 4, 7, 8, 9
+
+
+def build(force=False):
+    """Compile liboracle.so with g++ -O2 -ffp-contract=off (no FMA contraction)."""
+    srcs = [os.path.join(_HERE, s) for s in _SOURCES]
+    deps = srcs + [os.path.join(_HERE, "orc.hpp")]
+    if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in deps):
+        return _LIB
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-o", _LIB] + srcs
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        L = _lib
+        dp, vp, i32, f64 = ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.orc_new.restype = vp
+        L.orc_free.argtypes = [vp]
+        L.orc_set.argtypes = [vp, ctypes.c_char_p, f64]
+        L.orc_set_array.argtypes = [vp, ctypes.c_char_p, vp, i32]
+        L.orc_set_table.argtypes = [vp, vp, vp, vp]
+        L.orc_finalize.argtypes = [vp]
+        L.orc_set_grid.argtypes = [vp, i32, i32, i32, i32, f64, f64, f64]
+        L.orc_fill_ghosts.argtypes = [vp, vp, i32, vp]
+        L.orc_con2prim.argtypes = [vp, vp, vp, vp]
+        L.orc_prim2con.argtypes = [vp, vp, vp]
+        for name in ("orc_rhs", "orc_rhs_ccz4", "orc_rhs_grmhd"):
+            getattr(L, name).argtypes = [vp, vp, vp, vp]
+        L.orc_rk_combine.argtypes = [vp, i32, vp, vp, i32, vp, vp, f64]
+        L.orc_evolve.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, f64, i32]
+        for name, n in (("orc_d1", 1), ("orc_d2", 1)):
+            getattr(L, name).argtypes = [vp, ctypes.c_long, f64]
+            getattr(L, name).restype = f64
+        L.orc_d11.argtypes = [vp, ctypes.c_long, f64, ctypes.c_long, f64]
+        L.orc_d11.restype = f64
+        L.orc_dadv.argtypes = [vp, ctypes.c_long, f64, f64]
+        L.orc_dadv.restype = f64
+        L.orc_dko.argtypes = [vp, ctypes.c_long, f64, f64]
+        L.orc_dko.restype = f64
+        L.orc_mp5.argtypes = [f64] * 6
+        L.orc_mp5.restype = f64
+        L.orc_eos.argtypes = [vp, f64, f64, f64, vp]
+        L.orc_eos_eps_from_T.argtypes = [vp, f64, f64, f64]
+        L.orc_eos_eps_from_T.restype = f64
+        L.orc_con2prim_point.argtypes = [vp, vp, f64, f64, vp, vp]
+        L.orc_con2prim_point.restype = i32
+        L.orc_prim2con_point.argtypes = [vp, vp, vp, vp]
+    return _lib
+
+
+def _ptr(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+class Oracle:
+    """One oracle instance = parameters + grid. Arrays are numpy float64, SoA (field, k, j, i)."""
+
+    def __init__(self, params, nx, ny, nz, ng, dx, dy=None, dz=None, table=None):
+        L = lib()
+        self.h = L.orc_new()
+        self._keep = []
+        for k, v in params.items():
+            if isinstance(v, (list, tuple, np.ndarray)):
+                arr = _f64(v)
+                if L.orc_set_array(self.h, k.encode(), _ptr(arr), arr.size) != 0:
+                    raise KeyError(k)
+            elif L.orc_set(self.h, k.encode(), float(v)) != 0:
+                raise KeyError(k)
+        if table is not None:
+            for k in ("n_rho", "n_T", "n_ye", "lr0", "dlr", "lT0", "dlT", "ye0", "dye", "tab_eps_shift", "tab_h0"):
+                L.orc_set(self.h, k.encode(), float(table[k]))
+            self._keep = [_f64(table["logp"]), _f64(table["loge"]), _f64(table["cs2"])]
+            L.orc_set_table(self.h, *[_ptr(a) for a in self._keep])
+        L.orc_finalize(self.h)
+        dy = dx if dy is None else dy
+        dz = dx if dz is None else dz
+        L.orc_set_grid(self.h, nx, ny, nz, ng, dx, dy, dz)
+        self.shape = (nz + 2 * ng, ny + 2 * ng, nx + 2 * ng)
+        self.npts = int(np.prod(self.shape))
+        self.ng = ng
+
+    def __del__(self):
+        try:
+            lib().orc_free(self.h)
+        except Exception:
+            pass
+
+    def fill_ghosts(self, U, bc):
+        assert U.dtype == np.float64 and U.flags.c_contiguous
+        b = np.asarray(bc, dtype=np.int32)
+        lib().orc_fill_ghosts(self.h, _ptr(U), U.shape[0], _ptr(b))
+        return U
+
+    def con2prim(self, U):
+        P = np.zeros((NPRIM,) + self.shape)
+        flags = np.zeros(self.shape, dtype=np.uint8)
+        lib().orc_con2prim(self.h, _ptr(U), _ptr(P), _ptr(flags))
+        return P, flags
+
+    def prim2con(self, U, P):
+        """P: rho, Ye, eps, v^i given; fills p, W, T, cs2 in P and the fluid conserved fields in U (in place)."""
+        assert P.dtype == np.float64 and P.flags.c_contiguous and U.flags.c_contiguous
+        lib().orc_prim2con(self.h, _ptr(U), _ptr(P))
+        return U, P
+
+    def rhs(self, U, P, part="all"):
+        K = np.zeros_like(U)
+        fn = {"all": "orc_rhs", "ccz4": "orc_rhs_ccz4", "grmhd": "orc_rhs_grmhd"}[part]
+        getattr(lib(), fn)(self.h, _ptr(U), _ptr(P), _ptr(K))
+        return K
+
+    def rk_combine(self, U0, Ks, coef, dt):
+        out = U0.copy()
+        ptrs = (ctypes.c_void_p * len(Ks))(*[k.ctypes.data for k in Ks])
+        c = _f64(coef)
+        lib().orc_rk_combine(self.h, U0.shape[0], _ptr(out), _ptr(U0), len(Ks), ptrs, _ptr(c), float(dt))
+        return out
+
+    def evolve(self, U, bc, a_expl, w_expl, dt, n_steps):
+        """Advance U in place by n_steps full RK steps; returns (P, flags) of the final state."""
+        P = np.zeros((NPRIM,) + self.shape)
+        flags = np.zeros(self.shape, dtype=np.uint8)
+        a = _f64(a_expl)
+        w = _f64(w_expl)
+        b = np.asarray(bc, dtype=np.int32)
+        lib().orc_evolve(self.h, _ptr(U), _ptr(P), _ptr(flags), _ptr(b), len(w), _ptr(a), _ptr(w), float(dt), int(n_steps))
+        return P, flags
+
+    def eos(self, rho, eps, ye=0.3):
+        out = np.zeros(3)
+        lib().orc_eos(self.h, rho, eps, ye, _ptr(out))
+        return out  # p, T, cs2
+
+    def eps_from_T(self, rho, T, ye):
+        return lib().orc_eos_eps_from_T(self.h, rho, T, ye)
+
+    def con2prim_point(self, gt, chi, alpha, ucons):
+        gt = _f64(gt)
+        uc = _f64(ucons).copy()
+        prim = np.zeros(NPRIM)
+        flag = lib().orc_con2prim_point(self.h, _ptr(gt), chi, alpha, _ptr(uc), _ptr(prim))
+        return prim, flag, uc
+
+
+def prim2con_point(gl, prim, B):
+    out = np.zeros(5)
+    lib().orc_prim2con_point(_ptr(_f64(gl)), _ptr(_f64(prim)), _ptr(_f64(B)), _ptr(out))
+    return out  # D, tau, S_x, S_y, S_z
+
+
+def stencil(name, u, s, h, *extra):
+    """Apply one oracle stencil at the centre element of the 1-D/2-D numpy array u (for the pins)."""
+    u = _f64(u)
+    L = lib()
+    flat = u.reshape(-1)
+    c = flat.size // 2
+    p = ctypes.c_void_p(flat.ctypes.data + 8 * c)
+    return getattr(L, "orc_" + name)(p, s, h, *extra)

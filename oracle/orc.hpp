@@ -1,0 +1,118 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, single-threaded FP64 C++ restatement of the per-stage hot path of
+// MHDuet (arXiv 2510.13965): ghost fill, con2prim, CCZ4+GRMHD right-hand side and
+// the explicit Runge-Kutta combine, written step by step from PAPER.md in the
+// paper's order and notation. It shares no code with the CUDA library under
+// paper_2510_13965_b200/csrc/. Only tests/, __graft_entry__.smoke() and the
+// cpu_baseline / --impl reference legs of bench.py may build, load or call it.
+// Compile with -O2 -ffp-contract=off (no FMA contraction).
+//
+// Citations are "PAPER.md:<line>" plus the equation they fall in. Readings of
+// silent / garbled passages are the R-numbers of DESIGN.md.
+//
+// Parity pins (tests/test_oracle_*.py): stencils (polynomial exactness + leading
+// error constants), CCZ4 (flat space = 0; manufactured wavy-Minkowski exact solution,
+// also with a Killing Z-vector), GRMHD (boosted magnetised fluid in wavy Minkowski;
+// TOV equilibrium; SRMHD Alfven wave; Riemann monotonicity), con2prim (round trip),
+// MP5 (Eq. 70 on smooth data, monotone on a step), RK (exp series).
+// PARITY UNPINNED: kappa_z/kappa_c/kappa_2 damping terms beyond "vanish with the
+// constraint" and a hand value; atmosphere / error-policy parameter values (R10);
+// outflow boundary order (R17).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+
+namespace orc {
+
+// ---- evolved state U (SoA, x fastest); PAPER.md:132 (conformal fields), :221 (conserved)
+enum {
+  GXX = 0, GXY, GXZ, GYY, GYZ, GZZ,        // conformal metric  gamma~_ij
+  AXX, AXY, AXZ, AYY, AYZ, AZZ,            // conformal trace-free extrinsic curvature A~_ij
+  CHI, KHAT, THETA,                        // chi, K^ = K - 2 Theta, Theta
+  GAMX, GAMY, GAMZ,                        // Gamma^^i = Gamma~^i + 2 Z^i / chi
+  ALPHA, BETAX, BETAY, BETAZ,              // lapse, shift
+  DBAR, DYEBAR, TAUBAR, SXBAR, SYBAR, SZBAR, BXBAR, BYBAR, BZBAR, PHIBAR,  // sqrt(gamma) * (D, D Ye, tau, S_i, B^i, phi)
+  NSTATE = 32, NSPACETIME = 22
+};
+// ---- primitives P
+enum { RHO = 0, YE, EPS, PRESS, VX, VY, VZ, WLOR, TEMP, CS2, NPRIM = 10 };
+
+// ---- flag bits (one byte per cell); PAPER.md:1157-1162 error policy
+enum {
+  FLAG_ATMO = 1, FLAG_EPS_LO = 2, FLAG_EPS_HI = 4, FLAG_VMAX = 8, FLAG_YE = 16,
+  FLAG_FATAL = 32, FLAG_NOCONV = 64, FLAG_M1FIX = 128
+};
+
+struct Grid {
+  int nx, ny, nz, ng;     // interior points per axis, ghost width
+  double dx, dy, dz;
+  int mx() const { return nx + 2 * ng; }
+  int my() const { return ny + 2 * ng; }
+  int mz() const { return nz + 2 * ng; }
+  size_t npts() const { return (size_t)mx() * my() * mz(); }
+  size_t idx(int i, int j, int k) const { return ((size_t)k * my() + j) * mx() + i; }
+};
+
+struct Params {
+  // EoS: 0 ideal gas p=(Gamma-1) rho eps; 1 hybrid piecewise polytrope (Eqs. 30-31); 2 table
+  int eos_kind;
+  double eos_gamma;        // kind 0
+  double eos_gamma_th;     // kinds 1
+  int n_pieces;            // kind 1 (<= 8)
+  double pp_K[8], pp_Gamma[8], pp_rho[8], pp_a[8];   // piece i valid for pp_rho[i-1] <= rho < pp_rho[i]
+  // kind 2: table of log10 p, log10 (eps + eps_shift), cs2 on (log10 rho, log10 T, Ye)
+  const double *tab_logp, *tab_loge, *tab_cs2;
+  int n_rho, n_T, n_ye;
+  double lr0, dlr, lT0, dlT, ye0, dye, tab_eps_shift, tab_h0;
+  // CCZ4 + gauge (Eqs. 13-20, 25-26)
+  double kappa_z, kappa_c, kappa_2, eta_shift, f_alpha, f_beta, beta0[3], grav_G;
+  double sigma_ko_spacetime, sigma_ko_matter;
+  // GRMHD (Eq. 28; MP5 alpha l.518)
+  double c_b, kappa_b, mp5_alpha;
+  // con2prim error policy (l.1153-1162)
+  double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
+  double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
+  int c2p_maxit;
+};
+
+// ---- stencils (Sec. III B)
+double d1(const double* u, long s, double h);                 // Eq. (60)
+double d2(const double* u, long s, double h);                 // Eq. (62)
+double d11(const double* u, long s1, double h1, long s2, double h2);  // Eq. (61)
+double dadv(const double* u, long s, double h, double beta);  // l.454-456
+double dko(const double* u, long s, double h, double sigma);  // l.460
+double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alpha);  // Eqs. (70)-(76)
+
+// ---- EoS
+struct EosOut { double p, T, cs2; };
+void eos_init(Params& par);                                   // fills pp_a by continuity (l.246)
+EosOut eos_from_rho_eps(const Params& par, double rho, double eps, double ye);
+void eos_eps_range(const Params& par, double rho, double ye, double& emin, double& emax);
+void eos_rho_range(const Params& par, double& rmin, double& rmax);
+double eos_h0(const Params& par);
+double eos_eps_from_T(const Params& par, double rho, double T, double ye);
+
+// ---- pointwise physics
+// prim -> conserved (undensitised), Eq. (29); gl = physical metric gamma_ij (6 comps)
+void prim2con_point(const double gl[6], const double prim[NPRIM], const double B[3],
+                    double& D, double& tau, double S[3]);
+// con -> prim, App. D; returns flag byte; may modify the conserved fields (R11)
+uint8_t con2prim_point(const Params& par, const double gt[6], double chi, double alpha,
+                       double ucons[10], double prim[NPRIM]);
+
+// ---- whole-patch operations (a1..a9)
+void fill_ghosts(const Grid& g, double* U, int nfields, const int bc[6]);
+void con2prim(const Params& par, const Grid& g, double* U, double* P, uint8_t* flags);
+void prim2con(const Params& par, const Grid& g, double* U, double* P);   // densitises; uses metric in U
+void rhs(const Params& par, const Grid& g, const double* U, const double* P, double* K);
+void rhs_ccz4(const Params& par, const Grid& g, const double* U, const double* P, double* K);
+void rhs_grmhd(const Params& par, const Grid& g, const double* U, const double* P, double* K);
+void rk_combine(const Grid& g, int nfields, double* Uout, const double* U0, int nk,
+                const double* const* K, const double* coef, double dt);
+// n_steps full RK steps: per stage fill -> con2prim -> rhs -> combine (Eq. 53)
+void evolve(const Params& par, const Grid& g, double* U, double* P, uint8_t* flags,
+            const int bc[6], int stages, const double* a_expl, const double* w_expl,
+            double dt, int n_steps);
+
+}  // namespace orc

@@ -1,0 +1,96 @@
+// ORACLE (test infrastructure) — plain C entry points for the ctypes binding in oracle/__init__.py.
+#include <cstring>
+#include <string>
+#include "orc.hpp"
+
+using namespace orc;
+
+namespace {
+struct Handle { Params par; Grid grid; };
+
+bool set_scalar(Params& p, const std::string& k, double v) {
+#define D(name) if (k == #name) { p.name = v; return true; }
+#define I(name) if (k == #name) { p.name = (int)v; return true; }
+  I(eos_kind) D(eos_gamma) D(eos_gamma_th) I(n_pieces)
+  D(kappa_z) D(kappa_c) D(kappa_2) D(eta_shift) D(f_alpha) D(f_beta) D(grav_G)
+  D(sigma_ko_spacetime) D(sigma_ko_matter) D(c_b) D(kappa_b) D(mp5_alpha)
+  D(rho_atmo) D(rho_cut) D(rho_low) D(alpha_bh) D(w_max) D(rho_max) D(eps_min) D(eps_max)
+  D(ye_min) D(ye_max) D(ye_atmo) D(eps_atmo) D(T_atmo) I(c2p_maxit)
+  I(n_rho) I(n_T) I(n_ye) D(lr0) D(dlr) D(lT0) D(dlT) D(ye0) D(dye) D(tab_eps_shift) D(tab_h0)
+#undef D
+#undef I
+  return false;
+}
+}  // namespace
+
+extern "C" {
+
+void* orc_new() {
+  Handle* h = new Handle();
+  std::memset(&h->par, 0, sizeof(Params));
+  std::memset(&h->grid, 0, sizeof(Grid));
+  return h;
+}
+void orc_free(void* h) { delete (Handle*)h; }
+
+int orc_set(void* h, const char* key, double v) { return set_scalar(((Handle*)h)->par, key, v) ? 0 : -1; }
+
+int orc_set_array(void* hh, const char* key, const double* v, int n) {
+  Params& p = ((Handle*)hh)->par;
+  const std::string k = key;
+  double* dst = nullptr;
+  int cap = 8;
+  if (k == "pp_K") dst = p.pp_K;
+  else if (k == "pp_Gamma") dst = p.pp_Gamma;
+  else if (k == "pp_rho") dst = p.pp_rho;
+  else if (k == "beta0") { dst = p.beta0; cap = 3; }
+  if (!dst || n > cap) return -1;
+  for (int i = 0; i < n; ++i) dst[i] = v[i];
+  return 0;
+}
+// table pointers are borrowed (caller keeps the arrays alive)
+void orc_set_table(void* hh, const double* logp, const double* loge, const double* cs2) {
+  Params& p = ((Handle*)hh)->par;
+  p.tab_logp = logp; p.tab_loge = loge; p.tab_cs2 = cs2;
+}
+void orc_finalize(void* hh) { eos_init(((Handle*)hh)->par); }
+
+void orc_set_grid(void* hh, int nx, int ny, int nz, int ng, double dx, double dy, double dz) {
+  ((Handle*)hh)->grid = Grid{nx, ny, nz, ng, dx, dy, dz};
+}
+
+void orc_fill_ghosts(void* hh, double* U, int nfields, const int* bc) { fill_ghosts(((Handle*)hh)->grid, U, nfields, bc); }
+void orc_con2prim(void* hh, double* U, double* P, uint8_t* flags) { Handle* h = (Handle*)hh; con2prim(h->par, h->grid, U, P, flags); }
+void orc_prim2con(void* hh, double* U, double* P) { Handle* h = (Handle*)hh; prim2con(h->par, h->grid, U, P); }
+void orc_rhs(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs(h->par, h->grid, U, P, K); }
+void orc_rhs_ccz4(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_ccz4(h->par, h->grid, U, P, K); }
+void orc_rhs_grmhd(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_grmhd(h->par, h->grid, U, P, K); }
+void orc_rk_combine(void* hh, int nfields, double* Uout, const double* U0, int nk, const double* const* K, const double* coef, double dt) {
+  rk_combine(((Handle*)hh)->grid, nfields, Uout, U0, nk, K, coef, dt);
+}
+void orc_evolve(void* hh, double* U, double* P, uint8_t* flags, const int* bc, int stages,
+                const double* a_expl, const double* w_expl, double dt, int n_steps) {
+  Handle* h = (Handle*)hh;
+  evolve(h->par, h->grid, U, P, flags, bc, stages, a_expl, w_expl, dt, n_steps);
+}
+
+// ---- pointwise helpers for the pins
+double orc_d1(const double* u, long s, double h) { return d1(u, s, h); }
+double orc_d2(const double* u, long s, double h) { return d2(u, s, h); }
+double orc_d11(const double* u, long s1, double h1, long s2, double h2) { return d11(u, s1, h1, s2, h2); }
+double orc_dadv(const double* u, long s, double h, double beta) { return dadv(u, s, h, beta); }
+double orc_dko(const double* u, long s, double h, double sigma) { return dko(u, s, h, sigma); }
+double orc_mp5(double a, double b, double c, double d, double e, double alpha) { return mp5(a, b, c, d, e, alpha); }
+void orc_eos(void* hh, double rho, double eps, double ye, double* out3) {
+  const EosOut e = eos_from_rho_eps(((Handle*)hh)->par, rho, eps, ye);
+  out3[0] = e.p; out3[1] = e.T; out3[2] = e.cs2;
+}
+double orc_eos_eps_from_T(void* hh, double rho, double T, double ye) { return eos_eps_from_T(((Handle*)hh)->par, rho, T, ye); }
+int orc_con2prim_point(void* hh, const double* gt, double chi, double alpha, double* ucons, double* prim) {
+  return con2prim_point(((Handle*)hh)->par, gt, chi, alpha, ucons, prim);
+}
+void orc_prim2con_point(const double* gl, const double* prim, const double* B, double* out5) {
+  prim2con_point(gl, prim, B, out5[0], out5[1], out5 + 2);
+}
+
+}  // extern "C"
