@@ -1,0 +1,166 @@
+/* mhd.h — C ABI of the B200-native per-stage hot path of MHDuet (arXiv 2510.13965) on one uniform,
+ * ghosted, vertex-centred grid patch.
+ *
+ * One RK stage (Eq. 53, l.384-387; App. C step C3) is the call sequence
+ *     mhd_fill_ghosts -> mhd_con2prim -> mhd_rhs -> mhd_rk_stage
+ * every step of which runs in hand-written sm_100a CUDA kernels. There is no CPU fallback.
+ *
+ * Memory model. The CALLER owns all field memory (device pointers, e.g. torch tensors) and binds it to
+ * numbered slots with mhd_patch_bind; the library allocates only a few hundred bytes of device scratch at
+ * create time, allocates nothing per call, launches asynchronously on the caller's stream
+ * (a cudaStream_t passed as void*; NULL = legacy default stream) and never synchronises except in
+ * mhd_patch_status and the *_host entry points. All floating point is FP64.
+ *
+ * Layout. A slot holds n_fields fields, SoA: value of field f at grid point (i,j,k) is
+ *     base[f * field_stride + (k * MY + j) * MX + i],   MX = nx + 2 ng  (x fastest), 0 <= i < MX ...
+ * Interior points are ng <= i < ng + nx. field_stride >= MX*MY*MZ (elements).
+ *
+ * State fields U (32): 0-5 gamma~_ij (xx,xy,xz,yy,yz,zz), 6-11 A~_ij, 12 chi, 13 K^, 14 Theta,
+ *   15-17 Gamma^^i, 18 alpha, 19-21 beta^i (Eqs. 13-26);
+ *   22 Dbar, 23 DYebar, 24 taubar, 25-27 Sbar_i, 28-30 Bbar^i, 31 phibar = sqrt(gamma) x Eq. (29).
+ * Primitive fields P (10): rho, Ye, eps, p, v^x, v^y, v^z (contravariant), W, T, cs2.
+ * Flags: one byte per grid point, bits = MHD_FLAG_*.
+ *
+ * Errors. Every function returns MHD_OK (0) or a negative MHD_E_* code; nothing throws or aborts.
+ * The paper's "fatal error, stop the code" is a flag bit plus a counter.
+ */
+#ifndef MHD_H
+#define MHD_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MHD_NSTATE 32
+#define MHD_NPRIM 10
+#define MHD_MAX_STAGES 8
+#define MHD_MAX_PIECES 8
+
+/* slots */
+enum {
+  MHD_SLOT_U = 0,      /* current stage state U^(i)                      (MHD_NSTATE fields) */
+  MHD_SLOT_U0 = 1,     /* U^n, saved by mhd_rk_stage(stage = 0)          (MHD_NSTATE fields) */
+  MHD_SLOT_P = 2,      /* primitives                                     (MHD_NPRIM fields)  */
+  MHD_SLOT_FLAGS = 3,  /* uint8 flags, one field                                             */
+  MHD_SLOT_K1 = 4,     /* K_1 ... K_s = F(U^(j)): MHD_SLOT_K1 + j - 1    (MHD_NSTATE fields) */
+  MHD_NSLOTS = 4 + MHD_MAX_STAGES
+};
+
+/* flag bits: error policy of PAPER.md:1157-1162 */
+enum {
+  MHD_FLAG_ATMO = 1,     /* rule 1: reset to atmosphere                    */
+  MHD_FLAG_EPS_LO = 2,   /* rule 3: eps raised to eps_min                  */
+  MHD_FLAG_EPS_HI = 4,   /* rule 4: eps lowered to eps_max                 */
+  MHD_FLAG_VMAX = 8,     /* rule 5: velocity rescaled to W_max             */
+  MHD_FLAG_YE = 16,      /* rule 6: Ye reset                               */
+  MHD_FLAG_FATAL = 32,   /* rules 2, 4-6 outside low-density / BH regions  */
+  MHD_FLAG_NOCONV = 64,  /* a root find hit the iteration cap              */
+  MHD_FLAG_M1FIX = 128   /* reserved: M1 fix-up                            */
+};
+
+enum {
+  MHD_OK = 0,
+  MHD_E_ARG = -1,        /* null pointer / out-of-range argument            */
+  MHD_E_UNBOUND = -2,    /* a slot needed by the call has not been bound    */
+  MHD_E_CUDA = -3,       /* CUDA runtime error (launch, copy, allocation)   */
+  MHD_E_UNSUPPORTED = -4 /* feature not built (e.g. n_species != 0)         */
+};
+
+/* Plain data, copied at create time. Pointers inside are DEVICE pointers that must outlive the patch. */
+typedef struct {
+  int nx, ny, nz, ng;              /* interior points per axis; ghost width (>= 3: MP5/KO/advective stencils) */
+  double dx, dy, dz;               /* uniform spacing */
+  int n_species;                   /* 0 (M1 off); 3 is reserved */
+  /* EoS: 0 ideal gas p=(Gamma-1) rho eps; 1 hybrid piecewise polytrope (Eqs. 30-31); 2 table */
+  int eos_kind;
+  double eos_gamma;                /* kind 0 */
+  double eos_gamma_th;             /* kind 1 */
+  int n_pieces;                    /* kind 1; piece i holds for pp_rho[i-1] <= rho < pp_rho[i]; K_i, a_i (i>0) by continuity */
+  double pp_K[MHD_MAX_PIECES], pp_Gamma[MHD_MAX_PIECES], pp_rho[MHD_MAX_PIECES];
+  /* kind 2: log10 p, log10(eps + tab_eps_shift), cs2 tabulated on (log10 rho, log10 T, Ye), rho fastest; DEVICE pointers */
+  const double *tab_logp, *tab_loge, *tab_cs2;
+  int n_rho, n_T, n_ye;
+  double lr0, dlr, lT0, dlT, ye0, dye, tab_eps_shift, tab_h0;
+  /* CCZ4 + gauge, Eqs. (13)-(20), (25)-(26) */
+  double kappa_z, kappa_c, kappa_2, eta_shift, f_alpha, f_beta, beta0[3];
+  double grav_G;                   /* the explicit G of 8 pi G in Eqs. (14),(16),(17),(19); 0 decouples matter */
+  double sigma_ko_spacetime, sigma_ko_matter;   /* Kreiss-Oliger sigma */
+  /* GRMHD: divergence cleaning speed and damping (Eq. 28), MP5 alpha */
+  double c_b, kappa_b, mp5_alpha;
+  /* con2prim error policy */
+  double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
+  double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
+  int c2p_maxit;
+} mhd_patch_desc;
+
+/* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */
+typedef struct {
+  int stages;
+  const double *a_expl, *w_expl, *a_impl, *w_impl;
+} mhd_tableau;
+
+typedef struct {
+  unsigned long long n_points, n_atmo, n_eps_lo, n_eps_hi, n_vmax, n_ye, n_fatal, n_noconv, n_m1fix;
+} mhd_status;
+
+typedef struct mhd_patch mhd_patch;   /* opaque */
+
+size_t mhd_desc_sizeof(void);         /* sizeof(mhd_patch_desc) as compiled, for binding self-checks */
+
+/* Create / destroy. *out owns a copy of desc and a small device scratch buffer. */
+int mhd_patch_create(const mhd_patch_desc *desc, mhd_patch **out);
+void mhd_patch_destroy(mhd_patch *p);
+
+/* Bind caller-owned DEVICE memory to a slot. field_stride in elements (doubles; bytes for MHD_SLOT_FLAGS). */
+int mhd_patch_bind(mhd_patch *p, int slot, void *dev_ptr, size_t field_stride);
+
+/* a1 — ghost fill: bc[6] = {x-,x+,y-,y+,z-,z+}, 0 periodic wrap, 1 outflow (copy of the nearest
+ * interior value). Fills all ng ghost layers incl. edges and corners of every field of the slot, in place. */
+int mhd_fill_ghosts(mhd_patch *p, int slot_state, const int bc[6], void *cuda_stream);
+
+/* a2 — conserved -> primitive at every grid point incl. ghosts (App. D, Eqs. D1-D15, error policy
+ * l.1157-1162). Writes the 10 primitives and the flag byte; where a rule changed a primitive the fluid conserved
+ * fields of slot_state are reset from the corrected primitives (Bbar, phibar untouched). */
+int mhd_con2prim(mhd_patch *p, int slot_state, int slot_prim, int slot_flags, void *cuda_stream);
+
+/* inverse of a2 for initial data (Eq. 29): slot_prim holds rho, Ye, eps, v^i; fills p, W, T, cs2 there and
+ * Dbar, DYebar, taubar, Sbar_i in slot_state from them, the metric and Bbar^i already in slot_state. */
+int mhd_prim2con(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream);
+
+/* a3-a8 — right-hand side F(U) on the interior: CCZ4 + gauge (Eqs. 13-26; FD Eqs. 60-62, upwind l.454-456,
+ * KO l.460), GRMHD flux divergence (Eq. 32 with Eqs. 63-76, speeds App. B) and sources. Ghost points of
+ * slot_rhs are not written. Needs filled ghosts in slot_state and primitives at all points. */
+int mhd_rhs(mhd_patch *p, int slot_state, int slot_prim, int slot_rhs, void *cuda_stream);
+
+/* a9 — explicit RK combine on the interior (Eq. 53).
+ *   stage = 0          : U0 <- U  (start of a step)
+ *   1 <= stage < s     : U <- U0 + dt * sum_{j<=stage} a_expl[stage][j-1] K_j      (= U^(stage+1))
+ *   stage = s          : U <- U0 + dt * sum_j w_expl[j-1] K_j                      (= U^{n+1})
+ * K_j is slot MHD_SLOT_K1 + j - 1; zero coefficients are skipped (their slots need not be bound). */
+int mhd_rk_stage(mhd_patch *p, const mhd_tableau *t, int stage, double dt, void *cuda_stream);
+
+/* n_steps full RK steps, device resident: per stage fill -> con2prim -> rhs(K_stage) -> rk_stage; the state is
+ * left with ghosts filled and primitives/flags consistent. Asynchronous. */
+int mhd_advance(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
+
+/* Same, end to end with HOST buffers: copies host_U (MHD_NSTATE fields, packed, field_stride = MX*MY*MZ) to
+ * slot U, advances, copies U back into host_U and the flags into host_flags (may be NULL), then synchronises
+ * the stream. Pinned host memory makes the copies asynchronous with respect to the host. */
+int mhd_advance_host(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps,
+                     double *host_U, uint8_t *host_flags, void *cuda_stream);
+
+/* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */
+int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_stream);
+
+/* Measured FP64 FMA throughput of the device (register-resident DFMA chains on every SM), in FLOP/s;
+ * used as the FP64 roofline denominator. Synchronises. Returns < 0 on error. */
+double mhd_probe_fp64_flops(void *cuda_stream);
+
+const char *mhd_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_H */

@@ -1,0 +1,224 @@
+// C ABI of libmhd_b200 (see include/mhd.h): argument checking, slot bookkeeping and kernel sequencing only.
+#include <math.h>
+#include <new>
+#include <string.h>
+#include "mhd_internal.cuh"
+
+using namespace mhd;
+
+namespace {
+
+int slot_fields(int slot) {
+  if (slot == MHD_SLOT_P) return MHD_NPRIM;
+  if (slot == MHD_SLOT_FLAGS) return 1;
+  return MHD_NSTATE;
+}
+bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLOTS && p->slot[slot].ptr != nullptr; }
+bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || (slot >= MHD_SLOT_K1 && slot < MHD_NSLOTS); }
+double* dptr(const mhd_patch* p, int slot) { return (double*)p->slot[slot].ptr; }
+
+// piecewise-polytrope continuity constants: K_i, a_i for i > 0
+void finish_eos(Par& q) {
+  q.pp_a[0] = 0.0;
+  for (int i = 1; i < q.n_pieces; ++i) {
+    const double rb = q.pp_rho[i - 1];
+    q.pp_K[i] = q.pp_K[i - 1] * pow(rb, q.pp_Gamma[i - 1] - q.pp_Gamma[i]);
+    const double em = q.pp_a[i - 1] + q.pp_K[i - 1] / (q.pp_Gamma[i - 1] - 1.0) * pow(rb, q.pp_Gamma[i - 1] - 1.0);
+    q.pp_a[i] = em - q.pp_K[i] / (q.pp_Gamma[i] - 1.0) * pow(rb, q.pp_Gamma[i] - 1.0);
+  }
+}
+
+int stage_sequence(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, cudaStream_t s) {
+  int rc;
+  for (int step = 0; step < n_steps; ++step) {
+    if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
+    if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return rc;
+    if ((rc = mhd_rk_stage(p, t, 0, dt, s)) != MHD_OK) return rc;
+    for (int st = 1; st <= t->stages; ++st) {
+      if (st > 1) {
+        if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
+        if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return rc;
+      }
+      if ((rc = mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st - 1, s)) != MHD_OK) return rc;
+      if ((rc = mhd_rk_stage(p, t, st, dt, s)) != MHD_OK) return rc;
+    }
+  }
+  if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
+  return mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s);
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t mhd_desc_sizeof(void) { return sizeof(mhd_patch_desc); }
+
+int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
+  if (!desc || !out) return MHD_E_ARG;
+  if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1 || desc->ng < 3) return MHD_E_ARG;
+  if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
+  if (desc->n_species != 0) return MHD_E_UNSUPPORTED;
+  if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
+  if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
+  if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2)) return MHD_E_ARG;
+  mhd_patch* p = new (std::nothrow) mhd_patch();
+  if (!p) return MHD_E_ARG;
+  p->desc = *desc;
+  Dims& d = p->dims;
+  d.nx = desc->nx; d.ny = desc->ny; d.nz = desc->nz; d.ng = desc->ng;
+  d.mx = d.nx + 2 * d.ng; d.my = d.ny + 2 * d.ng; d.mz = d.nz + 2 * d.ng;
+  d.sy = d.mx; d.sz = (long long)d.mx * d.my; d.npts = d.sz * d.mz;
+  d.dx = desc->dx; d.dy = desc->dy; d.dz = desc->dz;
+  Par& q = p->par;
+  memset(&q, 0, sizeof(q));
+  q.eos_kind = desc->eos_kind; q.n_pieces = desc->n_pieces; q.eos_gamma = desc->eos_gamma; q.eos_gamma_th = desc->eos_gamma_th;
+  for (int i = 0; i < MHD_MAX_PIECES; ++i) { q.pp_K[i] = desc->pp_K[i]; q.pp_Gamma[i] = desc->pp_Gamma[i]; q.pp_rho[i] = desc->pp_rho[i]; }
+  if (q.eos_kind == 1) finish_eos(q);
+  q.tab_logp = desc->tab_logp; q.tab_loge = desc->tab_loge; q.tab_cs2 = desc->tab_cs2;
+  q.n_rho = desc->n_rho; q.n_T = desc->n_T; q.n_ye = desc->n_ye;
+  q.lr0 = desc->lr0; q.dlr = desc->dlr; q.lT0 = desc->lT0; q.dlT = desc->dlT; q.ye0 = desc->ye0; q.dye = desc->dye;
+  q.tab_eps_shift = desc->tab_eps_shift; q.tab_h0 = desc->tab_h0;
+  q.kappa_z = desc->kappa_z; q.kappa_c = desc->kappa_c; q.kappa_2 = desc->kappa_2; q.eta_shift = desc->eta_shift;
+  q.f_alpha = desc->f_alpha; q.f_beta = desc->f_beta; q.grav_G = desc->grav_G;
+  for (int i = 0; i < 3; ++i) q.beta0[i] = desc->beta0[i];
+  q.sigma_ko_spacetime = desc->sigma_ko_spacetime; q.sigma_ko_matter = desc->sigma_ko_matter;
+  q.c_b = desc->c_b; q.kappa_b = desc->kappa_b; q.mp5_alpha = desc->mp5_alpha;
+  q.rho_atmo = desc->rho_atmo; q.rho_cut = desc->rho_cut; q.rho_low = desc->rho_low; q.alpha_bh = desc->alpha_bh;
+  q.w_max = desc->w_max; q.rho_max = desc->rho_max; q.eps_min = desc->eps_min; q.eps_max = desc->eps_max;
+  q.ye_min = desc->ye_min; q.ye_max = desc->ye_max; q.ye_atmo = desc->ye_atmo; q.eps_atmo = desc->eps_atmo; q.T_atmo = desc->T_atmo;
+  q.c2p_maxit = desc->c2p_maxit > 0 ? desc->c2p_maxit : 100;
+  p->d_counts = nullptr;
+  if (cudaMalloc(&p->d_counts, 8 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
+  *out = p;
+  return MHD_OK;
+}
+
+void mhd_patch_destroy(mhd_patch* p) {
+  if (!p) return;
+  if (p->d_counts) cudaFree(p->d_counts);
+  delete p;
+}
+
+int mhd_patch_bind(mhd_patch* p, int slot, void* dev_ptr, size_t field_stride) {
+  if (!p || slot < 0 || slot >= MHD_NSLOTS || !dev_ptr) return MHD_E_ARG;
+  if (field_stride < (size_t)p->dims.npts) return MHD_E_ARG;
+  p->slot[slot].ptr = dev_ptr;
+  p->slot[slot].stride = field_stride;
+  return MHD_OK;
+}
+
+int mhd_fill_ghosts(mhd_patch* p, int slot_state, const int bc[6], void* stream) {
+  if (!p || !bc) return MHD_E_ARG;
+  for (int a = 0; a < 6; ++a) if (bc[a] != 0 && bc[a] != 1) return MHD_E_ARG;
+  if (slot_state < 0 || slot_state >= MHD_NSLOTS || slot_state == MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (!slot_ok(p, slot_state)) return MHD_E_UNBOUND;
+  return launch_fill_ghosts(p->dims, dptr(p, slot_state), p->slot[slot_state].stride, slot_fields(slot_state), bc, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_con2prim(mhd_patch* p, int slot_state, int slot_prim, int slot_flags, void* stream) {
+  if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || slot_flags != MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_flags)) return MHD_E_UNBOUND;
+  return launch_con2prim(p->dims, p->par, dptr(p, slot_state), p->slot[slot_state].stride, dptr(p, slot_prim), p->slot[slot_prim].stride,
+                         (uint8_t*)p->slot[slot_flags].ptr, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_prim2con(mhd_patch* p, int slot_state, int slot_prim, void* stream) {
+  if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P) return MHD_E_ARG;
+  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim)) return MHD_E_UNBOUND;
+  return launch_prim2con(p->dims, p->par, dptr(p, slot_state), p->slot[slot_state].stride, dptr(p, slot_prim), p->slot[slot_prim].stride,
+                         (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* stream) {
+  if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || !is_state_slot(slot_rhs) || slot_rhs == slot_state) return MHD_E_ARG;
+  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_rhs)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  const double* U = dptr(p, slot_state);
+  const double* P = dptr(p, slot_prim);
+  double* K = dptr(p, slot_rhs);
+  const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
+  if (launch_rhs_ccz4(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
+  if (launch_rhs_flux(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
+  return MHD_OK;
+}
+
+int mhd_rk_stage(mhd_patch* p, const mhd_tableau* t, int stage, double dt, void* stream) {
+  if (!p || !t || !t->a_expl || !t->w_expl || t->stages < 1 || t->stages > MHD_MAX_STAGES || stage < 0 || stage > t->stages) return MHD_E_ARG;
+  if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_U0)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (stage == 0)
+    return launch_copy_fields(p->dims, MHD_NSTATE, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+  const double* coef = stage < t->stages ? t->a_expl + (size_t)stage * t->stages : t->w_expl;
+  const int nmax = stage < t->stages ? stage : t->stages;
+  const double* Kp[MHD_MAX_STAGES];
+  size_t sk[MHD_MAX_STAGES];
+  double c[MHD_MAX_STAGES];
+  int nk = 0;
+  for (int j = 0; j < nmax; ++j) {
+    if (coef[j] == 0.0) continue;
+    if (!slot_ok(p, MHD_SLOT_K1 + j)) return MHD_E_UNBOUND;
+    Kp[nk] = dptr(p, MHD_SLOT_K1 + j); sk[nk] = p->slot[MHD_SLOT_K1 + j].stride; c[nk] = coef[j]; ++nk;
+  }
+  if (nk == 0)   // U <- U0
+    return launch_copy_fields(p->dims, MHD_NSTATE, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+  return launch_rk_combine(p->dims, MHD_NSTATE, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride,
+                           nk, Kp, sk, c, dt, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_advance(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, void* stream) {
+  if (!p || !t || !bc || n_steps < 0) return MHD_E_ARG;
+  return stage_sequence(p, t, bc, dt, n_steps, (cudaStream_t)stream);
+}
+
+int mhd_advance_host(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, double* host_U, uint8_t* host_flags, void* stream) {
+  if (!p || !t || !bc || !host_U || n_steps < 0) return MHD_E_ARG;
+  if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_FLAGS)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n = (size_t)p->dims.npts, su = p->slot[MHD_SLOT_U].stride;
+  double* U = dptr(p, MHD_SLOT_U);
+  if (su == n) {
+    if (cudaMemcpyAsync(U, host_U, n * MHD_NSTATE * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess) return MHD_E_CUDA;
+  } else {
+    for (int f = 0; f < MHD_NSTATE; ++f)
+      if (cudaMemcpyAsync(U + f * su, host_U + f * n, n * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess) return MHD_E_CUDA;
+  }
+  const int rc = stage_sequence(p, t, bc, dt, n_steps, s);
+  if (rc != MHD_OK) return rc;
+  if (su == n) {
+    if (cudaMemcpyAsync(host_U, U, n * MHD_NSTATE * sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  } else {
+    for (int f = 0; f < MHD_NSTATE; ++f)
+      if (cudaMemcpyAsync(host_U + f * n, U + f * su, n * sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  }
+  if (host_flags && cudaMemcpyAsync(host_flags, p->slot[MHD_SLOT_FLAGS].ptr, n, cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  return cudaStreamSynchronize(s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream) {
+  if (!p || !out || slot_flags != MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (!slot_ok(p, slot_flags)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (launch_count_flags(p->dims, (const uint8_t*)p->slot[slot_flags].ptr, p->d_counts, s) != cudaSuccess) return MHD_E_CUDA;
+  unsigned long long h[8];
+  if (cudaMemcpyAsync(h, p->d_counts, sizeof(h), cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return MHD_E_CUDA;
+  out->n_points = (unsigned long long)p->dims.npts;
+  out->n_atmo = h[0]; out->n_eps_lo = h[1]; out->n_eps_hi = h[2]; out->n_vmax = h[3];
+  out->n_ye = h[4]; out->n_fatal = h[5]; out->n_noconv = h[6]; out->n_m1fix = h[7];
+  return MHD_OK;
+}
+
+double mhd_probe_fp64_flops(void* stream) { return probe_fp64((cudaStream_t)stream); }
+
+const char* mhd_strerror(int code) {
+  switch (code) {
+    case MHD_OK: return "ok";
+    case MHD_E_ARG: return "invalid argument";
+    case MHD_E_UNBOUND: return "slot not bound";
+    case MHD_E_CUDA: return "CUDA runtime error";
+    case MHD_E_UNSUPPORTED: return "feature not supported by this build";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

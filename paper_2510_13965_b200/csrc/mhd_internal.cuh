@@ -1,0 +1,66 @@
+// Internal declarations of libmhd_b200 (CUDA, sm_100a). Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/mhd.h"
+
+namespace mhd {
+
+// field indices of the state and primitive slots (see include/mhd.h)
+enum {
+  GXX = 0, GXY, GXZ, GYY, GYZ, GZZ, AXX, AXY, AXZ, AYY, AYZ, AZZ, CHI, KHAT, THETA, GAMX, GAMY, GAMZ,
+  ALPHA, BETAX, BETAY, BETAZ, DBAR, DYEBAR, TAUBAR, SXBAR, SYBAR, SZBAR, BXBAR, BYBAR, BZBAR, PHIBAR
+};
+enum { RHO = 0, YE, EPS, PRESS, VX, VY, VZ, WLOR, TEMP, CS2 };
+
+struct Dims {
+  int nx, ny, nz, ng, mx, my, mz;
+  long long sy, sz;          // strides of j and k in elements
+  long long npts;            // mx*my*mz
+  double dx, dy, dz;
+};
+
+// device-side parameter block, passed by value as a __grid_constant__ kernel argument
+struct Par {
+  int eos_kind, n_pieces;
+  double eos_gamma, eos_gamma_th;
+  double pp_K[MHD_MAX_PIECES], pp_Gamma[MHD_MAX_PIECES], pp_rho[MHD_MAX_PIECES], pp_a[MHD_MAX_PIECES];
+  const double *tab_logp, *tab_loge, *tab_cs2;
+  int n_rho, n_T, n_ye;
+  double lr0, dlr, lT0, dlT, ye0, dye, tab_eps_shift, tab_h0;
+  double kappa_z, kappa_c, kappa_2, eta_shift, f_alpha, f_beta, beta0[3], grav_G;
+  double sigma_ko_spacetime, sigma_ko_matter;
+  double c_b, kappa_b, mp5_alpha;
+  double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
+  double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
+  int c2p_maxit;
+};
+
+struct Slot {
+  void* ptr = nullptr;
+  size_t stride = 0;
+};
+
+}  // namespace mhd
+
+struct mhd_patch {
+  mhd_patch_desc desc;
+  mhd::Dims dims;
+  mhd::Par par;
+  mhd::Slot slot[MHD_NSLOTS];
+  unsigned long long* d_counts;   // 8 counters for mhd_patch_status
+};
+
+namespace mhd {
+// kernel launchers (one per translation unit); all return cudaGetLastError()
+cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], cudaStream_t s);
+cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, cudaStream_t s);
+cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
+cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_rhs_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
+                              int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s);
+cudaError_t launch_copy_fields(const Dims& d, int nfields, double* dst, size_t sd, const double* src, size_t ss, cudaStream_t s);
+cudaError_t launch_count_flags(const Dims& d, const uint8_t* flags, unsigned long long* counts, cudaStream_t s);
+double probe_fp64(cudaStream_t s);
+}  // namespace mhd
