@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py — zone-stage updates/s of the MHDuet per-stage hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1|c3|c4] [--n SIZE] [--impl ours|reference]
+
+A "step" is one full explicit RK4 time step of one patch = 4 passes of the whole hot path
+(fill_ghosts -> con2prim -> rhs -> rk_stage), so one step performs 4 * n^3 zone-stage updates.
+N > 1 (torchrun): the path does not shard (north_star: no multi-GPU decomposition) -> N independent replicas,
+weak scaling, value = sum over ranks / max-over-ranks time.
+
+One JSON line is printed by rank 0; see DESIGN.md "Measurement" for the roofline arithmetic.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "zone-stage updates/s"
+STAGES = 4
+
+
+def workload_inputs(name, n):
+    """Seeded synthetic inputs (paper_2510_13965_b200.synth); returns cfg dict with U (metric, Bbar), P (rho, Ye, eps, v)."""
+    from paper_2510_13965_b200 import synth
+    if name == "c1":
+        base = synth.config1(n=min(n, 32))
+        if n > 32:                      # periodic data: tile the 32^3 box (same spacing), keeps every field smooth
+            reps = (n + 31) // 32
+            ng = base["ng"]
+
+            def tile(A):
+                inner = A[:, ng:-ng, ng:-ng, ng:-ng]
+                big = np.tile(inner, (1, reps, reps, reps))[:, :n, :n, :n]
+                return np.ascontiguousarray(np.pad(big, ((0, 0), (ng, ng), (ng, ng), (ng, ng)), mode="wrap"))
+            base["U"], base["P"] = tile(base["U"]), tile(base["P"])
+            base["n"] = (n, n, n)
+        return base
+    if name == "c3":
+        return synth.config3(n=n)
+    if name == "c4":
+        return synth.config4(n=n)
+    raise ValueError(name)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for i, nm in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+def oracle_leg(cfg_name, n_sample, steps):
+    """The oracle as it stands, single thread, on a bounded sample of the workload; returns (value, seconds, zone_stages)."""
+    import oracle
+    from paper_2510_13965_b200 import synth
+    cfg = workload_inputs(cfg_name, n_sample)
+    n = cfg["n"]
+    o = oracle.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"], table=cfg.get("table"))
+    U, P = cfg["U"].copy(), cfg["P"].copy()
+    o.prim2con(U, P)
+    a, w = synth.tableau("rk4")
+    dt = 0.25 * cfg["dx"]
+    t0 = time.perf_counter()
+    o.evolve(U, cfg["bc"], a, w, dt, steps)
+    sec = time.perf_counter() - t0
+    zs = float(n[0] * n[1] * n[2] * STAGES * steps)
+    return zs / sec, sec, zs
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_s = args.ref_n
+    vals = []
+    for _ in range(args.warmup):
+        oracle_leg(args.workload, 16, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        v, sec, zs = oracle_leg(args.workload, n_s, 1)
+        vals.append((zs, sec))
+    total = time.perf_counter() - t0
+    value = sum(z for z, _ in vals) / sum(s for _, s in vals)
+    sample = "%d^3 crop-sized instance of workload %s, 1 RK4 step per bench step, single thread" % (n_s, args.workload)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "zone-stages/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s_%d" % (args.workload, args.n), "bounded_sample": sample},
+        "cpu_baseline": {"value": value, "unit": "zone-stages/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "zone-stages/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c1")
+    ap.add_argument("--n", type=int, default=256)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-n", type=int, default=40, help="sample size of the oracle legs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2510_13965_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = workload_inputs(args.workload, args.n)
+    n, ng = cfg["n"], cfg["ng"]
+    zones = n[0] * n[1] * n[2]
+    patch = binding.Patch(cfg["params"], n, ng, cfg["dx"], stages=STAGES, table=cfg.get("table"), device="cuda:%d" % local)
+    a, w = synth.tableau("rk4")
+    tab = binding.make_tableau(a, w)
+    dt = 0.25 * cfg["dx"]
+    # initial data: metric + Bbar in U, (rho, Ye, eps, v) in P; conserved fields from the library's own prim2con kernel
+    patch.upload(U=cfg["U"], P=cfg["P"])
+    patch.prim2con()
+    patch.fill_ghosts(cfg["bc"])
+    U_init = patch.U.clone()
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        patch.advance(tab, cfg["bc"], dt, 1)
+    torch.cuda.synchronize()
+    patch.U.copy_(U_init)
+    patch.profile(True)
+    patch.profile_read()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        patch.advance(tab, cfg["bc"], dt, 1)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop()
+    prof = patch.profile_read()
+    patch.profile(False)
+    status = patch.status()
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * zones * STAGES * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (H2D of the state, advance, D2H of state + flags) ------
+    e2e = None
+    if not args.no_e2e:
+        hostU = U_init.cpu().pin_memory()
+        hostF = torch.zeros(patch.flags.shape[1:], dtype=torch.uint8).pin_memory()
+        src = hostU.clone()
+        e_steps = max(1, min(args.steps, 3))
+        patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)     # warm-up
+        hostU.copy_(src)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+        tt = torch.tensor([sec], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        sec = float(tt.item())
+        nbytes = hostU.numel() * 8
+        e2e = {"value": world * zones * STAGES * e_steps / sec, "unit": "zone-stages/s", "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes + hostF.numel(), "steps": e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------------------
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak, hbm_src = (peaks["hbm_gbs"], "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
+    fp64_peak = binding.mhd_probe_fp64_flops(patch.stream()) / 1e12
+    total_kernel_ms = sum(v[0] for v in prof.values())
+    dom = max(prof, key=lambda k: prof[k][0])
+    dom_ms, dom_launches = prof[dom]
+    # algorithmic doubles moved per zone by each kernel class: reads + writes at the minimum
+    alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "rhs_ccz4": 22 + 10 + 5 + 32, "rhs_flux_x": 21 + 8 + 20,
+                   "rhs_flux_y": 21 + 8 + 20, "rhs_flux_z": 21 + 8 + 20, "rk_combine": 3.75 * 32}
+    per_launch_bytes = alg_doubles[dom] * 8.0 * zones
+    achieved = per_launch_bytes / (dom_ms / dom_launches * 1e-3) / 1e9 if dom_launches else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                "peak_source": hbm_src, "traffic": None, "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
+                "share_of_step": dom_ms / total_kernel_ms if total_kernel_ms else None,
+                "fp64_peak_tflops_measured": fp64_peak,
+                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+                # whole-step view: algorithmic 1.28 kB per zone-stage against the HBM peak
+                "step_alg_bytes_per_zone_stage": 1280, "step_hbm_frac": 1280.0 * value / world / 1e9 / hbm_peak}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, sec, zs = oracle_leg(args.workload, args.ref_n, 1)
+        cpu = {"value": v, "unit": "zone-stages/s", "cores": 1, "kind": "oracle",
+               "sample": "%d^3 instance of workload %s, 1 RK4 step (%.1f s), single thread" % (args.ref_n, args.workload, sec)}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": "zone-stages/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "%s_%d" % (args.workload, args.n), "grid": list(n), "ghosts": ng, "rk": "rk4", "eos_kind": cfg["params"]["eos_kind"],
+                   "l2": "inputs (32 fields x %.0f MB) far larger than L2; no flush needed" % (patch.npts * 8 / 1e6),
+                   "non_atmosphere_fraction": 1.0 - status["n_atmo"] / status["n_points"], "parallelism": "replicas" if world > 1 else "single"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(v[1] for v in prof.values())),
+        "roofline": roofline, "cpu_baseline": cpu, "flags": {k: v for k, v in status.items() if k != "n_points"},
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

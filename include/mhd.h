@@ -154,6 +154,14 @@ int mhd_advance_host(mhd_patch *p, const mhd_tableau *t, const int bc[6], double
 /* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */
 int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_stream);
 
+/* Per-kernel device timing (CUDA events recorded on the launching stream around every kernel of the library).
+ * mhd_patch_profile(p, 1) starts collecting, (p, 0) stops. mhd_patch_profile_read synchronises the stream, adds up
+ * the elapsed milliseconds and launch counts per kernel class since the last read, and resets them.
+ * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 (+sources), 3 flux x, 4 flux y, 5 flux z, 6 rk combine / copy. */
+#define MHD_NKERNELS 7
+int mhd_patch_profile(mhd_patch *p, int enable);
+int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void *cuda_stream);
+
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains on every SM), in FLOP/s;
  * used as the FP64 roofline denominator. Synchronises. Returns < 0 on error. */
 double mhd_probe_fp64_flops(void *cuda_stream);

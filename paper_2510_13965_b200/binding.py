@@ -51,7 +51,9 @@ class mhd_status(ctypes.Structure):
 
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
-           "mhd_probe_fp64_flops", "mhd_strerror"]
+           "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror"]
+NKERNELS = 7
+KERNEL_CLASSES = ["fill_ghosts", "con2prim", "rhs_ccz4", "rhs_flux_x", "rhs_flux_y", "rhs_flux_z", "rk_combine"]
 
 _lib = None
 
@@ -76,6 +78,8 @@ def lib():
         L.mhd_advance.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_advance_host.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p, _p, _p]
         L.mhd_patch_status.argtypes = [_p, _i, ctypes.POINTER(mhd_status), _p]
+        L.mhd_patch_profile.argtypes = [_p, _i]
+        L.mhd_patch_profile_read.argtypes = [_p, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_ulonglong), _p]
         L.mhd_probe_fp64_flops.argtypes = [_p]
         L.mhd_probe_fp64_flops.restype = _d
         L.mhd_strerror.argtypes = [_i]
@@ -185,6 +189,17 @@ def mhd_patch_status(h, slot_flags=SLOT_FLAGS, stream=None):
     return {n: getattr(st, n) for n, _ in mhd_status._fields_}
 
 
+def mhd_patch_profile(h, enable):
+    _check(lib().mhd_patch_profile(h, int(enable)))
+
+
+def mhd_patch_profile_read(h, stream=None):
+    ms = (_d * NKERNELS)()
+    n = (ctypes.c_ulonglong * NKERNELS)()
+    _check(lib().mhd_patch_profile_read(h, ms, n, stream))
+    return {k: (ms[i], int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+
 def mhd_probe_fp64_flops(stream=None):
     return lib().mhd_probe_fp64_flops(stream)
 
@@ -263,6 +278,13 @@ class Patch:
         """host_U: pinned CPU float64 tensor (NSTATE, MZ, MY, MX), updated in place; host_flags: uint8 tensor or None."""
         mhd_advance_host(self.h, tableau, bc, dt, n_steps, host_U.data_ptr(),
                          None if host_flags is None else host_flags.data_ptr(), self.stream())
+
+    def profile(self, enable):
+        mhd_patch_profile(self.h, enable)
+
+    def profile_read(self):
+        """{kernel class: (milliseconds, launches)} since the last read (CUDA events on the launching stream)"""
+        return mhd_patch_profile_read(self.h, self.stream())
 
     def status(self):
         return mhd_patch_status(self.h, SLOT_FLAGS, self.stream())

@@ -28,6 +28,23 @@ void finish_eos(Par& q) {
   }
 }
 
+// RAII event pair around one kernel launch when profiling is on
+struct Timed {
+  mhd_patch* p; cudaStream_t s; mhd_patch::Ev ev; bool on;
+  Timed(mhd_patch* p_, int cls, cudaStream_t s_) : p(p_), s(s_), on(p_->profiling) {
+    if (!on) return;
+    if (!p->pool.empty()) { ev = p->pool.back(); p->pool.pop_back(); }
+    else { cudaEventCreate(&ev.a); cudaEventCreate(&ev.b); }
+    ev.cls = cls;
+    cudaEventRecord(ev.a, s);
+  }
+  ~Timed() {
+    if (!on) return;
+    cudaEventRecord(ev.b, s);
+    p->events.push_back(ev);
+  }
+};
+
 int stage_sequence(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, cudaStream_t s) {
   int rc;
   for (int step = 0; step < n_steps; ++step) {
@@ -95,6 +112,8 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
 
 void mhd_patch_destroy(mhd_patch* p) {
   if (!p) return;
+  for (auto& e : p->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  for (auto& e : p->pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   if (p->d_counts) cudaFree(p->d_counts);
   delete p;
 }
@@ -112,12 +131,14 @@ int mhd_fill_ghosts(mhd_patch* p, int slot_state, const int bc[6], void* stream)
   for (int a = 0; a < 6; ++a) if (bc[a] != 0 && bc[a] != 1) return MHD_E_ARG;
   if (slot_state < 0 || slot_state >= MHD_NSLOTS || slot_state == MHD_SLOT_FLAGS) return MHD_E_ARG;
   if (!slot_ok(p, slot_state)) return MHD_E_UNBOUND;
+  Timed tm(p, 0, (cudaStream_t)stream);
   return launch_fill_ghosts(p->dims, dptr(p, slot_state), p->slot[slot_state].stride, slot_fields(slot_state), bc, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
 }
 
 int mhd_con2prim(mhd_patch* p, int slot_state, int slot_prim, int slot_flags, void* stream) {
   if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || slot_flags != MHD_SLOT_FLAGS) return MHD_E_ARG;
   if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_flags)) return MHD_E_UNBOUND;
+  Timed tm(p, 1, (cudaStream_t)stream);
   return launch_con2prim(p->dims, p->par, dptr(p, slot_state), p->slot[slot_state].stride, dptr(p, slot_prim), p->slot[slot_prim].stride,
                          (uint8_t*)p->slot[slot_flags].ptr, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
 }
@@ -137,8 +158,11 @@ int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* str
   const double* P = dptr(p, slot_prim);
   double* K = dptr(p, slot_rhs);
   const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
-  if (launch_rhs_ccz4(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
-  if (launch_rhs_flux(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
+  { Timed tm(p, 2, s); if (launch_rhs_ccz4(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
+  for (int dir = 0; dir < 3; ++dir) {
+    Timed tm(p, 3 + dir, s);
+    if (launch_rhs_flux(dir, p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
+  }
   return MHD_OK;
 }
 
@@ -146,6 +170,7 @@ int mhd_rk_stage(mhd_patch* p, const mhd_tableau* t, int stage, double dt, void*
   if (!p || !t || !t->a_expl || !t->w_expl || t->stages < 1 || t->stages > MHD_MAX_STAGES || stage < 0 || stage > t->stages) return MHD_E_ARG;
   if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_U0)) return MHD_E_UNBOUND;
   cudaStream_t s = (cudaStream_t)stream;
+  Timed tm(p, 6, s);
   if (stage == 0)
     return launch_copy_fields(p->dims, MHD_NSTATE, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
   const double* coef = stage < t->stages ? t->a_expl + (size_t)stage * t->stages : t->w_expl;
@@ -205,6 +230,26 @@ int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream
   out->n_points = (unsigned long long)p->dims.npts;
   out->n_atmo = h[0]; out->n_eps_lo = h[1]; out->n_eps_hi = h[2]; out->n_vmax = h[3];
   out->n_ye = h[4]; out->n_fatal = h[5]; out->n_noconv = h[6]; out->n_m1fix = h[7];
+  return MHD_OK;
+}
+
+int mhd_patch_profile(mhd_patch* p, int enable) {
+  if (!p) return MHD_E_ARG;
+  p->profiling = enable != 0;
+  return MHD_OK;
+}
+
+int mhd_patch_profile_read(mhd_patch* p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void* stream) {
+  if (!p || !ms || !launches) return MHD_E_ARG;
+  if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return MHD_E_CUDA;
+  for (int c = 0; c < MHD_NKERNELS; ++c) { ms[c] = 0.0; launches[c] = 0; }
+  for (auto& e : p->events) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, e.a, e.b) != cudaSuccess) return MHD_E_CUDA;
+    ms[e.cls] += t; launches[e.cls] += 1;
+    p->pool.push_back(e);
+  }
+  p->events.clear();
   return MHD_OK;
 }
 

@@ -204,10 +204,9 @@ cudaError_t launch_dir(const Dims& d, const Par& par, const double* U, size_t su
 
 }  // namespace
 
-cudaError_t launch_rhs_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  cudaError_t e;
-  if ((e = launch_dir<0, 64, 256>(d, par, U, su, P, sp, K, sk, s)) != cudaSuccess) return e;
-  if ((e = launch_dir<1, 16, 512>(d, par, U, su, P, sp, K, sk, s)) != cudaSuccess) return e;
+cudaError_t launch_rhs_flux(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
+  if (dir == 0) return launch_dir<0, 64, 256>(d, par, U, su, P, sp, K, sk, s);
+  if (dir == 1) return launch_dir<1, 16, 512>(d, par, U, su, P, sp, K, sk, s);
   return launch_dir<2, 16, 512>(d, par, U, su, P, sp, K, sk, s);
 }
 

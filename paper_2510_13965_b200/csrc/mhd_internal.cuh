@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <vector>
 #include "../../include/mhd.h"
 
 namespace mhd {
@@ -49,6 +50,11 @@ struct mhd_patch {
   mhd::Par par;
   mhd::Slot slot[MHD_NSLOTS];
   unsigned long long* d_counts;   // 8 counters for mhd_patch_status
+  // optional per-kernel timing (mhd_patch_profile)
+  bool profiling = false;
+  struct Ev { cudaEvent_t a, b; int cls; };
+  std::vector<Ev> events;         // recorded pairs since the last read
+  std::vector<Ev> pool;           // recycled events
 };
 
 namespace mhd {
@@ -57,7 +63,7 @@ cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfie
 cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, cudaStream_t s);
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
 cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
-cudaError_t launch_rhs_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_rhs_flux(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
 cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
                               int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s);
 cudaError_t launch_copy_fields(const Dims& d, int nfields, double* dst, size_t sd, const double* src, size_t ss, cudaStream_t s);
