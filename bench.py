@@ -241,8 +241,8 @@ def main():
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
     # algorithmic doubles moved per zone by each kernel class: reads + writes at the minimum
-    alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "rhs_ccz4": 22 + 10 + 5 + 32, "rhs_flux_x": 21 + 8 + 20,
-                   "rhs_flux_y": 21 + 8 + 20, "rhs_flux_z": 21 + 8 + 20, "rk_combine": 3.75 * 32}
+    alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "rhs_ccz4": 22 + 10 + 5 + 32, "rhs_flux_x": 21 + 20,
+                   "rhs_flux_y": 21 + 20, "rhs_flux_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33}
     per_launch_bytes = alg_doubles[dom] * 8.0 * zones
     achieved = per_launch_bytes / (dom_ms / dom_launches * 1e-3) / 1e9 if dom_launches else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,

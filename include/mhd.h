@@ -35,6 +35,7 @@ extern "C" {
 
 #define MHD_NSTATE 32
 #define MHD_NPRIM 10
+#define MHD_NWORK 33        /* 3 directions x (10 flux brackets of Eq. 32 + 1 speed bound of App. B) */
 #define MHD_MAX_STAGES 8
 #define MHD_MAX_PIECES 8
 
@@ -44,8 +45,9 @@ enum {
   MHD_SLOT_U0 = 1,     /* U^n, saved by mhd_rk_stage(stage = 0)          (MHD_NSTATE fields) */
   MHD_SLOT_P = 2,      /* primitives                                     (MHD_NPRIM fields)  */
   MHD_SLOT_FLAGS = 3,  /* uint8 flags, one field                                             */
-  MHD_SLOT_K1 = 4,     /* K_1 ... K_s = F(U^(j)): MHD_SLOT_K1 + j - 1    (MHD_NSTATE fields) */
-  MHD_NSLOTS = 4 + MHD_MAX_STAGES
+  MHD_SLOT_WORK = 4,   /* scratch of mhd_rhs: pointwise fluxes and speeds (MHD_NWORK fields) */
+  MHD_SLOT_K1 = 5,     /* K_1 ... K_s = F(U^(j)): MHD_SLOT_K1 + j - 1    (MHD_NSTATE fields) */
+  MHD_NSLOTS = 5 + MHD_MAX_STAGES
 };
 
 /* flag bits: error policy of PAPER.md:1157-1162 */
@@ -131,7 +133,9 @@ int mhd_prim2con(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream)
 
 /* a3-a8 — right-hand side F(U) on the interior: CCZ4 + gauge (Eqs. 13-26; FD Eqs. 60-62, upwind l.454-456,
  * KO l.460), GRMHD flux divergence (Eq. 32 with Eqs. 63-76, speeds App. B) and sources. Ghost points of
- * slot_rhs are not written. Needs filled ghosts in slot_state and primitives at all points. */
+ * slot_rhs are not written. Needs filled ghosts in slot_state and primitives at all points, and MHD_SLOT_WORK bound
+ * (overwritten: pointwise F^d(U,P) and speeds at every grid point, computed once and read by the three 1-D
+ * reconstruction passes). */
 int mhd_rhs(mhd_patch *p, int slot_state, int slot_prim, int slot_rhs, void *cuda_stream);
 
 /* a9 — explicit RK combine on the interior (Eq. 53).
@@ -157,8 +161,8 @@ int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_s
 /* Per-kernel device timing (CUDA events recorded on the launching stream around every kernel of the library).
  * mhd_patch_profile(p, 1) starts collecting, (p, 0) stops. mhd_patch_profile_read synchronises the stream, adds up
  * the elapsed milliseconds and launch counts per kernel class since the last read, and resets them.
- * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 (+sources), 3 flux x, 4 flux y, 5 flux z, 6 rk combine / copy. */
-#define MHD_NKERNELS 7
+ * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 (+sources), 3 reconstruction x, 4 y, 5 z, 6 rk combine / copy, 7 pointwise fluxes. */
+#define MHD_NKERNELS 8
 int mhd_patch_profile(mhd_patch *p, int enable);
 int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void *cuda_stream);
 

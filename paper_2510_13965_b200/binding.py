@@ -13,8 +13,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 
-NSTATE, NPRIM, MAX_STAGES, MAX_PIECES = 32, 10, 8, 8
-SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_K1 = 0, 1, 2, 3, 4
+NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
+SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p
@@ -52,8 +52,8 @@ class mhd_status(ctypes.Structure):
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror"]
-NKERNELS = 7
-KERNEL_CLASSES = ["fill_ghosts", "con2prim", "rhs_ccz4", "rhs_flux_x", "rhs_flux_y", "rhs_flux_z", "rk_combine"]
+NKERNELS = 8
+KERNEL_CLASSES = ["fill_ghosts", "con2prim", "rhs_ccz4", "rhs_flux_x", "rhs_flux_y", "rhs_flux_z", "rk_combine", "point_flux"]
 
 _lib = None
 
@@ -230,7 +230,8 @@ class Patch:
         self.U, self.U0, self.P = z(NSTATE), z(NSTATE), z(NPRIM)
         self.flags = z(1, torch.uint8)
         self.K = [z(NSTATE) for _ in range(stages)]
-        for slot, t in [(SLOT_U, self.U), (SLOT_U0, self.U0), (SLOT_P, self.P), (SLOT_FLAGS, self.flags)] + \
+        self.work = z(NWORK)
+        for slot, t in [(SLOT_U, self.U), (SLOT_U0, self.U0), (SLOT_P, self.P), (SLOT_FLAGS, self.flags), (SLOT_WORK, self.work)] + \
                        [(SLOT_K1 + j, k) for j, k in enumerate(self.K)]:
             mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
 

@@ -11,6 +11,7 @@ namespace {
 int slot_fields(int slot) {
   if (slot == MHD_SLOT_P) return MHD_NPRIM;
   if (slot == MHD_SLOT_FLAGS) return 1;
+  if (slot == MHD_SLOT_WORK) return MHD_NWORK;
   return MHD_NSTATE;
 }
 bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLOTS && p->slot[slot].ptr != nullptr; }
@@ -152,16 +153,19 @@ int mhd_prim2con(mhd_patch* p, int slot_state, int slot_prim, void* stream) {
 
 int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* stream) {
   if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || !is_state_slot(slot_rhs) || slot_rhs == slot_state) return MHD_E_ARG;
-  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_rhs)) return MHD_E_UNBOUND;
+  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_rhs) || !slot_ok(p, MHD_SLOT_WORK)) return MHD_E_UNBOUND;
   cudaStream_t s = (cudaStream_t)stream;
+  double* Wk = dptr(p, MHD_SLOT_WORK);
+  const size_t sw = p->slot[MHD_SLOT_WORK].stride;
   const double* U = dptr(p, slot_state);
   const double* P = dptr(p, slot_prim);
   double* K = dptr(p, slot_rhs);
   const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
   { Timed tm(p, 2, s); if (launch_rhs_ccz4(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
+  { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
   for (int dir = 0; dir < 3; ++dir) {
     Timed tm(p, 3 + dir, s);
-    if (launch_rhs_flux(dir, p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
+    if (launch_recon(dir, p->dims, p->par, U, su, Wk, sw, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
   }
   return MHD_OK;
 }

@@ -2,71 +2,108 @@
 // finite-difference HRSC scheme of Sec. III C: Lax-Friedrichs flux splitting (Eq. 65) with the speed bound of
 // App. B (Eqs. B1-B3, reading R12), MP5 reconstruction (Eqs. 67-76) and the flux sum (Eq. 69); Eq. (64).
 //
-// One kernel per direction, one thread per NODE of a line segment (interior nodes + 3 halo nodes per side):
-//   phase 1  every node evaluates its pointwise flux F^d(U,P) (10 fields), keeps its conserved state U and its
-//            speed bound s, and parks them in shared memory (computed once per node and direction);
-//   phase 2  every interface i+1/2 takes lambda = max s over its six stencil nodes, splits F+- = (F +- lambda U)/2,
-//            reconstructs F^L = MP5(F+ at i-2..i+2), F^R = MP5(F- at i+3..i-1) and sums them;
-//   phase 3  every interior node subtracts (F^_{i+1/2} - F^_{i-1/2}) / h from K (the sources were written by ccz4.cu).
-// Warps always run along x, so global loads/stores coalesce in all three directions; along y and z the line
-// neighbours sit 32 threads apart in shared memory (conflict-free, no shuffles needed).
+// Two steps:
+//   k_point_flux   every grid point (ghosts included) evaluates ONCE the flux brackets F^x, F^y, F^z of the 10 fluid
+//                  fields and the three speed bounds s^x, s^y, s^z (the inverse metric, covariant v and B, b^2 ...
+//                  are shared between the directions) and writes them to the 33-field work slot
+//                  (field 11 d + a: a = 0..9 flux of field a in direction d, a = 10 speed).
+//   k_recon<DIR>   streaming 1-D kernels: per interface lambda = max s over its six stencil nodes, F+- = F +- lambda U
+//                  (the factor 1/2 of Eq. 65 is applied after the reconstruction: R_MP5 is homogeneous of degree one
+//                  and scaling by 1/2 is exact), F^L = MP5(F+ at i-2..i+2), F^R = MP5(F- at i+3..i-1), Eq. (69),
+//                  and K -= (F^_{i+1/2} - F^_{i-1/2}) / h (the sources were written to K by ccz4.cu).
+//                  y and z: one thread marches along a segment of SEG zones with a 6-node register window per field,
+//                  warps run along x (coalesced), every node value is loaded once per segment.
+//                  x: one thread per interface, six L1-resident loads per array, the left neighbour's F^ comes by
+//                  warp shuffle.
+// MP5: the limiter of Eqs. (73)-(76) is needed only where the test of Eq. (72) fails; the branch is taken per warp
+// (__any_sync), so smooth regions run the 5-point formula of Eq. (70) alone. Sign / magnitude selections of
+// minmod are done on the integer pipe (bit patterns of non-negative doubles order like integers), which keeps
+// the FP64 pipe for arithmetic.
 #include "mhd_internal.cuh"
 
 namespace mhd {
 
 namespace {
 
-constexpr int NQ = 21;   // 10 fluxes + 10 conserved + 1 speed per node
+constexpr long long SIGN = (long long)0x8000000000000000ULL;
 
+__device__ __forceinline__ long long bits(double a) { return __double_as_longlong(a); }
+__device__ __forceinline__ double dbl(long long a) { return __longlong_as_double(a); }
+__device__ __forceinline__ double dmin(double a, double b) { return b < a ? b : a; }
+__device__ __forceinline__ double dmax(double a, double b) { return a < b ? b : a; }
+// max of two non-negative doubles on the integer pipe
+__device__ __forceinline__ double pmax(double a, double b) { return dbl(max(bits(a), bits(b))); }
+
+// minmod of two arguments: common sign x smallest magnitude, else 0 (R14)
 __device__ __forceinline__ double minmod2(double a, double b) {
-  const double m = fmin(fabs(a), fabs(b));
-  return (a > 0.0 && b > 0.0) ? m : ((a < 0.0 && b < 0.0) ? -m : 0.0);
+  const long long ia = bits(a), ib = bits(b);
+  const long long m = min(ia & ~SIGN, ib & ~SIGN);
+  return ((ia ^ ib) < 0) ? 0.0 : dbl(m | (ia & SIGN));
 }
 __device__ __forceinline__ double minmod4(double a, double b, double c, double d) {
-  const double m = fmin(fmin(fabs(a), fabs(b)), fmin(fabs(c), fabs(d)));
-  const bool pos = a > 0.0 && b > 0.0 && c > 0.0 && d > 0.0;
-  const bool neg = a < 0.0 && b < 0.0 && c < 0.0 && d < 0.0;
-  return pos ? m : (neg ? -m : 0.0);
-}
-// R_MP5(F_{i-2},...,F_{i+2}), Eqs. (70)-(76)
-__device__ __forceinline__ double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alpha) {
-  const double fhi = (2.0 * fm2 - 13.0 * fm1 + 47.0 * f0 + 27.0 * fp1 - 3.0 * fp2) * (1.0 / 60.0);
-  const double dmh = f0 - fm1, dph = fp1 - f0;
-  const double fmp = f0 + minmod2(dph, alpha * dmh);
-  if ((fhi - f0) * (fhi - fmp) < 0.0) return fhi;
-  const double dm1 = fm2 - 2.0 * fm1 + f0, d0 = fm1 - 2.0 * f0 + fp1, dp1 = f0 - 2.0 * fp1 + fp2;
-  const double d4p = minmod4(4.0 * d0 - dp1, 4.0 * dp1 - d0, d0, dp1);
-  const double d4m = minmod4(4.0 * dm1 - d0, 4.0 * d0 - dm1, dm1, d0);
-  const double ful = f0 + alpha * dmh;
-  const double fmd = 0.5 * (f0 + fp1) - 0.5 * d4p;
-  const double flc = f0 + 0.5 * dmh + (4.0 / 3.0) * d4m;
-  const double fmin_ = fmax(fmin(fmin(f0, fp1), fmd), fmin(fmin(f0, ful), flc));
-  const double fmax_ = fmin(fmax(fmax(f0, fp1), fmd), fmax(fmax(f0, ful), flc));
-  return fmin_ + minmod2(fhi - fmin_, fmax_ - fmin_);      // Median(fmin, fhi, fmax)
+  const long long ia = bits(a), ib = bits(b), ic = bits(c), id = bits(d);
+  const long long m = min(min(ia & ~SIGN, ib & ~SIGN), min(ic & ~SIGN, id & ~SIGN));
+  const bool neg = (ia & ib & ic & id) < 0, pos = (ia | ib | ic | id) >= 0;
+  return (neg || pos) ? dbl(m | (ia & SIGN)) : 0.0;
 }
 
-// pointwise flux brackets of Eq. (32) in direction DIR and the speed bound (App. B)
-template <int DIR>
-__device__ __forceinline__ void point_flux(const Par& par, const double* __restrict__ U, size_t su, const double* __restrict__ P, size_t sp,
-                                           size_t pt, double F[10], double uc[10], double& smax) {
+// R_MP5(F_{i-2},...,F_{i+2}), Eqs. (70)-(76)
+__device__ __forceinline__ double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alpha) {
+  const double fhi = (2.0 * fm2 - 13.0 * fm1 + 47.0 * f0 + 27.0 * fp1 - 3.0 * fp2) * (1.0 / 60.0);   // Eq. (70)
+  const double dmh = f0 - fm1, dph = fp1 - f0;
+  const double fmp = f0 + minmod2(dph, alpha * dmh);                                                 // Eq. (71)
+  const bool smooth = (fhi - f0) * (fhi - fmp) < 0.0;                                                // Eq. (72)
+  if (!__any_sync(__activemask(), !smooth)) return fhi;
+  const double dm1 = fm2 - 2.0 * fm1 + f0, d0 = fm1 - 2.0 * f0 + fp1, dp1 = f0 - 2.0 * fp1 + fp2;
+  const double d4p = minmod4(4.0 * d0 - dp1, 4.0 * dp1 - d0, d0, dp1);                               // Eq. (76)
+  const double d4m = minmod4(4.0 * dm1 - d0, 4.0 * d0 - dm1, dm1, d0);
+  const double ful = f0 + alpha * dmh;                                                               // Eq. (73)
+  const double fmd = 0.5 * (f0 + fp1) - 0.5 * d4p;                                                   // Eq. (74)
+  const double flc = f0 + 0.5 * dmh + (4.0 / 3.0) * d4m;                                             // Eq. (75)
+  const double lo = dmax(dmin(dmin(f0, fp1), fmd), dmin(dmin(f0, ful), flc));
+  const double hi = dmin(dmax(dmax(f0, fp1), fmd), dmax(dmax(f0, ful), flc));
+  const double med = lo + minmod2(fhi - lo, hi - lo);                                                // Median(lo, fhi, hi)
+  return smooth ? fhi : med;
+}
+
+// F^_{i+1/2} of one field from the six stencil nodes i-2..i+3 (index 0..5), Eqs. (65), (67)-(69)
+__device__ __forceinline__ double flux_hat(const double f[6], const double u[6], double lam, double alpha) {
+  double p[5], m[5];
+#pragma unroll
+  for (int n = 0; n < 5; ++n) { p[n] = fma(lam, u[n], f[n]); m[n] = fma(-lam, u[n + 1], f[n + 1]); }
+  return 0.5 * (mp5(p[0], p[1], p[2], p[3], p[4], alpha) + mp5(m[4], m[3], m[2], m[1], m[0], alpha));
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pointwise flux brackets of Eq. (32) in all three directions and the speed bounds of App. B (Eqs. B1-B3, R12)
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_point_flux(const __grid_constant__ Dims d, const __grid_constant__ Par par,
+                                                    const double* __restrict__ U, size_t su, const double* __restrict__ P, size_t sp,
+                                                    double* __restrict__ Wk, size_t sw) {
+  const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (pt >= d.npts) return;
   auto u = [&](int f) { return __ldg(U + (size_t)f * su + pt); };
   auto pr = [&](int f) { return __ldg(P + (size_t)f * sp + pt); };
   const double gxx = u(GXX), gxy = u(GXY), gxz = u(GXZ), gyy = u(GYY), gyz = u(GYZ), gzz = u(GZZ);
   const double chi = u(CHI), al = u(ALPHA);
   const double be[3] = {u(BETAX), u(BETAY), u(BETAZ)};
+  double uc[10];
 #pragma unroll
   for (int a = 0; a < 10; ++a) uc[a] = u(DBAR + a);
   const double rho = pr(RHO), eps = pr(EPS), p = pr(PRESS), W = pr(WLOR), cs2 = pr(CS2);
   const double v[3] = {pr(VX), pr(VY), pr(VZ)};
-  // row DIR of the inverse conformal metric (only gamma~^{DIR j} is needed)
   const double idet = 1.0 / (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz) + gxz * (gxy * gyz - gyy * gxz));
-  double gid[3];
-  if (DIR == 0) { gid[0] = (gyy * gzz - gyz * gyz) * idet; gid[1] = (gxz * gyz - gxy * gzz) * idet; gid[2] = (gxy * gyz - gxz * gyy) * idet; }
-  if (DIR == 1) { gid[0] = (gxz * gyz - gxy * gzz) * idet; gid[1] = (gxx * gzz - gxz * gxz) * idet; gid[2] = (gxy * gxz - gxx * gyz) * idet; }
-  if (DIR == 2) { gid[0] = (gxy * gyz - gxz * gyy) * idet; gid[1] = (gxy * gxz - gxx * gyz) * idet; gid[2] = (gxx * gyy - gxy * gxy) * idet; }
+  double gi[3][3];
+  gi[0][0] = (gyy * gzz - gyz * gyz) * idet;
+  gi[0][1] = gi[1][0] = (gxz * gyz - gxy * gzz) * idet;
+  gi[0][2] = gi[2][0] = (gxy * gyz - gxz * gyy) * idet;
+  gi[1][1] = (gxx * gzz - gxz * gxz) * idet;
+  gi[1][2] = gi[2][1] = (gxy * gxz - gxx * gyz) * idet;
+  gi[2][2] = (gxx * gyy - gxy * gxy) * idet;
   const double ichi = 1.0 / chi;
   const double isg = chi * sqrt(chi), sg = 1.0 / isg;   // 1/sqrt(gamma), sqrt(gamma)
-  // covariant velocity and magnetic field (physical metric gamma_ij = gamma~_ij / chi)
   const double Bu[3] = {uc[6] * isg, uc[7] * isg, uc[8] * isg};
   const double vl[3] = {ichi * (gxx * v[0] + gxy * v[1] + gxz * v[2]), ichi * (gxy * v[0] + gyy * v[1] + gyz * v[2]), ichi * (gxz * v[0] + gyz * v[1] + gzz * v[2])};
   const double Bl[3] = {ichi * (gxx * Bu[0] + gxy * Bu[1] + gxz * Bu[2]), ichi * (gxy * Bu[0] + gyy * Bu[1] + gyz * Bu[2]), ichi * (gxz * Bu[0] + gyz * Bu[1] + gzz * Bu[2])};
@@ -75,139 +112,152 @@ __device__ __forceinline__ void point_flux(const Par& par, const double* __restr
   const double Bv = Bu[0] * vl[0] + Bu[1] * vl[1] + Bu[2] * vl[2];
   const double iW2 = 1.0 / (W * W);
   const double Sl[3] = {uc[3] * isg, uc[4] * isg, uc[5] * isg};
-  // mixed stress S_i^DIR = gamma^{DIR j} S_ij with S_ij of l.260; gamma^{DIR j} gamma_ij = delta^DIR_i
-  const double vd = v[DIR];                                                     // gamma^{dj} v_j = v^d
-  const double Bd = Bu[DIR];
-  const double Sd = chi * (gid[0] * Sl[0] + gid[1] * Sl[1] + gid[2] * Sl[2]);   // S^d
-  const double ptot = p + 0.5 * (iW2 * B2 + Bv * Bv);                           // coefficient of gamma_ij in S_ij
-  const double vk = al * vd - be[DIR];
-  F[0] = vk * uc[0];
-  F[1] = vk * uc[1];
-  F[2] = -be[DIR] * uc[2] + al * (sg * Sd - uc[0] * vd);
-#pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    const double Sid = 0.5 * (vl[i] * Sd + vd * Sl[i]) + (i == DIR ? ptot : 0.0) - iW2 * Bl[i] * Bd - 0.5 * Bv * (Bl[i] * vd + Bd * vl[i]);
-    F[3 + i] = -be[DIR] * uc[3 + i] + al * sg * Sid;
-    F[6 + i] = uc[6 + i] * vk - uc[6 + DIR] * (al * v[i] - be[i]) + al * chi * gid[i] * uc[9];
-  }
-  F[9] = -be[DIR] * uc[9] + al * par.c_b * par.c_b * uc[6 + DIR];
-  // speed bound, Eqs. (B1)-(B3)
-  const double h = rho * (1.0 + eps) + p;
-  const double b2 = B2 * iW2 + Bv * Bv;
+  const double ptot = p + 0.5 * (iW2 * B2 + Bv * Bv);     // coefficient of gamma_ij in S_ij (l.260)
+  const double h = rho * (1.0 + eps) + p;                 // enthalpy density (l.232)
+  const double b2 = B2 * iW2 + Bv * Bv;                   // (B3)
   const double ca2 = b2 / (h + b2);
-  const double a2 = cs2 + ca2 - cs2 * ca2;
-  const double gdd = chi * gid[DIR];
-  const double disc = a2 * (1.0 - v2) * ((1.0 - v2 * a2) * gdd - (1.0 - a2) * vd * vd);
-  const double root = sqrt(fmax(disc, 0.0));
+  const double a2 = cs2 + ca2 - cs2 * ca2;                // (B2)
   const double pre = al / (1.0 - v2 * a2);
-  const double lp = -be[DIR] + pre * ((1.0 - a2) * vd + root);
-  const double lm = -be[DIR] + pre * ((1.0 - a2) * vd - root);
-  smax = fmax(fmax(fabs(lp), fabs(lm)), fabs(be[DIR]) + al * par.c_b * sqrt(gdd));
-}
-
-// NL nodes along the line per block; LS = distance in threads (and shared-memory slots) between line neighbours
-template <int DIR, int NL, int NT>
-__global__ void __launch_bounds__(NT) k_rhs_flux(const __grid_constant__ Dims d, const __grid_constant__ Par par,
-                                                const double* __restrict__ U, size_t su, const double* __restrict__ P, size_t sp,
-                                                double* __restrict__ K, size_t sk) {
-  extern __shared__ double sh[];           // [NQ][NT]
-  constexpr int TL = NL - 6;               // interior nodes per tile
-  constexpr int LS = DIR == 0 ? 1 : NT / NL;
-  const int tid = threadIdx.x;
-  const int lpos = DIR == 0 ? tid % NL : tid / LS;      // position along the line
-  const int lane = DIR == 0 ? tid / NL : tid % LS;      // which line of the block
-  int ijk[3];
-  bool valid;
-  if (DIR == 0) {
-    ijk[0] = d.ng - 3 + blockIdx.x * TL + lpos;
-    ijk[1] = d.ng + blockIdx.y * (NT / NL) + lane;
-    ijk[2] = d.ng + blockIdx.z;
-    valid = ijk[0] < d.mx - (d.ng - 3) && ijk[1] < d.ng + d.ny;
-  } else if (DIR == 1) {
-    ijk[0] = d.ng + blockIdx.x * LS + lane;
-    ijk[1] = d.ng - 3 + blockIdx.y * TL + lpos;
-    ijk[2] = d.ng + blockIdx.z;
-    valid = ijk[0] < d.ng + d.nx && ijk[1] < d.my - (d.ng - 3);
-  } else {
-    ijk[0] = d.ng + blockIdx.x * LS + lane;
-    ijk[1] = d.ng + blockIdx.y;
-    ijk[2] = d.ng - 3 + blockIdx.z * TL + lpos;
-    valid = ijk[0] < d.ng + d.nx && ijk[2] < d.mz - (d.ng - 3);
-  }
-  const size_t pt = (size_t)ijk[2] * d.sz + (size_t)ijk[1] * d.sy + ijk[0];
-  // ---- phase 1
-  if (valid) {
-    double F[10], uc[10], s;
-    point_flux<DIR>(par, U, su, P, sp, pt, F, uc, s);
+  const double cb2 = par.c_b * par.c_b;
 #pragma unroll
-    for (int a = 0; a < 10; ++a) { sh[a * NT + tid] = F[a]; sh[(10 + a) * NT + tid] = uc[a]; }
-    sh[20 * NT + tid] = s;
-  }
-  __syncthreads();
-  // ---- phase 2: interface between lpos and lpos+1
-  double Fh[10];
-  const bool has_if = lpos >= 2 && lpos <= NL - 4;
-  if (has_if) {
-    double lam = 0.0;
+  for (int dir = 0; dir < 3; ++dir) {
+    const double vd = v[dir], Bd = Bu[dir];
+    const double Sd = chi * (gi[dir][0] * Sl[0] + gi[dir][1] * Sl[1] + gi[dir][2] * Sl[2]);   // S^d
+    const double vk = al * vd - be[dir];
+    double* out = Wk + (size_t)(11 * dir) * sw + pt;
+    out[0] = vk * uc[0];
+    out[sw] = vk * uc[1];
+    out[2 * sw] = -be[dir] * uc[2] + al * (sg * Sd - uc[0] * vd);
 #pragma unroll
-    for (int m = -2; m <= 3; ++m) lam = fmax(lam, sh[20 * NT + tid + m * LS]);
-#pragma unroll
-    for (int a = 0; a < 10; ++a) {
-      double fp[6], fm[6];
-#pragma unroll
-      for (int m = 0; m < 6; ++m) {
-        const double f = sh[a * NT + tid + (m - 2) * LS], uu = sh[(10 + a) * NT + tid + (m - 2) * LS];
-        fp[m] = 0.5 * (f + lam * uu);                                            // Eq. (65)
-        fm[m] = 0.5 * (f - lam * uu);
-      }
-      Fh[a] = mp5(fp[0], fp[1], fp[2], fp[3], fp[4], par.mp5_alpha)              // Eq. (67)
-              + mp5(fm[5], fm[4], fm[3], fm[2], fm[1], par.mp5_alpha);           // Eqs. (68), (69)
+    for (int i = 0; i < 3; ++i) {
+      // mixed stress S_i^d = gamma^{dj} S_ij with S_ij of l.260 (gamma^{dj} gamma_ij = delta^d_i, gamma^{dj} v_j = v^d)
+      const double Sid = 0.5 * (vl[i] * Sd + vd * Sl[i]) + (i == dir ? ptot : 0.0) - iW2 * Bl[i] * Bd - 0.5 * Bv * (Bl[i] * vd + Bd * vl[i]);
+      out[(3 + i) * sw] = -be[dir] * uc[3 + i] + al * sg * Sid;
+      out[(6 + i) * sw] = uc[6 + i] * vk - uc[6 + dir] * (al * v[i] - be[i]) + al * chi * gi[dir][i] * uc[9];
     }
-  }
-  __syncthreads();
-  if (has_if) {
-#pragma unroll
-    for (int a = 0; a < 10; ++a) sh[a * NT + tid] = Fh[a];                        // F^_{lpos+1/2}
-  }
-  __syncthreads();
-  // ---- phase 3: interior nodes of this tile
-  const int gl = DIR == 0 ? ijk[0] : (DIR == 1 ? ijk[1] : ijk[2]);
-  const int nd = DIR == 0 ? d.nx : (DIR == 1 ? d.ny : d.nz);
-  if (valid && lpos >= 3 && lpos <= NL - 4 && gl < d.ng + nd) {
-    const double ih = 1.0 / (DIR == 0 ? d.dx : (DIR == 1 ? d.dy : d.dz));
-#pragma unroll
-    for (int a = 0; a < 10; ++a) {
-      double* kp = K + (size_t)(DBAR + a) * sk + pt;
-      *kp -= (sh[a * NT + tid] - sh[a * NT + tid - LS]) * ih;                      // Eq. (64)
-    }
+    out[9 * sw] = -be[dir] * uc[9] + al * cb2 * uc[6 + dir];
+    const double gdd = chi * gi[dir][dir];
+    const double disc = a2 * (1.0 - v2) * ((1.0 - v2 * a2) * gdd - (1.0 - a2) * vd * vd);
+    const double root = sqrt(fmax(disc, 0.0));
+    const double lp = -be[dir] + pre * ((1.0 - a2) * vd + root);                               // (B1)
+    const double lm = -be[dir] + pre * ((1.0 - a2) * vd - root);
+    out[10 * sw] = fmax(fmax(fabs(lp), fabs(lm)), fabs(be[dir]) + al * par.c_b * sqrt(gdd));
   }
 }
 
-template <int DIR, int NL, int NT>
-cudaError_t launch_dir(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  constexpr int TL = NL - 6;
-  constexpr size_t smem = (size_t)NQ * NT * sizeof(double);
-  auto kern = k_rhs_flux<DIR, NL, NT>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  dim3 grid;
-  if (DIR == 0) grid = dim3((d.nx + TL - 1) / TL, (d.ny + NT / NL - 1) / (NT / NL), d.nz);
-  if (DIR == 1) grid = dim3((d.nx + NT / NL - 1) / (NT / NL), (d.ny + TL - 1) / TL, d.nz);
-  if (DIR == 2) grid = dim3((d.nx + NT / NL - 1) / (NT / NL), d.ny, (d.nz + TL - 1) / TL);
-  kern<<<grid, NT, smem, s>>>(d, par, U, su, P, sp, K, sk);
+cudaError_t launch_point_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* Wk, size_t sw, cudaStream_t s) {
+  k_point_flux<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, Wk, sw);
   return cudaGetLastError();
+}
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------------
+// y / z: marching reconstruction. Thread = (x column, segment of SEG zones along the line). blockIdx.y = the third axis.
+// ---------------------------------------------------------------------------------------------------------------
+template <int DIR, int SEG>
+__global__ void __launch_bounds__(128) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
+                                                     const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.nx) return;
+  const int nline = DIR == 1 ? d.ny : d.nz;
+  const int mline = nline + 2 * d.ng;
+  const long long ls = DIR == 1 ? d.sy : d.sz;               // stride along the line
+  const int c0 = blockIdx.z * SEG;                           // first zone of the segment (interior index)
+  // base = node (c0 - 3) of the line, i.e. global line index c0 + ng - 3
+  const int other = blockIdx.y + d.ng;
+  const long long base = (DIR == 1 ? (long long)other * d.sz : (long long)other * d.sy) + (i + d.ng);
+  const int g0 = c0 + d.ng - 3;
+  auto node = [&](int n) { return base + (long long)min(g0 + n, mline - 1) * ls; };   // clamped: the ragged tail never reads past the field
+  // lambda of the SEG+1 interfaces: interface m lies between nodes m+2 and m+3 (relative to g0), stencil nodes m..m+5
+  double lam[SEG + 1];
+  {
+    const double* s = Wk + (size_t)(11 * DIR + 10) * sw;
+    double w[6];
+#pragma unroll
+    for (int n = 0; n < 5; ++n) w[n] = __ldg(s + node(n));
+#pragma unroll
+    for (int m = 0; m <= SEG; ++m) {
+      w[(m + 5) % 6] = __ldg(s + node(m + 5));
+      lam[m] = pmax(pmax(pmax(w[0], w[1]), pmax(w[2], w[3])), pmax(w[4], w[5]));
+    }
+  }
+  const double ih = 1.0 / (DIR == 1 ? d.dy : d.dz);
+#pragma unroll 1
+  for (int a = 0; a < 10; ++a) {
+    const double* f = Wk + (size_t)(11 * DIR + a) * sw;
+    const double* u = U + (size_t)(DBAR + a) * su;
+    double* k = K + (size_t)(DBAR + a) * sk;
+    double fw[6], uw[6];
+#pragma unroll
+    for (int n = 0; n < 5; ++n) { fw[n] = __ldg(f + node(n)); uw[n] = __ldg(u + node(n)); }
+    double prev = 0.0;
+#pragma unroll
+    for (int m = 0; m <= SEG; ++m) {
+      fw[5] = __ldg(f + node(m + 5)); uw[5] = __ldg(u + node(m + 5));
+      const double fh = flux_hat(fw, uw, lam[m], alpha);
+      if (m > 0 && c0 + m - 1 < nline) {
+        const long long pt = base + (long long)(g0 + m + 2) * ls;     // zone c0 + m - 1
+        k[pt] -= (fh - prev) * ih;                                     // Eq. (64)
+      }
+      prev = fh;
+#pragma unroll
+      for (int n = 0; n < 5; ++n) { fw[n] = fw[n + 1]; uw[n] = uw[n + 1]; }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// x: one thread per interface; a warp covers 32 interfaces = 31 zones (lane 31 only supplies F^ to lane 30).
+// ---------------------------------------------------------------------------------------------------------------
+template <int WARPS>
+__global__ void __launch_bounds__(32 * WARPS) k_recon_x(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
+                                                       const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int row = blockIdx.y * WARPS + warp;                 // j index (interior)
+  if (row >= d.ny) return;                                   // whole warp leaves
+  const int z0 = blockIdx.x * 31;                            // first zone of this warp
+  const int zone = z0 + lane;                                // lane l: interface zone-1/2 (left face of its zone)
+  // left face of zone: between nodes zone-1 and zone -> stencil nodes zone-3 .. zone+2 ; global x index = zone + ng - 3 + n
+  const long long base = (long long)(blockIdx.z + d.ng) * d.sz + (long long)(row + d.ng) * d.sy;
+  const int g0 = zone + d.ng - 3;
+  auto node = [&](int n) { return base + min(g0 + n, d.mx - 1); };
+  double lam;
+  {
+    const double* s = Wk + (size_t)10 * sw;
+    lam = pmax(pmax(pmax(__ldg(s + node(0)), __ldg(s + node(1))), pmax(__ldg(s + node(2)), __ldg(s + node(3)))), pmax(__ldg(s + node(4)), __ldg(s + node(5))));
+  }
+  const double ih = 1.0 / d.dx;
+  const bool store = lane < 31 && zone < d.nx;
+#pragma unroll 2
+  for (int a = 0; a < 10; ++a) {
+    const double* f = Wk + (size_t)a * sw;
+    const double* u = U + (size_t)(DBAR + a) * su;
+    double fw[6], uw[6];
+#pragma unroll
+    for (int n = 0; n < 6; ++n) { fw[n] = __ldg(f + node(n)); uw[n] = __ldg(u + node(n)); }
+    const double fl = flux_hat(fw, uw, lam, alpha);            // F^ at zone - 1/2
+    const double fr = __shfl_down_sync(0xffffffffu, fl, 1);    // F^ at zone + 1/2
+    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] -= (fr - fl) * ih;
+  }
 }
 
 }  // namespace
 
-cudaError_t launch_rhs_flux(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  if (dir == 0) return launch_dir<0, 64, 256>(d, par, U, su, P, sp, K, sk, s);
-  if (dir == 1) return launch_dir<1, 16, 512>(d, par, U, su, P, sp, K, sk, s);
-  return launch_dir<2, 16, 512>(d, par, U, su, P, sp, K, sk, s);
+cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
+  constexpr int SEG = 8;
+  if (dir == 0) {
+    constexpr int WARPS = 4;
+    dim3 grid((d.nx + 30) / 31, (d.ny + WARPS - 1) / WARPS, d.nz);
+    k_recon_x<WARPS><<<grid, 32 * WARPS, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  } else if (dir == 1) {
+    dim3 grid((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG);
+    k_recon_march<1, SEG><<<grid, 128, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  } else {
+    dim3 grid((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG);
+    k_recon_march<2, SEG><<<grid, 128, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  }
+  return cudaGetLastError();
 }
 
 }  // namespace mhd

@@ -63,7 +63,8 @@ cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfie
 cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, cudaStream_t s);
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
 cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
-cudaError_t launch_rhs_flux(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_point_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* Wk, size_t sw, cudaStream_t s);
+cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s);
 cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
                               int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s);
 cudaError_t launch_copy_fields(const Dims& d, int nfields, double* dst, size_t sd, const double* src, size_t ss, cudaStream_t s);
