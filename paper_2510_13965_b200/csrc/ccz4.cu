@@ -5,88 +5,144 @@
 // sides of Eq. 32, l.256). Output: K_f for the 22 spacetime fields, and the source part of the 10 fluid fields
 // (the flux kernels of flux.cu subtract the flux divergence afterwards).
 //
-// One thread per interior point, x-contiguous warps. All stencils are evaluated on differences (note N1 of
-// DESIGN.md): algebraically identical to the printed coefficients, exact zeros in flat space, no cancellation noise.
-// The algebra is staged (Christoffels -> Ricci -> lapse Hessian -> shift terms -> curvature terms -> outputs) so
-// that second derivatives are contracted as soon as they are formed and never all live at once.
+// Two kernels:
+//   k_ccz4_algebra  everything that needs the radius-2 centred derivatives (Eqs. 60-62). A CTA of 256 threads owns a
+//                   16x4x4 tile, one point per thread. The 16 fields that are differentiated are staged one at a time
+//                   through a 3-deep shared-memory ring of 20x8x8 tiles (tile + halo 2) filled with cp.async, so
+//                   every stencil operand is an LDS with a compile-time offset and the copy of field f+2 overlaps the
+//                   arithmetic on field f. Phase 1 turns each tile into derivatives, contracts second derivatives at
+//                   once (gamma~^mn d_m d_n gamma~_ab, gamma~^jk d_j d_k beta^c, d_j d_k beta^k) and parks the 72
+//                   surviving numbers per point in a per-thread shared-memory scratch column; phase 2 is the
+//                   pointwise algebra of Eqs. (13)-(26) and the sources of Eq. (32) reading that scratch. Registers
+//                   then hold only the working set of the phase, not 130 derivatives at once.
+//   k_adv_ko        beta^k d_k u with the one-sided stencils plus the KO term, radius 3, 1-D along each axis, added to
+//                   K for the 22 spacetime fields (and KO alone for the matter fields when sigma_ko_matter != 0).
+//                   A thread marches 8 zones along z with a 7-value register window; x / y neighbours come from L1.
+//
+// All stencils are evaluated on differences (note N1 of DESIGN.md): algebraically identical to the printed
+// coefficients, exact zeros in flat space, no cancellation noise.
 #include "mhd_internal.cuh"
 
 namespace mhd {
 
 namespace {
 
-__device__ __forceinline__ int sym(int i, int j) { return i <= j ? (i * (5 - i)) / 2 + j : (j * (5 - j)) / 2 + i; }   // (0,0)=0 (0,1)=1 (0,2)=2 (1,1)=3 (1,2)=4 (2,2)=5
+__device__ __forceinline__ constexpr int sym(int i, int j) { return i <= j ? (i * (5 - i)) / 2 + j : (j * (5 - j)) / 2 + i; }   // (0,0)=0 (0,1)=1 (0,2)=2 (1,1)=3 (1,2)=4 (2,2)=5
 
-struct Stencil {
-  long long s[3];      // strides
-  double i12h[3];      // 1/(12 h)
-  double i12h2[3];     // 1/(12 h^2)
-  double i64h[3];      // 1/(64 h)
+// ------------------------------------------------------------------------------------------------ tile geometry
+constexpr int TX = 16, TY = 4, TZ = 4, RH = 2;
+constexpr int SX = TX + 2 * RH, SY = TY + 2 * RH, SZ = TZ + 2 * RH;   // 20 x 8 x 8
+constexpr int TILE = SX * SY * SZ;                                    // 1280 doubles
+constexpr int NT = TX * TY * TZ;                                      // 256 threads
+constexpr int NLD = TILE / NT;                                        // 5 cp.async per thread and field
+static_assert(TILE % NT == 0, "tile must be a multiple of the CTA size");
+constexpr int NBUF = 3;
+constexpr int OX = 1, OY = SX, OZ = SX * SY;                          // shared-memory strides
+
+// scratch slots (per thread)
+enum {
+  S_DG = 0,       // 18: d_c gamma~_ab at S_DG + 6 c + ab
+  S_R = 18,       //  6: gamma~^mn d_m d_n gamma~_ab
+  S_DGH = 24,     //  9: d_a Gamma^^c at S_DGH + 3 a + c
+  S_DCHI = 33,    //  3
+  S_DDCHI = 36,   //  6
+  S_DAL = 42,     //  3
+  S_DDAL = 45,    //  6
+  S_DBE = 51,     //  9: d_a beta^c at S_DBE + 3 a + c
+  S_LAPB = 60,    //  3: gamma~^jk d_j d_k beta^c
+  S_DDIV = 63,    //  3: d_a d_k beta^k
+  S_DKH = 66,     //  3
+  S_DTH = 69,     //  3
+  NSCR = 72
 };
+constexpr size_t SMEM_BYTES = (size_t)(NBUF * TILE + NSCR * NT) * sizeof(double);
 
-__device__ __forceinline__ double ld(const double* p) { return __ldg(p); }
+__device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// Eq. (60)
-__device__ __forceinline__ double D1(const double* u, long long s, double i12h) {
-  return (8.0 * (ld(u + s) - ld(u - s)) - (ld(u + 2 * s) - ld(u - 2 * s))) * i12h;
+// unscaled Eq. (60): 12 h D u
+template <int O>
+__device__ __forceinline__ double d1u(const double* s) { return 8.0 * (s[O] - s[-O]) - (s[2 * O] - s[-2 * O]); }
+// unscaled Eq. (62): 12 h^2 D^2 u, on differences from the centre
+template <int O>
+__device__ __forceinline__ double d2u(const double* s, double u0) {
+  return 16.0 * ((s[O] - u0) + (s[-O] - u0)) - ((s[2 * O] - u0) + (s[-2 * O] - u0));
 }
-// Eq. (62)
-__device__ __forceinline__ double D2(const double* u, long long s, double i12h2) {
-  const double u0 = ld(u);
-  return (16.0 * ((ld(u + s) - u0) + (ld(u - s) - u0)) - ((ld(u + 2 * s) - u0) + (ld(u - 2 * s) - u0))) * i12h2;
+// unscaled Eq. (61): 144 h_a h_b D_b (D_a u)
+template <int OA, int OB>
+__device__ __forceinline__ double d11u(const double* s) {
+  return 8.0 * (d1u<OA>(s + OB) - d1u<OA>(s - OB)) - (d1u<OA>(s + 2 * OB) - d1u<OA>(s - 2 * OB));
 }
-// Eq. (61): D_b (D_a u)
-__device__ __forceinline__ double D11(const double* u, long long sa, double ia, long long sb, double ib) {
-  const double p1 = D1(u + sb, sa, ia), m1 = D1(u - sb, sa, ia), p2 = D1(u + 2 * sb, sa, ia), m2 = D1(u - 2 * sb, sa, ia);
-  return (8.0 * (p1 - m1) - (p2 - m2)) * ib;
+
+struct Scale { double i12h[3], i12h2[3], i144[3]; };   // i144: xy, xz, yz
+
+__device__ __forceinline__ void first(const double* s, const Scale& sc, double o[3]) {
+  o[0] = d1u<OX>(s) * sc.i12h[0]; o[1] = d1u<OY>(s) * sc.i12h[1]; o[2] = d1u<OZ>(s) * sc.i12h[2];
 }
-// beta^k D_k u with the one-sided stencils of l.454-456 (beta >= 0 takes the "beta > 0" branch) + KO of l.460, all 3 axes
-__device__ __forceinline__ double adv_ko(const double* u, const Stencil& st, const double be[3], double sigma) {
-  const double u0 = ld(u);
-  double acc = 0.0;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    const long long s = st.s[k];
-    const double m3 = ld(u - 3 * s) - u0, m2 = ld(u - 2 * s) - u0, m1 = ld(u - s) - u0;
-    const double p1 = ld(u + s) - u0, p2 = ld(u + 2 * s) - u0, p3 = ld(u + 3 * s) - u0;
-    const double up = (p3 - 6.0 * p2 + 18.0 * p1 - 3.0 * m1);       // beta > 0
-    const double dn = (-m3 + 6.0 * m2 - 18.0 * m1 + 3.0 * p1);      // beta < 0
-    acc += be[k] * ((be[k] < 0.0 ? dn : up) * st.i12h[k]);
-    acc += sigma * st.i64h[k] * ((m3 + p3) - 6.0 * (m2 + p2) + 15.0 * (m1 + p1));
-  }
-  return acc;
+// second derivatives in sym order xx, xy, xz, yy, yz, zz
+__device__ __forceinline__ void second(const double* s, const Scale& sc, double o[6]) {
+  const double u0 = s[0];
+  o[0] = d2u<OX>(s, u0) * sc.i12h2[0]; o[3] = d2u<OY>(s, u0) * sc.i12h2[1]; o[5] = d2u<OZ>(s, u0) * sc.i12h2[2];
+  o[1] = d11u<OX, OY>(s) * sc.i144[0]; o[2] = d11u<OX, OZ>(s) * sc.i144[1]; o[4] = d11u<OY, OZ>(s) * sc.i144[2];
 }
 
 }  // namespace
 
-__global__ void __launch_bounds__(256, 1)
-k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
-           const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i >= d.nx || j >= d.ny || k >= d.nz) return;
-  const size_t pt = (size_t)(k + d.ng) * d.sz + (size_t)(j + d.ng) * d.sy + (i + d.ng);
-  Stencil st;
-  st.s[0] = 1; st.s[1] = d.sy; st.s[2] = d.sz;
+// order in which the differentiated fields pass through the ring
+__device__ constexpr int FORDER[16] = {GXX, GXY, GXZ, GYY, GYZ, GZZ, GAMX, GAMY, GAMZ, CHI, ALPHA, BETAX, BETAY, BETAZ, KHAT, THETA};
+
+__global__ void __launch_bounds__(NT, 1)
+k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
+               const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk) {
+  extern __shared__ __align__(16) double smem[];
+  double* ring = smem;
+  const int tid = threadIdx.x;
+  double* scr = smem + NBUF * TILE + tid;
+#define SCR(slot) scr[(slot) * NT]
+  const int tx = tid % TX, ty = (tid / TX) % TY, tz = tid / (TX * TY);
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, k0 = blockIdx.z * TZ;
+  const int i = i0 + tx, j = j0 + ty, k = k0 + tz;
+  const bool inside = i < d.nx && j < d.ny && k < d.nz;
+  // centre point (clamped for the threads of a ragged tile: they take part in the copies and barriers only)
+  const size_t pt = (size_t)(min(k, d.nz - 1) + d.ng) * d.sz + (size_t)(min(j, d.ny - 1) + d.ng) * d.sy + (min(i, d.nx - 1) + d.ng);
+
+  // global offsets of the NLD tile elements this thread copies (clamped into the ghosted array)
+  int goff[NLD];
+#pragma unroll
+  for (int m = 0; m < NLD; ++m) {
+    const int e = tid + m * NT;
+    const int x = e % SX, y = (e / SX) % SY, z = e / (SX * SY);
+    const int gx = min(i0 + x - RH + d.ng, d.mx - 1), gy = min(j0 + y - RH + d.ng, d.my - 1), gz = min(k0 + z - RH + d.ng, d.mz - 1);
+    goff[m] = (int)(gz * d.sz + gy * d.sy + gx);
+  }
+  auto issue = [&](int f, int buf) {
+    const double* src = U + (size_t)f * su;
+    double* dst = ring + buf * TILE + tid;
+#pragma unroll
+    for (int m = 0; m < NLD; ++m) cp_async8(dst + m * NT, src + goff[m]);
+    cp_commit();
+  };
+  issue(FORDER[0], 0);
+  issue(FORDER[1], 1);
+
+  Scale sc;
   {
     const double h[3] = {d.dx, d.dy, d.dz};
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { st.i12h[a] = 1.0 / (12.0 * h[a]); st.i12h2[a] = 1.0 / (12.0 * h[a] * h[a]); st.i64h[a] = 1.0 / (64.0 * h[a]); }
+    for (int a = 0; a < 3; ++a) { sc.i12h[a] = 1.0 / (12.0 * h[a]); sc.i12h2[a] = 1.0 / (12.0 * h[a] * h[a]); }
+    sc.i144[0] = sc.i12h[0] * sc.i12h[1]; sc.i144[1] = sc.i12h[0] * sc.i12h[2]; sc.i144[2] = sc.i12h[1] * sc.i12h[2];
   }
-  auto F = [&](int f) { return U + (size_t)f * su + pt; };
-  auto d1 = [&](int f, int a) { return D1(F(f), st.s[a], st.i12h[a]); };
-  auto d2 = [&](int f, int a, int b) {
-    return a == b ? D2(F(f), st.s[a], st.i12h2[a]) : D11(F(f), st.s[a], st.i12h[a], st.s[b], st.i12h[b]);
-  };
-  auto OUT = [&](int f) -> double& { return K[(size_t)f * sk + pt]; };
+  auto F = [&](int f) { return __ldg(U + (size_t)f * su + pt); };
 
-  // ---- point values
+  // ---- point values of the conformal metric and its inverse (needed to contract second derivatives in phase 1)
   double g[6], gi[6];
 #pragma unroll
-  for (int a = 0; a < 6; ++a) g[a] = ld(F(GXX + a));
-  const double chi = ld(F(CHI)), al = ld(F(ALPHA));
-  const double be[3] = {ld(F(BETAX)), ld(F(BETAY)), ld(F(BETAZ))};
+  for (int a = 0; a < 6; ++a) g[a] = F(GXX + a);
   const double detg = g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]);
   {
     const double idet = 1.0 / detg;
@@ -97,25 +153,69 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
     gi[4] = (g[1] * g[2] - g[0] * g[4]) * idet;
     gi[5] = (g[0] * g[3] - g[1] * g[1]) * idet;
   }
-  const double ichi = 1.0 / chi;
 #define G_(i, j) g[sym(i, j)]
 #define GI(i, j) gi[sym(i, j)]
 
+  // ================================================================= phase 1: derivatives, field by field
+  const int ctr = ((tz + RH) * SY + (ty + RH)) * SX + (tx + RH);
+  double chi = 1.0, al = 1.0, be[3] = {0, 0, 0}, Gh[3] = {0, 0, 0}, Kh = 0.0, Th = 0.0;
+  double ddiv[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int n = 0; n < 16; ++n) {
+    if (n + 1 < 16) cp_wait<1>(); else cp_wait<0>();
+    __syncthreads();
+    if (n + 2 < 16) issue(FORDER[n + 2], (n + 2) % NBUF);
+    const double* s = ring + (n % NBUF) * TILE + ctr;
+    double d1[3];
+    first(s, sc, d1);
+    if (n < 6) {                       // gamma~_ab, ab = n
+      double dd[6];
+      second(s, sc, dd);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) SCR(S_DG + 6 * c + n) = d1[c];
+      SCR(S_R + n) = 0.5 * (gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5]) + (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
+    } else if (n < 9) {                // Gamma^^c, c = n - 6
+      Gh[n - 6] = s[0];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) SCR(S_DGH + 3 * a + (n - 6)) = d1[a];
+    } else if (n == 9 || n == 10) {    // chi, alpha
+      double dd[6];
+      second(s, sc, dd);
+      if (n == 9) chi = s[0]; else al = s[0];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) SCR((n == 9 ? S_DCHI : S_DAL) + a) = d1[a];
+#pragma unroll
+      for (int a = 0; a < 6; ++a) SCR((n == 9 ? S_DDCHI : S_DDAL) + a) = dd[a];
+    } else if (n < 14) {               // beta^c, c = n - 11
+      const int c = n - 11;
+      double dd[6];
+      second(s, sc, dd);
+      be[c] = s[0];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { SCR(S_DBE + 3 * a + c) = d1[a]; ddiv[a] += dd[sym(a, c)]; }
+      SCR(S_LAPB + c) = gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
+    } else {                           // K^, Theta
+      if (n == 14) Kh = s[0]; else Th = s[0];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) SCR((n == 14 ? S_DKH : S_DTH) + a) = d1[a];
+    }
+  }
+  if (!inside) return;
+  (void)be;
+
+  // ================================================================= phase 2: pointwise algebra
+  auto OUT = [&](int f) -> double& { return K[(size_t)f * sk + pt]; };
+  const double ichi = 1.0 / chi;
+
   // ---- Christoffels of the conformal metric: Gl[k][ij] = Gamma~_kij, Gu[k][ij] = Gamma~^k_ij
   double Gl[3][6], Gu[3][6], Gt[3];
-  {
-    double dg[3][6];   // dg[k][ij] = d_k gamma~_ij
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
+  for (int c = 0; c < 3; ++c)
 #pragma unroll
-      for (int a = 0; a < 6; ++a) dg[c][a] = d1(GXX + a, c);
+    for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = a; b < 3; ++b) Gl[c][sym(a, b)] = 0.5 * (dg[a][sym(c, b)] + dg[b][sym(c, a)] - dg[c][sym(a, b)]);
-  }
+      for (int b = a; b < 3; ++b)
+        Gl[c][sym(a, b)] = 0.5 * (SCR(S_DG + 6 * a + sym(c, b)) + SCR(S_DG + 6 * b + sym(c, a)) - SCR(S_DG + 6 * c + sym(a, b)));
 #pragma unroll
   for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -123,53 +223,41 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
 #pragma unroll
   for (int c = 0; c < 3; ++c)
     Gt[c] = gi[0] * Gu[c][0] + gi[3] * Gu[c][3] + gi[5] * Gu[c][5] + 2.0 * (gi[1] * Gu[c][1] + gi[2] * Gu[c][2] + gi[4] * Gu[c][4]);
-
-  const double Gh[3] = {ld(F(GAMX)), ld(F(GAMY)), ld(F(GAMZ))};
   double Z[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) Z[c] = 0.5 * chi * (Gh[c] - Gt[c]);          // l.132
 
   // ---- chi R^_ij  (Eq. 23 times chi), accumulated component by component
   double X[6];   // becomes alpha (chi R^_ij + chi R^chi_ij - 8 pi G chi S_ij) - chi D_i D_j alpha
-  {
-    double dGh[3][3];   // dGh[a][c] = d_a Gamma^^c
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
+  for (int a = 0; a < 3; ++a)
 #pragma unroll
-      for (int c = 0; c < 3; ++c) dGh[a][c] = d1(GAMX + c, a);
+    for (int b = a; b < 3; ++b) {
+      const int ab = sym(a, b);
+      double r = -SCR(S_R + ab);                                              // -1/2 gamma~^mn d_m d_n gamma~_ab
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-      for (int b = a; b < 3; ++b) {
-        const int ab = sym(a, b);
-        double r = 0.0;
-        // -1/2 gamma~^mn d_m d_n gamma~_ab
-        r -= 0.5 * (gi[0] * d2(GXX + ab, 0, 0) + gi[3] * d2(GXX + ab, 1, 1) + gi[5] * d2(GXX + ab, 2, 2));
-        r -= gi[1] * d2(GXX + ab, 0, 1) + gi[2] * d2(GXX + ab, 0, 2) + gi[4] * d2(GXX + ab, 1, 2);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          r += 0.5 * (G_(c, a) * dGh[b][c] + G_(c, b) * dGh[a][c]);           // gamma~_k(i d_j) Gamma^^k
-          r += 0.5 * Gh[c] * (Gl[a][sym(b, c)] + Gl[b][sym(a, c)]);           // Gamma^^k Gamma~_(ij)k
-        }
-#pragma unroll
-        for (int m = 0; m < 3; ++m)
-#pragma unroll
-          for (int n = 0; n < 3; ++n) {
-            double t = 0.0;
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-              t += Gu[c][sym(m, a)] * Gl[b][sym(c, n)] + Gu[c][sym(m, b)] * Gl[a][sym(c, n)] + Gu[c][sym(m, a)] * Gl[c][sym(n, b)];
-            r += GI(m, n) * t;
-          }
-        X[ab] = chi * r;
+      for (int c = 0; c < 3; ++c) {
+        r += 0.5 * (G_(c, a) * SCR(S_DGH + 3 * b + c) + G_(c, b) * SCR(S_DGH + 3 * a + c));   // gamma~_k(i d_j) Gamma^^k
+        r += 0.5 * Gh[c] * (Gl[a][sym(b, c)] + Gl[b][sym(a, c)]);                                // Gamma^^k Gamma~_(ij)k
       }
-  }
+#pragma unroll
+      for (int m = 0; m < 3; ++m)
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          double t = 0.0;
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+            t += Gu[c][sym(m, a)] * Gl[b][sym(c, n)] + Gu[c][sym(m, b)] * Gl[a][sym(c, n)] + Gu[c][sym(m, a)] * Gl[c][sym(n, b)];
+          r += GI(m, n) * t;
+        }
+      X[ab] = chi * r;
+    }
   double Rtr = 0.0;   // gamma^ij (R_ij + 2 D_(i Z_j)) = gamma~^ij (chi R^_ij + chi R^chi_ij)
 
-  // ---- chi R^chi_ij (Eq. 22), physical Hessian of the lapse (R25), matter (l.188-192, l.260)
+  // ---- chi R^chi_ij (Eq. 22), physical Hessian of the lapse (R25)
   double dchi[3], dal[3];
 #pragma unroll
-  for (int a = 0; a < 3; ++a) { dchi[a] = d1(CHI, a); dal[a] = d1(ALPHA, a); }
+  for (int a = 0; a < 3; ++a) { dchi[a] = SCR(S_DCHI + a); dal[a] = SCR(S_DAL + a); }
   double gdchi[3];   // gamma~^kl d_l chi
 #pragma unroll
   for (int c = 0; c < 3; ++c) gdchi[c] = GI(c, 0) * dchi[0] + GI(c, 1) * dchi[1] + GI(c, 2) * dchi[2];
@@ -177,9 +265,7 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
   {
     double ddchi[6], ddal[6];
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-      for (int b = a; b < 3; ++b) { ddchi[sym(a, b)] = d2(CHI, a, b); ddal[sym(a, b)] = d2(ALPHA, a, b); }
+    for (int a = 0; a < 6; ++a) { ddchi[a] = SCR(S_DDCHI + a); ddal[a] = SCR(S_DDAL + a); }
     double lapchi = 0.0, Ghdchi = 0.0, Zl[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
@@ -216,19 +302,19 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
         X[ab] = al * ric - chi * DDal;
       }
   }
-  // ---- matter
+  // ---- matter (l.188-192, l.260)
   const double G8 = 8.0 * 3.14159265358979323846 * par.grav_G;
   const double isg = chi * sqrt(chi);   // 1/sqrt(gamma)
   double uc[10];
 #pragma unroll
-  for (int a = 0; a < 10; ++a) uc[a] = ld(F(DBAR + a));
+  for (int a = 0; a < 10; ++a) uc[a] = F(DBAR + a);
   double Sij[6];   // undensitised S_ij, l.260
-  double E, Sl[3], vu[3];
+  double E, Sl[3];
   {
-    const double W = ld(P + (size_t)WLOR * sp + pt), pr = ld(P + (size_t)PRESS * sp + pt);
-    double vl[3], Bu[3], Bl[3];
+    const double W = __ldg(P + (size_t)WLOR * sp + pt), pr = __ldg(P + (size_t)PRESS * sp + pt);
+    double vu[3], vl[3], Bu[3], Bl[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { vu[a] = ld(P + (size_t)(VX + a) * sp + pt); Bu[a] = uc[6 + a] * isg; Sl[a] = uc[3 + a] * isg; }
+    for (int a = 0; a < 3; ++a) { vu[a] = __ldg(P + (size_t)(VX + a) * sp + pt); Bu[a] = uc[6 + a] * isg; Sl[a] = uc[3 + a] * isg; }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       vl[a] = ichi * (G_(a, 0) * vu[0] + G_(a, 1) * vu[1] + G_(a, 2) * vu[2]);
@@ -269,14 +355,13 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
 #pragma unroll
   for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) dbe[a][c] = d1(BETAX + c, a);
+    for (int c = 0; c < 3; ++c) dbe[a][c] = SCR(S_DBE + 3 * a + c);
   const double divb = dbe[0][0] + dbe[1][1] + dbe[2][2];
 
   // ---- curvature fields
   double A[6];
 #pragma unroll
-  for (int a = 0; a < 6; ++a) A[a] = ld(F(AXX + a));
-  const double Kh = ld(F(KHAT)), Th = ld(F(THETA));
+  for (int a = 0; a < 6; ++a) A[a] = F(AXX + a);
   const double Ktot = Kh + 2.0 * Th;
   double Aud[3][3];   // A~^a_b
 #pragma unroll
@@ -295,15 +380,14 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
 #pragma unroll
     for (int b = a; b < 3; ++b) Auu[sym(a, b)] = Aud[a][0] * GI(0, b) + Aud[a][1] * GI(1, b) + Aud[a][2] * GI(2, b);
 
-  const double sig = par.sigma_ko_spacetime;
   const double logdet = log(detg);
-  // ---- Eq. (13)
+  // ---- Eq. (13) without the advective / KO part (k_adv_ko adds it)
 #pragma unroll
   for (int a = 0; a < 3; ++a)
 #pragma unroll
     for (int b = a; b < 3; ++b) {
       const int ab = sym(a, b);
-      double s = adv_ko(F(GXX + ab), st, be, sig);
+      double s = 0.0;
 #pragma unroll
       for (int c = 0; c < 3; ++c) s += G_(a, c) * dbe[b][c] + G_(c, b) * dbe[a][c];
       s += -(2.0 / 3.0) * g[ab] * divb - 2.0 * al * (A[ab] - g[ab] * trA * (1.0 / 3.0)) - al * (1.0 / 3.0) * par.kappa_c * g[ab] * logdet;
@@ -315,8 +399,7 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
 #pragma unroll
     for (int b = a; b < 3; ++b) {
       const int ab = sym(a, b);
-      double s = adv_ko(F(AXX + ab), st, be, sig);
-      double AAab = 0.0;
+      double s = 0.0, AAab = 0.0;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         s += A[sym(a, c)] * dbe[b][c] + A[sym(c, b)] * dbe[a][c];
@@ -326,33 +409,20 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
       OUT(AXX + ab) = s;
     }
   // ---- Eq. (15)
-  OUT(CHI) = adv_ko(F(CHI), st, be, sig) + (2.0 / 3.0) * chi * (al * Ktot - divb);
+  OUT(CHI) = (2.0 / 3.0) * chi * (al * Ktot - divb);
   // ---- Eqs. (16), (17)
   const double Zdal = Z[0] * dal[0] + Z[1] * dal[1] + Z[2] * dal[2];
-  OUT(KHAT) = adv_ko(F(KHAT), st, be, sig) - lapal + al * (Ktot * Ktot * (1.0 / 3.0) + AA + 0.5 * G8 * (E + Str) + par.kappa_z * (1.0 - par.kappa_2) * Th) + 2.0 * Zdal;
-  OUT(THETA) = adv_ko(F(THETA), st, be, sig) + 0.5 * al * (Rtr + (2.0 / 3.0) * Kh * Kh + (2.0 / 3.0) * Th * (Kh - 2.0 * Th) - AA) - Zdal
+  OUT(KHAT) = -lapal + al * (Ktot * Ktot * (1.0 / 3.0) + AA + 0.5 * G8 * (E + Str) + par.kappa_z * (1.0 - par.kappa_2) * Th) + 2.0 * Zdal;
+  OUT(THETA) = 0.5 * al * (Rtr + (2.0 / 3.0) * Kh * Kh + (2.0 / 3.0) * Th * (Kh - 2.0 * Th) - AA) - Zdal
                - al * (G8 * E + par.kappa_z * (2.0 + par.kappa_2) * Th);
   // ---- Eqs. (18)-(20)
   {
-    double dKh[3], dTh[3];
+    double dKh[3], dTh[3], lapb[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { dKh[a] = d1(KHAT, a); dTh[a] = d1(THETA, a); }
-    // second derivatives of the shift, contracted at once: lapb[c] = gamma~^jk d_j d_k beta^c, ddiv[j] = d_j d_k beta^k
-    double lapb[3], ddiv[3] = {0.0, 0.0, 0.0};
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      double dd[6];
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = a; b < 3; ++b) dd[sym(a, b)] = d2(BETAX + c, a, b);
-      lapb[c] = gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
-#pragma unroll
-      for (int a = 0; a < 3; ++a) ddiv[a] += dd[sym(a, c)];
-    }
+    for (int a = 0; a < 3; ++a) { dKh[a] = SCR(S_DKH + a); dTh[a] = SCR(S_DTH + a); lapb[a] = SCR(S_LAPB + a); }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-      double s = adv_ko(F(GAMX + a), st, be, sig) + (2.0 / 3.0) * Gh[a] * divb + lapb[a];
+      double s = (2.0 / 3.0) * Gh[a] * divb + lapb[a];
       double b1 = 0.0, b2 = 0.0;
 #pragma unroll
       for (int b = 0; b < 3; ++b) {
@@ -367,9 +437,9 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
     }
   }
   // ---- gauge, Eqs. (25)-(26)
-  OUT(ALPHA) = adv_ko(F(ALPHA), st, be, sig) - 2.0 * al * par.f_alpha * Kh;
+  OUT(ALPHA) = -2.0 * al * par.f_alpha * Kh;
 #pragma unroll
-  for (int a = 0; a < 3; ++a) OUT(BETAX + a) = adv_ko(F(BETAX + a), st, be, sig) + 0.75 * par.f_beta * Gh[a] - par.eta_shift * (be[a] - par.beta0[a]);
+  for (int a = 0; a < 3; ++a) OUT(BETAX + a) = 0.75 * par.f_beta * Gh[a] - par.eta_shift * (be[a] - par.beta0[a]);
 
   // ---- sources of the GRMHD system (right-hand sides of Eq. 32); the flux divergence is subtracted by flux.cu
   {
@@ -421,20 +491,88 @@ k_rhs_ccz4(const __grid_constant__ Dims d, const __grid_constant__ Par par, cons
       OUT(BXBAR + a) = uc[9] * sb;
     }
     OUT(PHIBAR) = -al * cb2 * uc[9] * Ktot - al * par.kappa_b * uc[9] + cb2 * (uc[6] * dal[0] + uc[7] * dal[1] + uc[8] * dal[2]);
-    if (par.sigma_ko_matter != 0.0) {                                        // R16: optional KO on the matter fields
-      const double zero[3] = {0.0, 0.0, 0.0};
-#pragma unroll 1
-      for (int a = 0; a < 10; ++a) OUT(DBAR + a) += adv_ko(F(DBAR + a), st, zero, par.sigma_ko_matter);
-    }
   }
 #undef G_
 #undef GI
+#undef SCR
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// beta^k D_k u (one-sided 4th-order stencils of l.454-456; beta >= 0 takes the "beta > 0" branch, R15) + KO (l.460),
+// added to K. The beta < 0 stencil is the mirror image of the beta > 0 one, so the operands are selected by the sign
+// of beta (integer selects) and one 4-term combination is evaluated:  beta D u = |beta| (a3 - 6 a2 + 18 a1 - 3 b1)/(12h)
+// with (a, b) = (+, -) differences from the centre for beta >= 0 and (-, +) for beta < 0.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr int AZ = 8;   // zones marched along z per thread
+
+template <bool ADV>
+__device__ __forceinline__ double adv_ko_axis(double m3, double m2, double m1, double p1, double p2, double p3, double cb, double cko) {
+  double acc = cko * ((m3 + p3) - 6.0 * (m2 + p2) + 15.0 * (m1 + p1));
+  if (ADV) {
+    const bool up = cb >= 0.0;
+    const double a3 = up ? p3 : m3, a2 = up ? p2 : m2, a1 = up ? p1 : m1, b1 = up ? m1 : p1;
+    acc += fabs(cb) * (a3 - 6.0 * a2 + 18.0 * a1 - 3.0 * b1);
+  }
+  return acc;
+}
+
+template <bool ADV>
+__global__ void __launch_bounds__(256) k_adv_ko(const __grid_constant__ Dims d, double sigma, int f0, int nf,
+                                                const double* __restrict__ U, size_t su, double* __restrict__ K, size_t sk) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k0 = blockIdx.z * AZ;
+  if (i >= d.nx || j >= d.ny) return;
+  const int nzl = min(AZ, d.nz - k0);
+  const long long sy = d.sy, sz = d.sz;
+  const size_t base = (size_t)(k0 + d.ng) * sz + (size_t)(j + d.ng) * sy + (i + d.ng);
+  const double i12h[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
+  const double cko[3] = {sigma / (64.0 * d.dx), sigma / (64.0 * d.dy), sigma / (64.0 * d.dz)};
+  double cb[AZ][3];   // beta^a / (12 h_a) on the AZ planes
+#pragma unroll
+  for (int kk = 0; kk < AZ; ++kk)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) cb[kk][a] = (ADV && kk < nzl) ? __ldg(U + (size_t)(BETAX + a) * su + base + kk * sz) * i12h[a] : 0.0;
+#pragma unroll 1
+  for (int f = f0; f < f0 + nf; ++f) {
+    const double* u = U + (size_t)f * su + base;
+    double* ko = K + (size_t)f * sk + base;
+    double w[7];
+#pragma unroll
+    for (int n = 0; n < 6; ++n) w[n] = __ldg(u + (n - 3) * sz);
+#pragma unroll
+    for (int kk = 0; kk < AZ; ++kk) {
+      if (kk < nzl) {
+        const double* c = u + kk * sz;
+        w[6] = __ldg(c + 3 * sz);
+        const double u0 = w[3];
+        double acc = adv_ko_axis<ADV>(w[0] - u0, w[1] - u0, w[2] - u0, w[4] - u0, w[5] - u0, w[6] - u0, cb[kk][2], cko[2]);
+        acc += adv_ko_axis<ADV>(__ldg(c - 3) - u0, __ldg(c - 2) - u0, __ldg(c - 1) - u0, __ldg(c + 1) - u0, __ldg(c + 2) - u0, __ldg(c + 3) - u0, cb[kk][0], cko[0]);
+        acc += adv_ko_axis<ADV>(__ldg(c - 3 * sy) - u0, __ldg(c - 2 * sy) - u0, __ldg(c - sy) - u0, __ldg(c + sy) - u0, __ldg(c + 2 * sy) - u0,
+                                __ldg(c + 3 * sy) - u0, cb[kk][1], cko[1]);
+        ko[kk * sz] += acc;
+#pragma unroll
+        for (int n = 0; n < 6; ++n) w[n] = w[n + 1];
+      }
+    }
+  }
+}
+}  // namespace
+
 cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  dim3 block(32, 4, 2);
-  dim3 grid((d.nx + block.x - 1) / block.x, (d.ny + block.y - 1) / block.y, (d.nz + block.z - 1) / block.z);
-  k_rhs_ccz4<<<grid, block, 0, s>>>(d, par, U, su, P, sp, K, sk);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
+  k_ccz4_algebra<<<grid, NT, SMEM_BYTES, s>>>(d, par, U, su, P, sp, K, sk);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  dim3 ablock(32, 8), agrid((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + AZ - 1) / AZ);
+  k_adv_ko<true><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  if (par.sigma_ko_matter != 0.0)                                          // R16: optional KO on the matter fields
+    k_adv_ko<false><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
   return cudaGetLastError();
 }
 
