@@ -21,6 +21,7 @@
 //
 // All stencils are evaluated on differences (note N1 of DESIGN.md): algebraically identical to the printed
 // coefficients, exact zeros in flat space, no cancellation noise.
+#include <stdlib.h>
 #include "mhd_internal.cuh"
 
 namespace mhd {
@@ -498,60 +499,54 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// beta^k D_k u (one-sided 4th-order stencils of l.454-456; beta >= 0 takes the "beta > 0" branch, R15) + KO (l.460),
-// added to K. The beta < 0 stencil is the mirror image of the beta > 0 one, so the operands are selected by the sign
-// of beta (integer selects) and one 4-term combination is evaluated:  beta D u = |beta| (a3 - 6 a2 + 18 a1 - 3 b1)/(12h)
-// with (a, b) = (+, -) differences from the centre for beta >= 0 and (-, +) for beta < 0.
+// beta^k D_k u (one-sided 4th-order stencils of l.454-456) + KO (l.460), added to K.
+// With p_n = u_{i+n} - u_i, m_n = u_{i-n} - u_i the two one-sided stencils are
+//     12 h D^+ u = p3 - 6 p2 + 18 p1 - 3 m1 = (Q + A)/2,      12 h D^- u = -(m3 - 6 m2 + 18 m1 - 3 p1) = (A - Q)/2,
+//     Q = (p3 + m3) - 6 (p2 + m2) + 15 (p1 + m1)   (the KO combination itself),   A = (p3 - m3) - 6 (p2 - m2) + 21 (p1 - m1),
+// so  beta D^{sign beta} u + sigma Q / (64 h) = beta A / (24 h) + (|beta| / (24 h) + sigma / (64 h)) Q :
+// no branch on the sign of beta (R15: the two branches agree at beta = 0), one pass over the six differences.
 // ---------------------------------------------------------------------------------------------------------------
 namespace {
-constexpr int AZ = 8;   // zones marched along z per thread
 
 template <bool ADV>
-__device__ __forceinline__ double adv_ko_axis(double m3, double m2, double m1, double p1, double p2, double p3, double cb, double cko) {
-  double acc = cko * ((m3 + p3) - 6.0 * (m2 + p2) + 15.0 * (m1 + p1));
-  if (ADV) {
-    const bool up = cb >= 0.0;
-    const double a3 = up ? p3 : m3, a2 = up ? p2 : m2, a1 = up ? p1 : m1, b1 = up ? m1 : p1;
-    acc += fabs(cb) * (a3 - 6.0 * a2 + 18.0 * a1 - 3.0 * b1);
-  }
-  return acc;
+__device__ __forceinline__ double adv_ko_axis(double um3, double um2, double um1, double u0, double up1, double up2, double up3, double cbh, double cko) {
+  const double q = ((up3 - u0) + (um3 - u0)) - 6.0 * ((up2 - u0) + (um2 - u0)) + 15.0 * ((up1 - u0) + (um1 - u0));
+  if (!ADV) return cko * q;
+  const double a = (up3 - um3) - 6.0 * (up2 - um2) + 21.0 * (up1 - um1);
+  return fma(cko + fabs(cbh), q, cbh * a);
 }
 
-template <bool ADV>
-__global__ void __launch_bounds__(256) k_adv_ko(const __grid_constant__ Dims d, double sigma, int f0, int nf,
-                                                const double* __restrict__ U, size_t su, double* __restrict__ K, size_t sk) {
+template <bool ADV, int AZ, int MINB>
+__global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Dims d, double sigma, int f0, int nf,
+                                                      const double* __restrict__ U, size_t su, double* __restrict__ K, size_t sk) {
   const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k0 = blockIdx.z * AZ;
   if (i >= d.nx || j >= d.ny) return;
   const int nzl = min(AZ, d.nz - k0);
   const long long sy = d.sy, sz = d.sz;
   const size_t base = (size_t)(k0 + d.ng) * sz + (size_t)(j + d.ng) * sy + (i + d.ng);
-  const double i12h[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
+  const double i24h[3] = {1.0 / (24.0 * d.dx), 1.0 / (24.0 * d.dy), 1.0 / (24.0 * d.dz)};
   const double cko[3] = {sigma / (64.0 * d.dx), sigma / (64.0 * d.dy), sigma / (64.0 * d.dz)};
-  double cb[AZ][3];   // beta^a / (12 h_a) on the AZ planes
+  double cb[AZ][3];   // beta^a / (24 h_a) on the AZ planes
 #pragma unroll
   for (int kk = 0; kk < AZ; ++kk)
 #pragma unroll
-    for (int a = 0; a < 3; ++a) cb[kk][a] = (ADV && kk < nzl) ? __ldg(U + (size_t)(BETAX + a) * su + base + kk * sz) * i12h[a] : 0.0;
+    for (int a = 0; a < 3; ++a) cb[kk][a] = (ADV && kk < nzl) ? __ldg(U + (size_t)(BETAX + a) * su + base + kk * sz) * i24h[a] : 0.0;
 #pragma unroll 1
   for (int f = f0; f < f0 + nf; ++f) {
     const double* u = U + (size_t)f * su + base;
     double* ko = K + (size_t)f * sk + base;
-    double w[7];
+    double w[AZ + 6];   // the z column k0-3 .. k0+AZ+2 (clamped for a ragged last block: those planes are not used)
 #pragma unroll
-    for (int n = 0; n < 6; ++n) w[n] = __ldg(u + (n - 3) * sz);
+    for (int n = 0; n < AZ + 6; ++n) w[n] = __ldg(u + (long long)min(n - 3, nzl + 2) * sz);
 #pragma unroll
     for (int kk = 0; kk < AZ; ++kk) {
       if (kk < nzl) {
         const double* c = u + kk * sz;
-        w[6] = __ldg(c + 3 * sz);
-        const double u0 = w[3];
-        double acc = adv_ko_axis<ADV>(w[0] - u0, w[1] - u0, w[2] - u0, w[4] - u0, w[5] - u0, w[6] - u0, cb[kk][2], cko[2]);
-        acc += adv_ko_axis<ADV>(__ldg(c - 3) - u0, __ldg(c - 2) - u0, __ldg(c - 1) - u0, __ldg(c + 1) - u0, __ldg(c + 2) - u0, __ldg(c + 3) - u0, cb[kk][0], cko[0]);
-        acc += adv_ko_axis<ADV>(__ldg(c - 3 * sy) - u0, __ldg(c - 2 * sy) - u0, __ldg(c - sy) - u0, __ldg(c + sy) - u0, __ldg(c + 2 * sy) - u0,
-                                __ldg(c + 3 * sy) - u0, cb[kk][1], cko[1]);
+        const double u0 = w[kk + 3];
+        double acc = adv_ko_axis<ADV>(w[kk], w[kk + 1], w[kk + 2], u0, w[kk + 4], w[kk + 5], w[kk + 6], cb[kk][2], cko[2]);
+        acc += adv_ko_axis<ADV>(__ldg(c - 3), __ldg(c - 2), __ldg(c - 1), u0, __ldg(c + 1), __ldg(c + 2), __ldg(c + 3), cb[kk][0], cko[0]);
+        acc += adv_ko_axis<ADV>(__ldg(c - 3 * sy), __ldg(c - 2 * sy), __ldg(c - sy), u0, __ldg(c + sy), __ldg(c + 2 * sy), __ldg(c + 3 * sy), cb[kk][1], cko[1]);
         ko[kk * sz] += acc;
-#pragma unroll
-        for (int n = 0; n < 6; ++n) w[n] = w[n + 1];
       }
     }
   }
@@ -560,19 +555,25 @@ __global__ void __launch_bounds__(256) k_adv_ko(const __grid_constant__ Dims d, 
 
 cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
   static bool attr_set = false;
+  static int variant = 0;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
     if (e != cudaSuccess) return e;
+    if (const char* v = getenv("MHD_ADV_VARIANT")) variant = atoi(v);
     attr_set = true;
   }
   dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
   k_ccz4_algebra<<<grid, NT, SMEM_BYTES, s>>>(d, par, U, su, P, sp, K, sk);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  dim3 ablock(32, 8), agrid((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + AZ - 1) / AZ);
-  k_adv_ko<true><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  dim3 ablock(32, 8);
+  auto agrid = [&](int az) { return dim3((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + az - 1) / az); };
+  if (variant == 0) k_adv_ko<true, 4, 4><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  else if (variant == 1) k_adv_ko<true, 8, 2><<<agrid(8), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  else if (variant == 2) k_adv_ko<true, 4, 3><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  else k_adv_ko<true, 8, 3><<<agrid(8), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
   if (par.sigma_ko_matter != 0.0)                                          // R16: optional KO on the matter fields
-    k_adv_ko<false><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
+    k_adv_ko<false, 4, 4><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
   return cudaGetLastError();
 }
 
