@@ -34,14 +34,48 @@ def build(force=False):
     return _LIB
 
 
-_lib = None
+_LIB_COUNT = os.path.join(_HERE, "liboracle_count.so")
+
+
+def build_counting(force=False):
+    """Operation-counting build (orc_count.cpp: the same sources with `double` replaced by a counting wrapper)."""
+    deps = [os.path.join(_HERE, s) for s in _SOURCES + ["orc.hpp", "orc_count.cpp"]]
+    if not force and os.path.exists(_LIB_COUNT) and all(os.path.getmtime(_LIB_COUNT) >= os.path.getmtime(d) for d in deps):
+        return _LIB_COUNT
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_COUNT, os.path.join(_HERE, "orc_count.cpp")]
+    subprocess.run(cmd, check=True)
+    return _LIB_COUNT
+
+
+_libs = {}
+_counting = False
+
+
+def use_counting(flag):
+    """Route every call of this module through the operation-counting library (for the F_alg measurement)."""
+    global _counting
+    _counting = bool(flag)
+
+
+def count_reset():
+    _load(True).orc_count_reset()
+
+
+def count_get():
+    """dict of operation counts since the last reset: add (incl. sub), mul, div, sqrt, cmp (incl. min/max), trans"""
+    out = (ctypes.c_ulonglong * 6)()
+    _load(True).orc_count_get(out)
+    return dict(zip(("add", "mul", "div", "sqrt", "cmp", "trans"), [int(v) for v in out]))
 
 
 def lib():
-    global _lib
-    if _lib is None:
-        _lib = ctypes.CDLL(build())
-        L = _lib
+    return _load(_counting)
+
+
+def _load(counting):
+    if counting not in _libs:
+        _libs[counting] = ctypes.CDLL(build_counting() if counting else build())
+        L = _libs[counting]
         dp, vp, i32, f64 = ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_int, ctypes.c_double
         L.orc_new.restype = vp
         L.orc_free.argtypes = [vp]
@@ -53,7 +87,7 @@ def lib():
         L.orc_fill_ghosts.argtypes = [vp, vp, i32, vp]
         L.orc_con2prim.argtypes = [vp, vp, vp, vp]
         L.orc_prim2con.argtypes = [vp, vp, vp]
-        for name in ("orc_rhs", "orc_rhs_ccz4", "orc_rhs_grmhd"):
+        for name in ("orc_rhs", "orc_rhs_ccz4", "orc_rhs_grmhd", "orc_rhs_grmhd_flux", "orc_rhs_grmhd_src"):
             getattr(L, name).argtypes = [vp, vp, vp, vp]
         L.orc_rk_combine.argtypes = [vp, i32, vp, vp, i32, vp, vp, f64]
         L.orc_evolve.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, f64, i32]
@@ -74,7 +108,7 @@ def lib():
         L.orc_con2prim_point.argtypes = [vp, vp, f64, f64, vp, vp]
         L.orc_con2prim_point.restype = i32
         L.orc_prim2con_point.argtypes = [vp, vp, vp, vp]
-    return _lib
+    return _libs[counting]
 
 
 def _ptr(a):
@@ -139,7 +173,8 @@ class Oracle:
 
     def rhs(self, U, P, part="all"):
         K = np.zeros_like(U)
-        fn = {"all": "orc_rhs", "ccz4": "orc_rhs_ccz4", "grmhd": "orc_rhs_grmhd"}[part]
+        fn = {"all": "orc_rhs", "ccz4": "orc_rhs_ccz4", "grmhd": "orc_rhs_grmhd", "grmhd_flux": "orc_rhs_grmhd_flux",
+              "grmhd_src": "orc_rhs_grmhd_src"}[part]
         getattr(lib(), fn)(self.h, _ptr(U), _ptr(P), _ptr(K))
         return K
 

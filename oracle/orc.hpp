@@ -108,6 +108,7 @@ void prim2con(const Params& par, const Grid& g, double* U, double* P);   // dens
 void rhs(const Params& par, const Grid& g, const double* U, const double* P, double* K);
 void rhs_ccz4(const Params& par, const Grid& g, const double* U, const double* P, double* K);
 void rhs_grmhd(const Params& par, const Grid& g, const double* U, const double* P, double* K);
+void rhs_grmhd_parts(const Params& par, const Grid& g, const double* U, const double* P, double* K, int parts);
 void rk_combine(const Grid& g, int nfields, double* Uout, const double* U0, int nk,
                 const double* const* K, const double* coef, double dt);
 // n_steps full RK steps: per stage fill -> con2prim -> rhs -> combine (Eq. 53)

@@ -65,6 +65,8 @@ void orc_prim2con(void* hh, double* U, double* P) { Handle* h = (Handle*)hh; pri
 void orc_rhs(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs(h->par, h->grid, U, P, K); }
 void orc_rhs_ccz4(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_ccz4(h->par, h->grid, U, P, K); }
 void orc_rhs_grmhd(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_grmhd(h->par, h->grid, U, P, K); }
+void orc_rhs_grmhd_flux(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_grmhd_parts(h->par, h->grid, U, P, K, 1); }
+void orc_rhs_grmhd_src(void* hh, const double* U, const double* P, double* K) { Handle* h = (Handle*)hh; rhs_grmhd_parts(h->par, h->grid, U, P, K, 2); }
 void orc_rk_combine(void* hh, int nfields, double* Uout, const double* U0, int nk, const double* const* K, const double* coef, double dt) {
   rk_combine(((Handle*)hh)->grid, nfields, Uout, U0, nk, K, coef, dt);
 }
