@@ -47,13 +47,21 @@ __device__ __forceinline__ double minmod4(double a, double b, double c, double d
   return (neg || pos) ? dbl(m | (ia & SIGN)) : 0.0;
 }
 
-// R_MP5(F_{i-2},...,F_{i+2}), Eqs. (70)-(76)
-__device__ __forceinline__ double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alpha) {
+// Eq. (70) and the test of Eq. (72). The test is a shortcut (DESIGN.md note N4): whenever f^hi lies between F_i and
+// f^MP = F_i + minmod(dph, alpha dmh) the limiter of Eqs. (73)-(76) returns it unchanged. With t = f^hi - F_i that is
+// "t between 0 and dph, and between 0 and alpha dmh": two products, no minmod. The closed interval (<=) is used: at
+// its end points (t = 0: constant data, e.g. atmosphere; t = dph; t = alpha dmh) the limiter is still the identity.
+__device__ __forceinline__ double mp5_hi(double fm2, double fm1, double f0, double fp1, double fp2, double alpha, bool& need) {
   const double fhi = (2.0 * fm2 - 13.0 * fm1 + 47.0 * f0 + 27.0 * fp1 - 3.0 * fp2) * (1.0 / 60.0);   // Eq. (70)
-  const double dmh = f0 - fm1, dph = fp1 - f0;
-  const double fmp = f0 + minmod2(dph, alpha * dmh);                                                 // Eq. (71)
-  const bool smooth = (fhi - f0) * (fhi - fmp) < 0.0;                                                // Eq. (72)
-  if (!__any_sync(__activemask(), !smooth)) return fhi;
+  const double t = fhi - f0;
+  need = !((t * (t - (fp1 - f0)) <= 0.0) && (t * (t - alpha * (f0 - fm1)) <= 0.0));                  // Eqs. (71)-(72)
+  return fhi;
+}
+
+// Median(f^hi, f^min, f^max) - f^hi, Eqs. (73)-(76): the correction the limiter applies to Eq. (70)
+__device__ __forceinline__ double mp5_correction(double fm2, double fm1, double f0, double fp1, double fp2, double alpha) {
+  const double fhi = (2.0 * fm2 - 13.0 * fm1 + 47.0 * f0 + 27.0 * fp1 - 3.0 * fp2) * (1.0 / 60.0);
+  const double dmh = f0 - fm1;
   const double dm1 = fm2 - 2.0 * fm1 + f0, d0 = fm1 - 2.0 * f0 + fp1, dp1 = f0 - 2.0 * fp1 + fp2;
   const double d4p = minmod4(4.0 * d0 - dp1, 4.0 * dp1 - d0, d0, dp1);                               // Eq. (76)
   const double d4m = minmod4(4.0 * dm1 - d0, 4.0 * d0 - dm1, dm1, d0);
@@ -62,16 +70,68 @@ __device__ __forceinline__ double mp5(double fm2, double fm1, double f0, double 
   const double flc = f0 + 0.5 * dmh + (4.0 / 3.0) * d4m;                                             // Eq. (75)
   const double lo = dmax(dmin(dmin(f0, fp1), fmd), dmin(dmin(f0, ful), flc));
   const double hi = dmin(dmax(dmax(f0, fp1), fmd), dmax(dmax(f0, ful), flc));
-  const double med = lo + minmod2(fhi - lo, hi - lo);                                                // Median(lo, fhi, hi)
-  return smooth ? fhi : med;
+  return (lo - fhi) + minmod2(fhi - lo, hi - lo);                                                    // Median(lo, fhi, hi) - fhi
 }
 
-// F^_{i+1/2} of one field from the six stencil nodes i-2..i+3 (index 0..5), Eqs. (65), (67)-(69)
-__device__ __forceinline__ double flux_hat(const double f[6], const double u[6], double lam, double alpha) {
+// ---------------------------------------------------------------------------------------------------------------
+// Warp-divergence control for the limiter. Only a fraction of the reconstructions fail the test of Eq. (72)
+// (near extrema, discontinuities), but in a 32-wide warp almost every warp holds one, so a per-lane branch would
+// run the limiter for everybody. Instead each lane pushes the five stencil values of its failing reconstructions
+// on a per-warp stack in shared memory; whenever 32 are pending the warp pops them and evaluates the limiter
+// densely, one entry per lane, and posts the correction to the owner's slot. The owner adds it afterwards.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int QCAP = 96;                 // 32 pending + up to 64 pushed between two flushes
+constexpr unsigned FULL = 0xffffffffu;
+
+struct LimQueue {
+  double* v;       // [5][QCAP] stencil values F_{i-2}..F_{i+2} of the pending reconstructions
+  int* tag;        // [QCAP]    owner lane | slot << 5
+  double* corr;    // [NSLOT][32] corrections by slot and owner lane
+  int count;       // pending entries (warp-uniform)
+};
+
+__device__ __forceinline__ void q_push(LimQueue& q, bool need, double fm2, double fm1, double f0, double fp1, double fp2, int slot, int lane) {
+  const unsigned b = __ballot_sync(FULL, need);
+  if (need) {
+    const int pos = q.count + __popc(b & ((1u << lane) - 1u));
+    q.v[pos] = fm2; q.v[QCAP + pos] = fm1; q.v[2 * QCAP + pos] = f0; q.v[3 * QCAP + pos] = fp1; q.v[4 * QCAP + pos] = fp2;
+    q.tag[pos] = lane | (slot << 5);
+  }
+  q.count += __popc(b);
+}
+// evaluate entries [first, first + n), n <= 32, one per lane
+__device__ __noinline__ void q_process(const double* v, const int* tag, double* corr, int first, int n, int lane, double alpha) {
+  __syncwarp();
+  if (lane < n) {
+    const int e = first + lane;
+    const int tg = tag[e];
+    corr[(tg >> 5) * 32 + (tg & 31)] = mp5_correction(v[e], v[QCAP + e], v[2 * QCAP + e], v[3 * QCAP + e], v[4 * QCAP + e], alpha);
+  }
+  __syncwarp();
+}
+__device__ __forceinline__ void q_flush(LimQueue& q, int lane, double alpha) {
+  while (q.count >= 32) { q.count -= 32; q_process(q.v, q.tag, q.corr, q.count, 32, lane, alpha); }
+}
+__device__ __forceinline__ void q_drain(LimQueue& q, int lane, double alpha) {
+  q_flush(q, lane, alpha);
+  if (q.count > 0) { q_process(q.v, q.tag, q.corr, 0, q.count, lane, alpha); q.count = 0; }
+}
+
+// Eqs. (65), (67)-(69) for one interface and one field from the six stencil nodes i-2..i+3 (index 0..5): returns
+// f^hi_L + f^hi_R (twice the unlimited F^) and queues the reconstructions that need the limiter (slots 2s, 2s+1).
+__device__ __forceinline__ double flux_hat2(LimQueue& q, const double f[6], const double u[6], double lam, double alpha, bool active,
+                                            int s, int lane, unsigned& mask) {
   double p[5], m[5];
 #pragma unroll
   for (int n = 0; n < 5; ++n) { p[n] = fma(lam, u[n], f[n]); m[n] = fma(-lam, u[n + 1], f[n + 1]); }
-  return 0.5 * (mp5(p[0], p[1], p[2], p[3], p[4], alpha) + mp5(m[4], m[3], m[2], m[1], m[0], alpha));
+  bool nl, nr;
+  const double fl = mp5_hi(p[0], p[1], p[2], p[3], p[4], alpha, nl);
+  const double fr = mp5_hi(m[4], m[3], m[2], m[1], m[0], alpha, nr);
+  nl = nl && active; nr = nr && active;
+  q_push(q, nl, p[0], p[1], p[2], p[3], p[4], 2 * s, lane);
+  q_push(q, nr, m[4], m[3], m[2], m[1], m[0], 2 * s + 1, lane);
+  mask |= ((unsigned)nl << (2 * s)) | ((unsigned)nr << (2 * s + 1));
+  return fl + fr;
 }
 
 }  // namespace
@@ -154,12 +214,21 @@ namespace {
 
 // ---------------------------------------------------------------------------------------------------------------
 // y / z: marching reconstruction. Thread = (x column, segment of SEG zones along the line). blockIdx.y = the third axis.
+// All 32 lanes of a warp stay alive (the limiter queue is warp-cooperative): columns past nx are clamped and masked.
 // ---------------------------------------------------------------------------------------------------------------
+constexpr int RW = 4;    // warps per CTA of the reconstruction kernels
+
 template <int DIR, int SEG>
-__global__ void __launch_bounds__(128) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
-                                                     const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= d.nx) return;
+__global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
+                                                            const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+  __shared__ double q_v[RW][5 * QCAP];
+  __shared__ int q_tag[RW][QCAP];
+  __shared__ double q_corr[RW][2 * (SEG + 1) * 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  LimQueue q = {q_v[warp], q_tag[warp], q_corr[warp], 0};
+  const int ii = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = ii < d.nx;
+  const int i = min(ii, d.nx - 1);
   const int nline = DIR == 1 ? d.ny : d.nz;
   const int mline = nline + 2 * d.ng;
   const long long ls = DIR == 1 ? d.sy : d.sz;               // stride along the line
@@ -182,39 +251,49 @@ __global__ void __launch_bounds__(128) k_recon_march(const __grid_constant__ Dim
       lam[m] = pmax(pmax(pmax(w[0], w[1]), pmax(w[2], w[3])), pmax(w[4], w[5]));
     }
   }
-  const double ih = 1.0 / (DIR == 1 ? d.dy : d.dz);
+  const double hih = 0.5 / (DIR == 1 ? d.dy : d.dz);         // the 1/2 of Eq. (65) and 1/h of Eq. (64)
 #pragma unroll 1
   for (int a = 0; a < 10; ++a) {
     const double* f = Wk + (size_t)(11 * DIR + a) * sw;
     const double* u = U + (size_t)(DBAR + a) * su;
     double* k = K + (size_t)(DBAR + a) * sk;
-    double fw[6], uw[6];
+    // the whole column of the segment (SEG + 6 nodes) is loaded up front: the warp-synchronous limiter queue below
+    // fences code motion, so loads issued inside the interface loop would each expose a full memory latency
+    double fc[SEG + 6], uc[SEG + 6], acc[SEG + 1];
+    unsigned mask = 0;
 #pragma unroll
-    for (int n = 0; n < 5; ++n) { fw[n] = __ldg(f + node(n)); uw[n] = __ldg(u + node(n)); }
-    double prev = 0.0;
+    for (int n = 0; n < SEG + 6; ++n) { fc[n] = __ldg(f + node(n)); uc[n] = __ldg(u + node(n)); }
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
-      fw[5] = __ldg(f + node(m + 5)); uw[5] = __ldg(u + node(m + 5));
-      const double fh = flux_hat(fw, uw, lam[m], alpha);
-      if (m > 0 && c0 + m - 1 < nline) {
-        const long long pt = base + (long long)(g0 + m + 2) * ls;     // zone c0 + m - 1
-        k[pt] -= (fh - prev) * ih;                                     // Eq. (64)
-      }
-      prev = fh;
-#pragma unroll
-      for (int n = 0; n < 5; ++n) { fw[n] = fw[n + 1]; uw[n] = uw[n + 1]; }
+      acc[m] = flux_hat2(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
+      q_flush(q, lane, alpha);
     }
+    q_drain(q, lane, alpha);
+#pragma unroll
+    for (int m = 0; m <= SEG; ++m) {
+      if (mask & (1u << (2 * m))) acc[m] += q.corr[(2 * m) * 32 + lane];
+      if (mask & (1u << (2 * m + 1))) acc[m] += q.corr[(2 * m + 1) * 32 + lane];
+    }
+#pragma unroll
+    for (int m = 1; m <= SEG; ++m)
+      if (active && c0 + m - 1 < nline) {
+        const long long pt = base + (long long)(g0 + m + 2) * ls;       // zone c0 + m - 1
+        k[pt] -= (acc[m] - acc[m - 1]) * hih;                           // Eq. (64)
+      }
   }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // x: one thread per interface; a warp covers 32 interfaces = 31 zones (lane 31 only supplies F^ to lane 30).
 // ---------------------------------------------------------------------------------------------------------------
-template <int WARPS>
-__global__ void __launch_bounds__(32 * WARPS) k_recon_x(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
-                                                       const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+__global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
+                                                        const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+  __shared__ double q_v[RW][5 * QCAP];
+  __shared__ int q_tag[RW][QCAP];
+  __shared__ double q_corr[RW][20 * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int row = blockIdx.y * WARPS + warp;                 // j index (interior)
+  LimQueue q = {q_v[warp], q_tag[warp], q_corr[warp], 0};
+  const int row = blockIdx.y * RW + warp;                    // j index (interior)
   if (row >= d.ny) return;                                   // whole warp leaves
   const int z0 = blockIdx.x * 31;                            // first zone of this warp
   const int zone = z0 + lane;                                // lane l: interface zone-1/2 (left face of its zone)
@@ -222,23 +301,43 @@ __global__ void __launch_bounds__(32 * WARPS) k_recon_x(const __grid_constant__ 
   const long long base = (long long)(blockIdx.z + d.ng) * d.sz + (long long)(row + d.ng) * d.sy;
   const int g0 = zone + d.ng - 3;
   auto node = [&](int n) { return base + min(g0 + n, d.mx - 1); };
+  const bool active = zone <= d.nx;                          // interfaces 0 .. nx
   double lam;
   {
     const double* s = Wk + (size_t)10 * sw;
     lam = pmax(pmax(pmax(__ldg(s + node(0)), __ldg(s + node(1))), pmax(__ldg(s + node(2)), __ldg(s + node(3)))), pmax(__ldg(s + node(4)), __ldg(s + node(5))));
   }
-  const double ih = 1.0 / d.dx;
+  const double hih = 0.5 / d.dx;
   const bool store = lane < 31 && zone < d.nx;
-#pragma unroll 2
-  for (int a = 0; a < 10; ++a) {
-    const double* f = Wk + (size_t)a * sw;
-    const double* u = U + (size_t)(DBAR + a) * su;
-    double fw[6], uw[6];
+  double acc[10];
+  unsigned mask = 0;
+  double fw[6], uw[6];
 #pragma unroll
-    for (int n = 0; n < 6; ++n) { fw[n] = __ldg(f + node(n)); uw[n] = __ldg(u + node(n)); }
-    const double fl = flux_hat(fw, uw, lam, alpha);            // F^ at zone - 1/2
-    const double fr = __shfl_down_sync(0xffffffffu, fl, 1);    // F^ at zone + 1/2
-    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] -= (fr - fl) * ih;
+  for (int n = 0; n < 6; ++n) { fw[n] = __ldg(Wk + node(n)); uw[n] = __ldg(U + (size_t)DBAR * su + node(n)); }
+#pragma unroll
+  for (int a = 0; a < 10; ++a) {
+    double fn[6], un[6];                                      // next field's stencil, in flight during this field's arithmetic
+    if (a < 9) {
+      const double* f = Wk + (size_t)(a + 1) * sw;
+      const double* u = U + (size_t)(DBAR + a + 1) * su;
+#pragma unroll
+      for (int n = 0; n < 6; ++n) { fn[n] = __ldg(f + node(n)); un[n] = __ldg(u + node(n)); }
+    }
+    acc[a] = flux_hat2(q, fw, uw, lam, alpha, active, a, lane, mask);   // twice F^ at zone - 1/2
+    q_flush(q, lane, alpha);
+    if (a < 9) {
+#pragma unroll
+      for (int n = 0; n < 6; ++n) { fw[n] = fn[n]; uw[n] = un[n]; }
+    }
+  }
+  q_drain(q, lane, alpha);
+#pragma unroll
+  for (int a = 0; a < 10; ++a) {
+    double fl = acc[a];
+    if (mask & (1u << (2 * a))) fl += q.corr[(2 * a) * 32 + lane];
+    if (mask & (1u << (2 * a + 1))) fl += q.corr[(2 * a + 1) * 32 + lane];
+    const double fr = __shfl_down_sync(FULL, fl, 1);           // F^ at zone + 1/2
+    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] -= (fr - fl) * hih;
   }
 }
 
@@ -247,9 +346,8 @@ __global__ void __launch_bounds__(32 * WARPS) k_recon_x(const __grid_constant__ 
 cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
   constexpr int SEG = 8;
   if (dir == 0) {
-    constexpr int WARPS = 4;
-    dim3 grid((d.nx + 30) / 31, (d.ny + WARPS - 1) / WARPS, d.nz);
-    k_recon_x<WARPS><<<grid, 32 * WARPS, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+    dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
+    k_recon_x<<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
   } else if (dir == 1) {
     dim3 grid((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG);
     k_recon_march<1, SEG><<<grid, 128, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
