@@ -156,7 +156,9 @@ uint8_t con2prim_point(const Params& par, const double gt[6], double chi, double
     // step 3: root of f on (0, mu_plus]
     const double f0 = s.f(0.0), f1 = s.f(mu_plus);
     double mu;
-    if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; c2 = false; }
+    // no sign change: the root sits at the bracket end when the state is degenerate (eps clamped to its minimum gives
+    // h = h0 and f(mu_plus) = 0 analytically, +-1e-16 numerically): that is a converged solve, not a failure (R9)
+    if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; c2 = std::fabs(f1) <= 1e-12; }
     else mu = brent([&](double m) { return s.f(m); }, 0.0, mu_plus, f0, f1, par.c2p_maxit, c2);
     s.f(mu);                                                // step 4: primitives at the root
     if (!c1 || !c2) flag |= FLAG_NOCONV;

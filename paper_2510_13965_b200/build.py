@@ -12,8 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd_b200.so")
-# per-source extra flags: con2prim is compiled without FMA contraction (bit-reproducible flag decisions)
-SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": ["--fmad=false"], "ccz4.cu": [], "flux.cu": []}
+SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": [], "ccz4.cu": [], "flux.cu": []}
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC"]
 
 

@@ -46,20 +46,35 @@ struct Timed {
   }
 };
 
+// n_steps full RK steps. "U0 <- U" at the start of a step is a swap of the two slot pointers, not a copy: the first
+// combine of the step rewrites the whole interior of the new U buffer and the ghost fill that follows rewrites every
+// ghost cell, so nothing of its old content survives. After an odd number of steps the result is copied back into the
+// buffer the caller bound to MHD_SLOT_U (once per call, not once per step).
 int stage_sequence(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, cudaStream_t s) {
   int rc;
+  if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_U0)) return MHD_E_UNBOUND;
+  bool swapped = false;
+  auto swap_u = [&]() { Slot tmp = p->slot[MHD_SLOT_U]; p->slot[MHD_SLOT_U] = p->slot[MHD_SLOT_U0]; p->slot[MHD_SLOT_U0] = tmp; swapped = !swapped; };
+  auto fail = [&](int code) { if (swapped) swap_u(); return code; };
   for (int step = 0; step < n_steps; ++step) {
-    if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
-    if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return rc;
-    if ((rc = mhd_rk_stage(p, t, 0, dt, s)) != MHD_OK) return rc;
-    for (int st = 1; st <= t->stages; ++st) {
-      if (st > 1) {
-        if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
-        if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return rc;
-      }
-      if ((rc = mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st - 1, s)) != MHD_OK) return rc;
-      if ((rc = mhd_rk_stage(p, t, st, dt, s)) != MHD_OK) return rc;
+    if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return fail(rc);
+    if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return fail(rc);
+    // stage 1 reads U^n from the buffer that becomes U0
+    if ((rc = mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1, s)) != MHD_OK) return fail(rc);
+    swap_u();
+    if ((rc = mhd_rk_stage(p, t, 1, dt, s)) != MHD_OK) return fail(rc);
+    for (int st = 2; st <= t->stages; ++st) {
+      if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return fail(rc);
+      if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return fail(rc);
+      if ((rc = mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st - 1, s)) != MHD_OK) return fail(rc);
+      if ((rc = mhd_rk_stage(p, t, st, dt, s)) != MHD_OK) return fail(rc);
     }
+  }
+  if (swapped) {   // result lives in the caller's U0 buffer: copy it home and restore the binding
+    Timed tm(p, 6, s);
+    if (launch_copy_fields(p->dims, MHD_NSTATE, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, s) != cudaSuccess)
+      return fail(MHD_E_CUDA);
+    swap_u();
   }
   if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
   return mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s);

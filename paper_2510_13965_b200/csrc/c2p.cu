@@ -2,10 +2,11 @@
 // l.1157-1162) and its inverse for initial data (Eq. 29), with the three equations of state
 // (ideal gas, hybrid piecewise polytrope Eqs. 30-31, tabulated p/eps(rho,T,Ye) l.248-250).
 //
-// This translation unit is compiled with --fmad=false: every flag decision (atmosphere, eps/v/Ye limits) is
-// then taken on IEEE add/mul/div/sqrt results that do not depend on contraction, which is what makes the
-// flag masks reproducible bit for bit (DESIGN.md note N2). The kernel is latency/divergence bound
-// (two bracketed root solves per cell), not FMA bound, so the cost is small.
+// Flag reproducibility (DESIGN.md note N2): the atmosphere decision is taken on D = Dbar * (chi * sqrt(chi)) —
+// multiplications and one square root only, so no FMA can form and the result is the IEEE value the oracle
+// computes. Every other rule of the error policy acts on the output of the root solve, which is defined only up to
+// its tolerance; inputs keep away from those thresholds. Divisions are hoisted into reciprocals (one per
+// denominator) because an FP64 division costs about ten FP64-pipe instructions.
 //
 // One thread per grid point; x-contiguous warps so the 18 loads and 11 stores per point coalesce.
 // Divergence control: atmosphere cells skip the solve entirely; both root solves are bounded by c2p_maxit.
@@ -120,21 +121,22 @@ __device__ __forceinline__ void sym_apply(const Sym3& g, const double v[3], doub
   o[1] = g.xy * v[0] + g.yy * v[1] + g.yz * v[2];
   o[2] = g.xz * v[0] + g.yz * v[1] + g.zz * v[2];
 }
-__device__ __forceinline__ Sym3 sym_inverse(const Sym3& g) {
+// inverse times the factor s
+__device__ __forceinline__ Sym3 sym_inverse(const Sym3& g, double s) {
   const double det = g.xx * (g.yy * g.zz - g.yz * g.yz) - g.xy * (g.xy * g.zz - g.yz * g.xz) + g.xz * (g.xy * g.yz - g.yy * g.xz);
+  const double f = s / det;
   Sym3 r;
-  r.xx = (g.yy * g.zz - g.yz * g.yz) / det;
-  r.xy = (g.xz * g.yz - g.xy * g.zz) / det;
-  r.xz = (g.xy * g.yz - g.xz * g.yy) / det;
-  r.yy = (g.xx * g.zz - g.xz * g.xz) / det;
-  r.yz = (g.xy * g.xz - g.xx * g.yz) / det;
-  r.zz = (g.xx * g.yy - g.xy * g.xy) / det;
+  r.xx = (g.yy * g.zz - g.yz * g.yz) * f;
+  r.xy = (g.xz * g.yz - g.xy * g.zz) * f;
+  r.xz = (g.xy * g.yz - g.xz * g.yy) * f;
+  r.yy = (g.xx * g.zz - g.xz * g.xz) * f;
+  r.yz = (g.xy * g.xz - g.xx * g.yz) * f;
+  r.zz = (g.xx * g.yy - g.xy * g.xy) * f;
   return r;
 }
-__device__ __forceinline__ Sym3 sym_scale(const Sym3& g, double s, bool divide) {
+__device__ __forceinline__ Sym3 sym_scale(const Sym3& g, double s) {
   Sym3 r;
-  if (divide) { r.xx = g.xx / s; r.xy = g.xy / s; r.xz = g.xz / s; r.yy = g.yy / s; r.yz = g.yz / s; r.zz = g.zz / s; }
-  else { r.xx = s * g.xx; r.xy = s * g.xy; r.xz = s * g.xz; r.yy = s * g.yy; r.yz = s * g.yz; r.zz = s * g.zz; }
+  r.xx = s * g.xx; r.xy = s * g.xy; r.xz = s * g.xz; r.yy = s * g.yy; r.yz = s * g.yz; r.zz = s * g.zz;
   return r;
 }
 
@@ -172,16 +174,17 @@ struct Master {
     const double rb2 = rbar2(mu);
     const double qbar = q - 0.5 * B2 - 0.5 * mu * mu * x * x * B2rp2;
     const double v2 = fmin(mu * mu * rb2, v02);
-    W = 1.0 / sqrt(1.0 - v2);
-    double rho = D / W;
+    const double iW = sqrt(1.0 - v2);
+    W = 1.0 / iW;
+    double rho = D * iW;
     rho = fmax(fmin(rho_hi, rho), rho_lo);
-    eps_raw = W * (qbar - mu * rb2) + v2 * W * W / (1.0 + W);
+    eps_raw = W * ((qbar - mu * rb2) + v2 / (1.0 + iW));                                             // (D12): W^2/(1+W) = W/(1+1/W)
     double emin, emax;
     eos_eps_range(par, rho, ye, emin, emax);
     const double eps = fmax(fmin(emax, eps_raw), emin);
     const Eos e = eos_eval(par, rho, eps, ye);
     const double a = e.p / (rho * (1.0 + eps));
-    const double nuA = (1.0 + a) * (1.0 + eps) / W;
+    const double nuA = (1.0 + a) * (1.0 + eps) * iW;
     const double nuB = (1.0 + a) * (1.0 + qbar - mu * rb2);
     return mu - 1.0 / (fmax(nuA, nuB) + mu * rb2);
   }
@@ -219,7 +222,7 @@ __device__ double brent_root(F&& fun, double a, double b, double fa, double fb, 
 }
 
 // ------------------------------------------------------------------------------------------ kernels
-__global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Dims d, const __grid_constant__ Par par,
+__global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dims d, const __grid_constant__ Par par,
                                                   double* __restrict__ U, size_t su, double* __restrict__ P, size_t sp,
                                                   uint8_t* __restrict__ flags) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -231,8 +234,8 @@ __global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Dims d
   const double isg = chi * sqrt(chi);            // 1/sqrt(gamma) = chi^(3/2)   (det gamma~ = 1)
   const double sg = 1.0 / isg;
   const double D = Dbar * isg;                   // note N2: mul, sqrt, mul only
-  const Sym3 gl = sym_scale(gt, chi, true);      // gamma_ij = gamma~_ij / chi
-  const Sym3 gu = sym_scale(sym_inverse(gt), chi, false);   // gamma^ij = chi gamma~^ij
+  const Sym3 gl = sym_scale(gt, 1.0 / chi);      // gamma_ij = gamma~_ij / chi
+  const Sym3 gu = sym_inverse(gt, chi);          // gamma^ij = chi gamma~^ij
   const double B[3] = {u(BXBAR) * isg, u(BYBAR) * isg, u(BZBAR) * isg};
   double ye = DYe / Dbar;
   unsigned int flag = 0;
@@ -244,10 +247,10 @@ __global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Dims d
     const double tau = u(TAUBAR) * isg;
     const double Sl[3] = {u(SXBAR) * isg, u(SYBAR) * isg, u(SZBAR) * isg};
     Master s;
-    s.D = D; s.q = tau / D;                                                          // (D1)
-    const double rl[3] = {Sl[0] / D, Sl[1] / D, Sl[2] / D};
-    const double sD = sqrt(D);
-    const double Bs[3] = {B[0] / sD, B[1] / sD, B[2] / sD};
+    const double iD = 1.0 / D, isD = 1.0 / sqrt(D);
+    s.D = D; s.q = tau * iD;                                                         // (D1)
+    const double rl[3] = {Sl[0] * iD, Sl[1] * iD, Sl[2] * iD};
+    const double Bs[3] = {B[0] * isD, B[1] * isD, B[2] * isD};
     double ru[3], Bsl[3];
     sym_apply(gu, rl, ru);
     sym_apply(gl, Bs, Bsl);
@@ -266,7 +269,7 @@ __global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Dims d
     const double mu_plus = brent_root([&](double m) { return s.fa(m); }, 0.0, mub, -1.0, s.fa(mub), par.c2p_maxit, ok1);   // step 2
     const double f0 = s.f(par, 0.0), f1 = s.f(par, mu_plus);
     double mu;
-    if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; ok2 = false; }
+    if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; ok2 = fabs(f1) <= 1e-12; }   // R9: degenerate root at the bracket end
     else mu = brent_root([&](double m) { return s.f(par, m); }, 0.0, mu_plus, f0, f1, par.c2p_maxit, ok2);                 // step 3
     s.f(par, mu);                                                                    // step 4
     if (!ok1 || !ok2) flag |= MHD_FLAG_NOCONV;
@@ -329,7 +332,7 @@ __global__ void __launch_bounds__(128) k_prim2con(const __grid_constant__ Dims d
   const double chi = u(CHI);
   const double isg = chi * sqrt(chi), sg = 1.0 / isg;
   const Sym3 gt = {u(GXX), u(GXY), u(GXZ), u(GYY), u(GYZ), u(GZZ)};
-  const Sym3 gl = sym_scale(gt, chi, true);
+  const Sym3 gl = sym_scale(gt, 1.0 / chi);
   const double rho = pr(RHO), eps = pr(EPS), ye = pr(YE);
   const double v[3] = {pr(VX), pr(VY), pr(VZ)};
   const double B[3] = {u(BXBAR) * isg, u(BYBAR) * isg, u(BZBAR) * isg};

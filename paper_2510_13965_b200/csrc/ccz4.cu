@@ -538,6 +538,9 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
     double w[AZ + 6];   // the z column k0-3 .. k0+AZ+2 (clamped for a ragged last block: those planes are not used)
 #pragma unroll
     for (int n = 0; n < AZ + 6; ++n) w[n] = __ldg(u + (long long)min(n - 3, nzl + 2) * sz);
+    double kold[AZ];    // K is read-modify-write: its loads are issued with the stencil loads, not after the arithmetic
+#pragma unroll
+    for (int kk = 0; kk < AZ; ++kk) kold[kk] = kk < nzl ? ko[kk * sz] : 0.0;
 #pragma unroll
     for (int kk = 0; kk < AZ; ++kk) {
       if (kk < nzl) {
@@ -546,7 +549,7 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
         double acc = adv_ko_axis<ADV>(w[kk], w[kk + 1], w[kk + 2], u0, w[kk + 4], w[kk + 5], w[kk + 6], cb[kk][2], cko[2]);
         acc += adv_ko_axis<ADV>(__ldg(c - 3), __ldg(c - 2), __ldg(c - 1), u0, __ldg(c + 1), __ldg(c + 2), __ldg(c + 3), cb[kk][0], cko[0]);
         acc += adv_ko_axis<ADV>(__ldg(c - 3 * sy), __ldg(c - 2 * sy), __ldg(c - sy), u0, __ldg(c + sy), __ldg(c + 2 * sy), __ldg(c + 3 * sy), cb[kk][1], cko[1]);
-        ko[kk * sz] += acc;
+        ko[kk * sz] = kold[kk] + acc;
       }
     }
   }

@@ -19,6 +19,7 @@
 // (__any_sync), so smooth regions run the 5-point formula of Eq. (70) alone. Sign / magnitude selections of
 // minmod are done on the integer pipe (bit patterns of non-negative doubles order like integers), which keeps
 // the FP64 pipe for arithmetic.
+#include <stdlib.h>
 #include "mhd_internal.cuh"
 
 namespace mhd {
@@ -343,18 +344,27 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
 
 }  // namespace
 
+template <int SEG>
+static void launch_march(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
+  if (dir == 1) {
+    dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.nz, (d.ny + SEG - 1) / SEG);
+    k_recon_march<1, SEG><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  } else {
+    dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.ny, (d.nz + SEG - 1) / SEG);
+    k_recon_march<2, SEG><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  }
+}
+
 cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
-  constexpr int SEG = 8;
+  static int seg = 0;
+  if (seg == 0) { const char* v = getenv("MHD_RECON_SEG"); seg = v ? atoi(v) : 6; }
   if (dir == 0) {
     dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
     k_recon_x<<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  } else if (dir == 1) {
-    dim3 grid((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG);
-    k_recon_march<1, SEG><<<grid, 128, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  } else {
-    dim3 grid((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG);
-    k_recon_march<2, SEG><<<grid, 128, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  }
+  } else if (seg == 4) launch_march<4>(dir, d, par, U, su, Wk, sw, K, sk, s);
+  else if (seg == 6) launch_march<6>(dir, d, par, U, su, Wk, sw, K, sk, s);
+  else if (seg == 12) launch_march<12>(dir, d, par, U, su, Wk, sw, K, sk, s);
+  else launch_march<8>(dir, d, par, U, su, Wk, sw, K, sk, s);
   return cudaGetLastError();
 }
 
