@@ -161,8 +161,9 @@ int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_s
 /* Per-kernel device timing (CUDA events recorded on the launching stream around every kernel of the library).
  * mhd_patch_profile(p, 1) starts collecting, (p, 0) stops. mhd_patch_profile_read synchronises the stream, adds up
  * the elapsed milliseconds and launch counts per kernel class since the last read, and resets them.
- * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 (+sources), 3 reconstruction x, 4 y, 5 z, 6 rk combine / copy, 7 pointwise fluxes. */
-#define MHD_NKERNELS 8
+ * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 algebra (+ fluid sources), 3 reconstruction x, 4 y, 5 z, 6 rk combine / copy,
+ * 7 pointwise fluxes, 8 advection + Kreiss-Oliger. */
+#define MHD_NKERNELS 9
 int mhd_patch_profile(mhd_patch *p, int enable);
 int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void *cuda_stream);
 

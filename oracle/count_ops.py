@@ -1,6 +1,6 @@
 """ORACLE (test infrastructure) — algorithmic operation count of the hot path (F_alg of SURVEY.md 8(d)).
 
-    python -m oracle.count_ops            # writes oracle/op_counts.json
+    python -m oracle.count_ops            # writes tests/golden/op_counts.json
 
 Runs the operation-counting build of the oracle (orc_count.cpp: the same sources, `double` replaced by a counting
 wrapper; no FMA can form) on a 16^3 instance of each workload and records, per interior zone and per step of the path,
@@ -65,7 +65,7 @@ def count(cfg):
 
 def main():
     res = {"c1": count(synth.config1(n=16))}
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "op_counts.json")
+    path = os.path.join(ROOT, "tests", "golden", "op_counts.json")
     with open(path, "w") as f:
         json.dump(res, f, indent=1, sort_keys=True)
     for k, v in res.items():

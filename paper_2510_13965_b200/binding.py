@@ -52,8 +52,8 @@ class mhd_status(ctypes.Structure):
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror"]
-NKERNELS = 8
-KERNEL_CLASSES = ["fill_ghosts", "con2prim", "rhs_ccz4", "rhs_flux_x", "rhs_flux_y", "rhs_flux_z", "rk_combine", "point_flux"]
+NKERNELS = 9
+KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko"]
 
 _lib = None
 

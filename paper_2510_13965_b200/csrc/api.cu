@@ -176,7 +176,8 @@ int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* str
   const double* P = dptr(p, slot_prim);
   double* K = dptr(p, slot_rhs);
   const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
-  { Timed tm(p, 2, s); if (launch_rhs_ccz4(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
+  { Timed tm(p, 2, s); if (launch_ccz4_algebra(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
+  { Timed tm(p, 8, s); if (launch_adv_ko(p->dims, p->par, U, su, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
   { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
   for (int dir = 0; dir < 3; ++dir) {
     Timed tm(p, 3 + dir, s);

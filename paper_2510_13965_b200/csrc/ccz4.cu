@@ -556,27 +556,24 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
 }
 }  // namespace
 
-cudaError_t launch_rhs_ccz4(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
+cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
   static bool attr_set = false;
-  static int variant = 0;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    if (const char* v = getenv("MHD_ADV_VARIANT")) variant = atoi(v);
     attr_set = true;
   }
   dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
   k_ccz4_algebra<<<grid, NT, SMEM_BYTES, s>>>(d, par, U, su, P, sp, K, sk);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  dim3 ablock(32, 8);
-  auto agrid = [&](int az) { return dim3((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + az - 1) / az); };
-  if (variant == 0) k_adv_ko<true, 4, 4><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
-  else if (variant == 1) k_adv_ko<true, 8, 2><<<agrid(8), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
-  else if (variant == 2) k_adv_ko<true, 4, 3><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
-  else k_adv_ko<true, 8, 3><<<agrid(8), ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, cudaStream_t s) {
+  constexpr int AZ = 4;
+  dim3 ablock(32, 8), agrid((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + AZ - 1) / AZ);
+  k_adv_ko<true, AZ, 3><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
   if (par.sigma_ko_matter != 0.0)                                          // R16: optional KO on the matter fields
-    k_adv_ko<false, 4, 4><<<agrid(4), ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
+    k_adv_ko<false, AZ, 4><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
   return cudaGetLastError();
 }
 

@@ -226,3 +226,201 @@ def config1(n=32, dx=0.1, seed=SEED_BASE + 1, gauge_perturbation=False, ng=NG):
     for i in range(3):
         P[VX + i] = v[i]
     return dict(U=U, P=P, n=(n, n, n), ng=ng, dx=dx, bc=[0] * 6, params=default_params())
+
+
+# ---- flat-space helpers -------------------------------------------------------------------------------
+def _flat_state(shape):
+    """22 spacetime fields of Minkowski space in the conformal variables: gamma~ = delta, chi = 1, alpha = 1, rest 0."""
+    U = np.zeros((NSTATE,) + shape)
+    U[GXX + 0] = U[GXX + 3] = U[GXX + 5] = 1.0
+    U[CHI] = 1.0
+    U[ALPHA] = 1.0
+    return U
+
+
+# ---- config 2: smooth convergence series (BASELINE.json configs[1]) ---------------------------------------
+def config2_gauge_wave(n=32, amplitude=1e-6, t=0.0, ng=NG, ny=None):
+    """Linearised gauge wave, 1-D in 3-D along x on the unit box: alpha = 1 + A sin k(x - sqrt2 t),
+    K = (sqrt2/2) A k cos k(x - sqrt2 t), flat metric, zero shift (f_beta = eta = 0), vacuum-like fluid (atmosphere,
+    grav_G = 0). Solves the linearised Eqs. (16), (25) (1+log slicing: speed sqrt 2); error floor O(A^2).
+    Returns the same dict as config1 plus `exact(t)` -> (alpha, Khat) arrays."""
+    L = 1.0
+    dx = L / n
+    ny = n if ny is None else ny                 # ny < n: thin slab for the (cheap) 1-D convergence pins
+    X, Y, Z = mesh(n, ny, ny, ng, dx)
+    k = 2.0 * math.pi / L
+
+    def exact(tt):
+        ph = k * (X - math.sqrt(2.0) * tt)
+        return 1.0 + amplitude * np.sin(ph), 0.5 * math.sqrt(2.0) * amplitude * k * np.cos(ph)
+
+    U = _flat_state(X.shape)
+    U[ALPHA], U[KHAT] = exact(t)
+    P = np.zeros((NPRIM,) + X.shape)
+    par = default_params(f_beta=0.0, eta_shift=0.0, kappa_z=0.0, kappa_c=0.0, grav_G=0.0)
+    P[RHO], P[YE], P[EPS] = par["rho_atmo"], par["ye_atmo"], par["eps_atmo"]
+    return dict(U=U, P=P, n=(n, ny, ny), ng=ng, dx=dx, bc=[0] * 6, params=par, exact=exact, L=L)
+
+
+def config2_alfven(n=32, t=0.0, ng=NG, rho=1.0, p=1.0, B0=1.0, eta=1.0, gamma=5.0 / 3.0, ny=None):
+    """Circularly polarised Alfven wave of arbitrary amplitude (an exact SRMHD solution; ref. [99] of the paper),
+    1-D in 3-D along x on the unit box, flat spacetime with grav_G = 0 so that the metric stays exactly flat.
+    B^x = B0, B^y = eta B0 cos k(x - vA t), B^z = eta B0 sin k(x - vA t), v^x = 0, v^{y,z} = -vA B^{y,z} / B0."""
+    L = 1.0
+    dx = L / n
+    ny = n if ny is None else ny                 # ny < n: thin slab for the (cheap) 1-D convergence pins
+    X, Y, Z = mesh(n, ny, ny, ng, dx)
+    k = 2.0 * math.pi / L
+    eps = p / ((gamma - 1.0) * rho)
+    rhoh = rho * (1.0 + eps) + p
+    den = rhoh + B0 * B0 * (1.0 + eta * eta)
+    vA = math.sqrt(B0 * B0 / den / (0.5 * (1.0 + math.sqrt(1.0 - (2.0 * eta * B0 * B0 / den) ** 2))))
+
+    def exact(tt):
+        ph = k * (X - vA * tt)
+        By, Bz = eta * B0 * np.cos(ph), eta * B0 * np.sin(ph)
+        return dict(B=[np.full_like(X, B0), By, Bz], v=[np.zeros_like(X), -vA * By / B0, -vA * Bz / B0])
+
+    U = _flat_state(X.shape)
+    e0 = exact(t)
+    P = np.zeros((NPRIM,) + X.shape)
+    P[RHO], P[YE], P[EPS] = rho, 0.3, eps
+    for i in range(3):
+        U[BXBAR + i] = e0["B"][i]
+        P[VX + i] = e0["v"][i]
+    par = default_params(eos_gamma=gamma, grav_G=0.0, rho_max=1e3, kappa_z=0.0, kappa_c=0.0)
+    return dict(U=U, P=P, n=(n, ny, ny), ng=ng, dx=dx, bc=[0] * 6, params=par, exact=exact, L=L, vA=vA)
+
+
+def riemann_1d(n=128, ng=NG, ny=4):
+    """1-D magnetised Riemann problem (Balsara-1 type states) along x on [-0.5, 0.5], outflow in x, periodic in y, z;
+    flat spacetime with grav_G = 0. Used for the monotonicity pin of the flux-splitting MP5 scheme."""
+    dx = 1.0 / n
+    X, Y, Z = mesh(n, ny, ny, ng, dx, x0=(-0.5 + 0.5 * dx, 0.0, 0.0))
+    left = X < 0.0
+    gamma = 2.0
+    U = _flat_state(X.shape)
+    P = np.zeros((NPRIM,) + X.shape)
+    P[RHO] = np.where(left, 1.0, 0.125)
+    pr = np.where(left, 1.0, 0.1)
+    P[EPS] = pr / ((gamma - 1.0) * P[RHO])
+    P[YE] = 0.3
+    U[BXBAR], U[BXBAR + 1] = 0.5, np.where(left, 1.0, -1.0)
+    par = default_params(eos_gamma=gamma, grav_G=0.0, rho_max=1e3, kappa_z=0.0, kappa_c=0.0)
+    return dict(U=U, P=P, n=(n, ny, ny), ng=ng, dx=dx, bc=[1, 1, 0, 0, 0, 0], params=par)
+
+
+# ---- TOV star in isotropic coordinates (initial data for configs 3-5) ---------------------------------------
+_TOV_CACHE = {}
+
+
+def tov_profile(K, Gamma, rho_c, dr=2.0e-3):
+    """Textbook TOV equations in the areal radius r for the polytrope p = K rho^Gamma, eps = p / ((Gamma-1) rho),
+    integrated with classical RK4 from the centre to the surface, together with the map to the isotropic radius rbar:
+      dm/dr = 4 pi r^2 e,  dp/dr = -(e + p)(m + 4 pi r^3 p) / (r (r - 2m)),  dnu/dr = (m + 4 pi r^3 p) / (r (r - 2m)),
+      d ln(rbar/r)/dr = (1/sqrt(1 - 2m/r) - 1) / r,   e = rho (1 + eps),
+    normalised to the exterior solution rbar = (r - M + sqrt(r^2 - 2 M r)) / 2, alpha = (1 - M/2rbar)/(1 + M/2rbar).
+    Returns a dict of 1-D arrays over rbar (interior) and the scalars M, Rbar."""
+    key = (K, Gamma, rho_c, dr)
+    if key in _TOV_CACHE:
+        return _TOV_CACHE[key]
+
+    def eos(p):
+        rho = (max(p, 0.0) / K) ** (1.0 / Gamma)
+        return rho, rho + max(p, 0.0) / (Gamma - 1.0)
+
+    def rhs(r, y):
+        m, p, nu, lq = y
+        rho, e = eos(p)
+        if r == 0.0:
+            return np.array([0.0, 0.0, 0.0, 0.0])
+        a = (m + 4.0 * math.pi * r ** 3 * p) / (r * (r - 2.0 * m))
+        return np.array([4.0 * math.pi * r * r * e, -(e + p) * a, a, (1.0 / math.sqrt(1.0 - 2.0 * m / r) - 1.0) / r])
+
+    p_c = K * rho_c ** Gamma
+    y = np.array([0.0, p_c, 0.0, 0.0])
+    r = 0.0
+    rs, ys = [r], [y.copy()]
+    p_stop = 1e-12 * p_c
+    while y[1] > p_stop and r < 100.0:
+        k1 = rhs(r, y)
+        k2 = rhs(r + 0.5 * dr, y + 0.5 * dr * k1)
+        k3 = rhs(r + 0.5 * dr, y + 0.5 * dr * k2)
+        k4 = rhs(r + dr, y + dr * k3)
+        yn = y + dr / 6.0 * (k1 + 2 * k2 + 2 * k3 + k4)
+        if yn[1] <= p_stop:                      # last partial step to the surface by linear interpolation in p
+            f = (y[1] - p_stop) / (y[1] - yn[1])
+            yn = y + f * (yn - y)
+            r += f * dr
+            yn[1] = 0.0
+            rs.append(r)
+            ys.append(yn)
+            break
+        r += dr
+        y = yn
+        rs.append(r)
+        ys.append(y.copy())
+    rs, ys = np.array(rs), np.array(ys)
+    M, R = ys[-1, 0], rs[-1]
+    Rbar = 0.5 * (R - M + math.sqrt(R * R - 2.0 * M * R))
+    lq = ys[:, 3] + (math.log(Rbar / R) - ys[-1, 3])             # ln(rbar / r), matched at the surface
+    rbar = rs * np.exp(lq)
+    nu = ys[:, 2] + (0.5 * math.log(1.0 - 2.0 * M / R) - ys[-1, 2])
+    p = np.maximum(ys[:, 1], 0.0)
+    rho = (p / K) ** (1.0 / Gamma)
+    psi = np.sqrt(np.where(rbar > 0, rs / np.where(rbar > 0, rbar, 1.0), np.exp(-lq[0])))
+    psi[0] = math.exp(-0.5 * lq[0])
+    out = dict(rbar=rbar, rho=rho, p=p, alpha=np.exp(nu), psi=psi, M=M, R=R, Rbar=Rbar, K=K, Gamma=Gamma)
+    _TOV_CACHE[key] = out
+    return out
+
+
+def tov_fields(prof, rb):
+    """rho, p, alpha, psi, dp/drbar at isotropic radii rb (array): interior by interpolation, exterior analytic."""
+    inside = rb < prof["Rbar"]
+    rr = np.minimum(rb, prof["Rbar"])
+    rho = np.where(inside, np.interp(rr, prof["rbar"], prof["rho"]), 0.0)
+    p = np.where(inside, np.interp(rr, prof["rbar"], prof["p"]), 0.0)
+    dpdr = np.where(inside, np.interp(rr, prof["rbar"], np.gradient(prof["p"], prof["rbar"])), 0.0)
+    M = prof["M"]
+    rsafe = np.maximum(rb, 1e-300)
+    psi = np.where(inside, np.interp(rr, prof["rbar"], prof["psi"]), 1.0 + M / (2.0 * rsafe))
+    alpha = np.where(inside, np.interp(rr, prof["rbar"], prof["alpha"]), (1.0 - M / (2.0 * rsafe)) / (1.0 + M / (2.0 * rsafe)))
+    return rho, p, alpha, psi, dpdr
+
+
+# ---- config 3: static magnetised TOV star (BASELINE.json configs[2]) --------------------------------------
+def config3(n=128, half_width=16.0, ng=NG, b_scale=1e-4, seed=SEED_BASE + 3):
+    """Polytrope K=100, Gamma=2, rho_c=1.28e-3 (M ~ 1.4) on an n^3 patch of the given half width, outflow boundaries.
+    gamma~_ij = delta_ij, chi = psi^-4, K_ij = 0, beta = 0, alpha from the TOV solution. Poloidal field from
+    A_phi = A0 max(P - 0.04 P_max, 0) varpi^2, i.e. Bbar = curl(A) (the densitised field IS the flat curl), scaled so
+    that max |B| = b_scale sqrt(P_max). Atmosphere rho = 1e-10 outside. Ideal gas Gamma = 2 (identical to the hybrid
+    EoS with one piece and Gamma_th = Gamma)."""
+    K, Gamma, rho_c = 100.0, 2.0, 1.28e-3
+    prof = tov_profile(K, Gamma, rho_c)
+    dx = 2.0 * half_width / n
+    x0 = -half_width + 0.5 * dx
+    X, Y, Z = mesh(n, n, n, ng, dx, x0=(x0, x0, x0))
+    rb = np.sqrt(X * X + Y * Y + Z * Z)
+    rho, p, alpha, psi, dpdr = tov_fields(prof, rb)
+    par = default_params(eos_gamma=Gamma, rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8)
+    U = _flat_state(X.shape)
+    U[CHI] = psi ** -4
+    U[ALPHA] = alpha
+    # conformally flat: Gamma~^i = 0, A~_ij = 0, K = 0
+    P = np.zeros((NPRIM,) + X.shape)
+    star = rho > 10.0 * par["rho_atmo"]
+    P[RHO] = np.where(star, rho, par["rho_atmo"])
+    P[EPS] = np.where(star, K * np.maximum(rho, 1e-300) ** (Gamma - 1.0) / (Gamma - 1.0), par["eps_atmo"])
+    P[YE] = par["ye_atmo"]
+    # vector potential A_x = -y Ab, A_y = x Ab, Ab = max(P - Pcut, 0):  Bbar = curl A
+    pmax = K * rho_c ** Gamma
+    on = p > 0.04 * pmax
+    Ab = np.where(on, p - 0.04 * pmax, 0.0)
+    dAb = np.where(on, dpdr, 0.0) / np.maximum(rb, 1e-300)       # (1/rbar) dAb/drbar, so that d_i Ab = x_i * dAb
+    Bx, By, Bz = -X * Z * dAb, -Y * Z * dAb, 2.0 * Ab + (X * X + Y * Y) * dAb
+    bmag = np.sqrt(Bx * Bx + By * By + Bz * Bz) * psi ** -4      # |B| = psi^-4 |Bbar|_flat
+    scale = b_scale * math.sqrt(pmax) / bmag.max() if bmag.max() > 0 else 0.0
+    U[BXBAR], U[BXBAR + 1], U[BXBAR + 2] = scale * Bx, scale * By, scale * Bz
+    frac = float(star[ng:-ng, ng:-ng, ng:-ng].mean())
+    return dict(U=U, P=P, n=(n, n, n), ng=ng, dx=dx, bc=[1] * 6, params=par, star_fraction=frac, tov=prof)
