@@ -32,18 +32,7 @@ def workload_inputs(name, n):
     """Seeded synthetic inputs (paper_2510_13965_b200.synth); returns cfg dict with U (metric, Bbar), P (rho, Ye, eps, v)."""
     from paper_2510_13965_b200 import synth
     if name == "c1":
-        base = synth.config1(n=min(n, 32))
-        if n > 32:                      # periodic data: tile the 32^3 box (same spacing), keeps every field smooth
-            reps = (n + 31) // 32
-            ng = base["ng"]
-
-            def tile(A):
-                inner = A[:, ng:-ng, ng:-ng, ng:-ng]
-                big = np.tile(inner, (1, reps, reps, reps))[:, :n, :n, :n]
-                return np.ascontiguousarray(np.pad(big, ((0, 0), (ng, ng), (ng, ng), (ng, ng)), mode="wrap"))
-            base["U"], base["P"] = tile(base["U"]), tile(base["P"])
-            base["n"] = (n, n, n)
-        return base
+        return synth.config1_tiled(n)
     if name == "c3":
         return synth.config3(n=n)
     if name == "c4":

@@ -424,3 +424,107 @@ def config3(n=128, half_width=16.0, ng=NG, b_scale=1e-4, seed=SEED_BASE + 3):
     U[BXBAR], U[BXBAR + 1], U[BXBAR + 2] = scale * Bx, scale * By, scale * Bz
     frac = float(star[ng:-ng, ng:-ng, ng:-ng].mean())
     return dict(U=U, P=P, n=(n, n, n), ng=ng, dx=dx, bc=[1] * 6, params=par, star_fraction=frac, tov=prof)
+
+
+# ---- config 4: hot rotating magnetised star with a synthetic tabulated EoS (BASELINE.json configs[3]) --------
+RHO_CGS_TO_CODE = 1.6199e-18          # G^3 Msun^2 / c^6 in cm^3 / g
+_TABLE_CACHE = {}
+
+
+def table_eos_analytic(rho, T, ye, K=2800.0, Gamma=2.5, gamma_th=1.75, cT=1.0e-3):
+    """The closed form the synthetic table is filled from (input recipe, not method arithmetic):
+    eps = K rho^(Gamma-1)/(Gamma-1) + cT T (1 + 0.2 (ye - 0.3)),  p = K rho^Gamma + (gamma_th - 1) rho eps_th,
+    cs2 = (dp/drho|eps + p/rho^2 dp/deps|rho) / h  (a one-piece hybrid EoS). rho in code units, T in MeV."""
+    eth = cT * T * (1.0 + 0.2 * (ye - 0.3))
+    ec = K * rho ** (Gamma - 1.0) / (Gamma - 1.0)
+    pc = K * rho ** Gamma
+    p = pc + (gamma_th - 1.0) * rho * eth
+    eps = ec + eth
+    h = 1.0 + eps + p / rho
+    dpdrho = Gamma * pc / rho + (gamma_th - 1.0) * eth - (gamma_th - 1.0) * pc / rho
+    cs2 = (dpdrho + p / (rho * rho) * (gamma_th - 1.0) * rho) / h
+    return p, eps, cs2
+
+
+def make_table(n_rho=180, n_T=120, n_ye=50):
+    """3-D table on (log10 rho[g/cc] in [3,16], log10 T[MeV] in [-1,2.3], Ye in [0.05,0.6]), rho fastest, then T, then Ye;
+    columns log10 p, log10(eps + shift), cs2. The density axis is stored in code units (log10 rho_cgs + log10 1.6199e-18)."""
+    key = (n_rho, n_T, n_ye)
+    if key in _TABLE_CACHE:
+        return _TABLE_CACHE[key]
+    lr = np.linspace(3.0, 16.0, n_rho) + math.log10(RHO_CGS_TO_CODE)
+    lT = np.linspace(-1.0, 2.3, n_T)
+    ye = np.linspace(0.05, 0.6, n_ye)
+    YE, LT, LR = np.meshgrid(ye, lT, lr, indexing="ij")
+    p, eps, cs2 = table_eos_analytic(10.0 ** LR, 10.0 ** LT, YE)
+    shift = 0.0
+    tab = dict(n_rho=n_rho, n_T=n_T, n_ye=n_ye, lr0=lr[0], dlr=lr[1] - lr[0], lT0=lT[0], dlT=lT[1] - lT[0],
+               ye0=ye[0], dye=ye[1] - ye[0], tab_eps_shift=shift, tab_h0=1.0,
+               logp=np.ascontiguousarray(np.log10(p)), loge=np.ascontiguousarray(np.log10(eps + shift)),
+               cs2=np.ascontiguousarray(np.minimum(cs2, 0.999)))
+    _TABLE_CACHE[key] = tab
+    return tab
+
+
+def config4(n=256, ng=NG, seed=SEED_BASE + 4, table_shape=(180, 120, 50), T_star=10.0, v_eq=0.2, b_scale=1e-4):
+    """Hot, rigidly rotating, magnetised star on an n^3 patch with the tabulated EoS (eos_kind = 2).
+    Cold part p = K rho^2.5 with K = 2800 (gives p_c close to the Gamma = 2, K = 100 polytrope at rho_c = 1.28e-3);
+    TOV-like profile of that cold EoS in isotropic coordinates; uniform temperature T_star inside, T_atmo outside;
+    rigid rotation about z with Omega such that v = v_eq at the equator; poloidal field as in config 3; density
+    multiplied by (1 + 1e-3 U(-1,1)) cell by cell (seeded). The patch width is Rbar / 0.46 (half width Rbar / 0.92), so that about 41 %
+    of the cells are star."""
+    Kc, Gc, rho_c = 2800.0, 2.5, 1.28e-3
+    tab = make_table(*table_shape)
+    prof = tov_profile(Kc, Gc, rho_c)
+    half = prof["Rbar"] / 0.92
+    dx = 2.0 * half / n
+    x0 = -half + 0.5 * dx
+    X, Y, Z = mesh(n, n, n, ng, dx, x0=(x0, x0, x0))
+    rb = np.sqrt(X * X + Y * Y + Z * Z)
+    rho, p, alpha, psi, dpdr = tov_fields(prof, rb)
+    par = default_params(eos_kind=2, rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, T_atmo=0.1, ye_min=0.05, ye_max=0.6,
+                         ye_atmo=0.3, rho_max=10.0 ** (tab["lr0"] + tab["dlr"] * (tab["n_rho"] - 1)), eps_max=1e3)
+    U = _flat_state(X.shape)
+    U[CHI] = psi ** -4
+    U[ALPHA] = alpha
+    rng = SplitMix64(seed)
+    noise = np.array([rng.uniform(-1.0, 1.0) for _ in range(4096)])
+    idx = (np.arange(X.size, dtype=np.int64) * 2654435761 % 4096).reshape(X.shape)        # cheap seeded scatter of 4096 draws
+    star = rho > 1e3 * par["rho_atmo"]
+    P = np.zeros((NPRIM,) + X.shape)
+    P[RHO] = np.where(star, rho * (1.0 + 1e-3 * noise[idx]), par["rho_atmo"])
+    P[YE] = np.where(star, 0.1 + 0.2 * np.exp(-(rb / prof["Rbar"]) ** 2), par["ye_atmo"])
+    Tf = np.where(star, T_star, par["T_atmo"])
+    P[EPS] = table_eos_analytic(P[RHO], Tf, P[YE])[1]
+    # atmosphere eps must be what the EoS returns for T_atmo through the table (interpolated), the kernels reset it anyway
+    omega = v_eq / prof["Rbar"]
+    P[VX] = np.where(star, -omega * Y, 0.0)
+    P[VX + 1] = np.where(star, omega * X, 0.0)
+    pmax = Kc * rho_c ** Gc
+    on = p > 0.04 * pmax
+    Ab = np.where(on, p - 0.04 * pmax, 0.0)
+    dAb = np.where(on, dpdr, 0.0) / np.maximum(rb, 1e-300)
+    Bx, By, Bz = -X * Z * dAb, -Y * Z * dAb, 2.0 * Ab + (X * X + Y * Y) * dAb
+    bmag = np.sqrt(Bx * Bx + By * By + Bz * Bz) * psi ** -4
+    scale = b_scale * math.sqrt(pmax) / bmag.max() if bmag.max() > 0 else 0.0
+    U[BXBAR], U[BXBAR + 1], U[BXBAR + 2] = scale * Bx, scale * By, scale * Bz
+    frac = float(star[ng:-ng, ng:-ng, ng:-ng].mean())
+    return dict(U=U, P=P, n=(n, n, n), ng=ng, dx=dx, bc=[1] * 6, params=par, table=tab, star_fraction=frac, tov=prof)
+
+
+def config1_tiled(n, **kw):
+    """Config 1 at n > 32: the periodic 32^3 box tiled to n^3 at the same spacing (every field stays smooth and periodic
+    when n is a multiple of 32; otherwise the wrap is a smooth-data jump the limiter handles). Bench workload c1_<n>."""
+    base = config1(n=min(n, 32), **kw)
+    if n <= 32:
+        return base
+    reps = (n + 31) // 32
+    ng = base["ng"]
+
+    def tile(A):
+        inner = A[:, ng:-ng, ng:-ng, ng:-ng]
+        big = np.tile(inner, (1, reps, reps, reps))[:, :n, :n, :n]
+        return np.ascontiguousarray(np.pad(big, ((0, 0), (ng, ng), (ng, ng), (ng, ng)), mode="wrap"))
+    base["U"], base["P"] = tile(base["U"]), tile(base["P"])
+    base["n"] = (n, n, n)
+    return base

@@ -21,6 +21,16 @@ def _rel(a, b, interior=True):
     return num / np.where(den > 0, den, 1.0), den
 
 
+def _rel_vec(a, b, groups):
+    """as _rel (all points), but the components of a vector share the norm of the vector: a component that vanishes in
+    the exact solution (v^x of a transverse wave) has no scale of its own"""
+    num = np.abs(a - b).reshape(a.shape[0], -1).max(axis=1)
+    den = np.abs(b).reshape(b.shape[0], -1).max(axis=1)
+    for g in groups:
+        den[list(g)] = den[list(g)].max()
+    return num / np.where(den > 0, den, 1.0)
+
+
 def _setup(oracle_mod, cfg):
     from paper_2510_13965_b200 import binding
     n = cfg["n"]
@@ -45,9 +55,9 @@ def _one_stage(oracle_mod, cfg, rhs_tol=1e-11, prim_tol=1e-12):
     patch.con2prim()
     Pg, Fg, Ug = patch.P.cpu().numpy(), patch.flags.cpu().numpy()[0], patch.U.cpu().numpy()
     assert np.array_equal(Fg, Fo), "flag masks must agree bit for bit"
-    rp, _ = _rel(Pg, Po, interior=False)
+    rp = _rel_vec(Pg, Po, [(4, 5, 6)])             # v^i share the norm of the vector (v^z = 0 exactly for rotation about z)
     assert np.all(rp < prim_tol), rp
-    ru, _ = _rel(Ug, Uo, interior=False)
+    ru = _rel_vec(Ug, Uo, [(25, 26, 27), (28, 29, 30)])
     assert np.all(ru < prim_tol), ru
     Kg = patch.rhs(1).cpu().numpy()
     rk, den = _rel(Kg, Ko)
@@ -167,4 +177,189 @@ def test_ten_rk_steps_parity(oracle_mod):
     hostF = torch.zeros(Fo.shape, dtype=torch.uint8).pin_memory()
     patch.advance_host(binding.make_tableau(a, w), cfg["bc"], dt, 10, hostU, hostF)
     assert np.array_equal(hostU.numpy(), Ug) and np.array_equal(hostF.numpy(), Fg)
+    patch.close()
+
+
+# ---- configs 2-4 and full-size sampled parity -----------------------------------------------------------------
+def _advance_both(oracle_mod, cfg, steps, courant=0.25):
+    from paper_2510_13965_b200 import binding
+    o, patch, U, P = _setup(oracle_mod, cfg)
+    a, w = synth.tableau("rk4")
+    dt = courant * cfg["dx"]
+    Uo = U.copy()
+    Po, Fo = o.evolve(Uo, cfg["bc"], a, w, dt, steps)
+    patch.upload(U=U)
+    patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, steps)
+    Ug, Pg, Fg = patch.U.cpu().numpy(), patch.P.cpu().numpy(), patch.flags.cpu().numpy()[0]
+    patch.close()
+    return (Ug, Pg, Fg), (Uo, Po, Fo)
+
+
+@pytest.mark.parametrize("n", [32, 64, 128])
+def test_config2_gauge_wave_100_steps(oracle_mod, n):
+    """BASELINE.json configs[1]: 100 full RK4 steps at Courant 0.25; slab n x 8 x 8 keeps the oracle to seconds."""
+    cfg = synth.config2_gauge_wave(n=n, ny=8)
+    (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 100)
+    assert np.array_equal(Fg, Fo)
+    # Tolerance (DESIGN.md "Parity tolerances"): north_star's 1e-9 relative per component, plus the rounding floor of a
+    # perturbative problem. The O(1) background fields (gamma~_ii, chi, alpha) carry one-ulp differences between the two
+    # summation orders; the second-derivative stencils amplify them by 1/h^2, each of the 400 stage evaluations adds
+    # dt times that to the O(1e-6) perturbative fields (A~_ij, Gamma^^i, Theta ...): floor = eps (dt / h^2) 400.
+    # Fields that stay exactly zero must do so on both sides.
+    d = np.abs(Ug - Uo).reshape(32, -1).max(axis=1)
+    scale = np.abs(Uo).reshape(32, -1).max(axis=1)
+    assert np.all(d[scale == 0.0] == 0.0)
+    floor = 2.2e-16 * (0.25 / cfg["dx"]) * 400
+    assert np.all(d <= 1e-9 * scale + floor), (d, scale, floor)
+    # and the wave itself (alpha - 1 ~ 1e-6) agrees to 1e-6 of ITS amplitude
+    assert np.abs(Ug[synth.ALPHA] - Uo[synth.ALPHA]).max() < 1e-6 * 1e-6
+
+
+@pytest.mark.parametrize("n", [32, 64, 128])
+def test_config2_alfven_wave_100_steps(oracle_mod, n):
+    cfg = synth.config2_alfven(n=n, ny=8)
+    (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 100)
+    assert np.array_equal(Fg, Fo)
+    ru = _rel_vec(Ug, Uo, [(25, 26, 27), (28, 29, 30)])
+    rp = _rel_vec(Pg, Po, [(4, 5, 6)])
+    assert np.all(ru < 1e-9) and np.all(rp < 1e-9), (ru, rp)
+
+
+def test_config2_observed_order_on_the_gpu():
+    """Convergence series 32^3, 64^3, 128^3 (full cubes, same end time t = 100 * 0.25 / 32) run by the CUDA path alone.
+    Alfven wave (exact nonlinear solution): order against the exact solution. Gauge wave (solves only the LINEARISED
+    equations, O(A^2) = 1e-12 floor): self-convergence (Richardson) on the points the three vertex-centred grids share."""
+    from paper_2510_13965_b200 import binding
+    a, w = synth.tableau("rk4")
+    for make, field, pick in ((synth.config2_gauge_wave, synth.ALPHA, None),
+                              (synth.config2_alfven, synth.BXBAR + 1, lambda e: e["B"][1])):
+        err, sol = {}, {}
+        for n in (32, 64, 128):
+            cfg = make(n=n)
+            steps = 100 * n // 32
+            dt = 0.25 * cfg["dx"]
+            patch = binding.Patch(cfg["params"], cfg["n"], cfg["ng"], cfg["dx"], stages=4)
+            patch.upload(U=cfg["U"], P=cfg["P"])
+            patch.prim2con()
+            patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, steps)
+            u = patch.U[field].cpu().numpy()[NG:-NG, NG:-NG, NG:-NG]
+            sol[n] = u[::n // 32, ::n // 32, ::n // 32]
+            if pick is not None:
+                err[n] = np.abs(u - pick(cfg["exact"](steps * dt))[NG:-NG, NG:-NG, NG:-NG]).max()
+            patch.close()
+        if pick is None:
+            d1, d2 = np.abs(sol[32] - sol[64]).max(), np.abs(sol[64] - sol[128]).max()
+            order = np.log2(d1 / d2)
+            print("gauge wave self-convergence: |u32-u64| = %.3e, |u64-u128| = %.3e, observed order %.2f" % (d1, d2, order))
+            assert 3.5 < order < 5.5, (d1, d2, order)
+        else:
+            o1, o2 = np.log2(err[32] / err[64]), np.log2(err[64] / err[128])
+            print("Alfven wave errors", err, "observed orders %.2f %.2f" % (o1, o2))
+            assert o1 > 3.8 and o2 > 3.8, (err, o1, o2)
+
+
+def test_config3_tov_parity(oracle_mod):
+    """Static magnetised TOV star, outflow boundaries, atmosphere: one-stage parity at 48^3 (flags bit-exact), 5 RK4 steps at 32^3."""
+    cfg = synth.config3(n=48)
+    _one_stage(oracle_mod, cfg)
+    cfg = synth.config3(n=32)
+    (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 5)
+    assert np.array_equal(Fg, Fo) and (Fo & 1).sum() > 0
+    ru, _ = _rel(Ug, Uo, interior=False)
+    rp, _ = _rel(Pg, Po, interior=False)
+    assert np.all(ru < 1e-9) and np.all(rp < 1e-9), (ru, rp)
+
+
+def test_config3_full_size_50_steps():
+    """BASELINE.json configs[2] at full size (128^3, 50 RK steps) on the CUDA path: equilibrium holds, nothing fatal."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config3(n=128)
+    a, w = synth.tableau("rk4")
+    patch = binding.Patch(cfg["params"], cfg["n"], cfg["ng"], cfg["dx"], stages=4)
+    patch.upload(U=cfg["U"], P=cfg["P"])
+    patch.prim2con()
+    rho0 = float(patch.P[synth.RHO].max())
+    patch.advance(binding.make_tableau(a, w), cfg["bc"], 0.25 * cfg["dx"], 50)
+    st = patch.status()
+    rho1 = float(patch.P[synth.RHO].max())
+    patch.close()
+    assert st["n_fatal"] == 0 and st["n_noconv"] == 0 and st["n_atmo"] > 0.5 * st["n_points"]
+    assert abs(rho1 / rho0 - 1.0) < 5e-3, (rho0, rho1)
+
+
+def test_config4_table_parity(oracle_mod):
+    """Hot rotating star with the full 180x120x50 table: one-stage parity at 32^3, 3 RK4 steps at 24^3."""
+    cfg = synth.config4(n=32)
+    _one_stage(oracle_mod, cfg, rhs_tol=1e-11, prim_tol=1e-11)     # eps through the T inversion: amplification note N3
+    cfg = synth.config4(n=24)
+    (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 3)
+    assert np.array_equal(Fg, Fo)
+    ru, _ = _rel(Ug, Uo, interior=False)
+    rp, _ = _rel(Pg, Po, interior=False)
+    assert np.all(ru < 1e-9) and np.all(rp < 1e-9), (ru, rp)
+
+
+def _crop_parity(oracle_mod, cfg, patch, boxes, m=12, rhs_tol=1e-11):
+    """Full-size run of the launch configuration bench.py times, checked on sampled sub-boxes the oracle can do one by
+    one: the oracle gets the box plus 3 layers of the surrounding (already ghost-filled) data as its ghosts."""
+    Ug_all = patch.U.cpu().numpy()
+    worst = 0.0
+    # R28: the norm of a component is taken over the interior of the WHOLE patch (a 12^3 box at a symmetry centre holds
+    # components that vanish there); it comes from the GPU result, whose samples are what is being checked
+    Kint = patch.K[0][:, NG:-NG, NG:-NG, NG:-NG]
+    gden = Kint.abs().reshape(Kint.shape[0], -1).max(dim=1).values.cpu().numpy()
+    # components of one tensor share its norm (off-diagonal gamma~_ij RHS of a conformally flat star are rounding noise)
+    for g in ((0, 1, 2, 3, 4, 5), (6, 7, 8, 9, 10, 11), (15, 16, 17), (19, 20, 21), (25, 26, 27), (28, 29, 30)):
+        gden[list(g)] = gden[list(g)].max()
+    for (i0, j0, k0) in boxes:
+        sl = (slice(None), slice(k0, k0 + m + 2 * NG), slice(j0, j0 + m + 2 * NG), slice(i0, i0 + m + 2 * NG))
+        o = oracle_mod.Oracle(cfg["params"], m, m, m, NG, cfg["dx"], table=cfg.get("table"))
+        Uc = np.ascontiguousarray(Ug_all[sl])
+        Po, Fo = o.con2prim(Uc)                                     # Uc is post-con2prim already: idempotent up to rounding
+        Ko = o.rhs(Uc, Po)
+        Kg = np.ascontiguousarray(patch.K[0][sl].cpu().numpy())
+        Fg = patch.flags[0][sl[1:]].cpu().numpy()
+        assert np.array_equal(Fg, Fo)
+        I3 = (slice(None), slice(NG, -NG), slice(NG, -NG), slice(NG, -NG))
+        num = np.abs(Kg[I3] - Ko[I3]).reshape(Kg.shape[0], -1).max(axis=1)
+        live = gden > 0
+        rk = num[live] / gden[live]
+        assert np.all(num[~live] == 0.0)
+        worst = max(worst, rk.max())
+        assert np.all(rk < rhs_tol), ((i0, j0, k0), rk)
+    return worst
+
+
+def test_full_size_256_sampled_parity(oracle_mod):
+    """BASELINE.json's 256^3 patch in bench.py's launch configuration (workload c1_256): fill -> con2prim -> rhs on the GPU,
+    compared with the oracle on 12^3 sub-boxes (first tile, a tile seam, the last ragged tiles at the far corner)."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config1_tiled(256)
+    patch = binding.Patch(cfg["params"], cfg["n"], cfg["ng"], cfg["dx"], stages=1)
+    patch.upload(U=cfg["U"], P=cfg["P"])
+    patch.prim2con()
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    patch.rhs(1)
+    n = 256
+    boxes = [(0, 0, 0), (n - 12, n - 12, n - 12), (122, 61, 200), (n - 12, 0, 97)]
+    worst = _crop_parity(oracle_mod, cfg, patch, boxes)
+    print("256^3 sampled parity, worst relative RHS difference %.2e" % worst)
+    patch.close()
+
+
+def test_config4_full_size_sampled_parity(oracle_mod):
+    """Config 4 at 128^3 with the full table (the 256^3 instance is the bench's c4 workload): sampled sub-boxes in the
+    stellar core, across the surface and in the atmosphere."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config4(n=128)
+    patch = binding.Patch(cfg["params"], cfg["n"], cfg["ng"], cfg["dx"], stages=1, table=cfg["table"])
+    patch.upload(U=cfg["U"], P=cfg["P"])
+    patch.prim2con()
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    patch.rhs(1)
+    boxes = [(58, 58, 58), (58, 58, 110), (0, 0, 0), (116, 116, 116), (20, 60, 60)]
+    worst = _crop_parity(oracle_mod, cfg, patch, boxes)
+    print("config 4 128^3 sampled parity, worst relative RHS difference %.2e" % worst)
     patch.close()

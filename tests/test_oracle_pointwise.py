@@ -223,3 +223,62 @@ def test_ghost_fill(oracle_mod):
     o.fill_ghosts(U, [0, 0, 1, 1, 0, 0])
     mixed = np.pad(np.pad(inner, ((0, 0), (0, 0), (ng, ng), (0, 0)), mode="edge"), ((0, 0), (ng, ng), (0, 0), (ng, ng)), mode="wrap")
     assert np.array_equal(U, mixed)
+
+
+# ---- tabulated EoS (config 4, reading R26) -------------------------------------------------------------------
+def _table_oracle(oracle_mod, shape=(60, 40, 12)):
+    tab = synth.make_table(*shape)
+    par = synth.default_params(eos_kind=2, ye_min=0.05, ye_max=0.6, eps_max=1e3,
+                               rho_max=10.0 ** (tab["lr0"] + tab["dlr"] * (tab["n_rho"] - 1)))
+    return oracle_mod.Oracle(par, 4, 4, 4, 3, 0.1, table=tab), tab
+
+
+def test_table_eos_exact_at_nodes_and_close_between(oracle_mod):
+    """At table nodes the interpolant returns the tabulated (analytic) values; between nodes it differs from the closed
+    form it was filled from only by the trilinear interpolation error; T(eps) inverts eps(T) exactly along the T axis."""
+    o, tab = _table_oracle(oracle_mod)
+    for (ir, it, iy) in ((5, 7, 3), (40, 20, 0), (58, 38, 10)):
+        rho = 10.0 ** (tab["lr0"] + ir * tab["dlr"])
+        T = 10.0 ** (tab["lT0"] + it * tab["dlT"])
+        ye = tab["ye0"] + iy * tab["dye"]
+        p_a, eps_a, cs2_a = synth.table_eos_analytic(rho, T, ye)
+        eps = o.eps_from_T(rho, T, ye)
+        assert abs(eps / eps_a - 1.0) < 1e-12
+        p, Tb, cs2 = o.eos(rho, eps, ye)
+        assert abs(p / p_a - 1.0) < 1e-11 and abs(Tb / T - 1.0) < 1e-11 and abs(cs2 - min(cs2_a, 0.999)) < 1e-11
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        rho = 10.0 ** rng.uniform(tab["lr0"] + 1.0, tab["lr0"] + 12.0)
+        T = 10.0 ** rng.uniform(-0.9, 2.2)
+        ye = rng.uniform(0.06, 0.59)
+        p_a, eps_a, cs2_a = synth.table_eos_analytic(rho, T, ye)
+        eps = o.eps_from_T(rho, T, ye)
+        p, Tb, cs2 = o.eos(rho, eps, ye)
+        assert abs(Tb / T - 1.0) < 1e-10                       # exact inversion of the interpolant
+        assert abs(eps / eps_a - 1.0) < 0.05 and abs(p / p_a - 1.0) < 0.05 and abs(cs2 - cs2_a) < 0.02   # coarse 60x40x12 table
+
+
+def test_table_con2prim_round_trip(oracle_mod):
+    """prim -> cons -> prim with the tabulated EoS (T inversion inside the mu iteration), north_star tolerance 1e-12 on rho, v;
+    eps carries the ~100x amplification of (D12) (note N3)."""
+    o, tab = _table_oracle(oracle_mod)
+    rng = np.random.default_rng(5)
+    gt = np.array([1.0, 0.0, 0.0, 1.0, 0.0, 1.0])
+    worst = 0.0
+    for _ in range(40):
+        rho = 10.0 ** rng.uniform(-9.0, -2.5)
+        T = 10.0 ** rng.uniform(-0.5, 1.8)
+        ye = rng.uniform(0.1, 0.5)
+        eps = o.eps_from_T(rho, T, ye)
+        v = rng.uniform(-0.3, 0.3, 3)
+        B = rng.uniform(-1.0, 1.0, 3) * math.sqrt(rho) * 0.1
+        p = o.eos(rho, eps, ye)[0]
+        prim = np.zeros(10)
+        prim[0], prim[1], prim[2], prim[3], prim[4:7] = rho, ye, eps, p, v
+        D, tau, Sx, Sy, Sz = oracle_mod.prim2con_point(gt, prim, B)
+        uc = np.array([D, D * ye, tau, Sx, Sy, Sz, B[0], B[1], B[2], 0.0])
+        out, flag, _ = o.con2prim_point(gt, 1.0, 1.0, uc)
+        assert flag == 0, flag
+        worst = max(worst, abs(out[0] / rho - 1.0), np.abs(out[4:7] - v).max())
+        assert abs(out[2] / eps - 1.0) < 1e-10
+    assert worst < 1e-12, worst
