@@ -95,6 +95,10 @@ typedef struct {
   double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
   double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
   int c2p_maxit;
+  /* M1 (n_species = 3): synthetic grey opacities kappa_a = kappa_s = m1_kappa0 (rho / m1_rho0)^2 m1_species_scale[s],
+   * eta = kappa_a T^4 (BASELINE.json configs[4]); energy floor, Newton tolerance / cap of App. C, baryon mass of l.316 */
+  double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
+  int m1_maxit;
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SOURCES = ["orc_stencil.cpp", "orc_eos.cpp", "orc_c2p.cpp", "orc_ccz4.cpp", "orc_grmhd.cpp",
-            "orc_rk.cpp", "orc_capi.cpp"]
+            "orc_rk.cpp", "orc_m1.cpp", "orc_m1_patch.cpp", "orc_capi.cpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 NSTATE, NPRIM = 32, 10
@@ -108,6 +108,15 @@ def _load(counting):
         L.orc_con2prim_point.argtypes = [vp, vp, f64, f64, vp, vp]
         L.orc_con2prim_point.restype = i32
         L.orc_prim2con_point.argtypes = [vp, vp, vp, vp]
+        L.orc_m1_closure_point.argtypes = [f64, vp, vp, f64, vp, vp, vp]
+        L.orc_m1_JH.argtypes = [f64, vp, vp, f64, vp, vp, f64, f64, vp]
+        L.orc_m1_jacobian.argtypes = [f64, vp, vp, f64, vp, vp, f64, f64, f64, f64, f64, vp]
+        L.orc_m1_implicit_point.argtypes = [vp, i32, vp, f64, f64, vp, f64, f64, f64, vp, vp, vp, vp]
+        L.orc_m1_implicit_point.restype = i32
+        L.orc_m1_rhs.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_m1_implicit.argtypes = [vp, vp, vp, vp, vp, f64, vp]
+        L.orc_m1_backreaction.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_evolve_imex.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, f64, i32]
     return _libs[counting]
 
 
@@ -225,3 +234,69 @@ def stencil(name, u, s, h, *extra):
     c = flat.size // 2
     p = ctypes.c_void_p(flat.ctypes.data + 8 * c)
     return getattr(L, "orc_" + name)(p, s, h, *extra)
+
+
+# ---- M1 (config 5) ------------------------------------------------------------------------------------------
+NM1 = 15
+
+
+def m1_closure_point(E, F, vu, W, gl, gu):
+    """Eqs. (42)-(50) at one point; gl, gu 3x3 physical metric and inverse. Returns dict xi, chi, J, Hn, H (3), P (3x3)."""
+    out = np.zeros(16)
+    lib().orc_m1_closure_point(float(E), _ptr(_f64(F)), _ptr(_f64(vu)), float(W), _ptr(_f64(gl)), _ptr(_f64(gu)), _ptr(out))
+    return dict(xi=out[0], chi=out[1], J=out[2], Hn=out[3], H=out[4:7].copy(), P=out[7:16].reshape(3, 3).copy())
+
+
+def m1_JH(E, F, vu, W, gl, gu, dthin, dthick):
+    out = np.zeros(4)
+    lib().orc_m1_JH(float(E), _ptr(_f64(F)), _ptr(_f64(vu)), float(W), _ptr(_f64(gl)), _ptr(_f64(gu)), float(dthin), float(dthick), _ptr(out))
+    return out[0], out[1:4].copy()
+
+
+def m1_jacobian(E, F, vu, W, gl, gu, dthin, dthick, alpha, ka, ks):
+    out = np.zeros(16)
+    lib().orc_m1_jacobian(float(E), _ptr(_f64(F)), _ptr(_f64(vu)), float(W), _ptr(_f64(gl)), _ptr(_f64(gu)), float(dthin), float(dthick),
+                          float(alpha), float(ka), float(ks), _ptr(out))
+    return out.reshape(4, 4)
+
+
+def _m1_implicit_point(self, species, Vstar, adt, alpha, vu, W, rho, T, gl, gu):
+    V, R = np.zeros(5), np.zeros(5)
+    flag = lib().orc_m1_implicit_point(self.h, int(species), _ptr(_f64(Vstar)), float(adt), float(alpha), _ptr(_f64(vu)), float(W), float(rho),
+                                       float(T), _ptr(_f64(gl)), _ptr(_f64(gu)), _ptr(V), _ptr(R))
+    return V, R, flag
+
+
+def _m1_rhs(self, U, P, V):
+    KV = np.zeros_like(V)
+    lib().orc_m1_rhs(self.h, _ptr(U), _ptr(P), _ptr(V), _ptr(KV))
+    return KV
+
+
+def _m1_implicit(self, U, P, V, adt, flags=None):
+    """V: V* in, V^(i) out (in place). Returns (R, flags)."""
+    R = np.zeros_like(V)
+    fl = np.zeros(self.shape, dtype=np.uint8) if flags is None else flags
+    lib().orc_m1_implicit(self.h, _ptr(U), _ptr(P), _ptr(V), _ptr(R), float(adt), _ptr(fl))
+    return R, fl
+
+
+def _m1_backreaction(self, U, P, R, K):
+    lib().orc_m1_backreaction(self.h, _ptr(U), _ptr(P), _ptr(R), _ptr(K))
+    return K
+
+
+def _evolve_imex(self, U, V, bc, a_expl, w_expl, a_impl, w_impl, dt, n_steps):
+    P = np.zeros((NPRIM,) + self.shape)
+    flags = np.zeros(self.shape, dtype=np.uint8)
+    ae, we, ai, wi = _f64(a_expl), _f64(w_expl), _f64(a_impl), _f64(w_impl)
+    b = np.asarray(bc, dtype=np.int32)
+    lib().orc_evolve_imex(self.h, _ptr(U), _ptr(V), _ptr(P), _ptr(flags), _ptr(b), len(we), _ptr(ae), _ptr(we), _ptr(ai), _ptr(wi), float(dt), int(n_steps))
+    return P, flags
+
+
+Oracle.m1_implicit_point = _m1_implicit_point
+Oracle.m1_rhs = _m1_rhs
+Oracle.m1_implicit = _m1_implicit
+Oracle.m1_backreaction = _m1_backreaction
+Oracle.evolve_imex = _evolve_imex

@@ -74,6 +74,10 @@ struct Params {
   double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
   double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
   int c2p_maxit;
+  // M1 (config 5): synthetic opacities kappa_a = kappa_s = m1_kappa0 (rho / m1_rho0)^2 * m1_species_scale[s],
+  // eta = kappa_a T^4 (BASELINE.json configs[4]); number opacities kappa_a^0 = kappa_a, eta^0 = eta (synthetic)
+  double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
+  int m1_maxit;
 };
 
 // ---- stencils (Sec. III B)
@@ -115,5 +119,28 @@ void rk_combine(const Grid& g, int nfields, double* Uout, const double* U0, int 
 void evolve(const Params& par, const Grid& g, double* U, double* P, uint8_t* flags,
             const int bc[6], int stages, const double* a_expl, const double* w_expl,
             double dt, int n_steps);
+
+// ---- M1 grey two-moment transport (Sec. II C, III D, App. B, App. C); V holds 15 fields: (Nbar, Ebar, Fbar_i) x 3 species
+enum { NM1 = 15, NSPECIES = 3 };
+struct M1Closure { double xi, chi, J, Hn, H[3], P[3][3]; int fix; };   // Eqs. (42)-(50); H[i] = gamma_ia H^a (covariant)
+// closure at one point from undensitised E, F_i (covariant), v^i, W and the physical metric gl = gamma_ij, gu = gamma^ij
+M1Closure m1_closure_point(double E, const double F[3], const double vu[3], double W, const double gl[3][3], const double gu[3][3]);
+// App. C Eqs. (C17)-(C27): J and H_i for given d_thin, d_thick
+void m1_JH_appC(double E, const double F[3], const double vu[3], double W, const double gl[3][3], const double gu[3][3],
+                double dthin, double dthick, double& J, double H[3]);
+// Jacobian of R_V w.r.t. (E, F_j), Eqs. (C28)-(C35), undensitised, closure frozen
+void m1_jacobian(double E, const double F[3], const double vu[3], double W, const double gl[3][3], const double gu[3][3],
+                 double dthin, double dthick, double alpha, double ka, double ks, double Jac[4][4]);
+void m1_opacities(const Params& par, int species, double rho, double T, double& ka, double& ks, double& eta);
+// pointwise implicit solve of App. C for one species: in Vstar = (N*, E*, F_i*) undensitised; out V, stiff source R (undensitised,
+// alpha (C, S_n, S_i)); returns flag bits (FLAG_M1FIX, FLAG_NOCONV)
+uint8_t m1_implicit_point(const Params& par, int species, const double Vstar[5], double adt, double alpha, const double vu[3], double W,
+                          double rho, double T, const double gl[3][3], const double gu[3][3], double V[5], double R[5]);
+// whole-patch operations
+void m1_rhs(const Params& par, const Grid& g, const double* U, const double* P, const double* V, double* KV);          // a11: explicit part
+void m1_implicit(const Params& par, const Grid& g, const double* U, const double* P, double* V, double* R, double adt, uint8_t* flags);  // a12
+void m1_backreaction(const Params& par, const Grid& g, const double* U, const double* P, const double* R, double* K);  // a8 (M1 part)
+void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double* P, uint8_t* flags, const int bc[6], int stages,
+                 const double* a_expl, const double* w_expl, const double* a_impl, const double* w_impl, double dt, int n_steps);
 
 }  // namespace orc

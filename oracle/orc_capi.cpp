@@ -16,6 +16,7 @@ bool set_scalar(Params& p, const std::string& k, double v) {
   D(sigma_ko_spacetime) D(sigma_ko_matter) D(c_b) D(kappa_b) D(mp5_alpha)
   D(rho_atmo) D(rho_cut) D(rho_low) D(alpha_bh) D(w_max) D(rho_max) D(eps_min) D(eps_max)
   D(ye_min) D(ye_max) D(ye_atmo) D(eps_atmo) D(T_atmo) I(c2p_maxit)
+  D(m1_kappa0) D(m1_rho0) D(m1_efloor) D(m1_tol) D(m1_mb) I(m1_maxit)
   I(n_rho) I(n_T) I(n_ye) D(lr0) D(dlr) D(lT0) D(dlT) D(ye0) D(dye) D(tab_eps_shift) D(tab_h0)
 #undef D
 #undef I
@@ -44,6 +45,7 @@ int orc_set_array(void* hh, const char* key, const double* v, int n) {
   else if (k == "pp_Gamma") dst = p.pp_Gamma;
   else if (k == "pp_rho") dst = p.pp_rho;
   else if (k == "beta0") { dst = p.beta0; cap = 3; }
+  else if (k == "m1_species_scale") { dst = p.m1_species_scale; cap = 3; }
   if (!dst || n > cap) return -1;
   for (int i = 0; i < n; ++i) dst[i] = v[i];
   return 0;
@@ -74,6 +76,34 @@ void orc_evolve(void* hh, double* U, double* P, uint8_t* flags, const int* bc, i
                 const double* a_expl, const double* w_expl, double dt, int n_steps) {
   Handle* h = (Handle*)hh;
   evolve(h->par, h->grid, U, P, flags, bc, stages, a_expl, w_expl, dt, n_steps);
+}
+
+// ---- M1
+void orc_m1_closure_point(double E, const double* F, const double* vu, double W, const double* gl, const double* gu, double* out16) {
+  const M1Closure c = m1_closure_point(E, F, vu, W, (const double (*)[3])gl, (const double (*)[3])gu);
+  out16[0] = c.xi; out16[1] = c.chi; out16[2] = c.J; out16[3] = c.Hn;
+  for (int i = 0; i < 3; ++i) { out16[4 + i] = c.H[i]; for (int j = 0; j < 3; ++j) out16[7 + 3 * i + j] = c.P[i][j]; }
+}
+void orc_m1_JH(double E, const double* F, const double* vu, double W, const double* gl, const double* gu, double dthin, double dthick, double* out4) {
+  m1_JH_appC(E, F, vu, W, (const double (*)[3])gl, (const double (*)[3])gu, dthin, dthick, out4[0], out4 + 1);
+}
+void orc_m1_jacobian(double E, const double* F, const double* vu, double W, const double* gl, const double* gu, double dthin, double dthick,
+                     double alpha, double ka, double ks, double* out16) {
+  m1_jacobian(E, F, vu, W, (const double (*)[3])gl, (const double (*)[3])gu, dthin, dthick, alpha, ka, ks, (double (*)[4])out16);
+}
+int orc_m1_implicit_point(void* hh, int species, const double* Vstar, double adt, double alpha, const double* vu, double W, double rho, double T,
+                          const double* gl, const double* gu, double* V, double* R) {
+  return m1_implicit_point(((Handle*)hh)->par, species, Vstar, adt, alpha, vu, W, rho, T, (const double (*)[3])gl, (const double (*)[3])gu, V, R);
+}
+void orc_m1_rhs(void* hh, const double* U, const double* P, const double* V, double* KV) { Handle* h = (Handle*)hh; m1_rhs(h->par, h->grid, U, P, V, KV); }
+void orc_m1_implicit(void* hh, const double* U, const double* P, double* V, double* R, double adt, uint8_t* flags) {
+  Handle* h = (Handle*)hh; m1_implicit(h->par, h->grid, U, P, V, R, adt, flags);
+}
+void orc_m1_backreaction(void* hh, const double* U, const double* P, const double* R, double* K) { Handle* h = (Handle*)hh; m1_backreaction(h->par, h->grid, U, P, R, K); }
+void orc_evolve_imex(void* hh, double* U, double* V, double* P, uint8_t* flags, const int* bc, int stages, const double* ae, const double* we,
+                     const double* ai, const double* wi, double dt, int n_steps) {
+  Handle* h = (Handle*)hh;
+  evolve_imex(h->par, h->grid, U, V, P, flags, bc, stages, ae, we, ai, wi, dt, n_steps);
 }
 
 // ---- pointwise helpers for the pins

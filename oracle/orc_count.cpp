@@ -68,6 +68,8 @@ using orc_cnt::Cnt;
 #include "orc_grmhd.cpp"
 #undef SYM
 #include "orc_rk.cpp"
+#include "orc_m1.cpp"
+#include "orc_m1_patch.cpp"
 #include "orc_capi.cpp"
 #undef double
 

@@ -37,6 +37,8 @@ class mhd_patch_desc(ctypes.Structure):
         ("rho_atmo", _d), ("rho_cut", _d), ("rho_low", _d), ("alpha_bh", _d), ("w_max", _d), ("rho_max", _d),
         ("eps_min", _d), ("eps_max", _d), ("ye_min", _d), ("ye_max", _d), ("ye_atmo", _d), ("eps_atmo", _d), ("T_atmo", _d),
         ("c2p_maxit", _i),
+        ("m1_kappa0", _d), ("m1_rho0", _d), ("m1_species_scale", _d * 3), ("m1_efloor", _d), ("m1_tol", _d), ("m1_mb", _d),
+        ("m1_maxit", _i),
     ]
 
 
@@ -113,7 +115,7 @@ def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, tab
             arr = getattr(d, k)
             for i, x in enumerate(v):
                 arr[i] = float(x)
-        elif k in ("eos_kind", "n_pieces", "c2p_maxit"):
+        elif k in ("eos_kind", "n_pieces", "c2p_maxit", "m1_maxit"):
             setattr(d, k, int(v))
         else:
             setattr(d, k, float(v))

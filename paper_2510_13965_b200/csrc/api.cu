@@ -120,6 +120,9 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.w_max = desc->w_max; q.rho_max = desc->rho_max; q.eps_min = desc->eps_min; q.eps_max = desc->eps_max;
   q.ye_min = desc->ye_min; q.ye_max = desc->ye_max; q.ye_atmo = desc->ye_atmo; q.eps_atmo = desc->eps_atmo; q.T_atmo = desc->T_atmo;
   q.c2p_maxit = desc->c2p_maxit > 0 ? desc->c2p_maxit : 100;
+  q.m1_kappa0 = desc->m1_kappa0; q.m1_rho0 = desc->m1_rho0 > 0.0 ? desc->m1_rho0 : 1.0; q.m1_efloor = desc->m1_efloor;
+  q.m1_tol = desc->m1_tol > 0.0 ? desc->m1_tol : 1e-13; q.m1_mb = desc->m1_mb; q.m1_maxit = desc->m1_maxit > 0 ? desc->m1_maxit : 30;
+  for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
   p->d_counts = nullptr;
   if (cudaMalloc(&p->d_counts, 8 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   *out = p;

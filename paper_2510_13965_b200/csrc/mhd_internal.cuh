@@ -35,6 +35,8 @@ struct Par {
   double rho_atmo, rho_cut, rho_low, alpha_bh, w_max, rho_max, eps_min, eps_max;
   double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
   int c2p_maxit;
+  double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
+  int m1_maxit;
 };
 
 struct Slot {

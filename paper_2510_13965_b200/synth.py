@@ -68,6 +68,23 @@ def tableau(name):
     return a, w
 
 
+def imex_tableau(name="imex332"):
+    """IMEX pair (a_expl, w_expl, a_impl, w_impl) in the form of PAPER.md Eqs. (53)-(55). The paper's Tables I, II have no
+    body (R1), so the implicit tableau is caller data; this 3-stage, 2nd-order, L-stable pair satisfies every condition the
+    paper states (sum w = 1, sum w c = sum w c~ = sum w~ c = sum w~ c~ = 1/2, DIRK, R(-inf) = 0)."""
+    if name != "imex332":
+        raise ValueError(name)
+    ae = np.zeros((3, 3))
+    ae[1, 0] = 0.5
+    ae[2, 0] = ae[2, 1] = 0.5
+    we = np.array([1 / 3, 1 / 3, 1 / 3])
+    ai = np.zeros((3, 3))
+    ai[0, 0] = ai[1, 1] = 0.25
+    ai[2, 0] = ai[2, 1] = ai[2, 2] = 1 / 3
+    wi = np.array([1 / 3, 1 / 3, 1 / 3])
+    return ae, we, ai, wi
+
+
 # ---- parameters ------------------------------------------------------------------------------------
 def default_params(**over):
     """Parameter dictionary (R3, R10, R16, R18 defaults; all damping terms non-zero so they are exercised)."""
@@ -80,6 +97,7 @@ def default_params(**over):
         rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, alpha_bh=0.1, w_max=100.0, rho_max=1.0,
         eps_min=0.0, eps_max=1e3, ye_min=0.0, ye_max=1.0, ye_atmo=0.3, eps_atmo=1e-8, T_atmo=0.1,
         c2p_maxit=100,
+        m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30,
     )
     p.update(over)
     return p
@@ -528,3 +546,60 @@ def config1_tiled(n, **kw):
     base["U"], base["P"] = tile(base["U"]), tile(base["P"])
     base["n"] = (n, n, n)
     return base
+
+
+# ---- config 5: two-star binary-like state + grey M1, 3 species (BASELINE.json configs[4]) ----------------------
+NM1 = 15
+
+
+def config5(n=192, half_width=60.0, separation=45.0, ng=NG, kappa0=1e-6, e_scale=1e-3, crop_on_star=False):
+    """Two Gamma = 2, K = 100, rho_c = 1.28e-3 TOV stars at x = +-separation/2 with Newtonian circular-orbit velocities
+    (+-v along y), conformal factors, lapses and a boost-like shift superposed (psi = 1 + sum (psi_i - 1),
+    alpha = 1 + sum (alpha_i - 1), beta = - sum v_i (1 - alpha_i)); conformally flat, K_ij = 0. Three neutrino species
+    with E = e_scale * scale_s * T^4 (T = p / rho, R27) inside the stars and a floor outside, F_i = 0, N = E.
+    crop_on_star: the patch is centred on one star and n * dx covers 2.2 stellar radii (about 40 % star), the variant
+    SURVEY.md 8(d) asks for so that the stiff-core path is exercised."""
+    K, Gamma, rho_c = 100.0, 2.0, 1.28e-3
+    prof = tov_profile(K, Gamma, rho_c)
+    if crop_on_star:
+        half_width = prof["Rbar"] / 0.92
+        centre = (0.5 * separation, 0.0, 0.0)
+    else:
+        centre = (0.0, 0.0, 0.0)
+    dx = 2.0 * half_width / n
+    x0 = tuple(c - half_width + 0.5 * dx for c in centre)
+    X, Y, Z = mesh(n, n, n, ng, dx, x0=x0)
+    vorb = 0.5 * math.sqrt(2.0 * prof["M"] / separation)
+    par = default_params(eos_gamma=Gamma, rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, m1_kappa0=kappa0)
+    psi, alpha = np.ones_like(X), np.ones_like(X)
+    beta = [np.zeros_like(X) for _ in range(3)]
+    rho, vy = np.zeros_like(X), np.zeros_like(X)
+    for sgn in (+1.0, -1.0):
+        rb = np.sqrt((X - sgn * 0.5 * separation) ** 2 + Y * Y + Z * Z)
+        r_, p_, a_, ps_, _ = tov_fields(prof, rb)
+        psi += ps_ - 1.0
+        alpha += a_ - 1.0
+        beta[1] += -sgn * vorb * (1.0 - a_)
+        rho += r_
+        vy += np.where(r_ > 0.0, sgn * vorb, 0.0)
+    U = _flat_state(X.shape)
+    U[CHI] = psi ** -4
+    U[ALPHA] = alpha
+    for i in range(3):
+        U[BETAX + i] = beta[i]
+    star = rho > 10.0 * par["rho_atmo"]
+    P = np.zeros((NPRIM,) + X.shape)
+    P[RHO] = np.where(star, rho, par["rho_atmo"])
+    P[EPS] = np.where(star, K * np.maximum(rho, 1e-300) ** (Gamma - 1.0) / (Gamma - 1.0), par["eps_atmo"])
+    P[YE] = par["ye_atmo"]
+    P[VX + 1] = np.where(star, vy, 0.0)
+    U[BXBAR + 2] = 1e-6 * np.where(star, rho / rho_c, 0.0)
+    T = np.where(star, (Gamma - 1.0) * P[EPS], 0.0)                 # T = p / rho for the ideal gas
+    V = np.zeros((NM1,) + X.shape)
+    sg = psi ** 6
+    for s in range(3):
+        E = np.maximum(e_scale * par["m1_species_scale"][s] * T ** 4, 1e-20)
+        V[5 * s] = sg * E
+        V[5 * s + 1] = sg * E
+    frac = float(star[ng:-ng, ng:-ng, ng:-ng].mean())
+    return dict(U=U, P=P, V=V, n=(n, n, n), ng=ng, dx=dx, bc=[1] * 6, params=par, star_fraction=frac, tov=prof)

@@ -1,0 +1,179 @@
+"""Pins of the M1 oracle: closure limits and exactness, App. C forms vs Sec. II C, Jacobian vs finite
+differences, implicit-solve limits, flux consistency, IMEX order conditions."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2510_13965_b200 import synth
+
+ID = np.eye(3)
+
+
+def _rand_state(rng, vmax=0.5, metric=True):
+    if metric:
+        A = ID + 0.2 * rng.standard_normal((3, 3))
+        gl = A @ A.T
+    else:
+        gl = ID.copy()
+    gu = np.linalg.inv(gl)
+    v = rng.uniform(-1, 1, 3)
+    v *= rng.uniform(0.05, vmax) / math.sqrt(v @ gl @ v)
+    W = 1.0 / math.sqrt(1.0 - v @ gl @ v)
+    E = 10.0 ** rng.uniform(-8, -2)
+    F = rng.uniform(-1, 1, 3)
+    F *= rng.uniform(0.05, 0.9) * E / math.sqrt(F @ gu @ F)
+    return E, F, v, W, gl, gu
+
+
+def test_closure_limits(oracle_mod):
+    E, F0, v0 = 2.5e-3, np.zeros(3), np.zeros(3)
+    c = oracle_mod.m1_closure_point(E, F0, v0, 1.0, ID, ID)
+    assert c["xi"] == 0.0 and abs(c["chi"] - 1 / 3) < 1e-16 and np.allclose(c["P"], E * ID / 3, rtol=1e-15, atol=0)
+    F = np.array([0.6, -0.48, 0.64]) * E                      # |F| = E
+    c = oracle_mod.m1_closure_point(E, F, v0, 1.0, ID, ID)
+    assert abs(c["xi"] - 1.0) < 1e-12 and abs(c["chi"] - 1.0) < 1e-12
+    assert np.allclose(c["P"], E * np.outer(F, F) / (F @ F), rtol=1e-14, atol=0)
+
+
+def test_closure_exact_in_thick_and_thin_limits(oracle_mod):
+    """Minerbo is exact for radiation isotropic in the fluid frame and for a single beam: build T^ab in flat
+    space from its definition, project with n^a, feed (E, F_i) to the closure and compare J, H, P_ij."""
+    rng = np.random.default_rng(1)
+    for _ in range(20):
+        v = rng.uniform(-0.5, 0.5, 3)
+        W = 1.0 / math.sqrt(1.0 - v @ v)
+        J0 = 10.0 ** rng.uniform(-6, -2)
+        E = 4 / 3 * J0 * W * W - J0 / 3
+        F = 4 / 3 * J0 * W * W * v
+        Pex = 4 / 3 * J0 * W * W * np.outer(v, v) + J0 / 3 * ID
+        c = oracle_mod.m1_closure_point(E, F, v, W, ID, ID)
+        assert c["xi"] < 1e-7 and abs(c["J"] / J0 - 1) < 1e-12 and np.abs(c["H"]).max() < 1e-12 * J0
+        assert np.abs(c["P"] - Pex).max() < 1e-12 * E
+        k = rng.standard_normal(3)
+        k /= np.linalg.norm(k)
+        Eb = 10.0 ** rng.uniform(-6, -2)
+        c = oracle_mod.m1_closure_point(Eb, Eb * k, v, W, ID, ID)
+        assert abs(c["xi"] - 1.0) < 1e-7 and np.abs(c["P"] - Eb * np.outer(k, k)).max() < 1e-7 * Eb
+        assert abs(c["J"] / (W * W * Eb * (1 - k @ v) ** 2) - 1) < 1e-12
+
+
+def test_closure_orthogonality_and_root(oracle_mod):
+    """H^a u_a = 0 (i.e. H.n + H_i v^i = 0) pins the mutual consistency of Eqs. (42)-(44); xi^2 J^2 = H_a H^a at the root."""
+    rng = np.random.default_rng(2)
+    for _ in range(50):
+        E, F, v, W, gl, gu = _rand_state(rng)
+        c = oracle_mod.m1_closure_point(E, F, v, W, gl, gu)
+        assert abs(c["Hn"] + c["H"] @ v) < 1e-13 * E
+        H2 = -c["Hn"] ** 2 + c["H"] @ gu @ c["H"]
+        assert 0.0 < c["xi"] < 1.0 and abs(c["xi"] ** 2 * c["J"] ** 2 - H2) < 1e-12 * E * E
+        assert abs(c["chi"] - (1 / 3 + c["xi"] ** 2 * (6 - 2 * c["xi"] + 6 * c["xi"] ** 2) / 15)) < 1e-15
+        assert np.allclose(c["P"], c["P"].T, rtol=0, atol=1e-18)
+
+
+def test_appC_forms_equal_section2C(oracle_mod):
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        E, F, v, W, gl, gu = _rand_state(rng)
+        c = oracle_mod.m1_closure_point(E, F, v, W, gl, gu)
+        dthin, dthick = 0.5 * (3 * c["chi"] - 1), 1.5 * (1 - c["chi"])
+        J, H = oracle_mod.m1_JH(E, F, v, W, gl, gu, dthin, dthick)
+        assert abs(J / c["J"] - 1) < 1e-12 and np.abs(H - c["H"]).max() < 1e-12 * E
+
+
+def _RV(oracle_mod, V, v, W, gl, gu, dthin, dthick, alpha, ka, ks, eta):
+    J, H = oracle_mod.m1_JH(V[0], V[1:], v, W, gl, gu, dthin, dthick)
+    vl = gl @ v
+    Sn = W * ((eta + ks * J) - (ka + ks) * (V[0] - V[1:] @ v))
+    Si = W * (eta - ka * J) * vl - (ka + ks) * H
+    return alpha * np.concatenate([[Sn], Si])
+
+
+def test_jacobian_matches_finite_differences(oracle_mod):
+    rng = np.random.default_rng(4)
+    for _ in range(10):
+        E, F, v, W, gl, gu = _rand_state(rng)
+        dthick = rng.uniform(0.0, 1.0)
+        dthin = 1.0 - dthick
+        alpha, ka, ks, eta = 0.8, 0.7, 0.4, 0.0          # the Jacobian does not depend on eta; eta >> E would only add rounding noise to the differences
+        Jac = oracle_mod.m1_jacobian(E, F, v, W, gl, gu, dthin, dthick, alpha, ka, ks)
+        V = np.concatenate([[E], F])
+        for j in range(4):
+            h = 1e-6 * E
+            Vp, Vm = V.copy(), V.copy()
+            Vp[j] += h
+            Vm[j] -= h
+            fd = (_RV(oracle_mod, Vp, v, W, gl, gu, dthin, dthick, alpha, ka, ks, eta) -
+                  _RV(oracle_mod, Vm, v, W, gl, gu, dthin, dthick, alpha, ka, ks, eta)) / (2 * h)
+            assert np.abs(fd - Jac[:, j]).max() < 1e-7 * np.abs(Jac).max(), (j, fd, Jac[:, j])
+
+
+def _oracle(oracle_mod, **over):
+    return oracle_mod.Oracle(synth.default_params(**over), 4, 4, 4, 3, 0.1)
+
+
+def test_implicit_solve_limits(oracle_mod):
+    rng = np.random.default_rng(5)
+    E, F, v, W, gl, gu = _rand_state(rng, vmax=0.3)
+    Vs = np.concatenate([[1e-4, E], F])
+    # no interaction: V = V*
+    o = _oracle(oracle_mod, m1_kappa0=0.0)
+    V, R, fl = o.m1_implicit_point(0, Vs, 0.1, 0.9, v, W, 1e-3, 0.02, gl, gu)
+    assert fl == 0 and np.array_equal(V, Vs) and np.all(R == 0.0)
+    # residual of (C13)-(C14) and (C10) at return
+    o = _oracle(oracle_mod, m1_kappa0=5.0)
+    for adt in (1e-3, 0.1, 10.0):
+        V, R, fl = o.m1_implicit_point(0, Vs, adt, 0.9, v, W, 1e-3, 0.3, gl, gu)
+        assert fl == 0
+        assert np.abs(V - Vs - adt * R).max() < 1e-12 * max(E, np.abs(V).max())
+    # v = 0, kappa dt -> infinity: J -> eta / kappa_a, H -> 0 (thermal equilibrium)
+    o = _oracle(oracle_mod, m1_kappa0=1e9)
+    V, R, fl = o.m1_implicit_point(0, Vs, 1.0, 1.0, np.zeros(3), 1.0, 1e-3, 0.3, ID, ID)
+    assert abs(V[1] / 0.3 ** 4 - 1) < 1e-8 and np.abs(V[2:]).max() < 1e-8 * V[1]
+    # v = 0: the system is linear; compare with the direct solve of Eq. (C6)
+    ka = 5.0 * 1.0
+    o = _oracle(oracle_mod, m1_kappa0=5.0)
+    al, adt, T = 0.9, 0.2, 0.3
+    V, R, fl = o.m1_implicit_point(0, Vs, adt, al, np.zeros(3), 1.0, 1e-3, T, ID, ID)
+    Eex = (Vs[1] + adt * al * ka * T ** 4) / (1 + adt * al * ka)          # S_n = eta - kappa_a E  (J = E at v = 0)
+    Fex = Vs[2:] / (1 + adt * al * 2 * ka)                                # S_i = -(kappa_a + kappa_s) F_i
+    assert abs(V[1] / Eex - 1) < 1e-12 and np.abs(V[2:] - Fex).max() < 1e-12 * np.abs(Fex).max()
+    Nex = (Vs[0] + adt * al * ka * T ** 4) / (1 + adt * al * ka)          # Gamma = 1
+    assert abs(V[0] / Nex - 1) < 1e-12
+
+
+def test_m1_rhs_constant_state_and_diffusion_limit(oracle_mod):
+    """Flat space, uniform fluid at rest, uniform radiation: flux divergence and geometric sources vanish exactly;
+    optically thick limit of Eq. (77): A -> 0 gives the centred flux (F_i + F_i+1)/2."""
+    n, ng, dx = 8, 3, 0.1
+    o = oracle_mod.Oracle(synth.default_params(), n, n, n, ng, dx)
+    U = synth._flat_state(o.shape)
+    P = np.zeros((10,) + o.shape)
+    P[synth.RHO], P[synth.WLOR], P[synth.TEMP] = 1e-3, 1.0, 0.01
+    V = np.zeros((15,) + o.shape)
+    for s in range(3):
+        V[5 * s], V[5 * s + 1], V[5 * s + 2] = 1e-4, 1e-5, 2e-6
+    KV = o.m1_rhs(U, P, V)
+    assert np.all(KV == 0.0)
+    # smooth E profile, F = 0, huge opacity: dF_x/dt = -d_x (E/3) with the centred 2nd-order difference
+    o2 = oracle_mod.Oracle(synth.default_params(m1_kappa0=1e12), n, n, n, ng, dx)
+    X = synth.mesh(n, n, n, ng, dx)[0]
+    V[:] = 0.0
+    V[1] = 1e-5 * (1.0 + 0.1 * np.sin(2 * math.pi * X / (n * dx)))
+    V[6] = V[11] = 1e-5
+    KV = o2.m1_rhs(U, P, V)
+    I = (slice(ng, -ng),) * 3
+    ref = -(V[1][:, :, ng + 1:-ng + 1 or None] - V[1][:, :, ng - 1:-ng - 1]) / (2 * dx) / 3.0
+    assert np.abs(KV[2][I] - ref[ng:-ng, ng:-ng]).max() < 1e-12 * np.abs(ref).max()
+
+
+def test_imex_tableau_conditions():
+    """R1: the conditions PAPER.md:389-408 states for the IMEX pair."""
+    ae, we, ai, wi = synth.imex_tableau()
+    ce, ci = ae.sum(axis=1), ai.sum(axis=1)
+    assert np.allclose(np.triu(ae), 0) and np.allclose(np.triu(ai, 1), 0)
+    assert abs(we.sum() - 1) < 1e-15 and abs(wi.sum() - 1) < 1e-15
+    for w in (we, wi):
+        for c in (ce, ci):
+            assert abs(w @ c - 0.5) < 1e-15
+    assert abs(1.0 - wi @ np.linalg.solve(ai, np.ones(3))) < 1e-14      # R(-inf) = 0: L-stable
