@@ -36,6 +36,8 @@ extern "C" {
 #define MHD_NSTATE 32
 #define MHD_NPRIM 10
 #define MHD_NWORK 33        /* 3 directions x (10 flux brackets of Eq. 32 + 1 speed bound of App. B) */
+#define MHD_NM1 15          /* (Nbar, Ebar, Fbar_i) x 3 neutrino species, field 5 s + {0..4} */
+#define MHD_NM1WORK 75      /* per species: 3 directions x (5 flux brackets + speed), kappa_a + kappa_s, P_ij */
 #define MHD_MAX_STAGES 8
 #define MHD_MAX_PIECES 8
 
@@ -47,7 +49,13 @@ enum {
   MHD_SLOT_FLAGS = 3,  /* uint8 flags, one field                                             */
   MHD_SLOT_WORK = 4,   /* scratch of mhd_rhs: pointwise fluxes and speeds (MHD_NWORK fields) */
   MHD_SLOT_K1 = 5,     /* K_1 ... K_s = F(U^(j)): MHD_SLOT_K1 + j - 1    (MHD_NSTATE fields) */
-  MHD_NSLOTS = 5 + MHD_MAX_STAGES
+  /* M1 (n_species = 3) */
+  MHD_SLOT_V = 5 + MHD_MAX_STAGES,        /* neutrino fields of the current stage            (MHD_NM1 fields)     */
+  MHD_SLOT_V0,                            /* V^n                                             (MHD_NM1 fields)     */
+  MHD_SLOT_M1WORK,                        /* scratch of mhd_m1_rhs                           (MHD_NM1WORK fields) */
+  MHD_SLOT_KV1,                           /* explicit parts F_V(U^(j)): MHD_SLOT_KV1 + j - 1 (MHD_NM1 fields)     */
+  MHD_SLOT_R1 = MHD_SLOT_KV1 + MHD_MAX_STAGES,   /* stiff sources R_V(U^(j)): MHD_SLOT_R1 + j - 1 (MHD_NM1 fields) */
+  MHD_NSLOTS = MHD_SLOT_R1 + MHD_MAX_STAGES
 };
 
 /* flag bits: error policy of PAPER.md:1157-1162 */
@@ -59,7 +67,7 @@ enum {
   MHD_FLAG_YE = 16,      /* rule 6: Ye reset                               */
   MHD_FLAG_FATAL = 32,   /* rules 2, 4-6 outside low-density / BH regions  */
   MHD_FLAG_NOCONV = 64,  /* a root find hit the iteration cap              */
-  MHD_FLAG_M1FIX = 128   /* reserved: M1 fix-up                            */
+  MHD_FLAG_M1FIX = 128   /* M1: E floored or |F| limited to E (reading R22) */
 };
 
 enum {
@@ -74,7 +82,7 @@ enum {
 typedef struct {
   int nx, ny, nz, ng;              /* interior points per axis; ghost width (>= 3: MP5/KO/advective stencils) */
   double dx, dy, dz;               /* uniform spacing */
-  int n_species;                   /* 0 (M1 off); 3 is reserved */
+  int n_species;                   /* 0 (M1 off) or 3 (grey M1: nu_e, anti-nu_e, nu_x) */
   /* EoS: 0 ideal gas p=(Gamma-1) rho eps; 1 hybrid piecewise polytrope (Eqs. 30-31); 2 table */
   int eos_kind;
   double eos_gamma;                /* kind 0 */
@@ -98,7 +106,7 @@ typedef struct {
   /* M1 (n_species = 3): synthetic grey opacities kappa_a = kappa_s = m1_kappa0 (rho / m1_rho0)^2 m1_species_scale[s],
    * eta = kappa_a T^4 (BASELINE.json configs[4]); energy floor, Newton tolerance / cap of App. C, baryon mass of l.316 */
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
-  int m1_maxit;
+  int m1_maxit, m1_odd_even;       /* m1_odd_even != 0: the A := 1 switch against odd-even decoupling (l.565-570) */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */
@@ -159,6 +167,22 @@ int mhd_advance(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, 
 int mhd_advance_host(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps,
                      double *host_U, uint8_t *host_flags, void *cuda_stream);
 
+/* ---- M1 (Sec. II C, III D, App. B, C); all need n_species = 3 ----
+ * a12 (+a10) — pointwise implicit solve at every grid point (App. C, Eqs. C10-C35): slot_V holds V* (densitised) on entry and
+ * V^(i) on exit; slot_R receives the densitised stiff source alpha sqrt(gamma) (C, S_n, S_i) evaluated at V^(i); adt = a_ii dt.
+ * Needs slot U (metric) and P (v^i, W, rho, T) consistent; ORs MHD_FLAG_M1FIX / MHD_FLAG_NOCONV into slot FLAGS. */
+int mhd_m1_implicit(mhd_patch *p, int slot_V, int slot_R, double adt, void *cuda_stream);
+/* a11 (+a10) — explicit part of Eqs. (38)-(40) on the interior: closure at every point, fluxes of Eqs. (77)-(78), geometric
+ * sources; slot_KV <- F_V. Needs filled ghosts in slot_V and slot U, primitives at all points, MHD_SLOT_M1WORK bound. */
+int mhd_m1_rhs(mhd_patch *p, int slot_V, int slot_KV, void *cuda_stream);
+/* a8 (M1 part) — neutrino back-reaction on the fluid: slot_K[taubar, Sbar_i] -= sum_species slot_R[Ebar, Fbar_i],
+ * slot_K[DYebar] -= m_b (R[Nbar]_nue - R[Nbar]_anti-nue), interior. */
+int mhd_m1_backreaction(mhd_patch *p, int slot_R, int slot_K, void *cuda_stream);
+/* n_steps full IMEX steps (Eq. 53, App. C steps C3-C4) of the coupled system, device resident; the tableau must carry
+ * a_impl (row-major, lower triangular incl. diagonal) and w_impl. Per stage: combine -> fill -> con2prim -> implicit solve ->
+ * rhs + back-reaction -> M1 explicit part. */
+int mhd_advance_imex(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
+
 /* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */
 int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_stream);
 
@@ -166,8 +190,9 @@ int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_s
  * mhd_patch_profile(p, 1) starts collecting, (p, 0) stops. mhd_patch_profile_read synchronises the stream, adds up
  * the elapsed milliseconds and launch counts per kernel class since the last read, and resets them.
  * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 algebra (+ fluid sources), 3 reconstruction x, 4 y, 5 z, 6 rk combine / copy,
- * 7 pointwise fluxes, 8 advection + Kreiss-Oliger. */
-#define MHD_NKERNELS 9
+ * 7 pointwise fluxes, 8 advection + Kreiss-Oliger, 9 M1 closure + pointwise fluxes, 10 M1 flux divergence + sources,
+ * 11 M1 implicit solve + back-reaction. */
+#define MHD_NKERNELS 12
 int mhd_patch_profile(mhd_patch *p, int enable);
 int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void *cuda_stream);
 

@@ -77,7 +77,7 @@ struct Params {
   // M1 (config 5): synthetic opacities kappa_a = kappa_s = m1_kappa0 (rho / m1_rho0)^2 * m1_species_scale[s],
   // eta = kappa_a T^4 (BASELINE.json configs[4]); number opacities kappa_a^0 = kappa_a, eta^0 = eta (synthetic)
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
-  int m1_maxit;
+  int m1_maxit, m1_odd_even;   // m1_odd_even: apply the A := 1 switch of l.565-570
 };
 
 // ---- stencils (Sec. III B)

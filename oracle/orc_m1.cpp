@@ -57,7 +57,7 @@ M1Closure m1_closure_point(double E, const double F[3], const double vu[3], doub
   raise(gu, F, Fu);
   lower(gl, vu, vl);
   double F2 = dot_ud(Fu, F);
-  if (F2 < 1e-60) F2 = 0.0;                                                                               // R22: f^ = 0
+  if (F2 < 1e-30 * E * E) F2 = 0.0;                                                                       // R22: f^ = 0 for |F| < 1e-15 E
   auto R = [&](double xi) {                                                                               // Eq. (50)
     moments_for_chi(eddington(xi), E, F, Fu, F2, vu, vl, W, gl, c);
     double Hu[3];
@@ -92,7 +92,7 @@ void m1_JH_appC(double E, const double F[3], const double vu[3], double W, const
   const double W2 = W * W, v2 = dot_ud(vu, vl), vF = dot_ud(vu, F);
   double F2 = dot_ud(Fu, F);
   double fh[3] = {0, 0, 0};
-  if (F2 >= 1e-60) { const double Fn = std::sqrt(F2); for (int i = 0; i < 3; ++i) fh[i] = F[i] / Fn; }
+  if (F2 >= 1e-30 * E * E) { const double Fn = std::sqrt(F2); for (int i = 0; i < 3; ++i) fh[i] = F[i] / Fn; }
   const double vf = dot_ud(vu, fh);
   const double B0 = W2 * (E - 2.0 * vF);                                                                  // (C19)
   const double Bthin = W2 * E * vf * vf;                                                                  // (C20)
@@ -114,7 +114,7 @@ void m1_jacobian(double E, const double F[3], const double vu[3], double W, cons
   const double W2 = W * W, W3 = W2 * W, v2 = dot_ud(vu, vl), kas = ka + ks;
   double F2 = dot_ud(Fu, F);
   double fh[3] = {0, 0, 0}, fhu[3] = {0, 0, 0}, iF = 0.0;
-  if (F2 >= 1e-60) { const double Fn = std::sqrt(F2); iF = 1.0 / Fn; for (int i = 0; i < 3; ++i) { fh[i] = F[i] / Fn; fhu[i] = Fu[i] / Fn; } }
+  if (F2 >= 1e-30 * E * E) { const double Fn = std::sqrt(F2); iF = 1.0 / Fn; for (int i = 0; i < 3; ++i) { fh[i] = F[i] / Fn; fhu[i] = Fu[i] / Fn; } }
   const double vf = dot_ud(vu, fh);
   const double dJdE = W2 + dthin * vf * vf * W2 + dthick * (3.0 - 2.0 * W2) * (W2 - 1.0) / (1.0 + 2.0 * W2);        // (C32)
   double dJdF[3], dHdE[3], dHdF[3][3];
@@ -200,7 +200,9 @@ uint8_t m1_implicit_point(const Params& par, int species, const double Vstar[5],
     stiff_terms(E, F, vu, W, gl, gu, dthin, dthick, alpha, ka, ks, eta, S, J);
     double G[4] = {E - Es - adt * S[0], F[0] - Fs[0] - adt * S[1], F[1] - Fs[1] - adt * S[2], F[2] - Fs[2] - adt * S[3]};   // (C13)-(C14)
     const double gn = std::max(std::max(std::fabs(G[0]), std::fabs(G[1])), std::max(std::fabs(G[2]), std::fabs(G[3])));
-    if (gn <= par.m1_tol * std::max(Es, par.m1_efloor)) { conv = true; break; }
+    // R21: the residual is measured against the size of the terms it is made of: E* and the stiff terms a_ii dt alpha W (eta, kappa_as E),
+    // whose rounding error bounds what Newton can reach when kappa dt >> 1
+    if (gn <= par.m1_tol * (std::max(Es, par.m1_efloor) + adt * alpha * W * (eta + (ka + ks) * std::max(Es, E)))) { conv = true; break; }
     double Jac[4][4], M[4][4];
     m1_jacobian(E, F, vu, W, gl, gu, dthin, dthick, alpha, ka, ks, Jac);
     for (int r = 0; r < 4; ++r) for (int q = 0; q < 4; ++q) M[r][q] = (r == q ? 1.0 : 0.0) - adt * Jac[r][q];               // (C16)

@@ -60,7 +60,7 @@ void m1_flux_point(const GeoPt& q, const double u[5], int d, double F[5], double
   // (B5); R32: the second candidate E |F^d| / F_k F^k equals the first when |F| = E (free streaming) but diverges for
   // |F| << E, where d_thin does not vanish if the fluid moves; no signal outruns light, so the bracket is capped at
   // the coordinate light speed sqrt(gamma^dd)
-  if (F2 >= 1e-60) thin += q.al * std::min(std::max(std::fabs(Fu[d]) / std::sqrt(F2), E * std::fabs(Fu[d]) / F2), std::sqrt(q.gu[d][d]));
+  if (F2 >= 1e-30 * E * E) thin += q.al * std::min(std::max(std::fabs(Fu[d]) / std::sqrt(F2), E * std::fabs(Fu[d]) / F2), std::sqrt(q.gu[d][d]));
   const double thick = std::fabs(q.be[d]) + q.al * std::max((2.0 * W2 * std::fabs(q.vu[d]) + std::sqrt(std::max((2.0 * W2 + 1.0) * q.gu[d][d] - 2.0 * W2 * q.vu[d] * q.vu[d], 0.0))) / (2.0 * W2 + 1.0),
                                                            std::fabs(q.vu[d]));                       // (B5)
   lam = 0.5 * (3.0 * c.chi - 1.0) * thin + 1.5 * (1.0 - c.chi) * thick;                                 // (B4)
@@ -106,7 +106,10 @@ void m1_rhs(const Params& par, const Grid& G, const double* U, const double* P, 
           const double dm = u[i] - u[i - 1], d0 = u[i + 1] - u[i], dp = u[i + 2] - u[i + 1];
           const double Phi = d0 == 0.0 ? 1.0 : std::max(0.0, std::min(1.0, std::min(2.0 * dm / d0, 2.0 * dp / d0)));   // Eq. (78), R20
           double A = A0;
-          if (dm * d0 < 0.0 && d0 * dp < 0.0) A = 1.0;              // odd-even decoupling, l.565-570
+          // odd-even decoupling, l.565-570. R33: the three differences must all exceed 1e-10 of the local magnitude —
+          // a zigzag of rounding noise on a flat profile is not an oscillation (and would make the switch irreproducible)
+          const double tiny = 1e-10 * std::max(std::max(std::fabs(u[i - 1]), std::fabs(u[i])), std::max(std::fabs(u[i + 1]), std::fabs(u[i + 2])));
+          if (par.m1_odd_even && dm * d0 < 0.0 && d0 * dp < 0.0 && std::min(std::min(std::fabs(dm), std::fabs(d0)), std::fabs(dp)) > tiny) A = 1.0;
           const double FHO = 0.5 * (F[i] + F[i + 1]);
           const double FLO = FHO - 0.5 * l * d0;                    // R20
           Fhat[f * (Md + 1) + i] = FHO - A * (1.0 - Phi) * (FHO - FLO);                                                 // Eq. (77)

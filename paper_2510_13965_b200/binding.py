@@ -15,6 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 
 NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
 SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
+NM1, NM1WORK = 15, 75
+SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1 = 13, 14, 15, 16, 24
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p
@@ -38,7 +40,7 @@ class mhd_patch_desc(ctypes.Structure):
         ("eps_min", _d), ("eps_max", _d), ("ye_min", _d), ("ye_max", _d), ("ye_atmo", _d), ("eps_atmo", _d), ("T_atmo", _d),
         ("c2p_maxit", _i),
         ("m1_kappa0", _d), ("m1_rho0", _d), ("m1_species_scale", _d * 3), ("m1_efloor", _d), ("m1_tol", _d), ("m1_mb", _d),
-        ("m1_maxit", _i),
+        ("m1_maxit", _i), ("m1_odd_even", _i),
     ]
 
 
@@ -53,9 +55,11 @@ class mhd_status(ctypes.Structure):
 
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
-           "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror"]
-NKERNELS = 9
-KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko"]
+           "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
+           "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_advance_imex"]
+NKERNELS = 12
+KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
+                  "m1_point", "m1_div", "m1_implicit"]
 
 _lib = None
 
@@ -85,6 +89,10 @@ def lib():
         L.mhd_probe_fp64_flops.argtypes = [_p]
         L.mhd_probe_fp64_flops.restype = _d
         L.mhd_strerror.argtypes = [_i]
+        L.mhd_m1_implicit.argtypes = [_p, _i, _i, _d, _p]
+        L.mhd_m1_rhs.argtypes = [_p, _i, _i, _p]
+        L.mhd_m1_backreaction.argtypes = [_p, _i, _i, _p]
+        L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
         if L.mhd_desc_sizeof() != ctypes.sizeof(mhd_patch_desc):
             raise RuntimeError("mhd_patch_desc layout mismatch between include/mhd.h and binding.py")
@@ -101,12 +109,12 @@ def _check(rc):
         raise MhdError("libmhd_b200: %s (%d)" % (lib().mhd_strerror(rc).decode(), rc))
 
 
-def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, table=None):
+def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, table=None, n_species=0):
     """Marshal a parameter dictionary (paper_2510_13965_b200.synth.default_params) into mhd_patch_desc."""
     d = mhd_patch_desc()
     d.nx, d.ny, d.nz, d.ng = nx, ny, nz, ng
     d.dx, d.dy, d.dz = dx, dx if dy is None else dy, dx if dz is None else dz
-    d.n_species = 0
+    d.n_species = n_species
     names = {f[0] for f in mhd_patch_desc._fields_}
     for k, v in params.items():
         if k not in names:
@@ -115,7 +123,7 @@ def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, tab
             arr = getattr(d, k)
             for i, x in enumerate(v):
                 arr[i] = float(x)
-        elif k in ("eos_kind", "n_pieces", "c2p_maxit", "m1_maxit"):
+        elif k in ("eos_kind", "n_pieces", "c2p_maxit", "m1_maxit", "m1_odd_even"):
             setattr(d, k, int(v))
         else:
             setattr(d, k, float(v))
@@ -128,13 +136,18 @@ def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, tab
     return d
 
 
-def make_tableau(a_expl, w_expl):
+def make_tableau(a_expl, w_expl, a_impl=None, w_impl=None):
     a = np.ascontiguousarray(a_expl, dtype=np.float64)
     w = np.ascontiguousarray(w_expl, dtype=np.float64)
     t = mhd_tableau()
     t.stages = len(w)
     t.a_expl, t.w_expl, t.a_impl, t.w_impl = a.ctypes.data, w.ctypes.data, None, None
     t._keep = (a, w)
+    if a_impl is not None:
+        ai = np.ascontiguousarray(a_impl, dtype=np.float64)
+        wi = np.ascontiguousarray(w_impl, dtype=np.float64)
+        t.a_impl, t.w_impl = ai.ctypes.data, wi.ctypes.data
+        t._keep = (a, w, ai, wi)
     return t
 
 
@@ -185,6 +198,22 @@ def mhd_advance_host(h, tableau, bc, dt, n_steps, host_U_ptr, host_flags_ptr=Non
     _check(lib().mhd_advance_host(h, ctypes.byref(tableau), _bc(bc), dt, n_steps, host_U_ptr, host_flags_ptr, stream))
 
 
+def mhd_m1_implicit(h, slot_V, slot_R, adt, stream=None):
+    _check(lib().mhd_m1_implicit(h, slot_V, slot_R, adt, stream))
+
+
+def mhd_m1_rhs(h, slot_V, slot_KV, stream=None):
+    _check(lib().mhd_m1_rhs(h, slot_V, slot_KV, stream))
+
+
+def mhd_m1_backreaction(h, slot_R, slot_K, stream=None):
+    _check(lib().mhd_m1_backreaction(h, slot_R, slot_K, stream))
+
+
+def mhd_advance_imex(h, tableau, bc, dt, n_steps, stream=None):
+    _check(lib().mhd_advance_imex(h, ctypes.byref(tableau), _bc(bc), dt, n_steps, stream))
+
+
 def mhd_patch_status(h, slot_flags=SLOT_FLAGS, stream=None):
     st = mhd_status()
     _check(lib().mhd_patch_status(h, slot_flags, ctypes.byref(st), stream))
@@ -209,7 +238,7 @@ def mhd_probe_fp64_flops(stream=None):
 class Patch:
     """Owns the torch device tensors of one patch and binds them to the library's slots."""
 
-    def __init__(self, params, n, ng, dx, stages=4, table=None, device="cuda:0"):
+    def __init__(self, params, n, ng, dx, stages=4, table=None, device="cuda:0", m1=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libmhd_b200 needs a CUDA device; there is no CPU fallback")
@@ -226,7 +255,7 @@ class Patch:
             self._table_t = [torch.as_tensor(np.ascontiguousarray(table[k], dtype=np.float64), device=self.device)
                              for k in ("logp", "loge", "cs2")]
             ptrs = [t.data_ptr() for t in self._table_t]
-        self.desc = make_desc(params, nx, ny, nz, ng, dx, table_ptrs=ptrs, table=table)
+        self.desc = make_desc(params, nx, ny, nz, ng, dx, table_ptrs=ptrs, table=table, n_species=3 if m1 else 0)
         self.h = mhd_patch_create(self.desc)
         z = lambda nf, dt=torch.float64: torch.zeros((nf,) + self.shape, dtype=dt, device=self.device)
         self.U, self.U0, self.P = z(NSTATE), z(NSTATE), z(NPRIM)
@@ -236,6 +265,28 @@ class Patch:
         for slot, t in [(SLOT_U, self.U), (SLOT_U0, self.U0), (SLOT_P, self.P), (SLOT_FLAGS, self.flags), (SLOT_WORK, self.work)] + \
                        [(SLOT_K1 + j, k) for j, k in enumerate(self.K)]:
             mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
+        if m1:                                              # grey M1, 3 species: V, V^n, per-stage explicit parts and stiff sources
+            self.V, self.V0, self.m1work = z(NM1), z(NM1), z(NM1WORK)
+            self.KV = [z(NM1) for _ in range(stages)]
+            self.R = [z(NM1) for _ in range(stages)]
+            for slot, t in [(SLOT_V, self.V), (SLOT_V0, self.V0), (SLOT_M1WORK, self.m1work)] + \
+                           [(SLOT_KV1 + j, k) for j, k in enumerate(self.KV)] + [(SLOT_R1 + j, k) for j, k in enumerate(self.R)]:
+                mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
+
+    def m1_implicit(self, adt, j=1):
+        """V* -> V^(i) in place; stiff source to R_j"""
+        mhd_m1_implicit(self.h, SLOT_V, SLOT_R1 + j - 1, adt, self.stream())
+        return self.R[j - 1]
+
+    def m1_rhs(self, j=1):
+        mhd_m1_rhs(self.h, SLOT_V, SLOT_KV1 + j - 1, self.stream())
+        return self.KV[j - 1]
+
+    def m1_backreaction(self, j=1):
+        mhd_m1_backreaction(self.h, SLOT_R1 + j - 1, SLOT_K1 + j - 1, self.stream())
+
+    def advance_imex(self, tableau, bc, dt, n_steps):
+        mhd_advance_imex(self.h, tableau, bc, dt, n_steps, self.stream())
 
     def close(self):
         if getattr(self, "h", None) is not None:

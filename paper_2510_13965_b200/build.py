@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd_b200.so")
-SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": [], "ccz4.cu": [], "flux.cu": []}
+SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": [], "ccz4.cu": [], "flux.cu": [], "m1.cu": []}
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC"]
 
 
@@ -21,7 +21,7 @@ def _newer(target, deps):
 
 
 def build(force=False, verbose=False):
-    headers = [os.path.join(CSRC, "mhd_internal.cuh"), os.path.join(HERE, "..", "include", "mhd.h"), os.path.abspath(__file__)]
+    headers = [os.path.join(CSRC, "mhd_internal.cuh"), os.path.join(CSRC, "rootfind.cuh"), os.path.join(HERE, "..", "include", "mhd.h"), os.path.abspath(__file__)]
     objs, jobs = [], []
     for src, extra in SOURCES.items():
         s = os.path.join(CSRC, src)

@@ -12,10 +12,13 @@ int slot_fields(int slot) {
   if (slot == MHD_SLOT_P) return MHD_NPRIM;
   if (slot == MHD_SLOT_FLAGS) return 1;
   if (slot == MHD_SLOT_WORK) return MHD_NWORK;
+  if (slot == MHD_SLOT_M1WORK) return MHD_NM1WORK;
+  if (slot >= MHD_SLOT_V) return MHD_NM1;
   return MHD_NSTATE;
 }
 bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLOTS && p->slot[slot].ptr != nullptr; }
-bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || (slot >= MHD_SLOT_K1 && slot < MHD_NSLOTS); }
+bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || (slot >= MHD_SLOT_K1 && slot < MHD_SLOT_K1 + MHD_MAX_STAGES); }
+bool is_m1_slot(int slot) { return slot >= MHD_SLOT_V && slot < MHD_NSLOTS && slot != MHD_SLOT_M1WORK; }
 double* dptr(const mhd_patch* p, int slot) { return (double*)p->slot[slot].ptr; }
 
 // piecewise-polytrope continuity constants: K_i, a_i for i > 0
@@ -90,7 +93,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (!desc || !out) return MHD_E_ARG;
   if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1 || desc->ng < 3) return MHD_E_ARG;
   if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
-  if (desc->n_species != 0) return MHD_E_UNSUPPORTED;
+  if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
   if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2)) return MHD_E_ARG;
@@ -123,6 +126,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.m1_kappa0 = desc->m1_kappa0; q.m1_rho0 = desc->m1_rho0 > 0.0 ? desc->m1_rho0 : 1.0; q.m1_efloor = desc->m1_efloor;
   q.m1_tol = desc->m1_tol > 0.0 ? desc->m1_tol : 1e-13; q.m1_mb = desc->m1_mb; q.m1_maxit = desc->m1_maxit > 0 ? desc->m1_maxit : 30;
   for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
+  q.m1_odd_even = desc->m1_odd_even;
   p->d_counts = nullptr;
   if (cudaMalloc(&p->d_counts, 8 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   *out = p;
@@ -240,6 +244,99 @@ int mhd_advance_host(mhd_patch* p, const mhd_tableau* t, const int bc[6], double
   }
   if (host_flags && cudaMemcpyAsync(host_flags, p->slot[MHD_SLOT_FLAGS].ptr, n, cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
   return cudaStreamSynchronize(s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_m1_implicit(mhd_patch* p, int slot_V, int slot_R, double adt, void* stream) {
+  if (!p || !is_m1_slot(slot_V) || !is_m1_slot(slot_R) || slot_V == slot_R || !(adt >= 0.0)) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  if (!slot_ok(p, slot_V) || !slot_ok(p, slot_R) || !slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_P) || !slot_ok(p, MHD_SLOT_FLAGS)) return MHD_E_UNBOUND;
+  Timed tm(p, 11, (cudaStream_t)stream);
+  return launch_m1_implicit(p->dims, p->par, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, dptr(p, MHD_SLOT_P), p->slot[MHD_SLOT_P].stride,
+                            dptr(p, slot_V), p->slot[slot_V].stride, dptr(p, slot_R), p->slot[slot_R].stride, adt,
+                            (uint8_t*)p->slot[MHD_SLOT_FLAGS].ptr, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_m1_rhs(mhd_patch* p, int slot_V, int slot_KV, void* stream) {
+  if (!p || !is_m1_slot(slot_V) || !is_m1_slot(slot_KV) || slot_V == slot_KV) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  if (!slot_ok(p, slot_V) || !slot_ok(p, slot_KV) || !slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_P) || !slot_ok(p, MHD_SLOT_M1WORK)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  const double* U = dptr(p, MHD_SLOT_U);
+  const size_t su = p->slot[MHD_SLOT_U].stride, sw = p->slot[MHD_SLOT_M1WORK].stride;
+  { Timed tm(p, 9, s);
+    if (launch_m1_point(p->dims, p->par, U, su, dptr(p, MHD_SLOT_P), p->slot[MHD_SLOT_P].stride, dptr(p, slot_V), p->slot[slot_V].stride,
+                        dptr(p, MHD_SLOT_M1WORK), sw, s) != cudaSuccess) return MHD_E_CUDA; }
+  Timed tm(p, 10, s);
+  return launch_m1_div(p->dims, p->par, U, su, dptr(p, slot_V), p->slot[slot_V].stride, dptr(p, MHD_SLOT_M1WORK), sw, dptr(p, slot_KV), p->slot[slot_KV].stride, s)
+         == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_m1_backreaction(mhd_patch* p, int slot_R, int slot_K, void* stream) {
+  if (!p || !is_m1_slot(slot_R) || !is_state_slot(slot_K)) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  if (!slot_ok(p, slot_R) || !slot_ok(p, slot_K)) return MHD_E_UNBOUND;
+  Timed tm(p, 11, (cudaStream_t)stream);
+  return launch_m1_backreact(p->dims, p->par, dptr(p, slot_R), p->slot[slot_R].stride, dptr(p, slot_K), p->slot[slot_K].stride, (cudaStream_t)stream)
+         == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+// V <- V0 + dt (sum_j ce[j] KV_j + sum_j ci[j] R_j), j < nj
+static int m1_combine(mhd_patch* p, int nj, const double* ce, const double* ci, double dt, cudaStream_t s) {
+  const double* Kp[MHD_MAX_STAGES];
+  size_t sk[MHD_MAX_STAGES];
+  double c[MHD_MAX_STAGES];
+  int nk = 0;
+  for (int pass = 0; pass < 2; ++pass)
+    for (int j = 0; j < nj; ++j) {
+      const double cj = pass == 0 ? ce[j] : ci[j];
+      if (cj == 0.0) continue;
+      const int slot = (pass == 0 ? MHD_SLOT_KV1 : MHD_SLOT_R1) + j;
+      if (!slot_ok(p, slot)) return MHD_E_UNBOUND;
+      if (nk == MHD_MAX_STAGES) return MHD_E_ARG;
+      Kp[nk] = dptr(p, slot); sk[nk] = p->slot[slot].stride; c[nk] = cj; ++nk;
+    }
+  Timed tm(p, 6, s);
+  if (nk == 0)
+    return launch_copy_fields(p->dims, MHD_NM1, dptr(p, MHD_SLOT_V), p->slot[MHD_SLOT_V].stride, dptr(p, MHD_SLOT_V0), p->slot[MHD_SLOT_V0].stride, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+  return launch_rk_combine(p->dims, MHD_NM1, dptr(p, MHD_SLOT_V), p->slot[MHD_SLOT_V].stride, dptr(p, MHD_SLOT_V0), p->slot[MHD_SLOT_V0].stride,
+                           nk, Kp, sk, c, dt, s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_advance_imex(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, void* stream) {
+  if (!p || !t || !bc || n_steps < 0 || !t->a_expl || !t->w_expl || !t->a_impl || !t->w_impl || t->stages < 1 || t->stages > MHD_MAX_STAGES) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  for (int sl : {MHD_SLOT_U, MHD_SLOT_U0, MHD_SLOT_P, MHD_SLOT_FLAGS, MHD_SLOT_V, MHD_SLOT_V0}) if (!slot_ok(p, sl)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int q = t->stages;
+  int rc;
+#define CK(call) if ((rc = (call)) != MHD_OK) return rc
+  for (int step = 0; step < n_steps; ++step) {
+    CK(mhd_fill_ghosts(p, MHD_SLOT_U, bc, s));
+    CK(mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s));
+    CK(mhd_fill_ghosts(p, MHD_SLOT_V, bc, s));
+    CK(mhd_rk_stage(p, t, 0, dt, s));                                                    // U0 <- U
+    { Timed tm(p, 6, s);
+      if (launch_copy_fields(p->dims, MHD_NM1, dptr(p, MHD_SLOT_V0), p->slot[MHD_SLOT_V0].stride, dptr(p, MHD_SLOT_V), p->slot[MHD_SLOT_V].stride, s) != cudaSuccess) return MHD_E_CUDA; }
+    for (int st = 0; st < q; ++st) {
+      if (st > 0) {                                                                      // explicit intermediate values (C3)
+        CK(mhd_rk_stage(p, t, st, dt, s));
+        CK(m1_combine(p, st, t->a_expl + (size_t)st * q, t->a_impl + (size_t)st * q, dt, s));
+        CK(mhd_fill_ghosts(p, MHD_SLOT_U, bc, s));
+        CK(mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s));
+        CK(mhd_fill_ghosts(p, MHD_SLOT_V, bc, s));
+      }
+      CK(mhd_m1_implicit(p, MHD_SLOT_V, MHD_SLOT_R1 + st, t->a_impl[(size_t)st * q + st] * dt, s));   // (C4)
+      CK(mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st, s));
+      CK(mhd_m1_backreaction(p, MHD_SLOT_R1 + st, MHD_SLOT_K1 + st, s));
+      CK(mhd_m1_rhs(p, MHD_SLOT_V, MHD_SLOT_KV1 + st, s));
+    }
+    CK(mhd_rk_stage(p, t, q, dt, s));
+    CK(m1_combine(p, q, t->w_expl, t->w_impl, dt, s));
+  }
+  CK(mhd_fill_ghosts(p, MHD_SLOT_U, bc, s));
+  CK(mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s));
+  return mhd_fill_ghosts(p, MHD_SLOT_V, bc, s);
+#undef CK
 }
 
 int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream) {

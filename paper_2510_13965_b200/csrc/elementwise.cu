@@ -69,15 +69,13 @@ struct RkArgs {
 };
 
 template <int NK>
-__global__ void __launch_bounds__(128) k_rk_combine(Dims d, double* __restrict__ Uout, size_t so,
+__global__ void __launch_bounds__(128) k_rk_combine(Dims d, int nfields, double* __restrict__ Uout, size_t so,
                                                     const double* __restrict__ U0, size_t s0, RkArgs a) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.nx) return;
   const size_t p = (size_t)(blockIdx.z + d.ng) * d.sz + (size_t)(blockIdx.y + d.ng) * d.sy + (i + d.ng);
-  const int f = threadIdx.y + blockDim.y * 0;   // fields are looped below
-  (void)f;
 #pragma unroll 4
-  for (int fld = 0; fld < MHD_NSTATE; ++fld) {
+  for (int fld = 0; fld < nfields; ++fld) {
     double acc = 0.0;
 #pragma unroll
     for (int m = 0; m < NK; ++m) acc = fma(a.c[m], __ldg(a.K[m] + (size_t)fld * a.sk[m] + p), acc);
@@ -87,13 +85,12 @@ __global__ void __launch_bounds__(128) k_rk_combine(Dims d, double* __restrict__
 
 cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
                               int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s) {
-  (void)nfields;
   RkArgs a;
   a.nk = nk;
   for (int m = 0; m < nk; ++m) { a.K[m] = K[m]; a.sk[m] = sk[m]; a.c[m] = dt * coef[m]; }
   dim3 grid((d.nx + 127) / 128, d.ny, d.nz), block(128);
   switch (nk) {
-#define CASE(N) case N: k_rk_combine<N><<<grid, block, 0, s>>>(d, Uout, so, U0, s0, a); break;
+#define CASE(N) case N: k_rk_combine<N><<<grid, block, 0, s>>>(d, nfields, Uout, so, U0, s0, a); break;
     CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
 #undef CASE
     default: return cudaErrorInvalidValue;

@@ -36,7 +36,7 @@ struct Par {
   double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
   int c2p_maxit;
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
-  int m1_maxit;
+  int m1_maxit, m1_odd_even;
 };
 
 struct Slot {
@@ -73,4 +73,11 @@ cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t s
 cudaError_t launch_copy_fields(const Dims& d, int nfields, double* dst, size_t sd, const double* src, size_t ss, cudaStream_t s);
 cudaError_t launch_count_flags(const Dims& d, const uint8_t* flags, unsigned long long* counts, cudaStream_t s);
 double probe_fp64(cudaStream_t s);
+cudaError_t launch_m1_point(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, const double* V, size_t sv,
+                            double* Wk, size_t sw, cudaStream_t s);
+cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
+                          double* KV, size_t sk, cudaStream_t s);
+cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* V, size_t sv,
+                               double* R, size_t sr, double adt, uint8_t* flags, cudaStream_t s);
+cudaError_t launch_m1_backreact(const Dims& d, const Par& par, const double* R, size_t sr, double* K, size_t sk, cudaStream_t s);
 }  // namespace mhd

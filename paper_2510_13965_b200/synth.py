@@ -97,7 +97,7 @@ def default_params(**over):
         rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, alpha_bh=0.1, w_max=100.0, rho_max=1.0,
         eps_min=0.0, eps_max=1e3, ye_min=0.0, ye_max=1.0, ye_atmo=0.3, eps_atmo=1e-8, T_atmo=0.1,
         c2p_maxit=100,
-        m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30,
+        m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30, m1_odd_even=1,
     )
     p.update(over)
     return p

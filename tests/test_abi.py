@@ -42,7 +42,7 @@ def test_argument_errors_without_gpu(built_lib):
     assert L.mhd_patch_create(ctypes.byref(d), ctypes.byref(h)) == -1
     assert L.mhd_patch_create(None, ctypes.byref(h)) == -1
     d = binding.make_desc(synth.default_params(), 8, 8, 8, 3, 0.1)
-    d.n_species = 3
+    d.n_species = 2                                                      # only 0 (M1 off) and 3 are built
     assert L.mhd_patch_create(ctypes.byref(d), ctypes.byref(h)) == -4
 
 

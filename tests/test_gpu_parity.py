@@ -363,3 +363,90 @@ def test_config4_full_size_sampled_parity(oracle_mod):
     worst = _crop_parity(oracle_mod, cfg, patch, boxes)
     print("config 4 128^3 sampled parity, worst relative RHS difference %.2e" % worst)
     patch.close()
+
+
+# ---- config 5: grey M1, IMEX stage -----------------------------------------------------------------------------
+def _m1_setup(oracle_mod, cfg, stages=3):
+    from paper_2510_13965_b200 import binding
+    n = cfg["n"]
+    o = oracle_mod.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"])
+    U, P, V = cfg["U"].copy(), cfg["P"].copy(), cfg["V"].copy()
+    o.prim2con(U, P)
+    patch = binding.Patch(cfg["params"], n, cfg["ng"], cfg["dx"], stages=stages, m1=True)
+    return o, patch, U, P, V
+
+
+def _rel_m1(a, b):
+    """per field of V (15), the three F_i of a species sharing the norm of the vector and E (|F| <= E)"""
+    num = np.abs(a - b).reshape(15, -1).max(axis=1)
+    den = np.abs(b).reshape(15, -1).max(axis=1)
+    for s in range(3):
+        den[5 * s + 2:5 * s + 5] = max(den[5 * s + 2:5 * s + 5].max(), den[5 * s + 1])
+    return num / np.where(den > 0, den, 1.0)
+
+
+@pytest.mark.parametrize("kappa0", [1e-6, 1e3])
+def test_config5_m1_pieces_parity(oracle_mod, kappa0):
+    """a10-a12 one by one on a star-centred crop of config 5 (about 40 % star): implicit solve (closure + Newton),
+    explicit part (closure, fluxes of Eqs. 77-78, sources), back-reaction; optically thin (BASELINE opacities) and stiff."""
+    cfg = synth.config5(n=24, crop_on_star=True, kappa0=kappa0)
+    o, patch, U, P, V = _m1_setup(oracle_mod, cfg)
+    rng = np.random.default_rng(9)
+    for s in range(3):                                   # non-zero fluxes of both signs, |F| < E
+        for i in range(3):
+            V[5 * s + 2 + i] = V[5 * s + 1] * rng.uniform(-0.3, 0.3) * (1.0 + 0.2 * np.sin(3.0 * (i + 1) * cfg["U"][synth.ALPHA]))
+    Uo = U.copy()
+    o.fill_ghosts(Uo, cfg["bc"])
+    Po, Fo = o.con2prim(Uo)
+    Vo = V.copy()
+    o.fill_ghosts(Vo, cfg["bc"])
+    adt = 0.25 * 0.25 * cfg["dx"]
+    Ro, Fo = o.m1_implicit(Uo, Po, Vo, adt, flags=Fo)
+    KVo = o.m1_rhs(Uo, Po, Vo)
+    Ko = o.rhs(Uo, Po)
+    o.m1_backreaction(Uo, Po, Ro, Ko)
+    patch.upload(U=U)
+    patch.V.copy_(patch.torch.as_tensor(V))
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    from paper_2510_13965_b200 import binding
+    patch.fill_ghosts(cfg["bc"], slot=binding.SLOT_V)
+    Rg = patch.m1_implicit(adt, 1).cpu().numpy()
+    Vg, Fg = patch.V.cpu().numpy(), patch.flags.cpu().numpy()[0]
+    assert np.array_equal(Fg, Fo), "flag masks (incl. M1 fix-ups) must agree bit for bit"
+    assert np.all(_rel_m1(Vg, Vo) < 1e-11), _rel_m1(Vg, Vo)
+    rr = np.abs(Rg - Ro).reshape(15, -1).max(axis=1) / np.abs(Ro).reshape(15, -1).max()
+    assert np.all(rr < 1e-10), rr
+    KVg = patch.m1_rhs(1).cpu().numpy()
+    I = (slice(None), slice(NG, -NG), slice(NG, -NG), slice(NG, -NG))
+    num = np.abs(KVg[I] - KVo[I]).reshape(15, -1).max(axis=1)
+    den = np.abs(KVo[I]).reshape(15, -1).max(axis=1)
+    for s in range(3):
+        den[5 * s + 2:5 * s + 5] = den[5 * s + 2:5 * s + 5].max()
+    assert np.all(num / den < 1e-11), num / den
+    Kg = patch.rhs(1)
+    patch.m1_backreaction(1)
+    rk, dk = _rel(Kg.cpu().numpy(), Ko)
+    assert np.all(rk[dk > 0] < 1e-11), rk
+    patch.close()
+
+
+@pytest.mark.parametrize("kappa0", [1e-6, 1e3])
+def test_config5_imex_steps_parity(oracle_mod, kappa0):
+    """Full IMEX steps (Eq. 53, App. C) of the coupled CCZ4 + GRMHD + M1 system: 3 steps at 20^3 on the star-centred crop."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config5(n=20, crop_on_star=True, kappa0=kappa0)
+    o, patch, U, P, V = _m1_setup(oracle_mod, cfg)
+    ae, we, ai, wi = synth.imex_tableau()
+    dt = 0.25 * cfg["dx"]
+    Uo, Vo = U.copy(), V.copy()
+    Po, Fo = o.evolve_imex(Uo, Vo, cfg["bc"], ae, we, ai, wi, dt, 3)
+    patch.upload(U=U)
+    patch.V.copy_(patch.torch.as_tensor(V))
+    patch.advance_imex(binding.make_tableau(ae, we, ai, wi), cfg["bc"], dt, 3)
+    Ug, Vg, Fg = patch.U.cpu().numpy(), patch.V.cpu().numpy(), patch.flags.cpu().numpy()[0]
+    assert np.array_equal(Fg, Fo)
+    ru = _rel_vec(Ug, Uo, [(25, 26, 27), (28, 29, 30), (19, 20, 21)])
+    assert np.all(ru < 1e-9), ru
+    assert np.all(_rel_m1(Vg, Vo) < 1e-9), _rel_m1(Vg, Vo)
+    patch.close()
