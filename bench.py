@@ -37,6 +37,10 @@ def workload_inputs(name, n):
         return synth.config3(n=n)
     if name == "c4":
         return synth.config4(n=n)
+    if name == "c5":                    # two stars + M1 on the full half-width-60 patch (0.3 % star)
+        return synth.config5(n=n)
+    if name == "c5crop":                # the same state on a patch centred on one star (40 % star): exercises the stiff cores
+        return synth.config5(n=n, crop_on_star=True)
     raise ValueError(name)
 
 
@@ -82,12 +86,18 @@ def oracle_leg(cfg_name, n_sample, steps):
     o = oracle.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"], table=cfg.get("table"))
     U, P = cfg["U"].copy(), cfg["P"].copy()
     o.prim2con(U, P)
-    a, w = synth.tableau("rk4")
     dt = 0.25 * cfg["dx"]
     t0 = time.perf_counter()
-    o.evolve(U, cfg["bc"], a, w, dt, steps)
+    if "V" in cfg:
+        ae, we, ai, wi = synth.imex_tableau()
+        o.evolve_imex(U, cfg["V"].copy(), cfg["bc"], ae, we, ai, wi, dt, steps)
+        nst = len(we)
+    else:
+        a, w = synth.tableau("rk4")
+        o.evolve(U, cfg["bc"], a, w, dt, steps)
+        nst = len(w)
     sec = time.perf_counter() - t0
-    zs = float(n[0] * n[1] * n[2] * STAGES * steps)
+    zs = float(n[0] * n[1] * n[2] * nst * steps)
     return zs / sec, sec, zs
 
 
@@ -147,15 +157,23 @@ def main():
     cfg = workload_inputs(args.workload, args.n)
     n, ng = cfg["n"], cfg["ng"]
     zones = n[0] * n[1] * n[2]
-    patch = binding.Patch(cfg["params"], n, ng, cfg["dx"], stages=STAGES, table=cfg.get("table"), device="cuda:%d" % local)
-    a, w = synth.tableau("rk4")
-    tab = binding.make_tableau(a, w)
+    m1 = "V" in cfg
+    nstages = 3 if m1 else STAGES
+    patch = binding.Patch(cfg["params"], n, ng, cfg["dx"], stages=nstages, table=cfg.get("table"), device="cuda:%d" % local, m1=m1)
+    if m1:                              # config 5: IMEX(3,3,2) pair (R1), 3 stages per step
+        tab = binding.make_tableau(*synth.imex_tableau())
+        patch.V.copy_(torch.as_tensor(cfg["V"]))
+        advance = patch.advance_imex
+    else:
+        tab = binding.make_tableau(*synth.tableau("rk4"))
+        advance = patch.advance
     dt = 0.25 * cfg["dx"]
     # initial data: metric + Bbar in U, (rho, Ye, eps, v) in P; conserved fields from the library's own prim2con kernel
     patch.upload(U=cfg["U"], P=cfg["P"])
     patch.prim2con()
     patch.fill_ghosts(cfg["bc"])
     U_init = patch.U.clone()
+    V_init = patch.V.clone() if m1 else None
     torch.cuda.synchronize()
 
     def barrier():
@@ -165,9 +183,11 @@ def main():
 
     # ---- device-resident timing -------------------------------------------------------------------------------
     for _ in range(args.warmup):
-        patch.advance(tab, cfg["bc"], dt, 1)
+        advance(tab, cfg["bc"], dt, 1)
     torch.cuda.synchronize()
     patch.U.copy_(U_init)
+    if m1:
+        patch.V.copy_(V_init)
     patch.profile(True)
     patch.profile_read()
     sampler = ClockSampler(local)
@@ -175,7 +195,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    patch.advance(tab, cfg["bc"], dt, args.steps)        # K full RK4 steps = 4K passes of the whole path, one C-ABI call
+    advance(tab, cfg["bc"], dt, args.steps)              # K full RK steps = 4K (IMEX: 3K) passes of the whole path, one C-ABI call
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
@@ -187,11 +207,11 @@ def main():
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms = float(t.item())
-    value = world * zones * STAGES * args.steps / (ms * 1e-3)
+    value = world * zones * nstages * args.steps / (ms * 1e-3)
 
     # ---- end to end through the host-buffer entry point (H2D of the state, advance, D2H of state + flags) ------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not m1:
         hostU = U_init.cpu().pin_memory()
         hostF = torch.zeros(patch.flags.shape[1:], dtype=torch.uint8).pin_memory()
         src = hostU.clone()
@@ -229,23 +249,29 @@ def main():
         pass
     hbm_peak, hbm_src = (peaks["hbm_gbs"], "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
     fp64_peak = binding.mhd_probe_fp64_flops(patch.stream()) / 1e12
-    oc = json.load(open(os.path.join(ROOT, "tests", "golden", "op_counts.json")))["c1"]
+    oc = json.load(open(os.path.join(ROOT, "tests", "golden", "op_counts.json")))["c5" if m1 else "c1"]
     pts_per_zone = patch.npts / zones
     # algorithmic flops per zone and launch of each kernel class (the oracle's count of the step(s) the kernel performs)
     alg_flops = {"fill_ghosts": 0.0, "con2prim": oc["con2prim_per_point"]["flops"] * pts_per_zone,
                  "ccz4_algebra": oc["ccz4_per_zone"]["flops"] - oc["adv_ko_per_zone"]["flops"] + oc["grmhd_src_per_zone"]["flops"],
                  "adv_ko": oc["adv_ko_per_zone"]["flops"], "point_flux": 0.0,
                  "recon_x": oc["grmhd_flux_per_zone"]["flops"] / 3, "recon_y": oc["grmhd_flux_per_zone"]["flops"] / 3,
-                 "recon_z": oc["grmhd_flux_per_zone"]["flops"] / 3, "rk_combine": 2.5 * oc["rk_combine_per_zone_per_term"]["flops"]}
+                 "recon_z": oc["grmhd_flux_per_zone"]["flops"] / 3, "rk_combine": 2.5 * oc["rk_combine_per_zone_per_term"]["flops"],
+                 # M1: not claimed. The oracle re-solves the closure by plain bisection (~60 evaluations) at every node of every
+                 # line and direction, so its count (tests/golden/op_counts.json, c5) says nothing about the work needed
+                 "m1_point": 0.0, "m1_div": 0.0, "m1_implicit": 0.0}
     # algorithmic doubles moved per zone and launch (reads + writes at the minimum)
     alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "ccz4_algebra": 22 + 10 + 5 + 32, "adv_ko": 22 * 3, "recon_x": 21 + 20,
-                   "recon_y": 21 + 20, "recon_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33}
+                   "recon_y": 21 + 20, "recon_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33,
+                   "m1_point": 21 + 15 + 75, "m1_div": 15 + 75 + 22 + 15, "m1_implicit": 21 + 15 + 30}
     total_kernel_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
     sec_per_launch = dom_ms / max(dom_launches, 1) * 1e-3
     achieved = alg_flops[dom] * zones / sec_per_launch / 1e12
     F_alg = oc["per_zone_stage_flops"]
+    if m1:                              # conservative: the M1 steps add time but no claimed flops
+        F_alg -= oc["m1_implicit_per_point"]["flops"] * pts_per_zone + oc["m1_rhs_per_zone"]["flops"]
     step_tflops = F_alg * value / world / 1e12
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
                 "peak_source": "measured: FP64 DFMA probe of the library (mhd_probe_fp64_flops); nominal 37.2",
