@@ -44,6 +44,22 @@ def workload_inputs(name, n):
     raise ValueError(name)
 
 
+def max_over_ranks(value, device=None):
+    """Replicas-only scaling: the only exchange of the N > 1 path is this reduction of the timed
+    region over ranks (MAX), after which value = world * units / time. Works on any torch.distributed backend."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(world, zones, stages, steps, ms_max):
+    """whole-job zone-stage updates per second of `world` independent replicas (weak scaling)"""
+    return world * zones * stages * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
@@ -203,11 +219,8 @@ def main():
     prof = patch.profile_read()
     patch.profile(False)
     status = patch.status()
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * zones * nstages * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, device="cuda")
+    value = aggregate_throughput(world, zones, nstages, args.steps, ms)
 
     # ---- end to end through the host-buffer entry point (H2D of the state, advance, D2H of state + flags) ------
     e2e = None
@@ -224,10 +237,7 @@ def main():
             patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)
         torch.cuda.synchronize()
         sec = time.perf_counter() - t0
-        tt = torch.tensor([sec], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        sec = float(tt.item())
+        sec = max_over_ranks(sec, device="cuda")
         nbytes = hostU.numel() * 8
         e2e = {"value": world * zones * STAGES * e_steps / sec, "unit": "zone-stages/s", "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes + hostF.numel(), "steps": e_steps}
