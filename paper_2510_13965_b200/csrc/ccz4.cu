@@ -31,32 +31,20 @@ namespace {
 __device__ __forceinline__ constexpr int sym(int i, int j) { return i <= j ? (i * (5 - i)) / 2 + j : (j * (5 - j)) / 2 + i; }   // (0,0)=0 (0,1)=1 (0,2)=2 (1,1)=3 (1,2)=4 (2,2)=5
 
 // ------------------------------------------------------------------------------------------------ tile geometry
-constexpr int TX = 16, TY = 4, TZ = 4, RH = 2;
-constexpr int SX = TX + 2 * RH, SY = TY + 2 * RH, SZ = TZ + 2 * RH;   // 20 x 8 x 8
-constexpr int TILE = SX * SY * SZ;                                    // 1280 doubles
-constexpr int NT = TX * TY * TZ;                                      // 256 threads
-constexpr int NLD = TILE / NT;                                        // 5 cp.async per thread and field
-static_assert(TILE % NT == 0, "tile must be a multiple of the CTA size");
+constexpr int TX = 16, TY = 4, RH = 2;                                // the tile depth TZ is a template parameter of the kernel
+constexpr int SX = TX + 2 * RH, SY = TY + 2 * RH;                     // 20 x 8 x (TZ + 4)
 constexpr int NBUF = 3;
 constexpr int OX = 1, OY = SX, OZ = SX * SY;                          // shared-memory strides
 
-// scratch slots (per thread)
+// scratch slots (per thread): only what the pointwise algebra needs more than once. Second derivatives, d Gamma^, d K^ and
+// d Theta enter the right-hand side linearly and are folded into register accumulators the moment they are computed.
 enum {
   S_DG = 0,       // 18: d_c gamma~_ab at S_DG + 6 c + ab
-  S_R = 18,       //  6: gamma~^mn d_m d_n gamma~_ab
-  S_DGH = 24,     //  9: d_a Gamma^^c at S_DGH + 3 a + c
-  S_DCHI = 33,    //  3
-  S_DDCHI = 36,   //  6
-  S_DAL = 42,     //  3
-  S_DDAL = 45,    //  6
-  S_DBE = 51,     //  9: d_a beta^c at S_DBE + 3 a + c
-  S_LAPB = 60,    //  3: gamma~^jk d_j d_k beta^c
-  S_DDIV = 63,    //  3: d_a d_k beta^k
-  S_DKH = 66,     //  3
-  S_DTH = 69,     //  3
-  NSCR = 72
+  S_DDAL = 18,    //  6: d_a d_b alpha
+  S_DBE = 24,     //  9: d_a beta^c at S_DBE + 3 a + c
+  NSCR = 33
 };
-constexpr size_t SMEM_BYTES = (size_t)(NBUF * TILE + NSCR * NT) * sizeof(double);
+template <int TZ> constexpr size_t smem_bytes() { return (size_t)(NBUF * SX * SY * (TZ + 2 * RH) + NSCR * TX * TY * TZ) * sizeof(double); }
 
 __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -97,9 +85,11 @@ __device__ __forceinline__ void second(const double* s, const Scale& sc, double 
 // order in which the differentiated fields pass through the ring
 __device__ constexpr int FORDER[16] = {GXX, GXY, GXZ, GYY, GYZ, GZZ, GAMX, GAMY, GAMZ, CHI, ALPHA, BETAX, BETAY, BETAZ, KHAT, THETA};
 
-__global__ void __launch_bounds__(NT, 1)
+template <int TZ>
+__global__ void __launch_bounds__(TX * TY * TZ, 1)
 k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk) {
+  constexpr int SZ = TZ + 2 * RH, TILE = SX * SY * SZ, NT = TX * TY * TZ, NLD = (TILE + NT - 1) / NT;
   extern __shared__ __align__(16) double smem[];
   double* ring = smem;
   const int tid = threadIdx.x;
@@ -116,7 +106,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
   int goff[NLD];
 #pragma unroll
   for (int m = 0; m < NLD; ++m) {
-    const int e = tid + m * NT;
+    const int e = min(tid + m * NT, TILE - 1);
     const int x = e % SX, y = (e / SX) % SY, z = e / (SX * SY);
     const int gx = min(i0 + x - RH + d.ng, d.mx - 1), gy = min(j0 + y - RH + d.ng, d.my - 1), gz = min(k0 + z - RH + d.ng, d.mz - 1);
     goff[m] = (int)(gz * d.sz + gy * d.sy + gx);
@@ -125,7 +115,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
     const double* src = U + (size_t)f * su;
     double* dst = ring + buf * TILE + tid;
 #pragma unroll
-    for (int m = 0; m < NLD; ++m) cp_async8(dst + m * NT, src + goff[m]);
+    for (int m = 0; m < NLD; ++m) if (TILE % NT == 0 || tid + m * NT < TILE) cp_async8(dst + m * NT, src + goff[m]);
     cp_commit();
   };
   issue(FORDER[0], 0);
@@ -159,8 +149,11 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 
   // ================================================================= phase 1: derivatives, field by field
   const int ctr = ((tz + RH) * SY + (ty + RH)) * SX + (tx + RH);
-  double chi = 1.0, al = 1.0, be[3] = {0, 0, 0}, Gh[3] = {0, 0, 0}, Kh = 0.0, Th = 0.0;
-  double ddiv[3] = {0.0, 0.0, 0.0};
+  const double chi = F(CHI), al = F(ALPHA);
+  double be[3] = {0, 0, 0}, Gh[3] = {0, 0, 0}, Kh = 0.0, Th = 0.0;
+  double Racc[6] = {0, 0, 0, 0, 0, 0};   // part of chi (R^_ab + R^chi_ab) that is linear in second derivatives and in d Gamma^
+  double GamAcc[3] = {0, 0, 0};          // gamma~^jk d_j d_k beta^a + 1/3 gamma~^ab d_b d_k beta^k - 2 alpha gamma~^ab (2/3 d_b K^ + 1/3 d_b Theta)
+  double dchi[3] = {0, 0, 0}, dal[3] = {0, 0, 0};
 #pragma unroll
   for (int n = 0; n < 16; ++n) {
     if (n + 1 < 16) cp_wait<1>(); else cp_wait<0>();
@@ -169,36 +162,50 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
     const double* s = ring + (n % NBUF) * TILE + ctr;
     double d1[3];
     first(s, sc, d1);
-    if (n < 6) {                       // gamma~_ab, ab = n
+    if (n < 6) {                       // gamma~_ab, ab = n: -1/2 gamma~^mn d_m d_n gamma~_ab of Eq. (23)
       double dd[6];
       second(s, sc, dd);
 #pragma unroll
       for (int c = 0; c < 3; ++c) SCR(S_DG + 6 * c + n) = d1[c];
-      SCR(S_R + n) = 0.5 * (gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5]) + (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
-    } else if (n < 9) {                // Gamma^^c, c = n - 6
-      Gh[n - 6] = s[0];
+      Racc[n] -= chi * (0.5 * (gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5]) + (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]));
+    } else if (n < 9) {                // Gamma^^c, c = n - 6: gamma~_k(i d_j) Gamma^^k
+      const int c = n - 6;
+      Gh[c] = s[0];
 #pragma unroll
-      for (int a = 0; a < 3; ++a) SCR(S_DGH + 3 * a + (n - 6)) = d1[a];
-    } else if (n == 9 || n == 10) {    // chi, alpha
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = a; b < 3; ++b) Racc[sym(a, b)] += 0.5 * chi * (G_(c, a) * d1[b] + G_(c, b) * d1[a]);
+    } else if (n == 9) {               // chi: 1/2 d_i d_j chi + 1/2 gamma~_ij gamma~^mn d_m d_n chi of Eq. (22)
       double dd[6];
       second(s, sc, dd);
-      if (n == 9) chi = s[0]; else al = s[0];
+      const double lap = gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
 #pragma unroll
-      for (int a = 0; a < 3; ++a) SCR((n == 9 ? S_DCHI : S_DAL) + a) = d1[a];
+      for (int a = 0; a < 3; ++a) dchi[a] = d1[a];
 #pragma unroll
-      for (int a = 0; a < 6; ++a) SCR((n == 9 ? S_DDCHI : S_DDAL) + a) = dd[a];
+      for (int a = 0; a < 6; ++a) Racc[a] += 0.5 * dd[a] + 0.5 * g[a] * lap;
+    } else if (n == 10) {              // alpha
+      double dd[6];
+      second(s, sc, dd);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) dal[a] = d1[a];
+#pragma unroll
+      for (int a = 0; a < 6; ++a) SCR(S_DDAL + a) = dd[a];
     } else if (n < 14) {               // beta^c, c = n - 11
       const int c = n - 11;
       double dd[6];
       second(s, sc, dd);
       be[c] = s[0];
 #pragma unroll
-      for (int a = 0; a < 3; ++a) { SCR(S_DBE + 3 * a + c) = d1[a]; ddiv[a] += dd[sym(a, c)]; }
-      SCR(S_LAPB + c) = gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
-    } else {                           // K^, Theta
+      for (int a = 0; a < 3; ++a) {
+        SCR(S_DBE + 3 * a + c) = d1[a];
+        GamAcc[a] += (1.0 / 3.0) * (GI(a, 0) * dd[sym(0, c)] + GI(a, 1) * dd[sym(1, c)] + GI(a, 2) * dd[sym(2, c)]);
+      }
+      GamAcc[c] += gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
+    } else {                           // K^ (weight 2/3), Theta (weight 1/3): -2 alpha gamma~^ab w d_b
       if (n == 14) Kh = s[0]; else Th = s[0];
+      const double w = -2.0 * al * (n == 14 ? 2.0 / 3.0 : 1.0 / 3.0);
 #pragma unroll
-      for (int a = 0; a < 3; ++a) SCR((n == 14 ? S_DKH : S_DTH) + a) = d1[a];
+      for (int a = 0; a < 3; ++a) GamAcc[a] += w * (GI(a, 0) * d1[0] + GI(a, 1) * d1[1] + GI(a, 2) * d1[2]);
     }
   }
   if (!inside) return;
@@ -235,12 +242,9 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 #pragma unroll
     for (int b = a; b < 3; ++b) {
       const int ab = sym(a, b);
-      double r = -SCR(S_R + ab);                                              // -1/2 gamma~^mn d_m d_n gamma~_ab
+      double r = 0.0;
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        r += 0.5 * (G_(c, a) * SCR(S_DGH + 3 * b + c) + G_(c, b) * SCR(S_DGH + 3 * a + c));   // gamma~_k(i d_j) Gamma^^k
-        r += 0.5 * Gh[c] * (Gl[a][sym(b, c)] + Gl[b][sym(a, c)]);                                // Gamma^^k Gamma~_(ij)k
-      }
+      for (int c = 0; c < 3; ++c) r += 0.5 * Gh[c] * (Gl[a][sym(b, c)] + Gl[b][sym(a, c)]);        // Gamma^^k Gamma~_(ij)k
 #pragma unroll
       for (int m = 0; m < 3; ++m)
 #pragma unroll
@@ -251,29 +255,26 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
             t += Gu[c][sym(m, a)] * Gl[b][sym(c, n)] + Gu[c][sym(m, b)] * Gl[a][sym(c, n)] + Gu[c][sym(m, a)] * Gl[c][sym(n, b)];
           r += GI(m, n) * t;
         }
-      X[ab] = chi * r;
+      X[ab] = Racc[ab] + chi * r;
     }
   double Rtr = 0.0;   // gamma^ij (R_ij + 2 D_(i Z_j)) = gamma~^ij (chi R^_ij + chi R^chi_ij)
 
   // ---- chi R^chi_ij (Eq. 22), physical Hessian of the lapse (R25)
-  double dchi[3], dal[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) { dchi[a] = SCR(S_DCHI + a); dal[a] = SCR(S_DAL + a); }
   double gdchi[3];   // gamma~^kl d_l chi
 #pragma unroll
   for (int c = 0; c < 3; ++c) gdchi[c] = GI(c, 0) * dchi[0] + GI(c, 1) * dchi[1] + GI(c, 2) * dchi[2];
   double lapal;      // D_i D^i alpha, Eq. (24)
   {
-    double ddchi[6], ddal[6];
+    double ddal[6];
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { ddchi[a] = SCR(S_DDCHI + a); ddal[a] = SCR(S_DDAL + a); }
+    for (int a = 0; a < 6; ++a) ddal[a] = SCR(S_DDAL + a);
     double lapchi = 0.0, Ghdchi = 0.0, Zl[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       Ghdchi += Gh[a] * dchi[a];
       Zl[a] = G_(a, 0) * Z[0] + G_(a, 1) * Z[1] + G_(a, 2) * Z[2];        // Z^k gamma~_ka
 #pragma unroll
-      for (int b = 0; b < 3; ++b) lapchi += GI(a, b) * (ddchi[sym(a, b)] - 1.5 * ichi * dchi[a] * dchi[b]);
+      for (int b = 0; b < 3; ++b) lapchi -= GI(a, b) * 1.5 * ichi * dchi[a] * dchi[b];   // its second-derivative part is in Racc
     }
     lapal = 0.0;
 #pragma unroll
@@ -290,7 +291,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 #pragma unroll
       for (int b = a; b < 3; ++b) {
         const int ab = sym(a, b);
-        double c_ = 0.5 * ddchi[ab] - 0.25 * ichi * dchi[a] * dchi[b];
+        double c_ = -0.25 * ichi * dchi[a] * dchi[b];
         double Gdal = 0.0;   // Gamma~^k_ab d_k alpha
 #pragma unroll
         for (int c = 0; c < 3; ++c) { c_ -= 0.5 * Gu[c][ab] * dchi[c]; Gdal += Gu[c][ab] * dal[c]; }
@@ -418,20 +419,17 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
                - al * (G8 * E + par.kappa_z * (2.0 + par.kappa_2) * Th);
   // ---- Eqs. (18)-(20)
   {
-    double dKh[3], dTh[3], lapb[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { dKh[a] = SCR(S_DKH + a); dTh[a] = SCR(S_DTH + a); lapb[a] = SCR(S_LAPB + a); }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-      double s = (2.0 / 3.0) * Gh[a] * divb + lapb[a];
+      double s = (2.0 / 3.0) * Gh[a] * divb + GamAcc[a];
       double b1 = 0.0, b2 = 0.0;
 #pragma unroll
       for (int b = 0; b < 3; ++b) {
-        s += -Gh[b] * dbe[b][a] + GI(a, b) * ddiv[b] * (1.0 / 3.0) - 2.0 * Auu[sym(a, b)] * dal[b];
+        s += -Gh[b] * dbe[b][a] - 2.0 * Auu[sym(a, b)] * dal[b];
 #pragma unroll
         for (int c = 0; c < 3; ++c) b1 += Gu[a][sym(b, c)] * Auu[sym(b, c)];
-        b1 += -1.5 * ichi * Auu[sym(a, b)] * dchi[b] - (2.0 / 3.0) * GI(a, b) * dKh[b] - G8 * GI(a, b) * Sl[b];
-        b2 -= GI(a, b) * (dTh[b] * (1.0 / 3.0) + Th / al * dal[b]);
+        b1 += -1.5 * ichi * Auu[sym(a, b)] * dchi[b] - G8 * GI(a, b) * Sl[b];
+        b2 -= GI(a, b) * (Th / al * dal[b]);
       }
       b2 -= Z[a] * ichi * (par.kappa_z + (2.0 / 3.0) * Ktot);
       OUT(GAMX + a) = s + 2.0 * al * (b1 + b2);
@@ -557,14 +555,19 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
 }  // namespace
 
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+  static int tz = 0;
+  if (tz == 0) {
+    const char* v = getenv("MHD_CCZ4_TZ");
+    tz = v ? atoi(v) : 4;
+    cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<4>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ccz4_algebra<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<5>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ccz4_algebra<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<6>());
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
-  dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
-  k_ccz4_algebra<<<grid, NT, SMEM_BYTES, s>>>(d, par, U, su, P, sp, K, sk);
+  auto grid = [&](int TZ) { return dim3((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ); };
+  if (tz == 6) k_ccz4_algebra<6><<<grid(6), TX * TY * 6, smem_bytes<6>(), s>>>(d, par, U, su, P, sp, K, sk);
+  else if (tz == 5) k_ccz4_algebra<5><<<grid(5), TX * TY * 5, smem_bytes<5>(), s>>>(d, par, U, su, P, sp, K, sk);
+  else k_ccz4_algebra<4><<<grid(4), TX * TY * 4, smem_bytes<4>(), s>>>(d, par, U, su, P, sp, K, sk);
   return cudaGetLastError();
 }
 
