@@ -119,7 +119,7 @@ __device__ __forceinline__ void opacities(const Par& par, int s, double rho, dou
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_m1_point(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
+__global__ void __launch_bounds__(128, 3) k_m1_point(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                   const double* __restrict__ P, size_t sp, const double* __restrict__ V, size_t sv,
                                                   double* __restrict__ Wk, size_t sw) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -174,7 +174,8 @@ namespace {
 // F^_{i+1/2} of Eq. (77) from u_{i-1..i+2}, the fluxes at i, i+1, lambda_{i+1/2} and A_{i+1/2}
 __device__ __forceinline__ double m1_face(double um, double u0, double up, double upp, double F0, double F1, double lam, double A0, bool oe) {
   const double dm = u0 - um, d0 = up - u0, dp = upp - up;
-  const double Phi = d0 == 0.0 ? 1.0 : fmax(0.0, fmin(1.0, fmin(2.0 * dm / d0, 2.0 * dp / d0)));        // Eq. (78), R20
+  const double r2 = 2.0 / d0;                                                                           // one reciprocal per face and field
+  const double Phi = d0 == 0.0 ? 1.0 : fmax(0.0, fmin(1.0, fmin(dm * r2, dp * r2)));                    // Eq. (78), R20
   const double tiny = 1e-10 * fmax(fmax(fabs(um), fabs(u0)), fmax(fabs(up), fabs(upp)));                // R33
   const double A = (oe && dm * d0 < 0.0 && d0 * dp < 0.0 && fmin(fmin(fabs(dm), fabs(d0)), fabs(dp)) > tiny) ? 1.0 : A0;   // l.565-570
   const double FHO = 0.5 * (F0 + F1);
@@ -185,7 +186,7 @@ __device__ __forceinline__ double d1c(const double* __restrict__ u, long long s,
 }
 }  // namespace
 
-__global__ void __launch_bounds__(128) k_m1_div(const __grid_constant__ Dims d, bool oe, const double* __restrict__ U, size_t su,
+__global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims d, bool oe, const double* __restrict__ U, size_t su,
                                                 const double* __restrict__ V, size_t sv, const double* __restrict__ Wk, size_t sw,
                                                 double* __restrict__ KV, size_t sk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -193,6 +194,36 @@ __global__ void __launch_bounds__(128) k_m1_div(const __grid_constant__ Dims d, 
   const size_t pt = (size_t)(blockIdx.z + d.ng) * d.sz + (size_t)(blockIdx.y + d.ng) * d.sy + (i + d.ng);
   const long long st[3] = {1, d.sy, d.sz};
   const double h[3] = {d.dx, d.dy, d.dz};
+#pragma unroll 1
+  for (int s = 0; s < 3; ++s) {
+    double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    const double* wk = Wk + (size_t)(M1W * s) * sw + pt;
+#pragma unroll
+    for (int dir = 0; dir < 3; ++dir) {
+      const long long ls = st[dir];
+      const double* wl = wk + (size_t)(6 * dir + 5) * sw;
+      const double* wkap = wk + (size_t)18 * sw;
+      const double lm = __ldg(wl - ls), l0 = __ldg(wl), lp = __ldg(wl + ls);
+      const double km = __ldg(wkap - ls), k0 = __ldg(wkap), kp = __ldg(wkap + ls);
+      const double lamL = fmax(lm, l0), lamR = fmax(l0, lp);
+      const double khL = 0.5 * (km + k0) * h[dir], khR = 0.5 * (k0 + kp) * h[dir];
+      // tanh(x) rounds to 1 in FP64 for x >= 20: optically thin faces skip the evaluation
+      const double AL = khL > 0.05 ? tanh(1.0 / khL) : 1.0, AR = khR > 0.05 ? tanh(1.0 / khR) : 1.0;
+      const double ih = 1.0 / h[dir];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const double* u = V + (size_t)(5 * s + f) * sv + pt;
+        const double* F = wk + (size_t)(6 * dir + f) * sw;
+        const double u2m = __ldg(u - 2 * ls), um = __ldg(u - ls), u0 = __ldg(u), up = __ldg(u + ls), u2p = __ldg(u + 2 * ls);
+        const double Fm = __ldg(F - ls), F0 = __ldg(F), Fp = __ldg(F + ls);
+        const double fR = m1_face(um, u0, up, u2p, F0, Fp, lamR, AR, oe);
+        const double fL = m1_face(u2m, um, u0, up, Fm, F0, lamL, AL, oe);
+        acc[f] -= (fR - fL) * ih;
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < 5; ++f) KV[(size_t)(5 * s + f) * sk + pt] = acc[f];
+  }
   // ---- geometry for the sources of Eqs. (39)-(40)
   double g[6], gu[6], dg[3][6], dchi[3], dal[3], dbe[3][3], At[6], be[3];
 #pragma unroll
@@ -220,30 +251,8 @@ __global__ void __launch_bounds__(128) k_m1_div(const __grid_constant__ Dims d, 
   const double sg = 1.0 / (chi * sqrt(chi)), ichi = 1.0 / chi;
 #pragma unroll 1
   for (int s = 0; s < 3; ++s) {
-    double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     const double* wk = Wk + (size_t)(M1W * s) * sw + pt;
-#pragma unroll
-    for (int dir = 0; dir < 3; ++dir) {
-      const long long ls = st[dir];
-      const double* wl = wk + (size_t)(6 * dir + 5) * sw;
-      const double* wkap = wk + (size_t)18 * sw;
-      const double lm = __ldg(wl - ls), l0 = __ldg(wl), lp = __ldg(wl + ls);
-      const double km = __ldg(wkap - ls), k0 = __ldg(wkap), kp = __ldg(wkap + ls);
-      const double lamL = fmax(lm, l0), lamR = fmax(l0, lp);
-      const double khL = 0.5 * (km + k0) * h[dir], khR = 0.5 * (k0 + kp) * h[dir];
-      const double AL = khL > 0.0 ? tanh(1.0 / khL) : 1.0, AR = khR > 0.0 ? tanh(1.0 / khR) : 1.0;
-      const double ih = 1.0 / h[dir];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        const double* u = V + (size_t)(5 * s + f) * sv + pt;
-        const double* F = wk + (size_t)(6 * dir + f) * sw;
-        const double u2m = __ldg(u - 2 * ls), um = __ldg(u - ls), u0 = __ldg(u), up = __ldg(u + ls), u2p = __ldg(u + 2 * ls);
-        const double Fm = __ldg(F - ls), F0 = __ldg(F), Fp = __ldg(F + ls);
-        const double fR = m1_face(um, u0, up, u2p, F0, Fp, lamR, AR, oe);
-        const double fL = m1_face(u2m, um, u0, up, Fm, F0, lamL, AL, oe);
-        acc[f] -= (fR - fL) * ih;
-      }
-    }
+    double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     // ---- geometric sources
     double Pl[6], ub[5];
 #pragma unroll
@@ -281,7 +290,7 @@ __global__ void __launch_bounds__(128) k_m1_div(const __grid_constant__ Dims d, 
       acc[2 + a] += sF + 0.5 * al * ichi * Pdg;
     }
 #pragma unroll
-    for (int f = 0; f < 5; ++f) KV[(size_t)(5 * s + f) * sk + pt] = acc[f];
+    for (int f = 1; f < 5; ++f) KV[(size_t)(5 * s + f) * sk + pt] += acc[f];
   }
 }
 
@@ -362,7 +371,7 @@ __device__ __forceinline__ bool solve4(double A[4][4], double b[4]) {
 }
 }  // namespace
 
-__global__ void __launch_bounds__(128) k_m1_implicit(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
+__global__ void __launch_bounds__(128, 3) k_m1_implicit(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                      const double* __restrict__ P, size_t sp, double* __restrict__ V, size_t sv,
                                                      double* __restrict__ R, size_t sr, double adt, uint8_t* __restrict__ flags) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
