@@ -177,3 +177,37 @@ def test_imex_tableau_conditions():
         for c in (ce, ci):
             assert abs(w @ c - 0.5) < 1e-15
     assert abs(1.0 - wi @ np.linalg.solve(ai, np.ones(3))) < 1e-14      # R(-inf) = 0: L-stable
+
+
+def test_odd_even_switch_fires_on_a_zigzag_only(oracle_mod):
+    """l.565-570 with reading R33: on a genuine zigzag (alternating E) in an optically thick medium the switch sets A = 1 and the
+    full Lax-Friedrichs dissipation acts; with the switch off the same data see A = tanh(1/(kappa dx)) ~ 0; on a smooth profile
+    with rounding-level noise the switch must NOT fire."""
+    n, ng, dx = 12, 3, 0.1
+    U = synth._flat_state((n + 6,) * 3)
+    P = np.zeros((10,) + U.shape[1:])
+    P[synth.RHO], P[synth.WLOR], P[synth.TEMP] = 1e-3, 1.0, 0.01
+    idx = np.arange(n + 6)
+    zig = 1e-5 * (1.0 + 0.1 * (-1.0) ** idx)[None, None, :] * np.ones(U.shape[1:])
+    V = np.zeros((15,) + U.shape[1:])
+    V[1] = zig
+    V[6] = V[11] = 1e-5
+    I = (slice(ng, -ng),) * 3
+    out = {}
+    for oe in (0, 1):
+        o = oracle_mod.Oracle(synth.default_params(m1_kappa0=1e6, m1_odd_even=oe), n, n, n, ng, dx)
+        out[oe] = o.m1_rhs(U, P, V)[1][I]
+    # switch off: A ~ 1e-5, the E equation sees (almost) no dissipation; switch on: -lambda (u_{i+1} - 2 u_i + u_{i-1}) / (2 dx) with lambda = 1/sqrt3
+    assert np.abs(out[0]).max() < 1e-3 * np.abs(out[1]).max()
+    lap = (zig[:, :, ng + 1:n + ng + 1] - 2 * zig[:, :, ng:n + ng] + zig[:, :, ng - 1:n + ng - 1])[ng:-ng, ng:-ng]
+    lam = 1.0 / np.sqrt(3.0)                       # (B5) thick limit at rest: sqrt(3 gamma^xx) / 3
+    assert np.abs(out[1] - 0.5 * lam * lap / dx).max() < 1e-9 * np.abs(out[1]).max()
+    # smooth profile + rounding noise: both settings agree
+    rng = np.random.default_rng(0)
+    X = synth.mesh(n, n, n, ng, dx)[0]
+    V[1] = 1e-5 * (1.0 + 0.1 * np.sin(2 * np.pi * X / (n * dx))) * (1.0 + 1e-15 * rng.standard_normal(X.shape))
+    res = []
+    for oe in (0, 1):
+        o = oracle_mod.Oracle(synth.default_params(m1_kappa0=1e6, m1_odd_even=oe), n, n, n, ng, dx)
+        res.append(o.m1_rhs(U, P, V)[1][I])
+    assert np.array_equal(res[0], res[1])
