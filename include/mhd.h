@@ -136,7 +136,9 @@ int mhd_fill_ghosts(mhd_patch *p, int slot_state, const int bc[6], void *cuda_st
 
 /* a2 — conserved -> primitive at every grid point incl. ghosts (App. D, Eqs. D1-D15, error policy
  * l.1157-1162). Writes the 10 primitives and the flag byte; where a rule changed a primitive the fluid conserved
- * fields of slot_state are reset from the corrected primitives (Bbar, phibar untouched). */
+ * fields of slot_state are reset from the corrected primitives (Bbar, phibar untouched). slot_prim is also READ: if it holds
+ * valid primitives (e.g. of the previous stage) they give the starting bracket of the root solve (warm start); the result is
+ * the same root to solver tolerance whatever slot_prim held, zeros and NaNs included. */
 int mhd_con2prim(mhd_patch *p, int slot_state, int slot_prim, int slot_flags, void *cuda_stream);
 
 /* inverse of a2 for initial data (Eq. 29): slot_prim holds rho, Ye, eps, v^i; fills p, W, T, cs2 there and

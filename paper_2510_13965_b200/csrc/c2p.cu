@@ -234,13 +234,32 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
     s.v02 = s.r2 / (s.h0 * s.h0 + s.r2);
     if (par.eos_kind == 2) { s.rho_lo = pow(10.0, par.lr0); s.rho_hi = pow(10.0, par.lr0 + par.dlr * (par.n_rho - 1)); }
     else { s.rho_lo = 0.0; s.rho_hi = par.rho_max; }
-    bool ok1, ok2 = true;
+    bool ok1 = true, ok2 = true;
     const double mub = 1.0 / s.h0;
-    const double mu_plus = brent_root([&](double m) { return s.fa(m); }, 0.0, mub, -1.0, s.fa(mub), par.c2p_maxit, ok1);   // step 2
-    const double f0 = s.f(par, 0.0), f1 = s.f(par, mu_plus);
-    double mu;
-    if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; ok2 = fabs(f1) <= 1e-12; }   // R9: degenerate root at the bracket end
-    else mu = brent_root([&](double m) { return s.f(par, m); }, 0.0, mu_plus, f0, f1, par.c2p_maxit, ok2);                 // step 3
+    double mu = 0.0;
+    // Warm start: the primitive slot still holds the solution of the previous stage, which for a time-stepped state lies
+    // within ~1e-3 of the new one. mu = 1 / (W h) of it, +-1 %, is tried as the bracket of step 3; it is used only if f
+    // changes sign on it (the root of f on (0, mu_+] is unique, and f grows beyond mu_+), otherwise the solve starts cold
+    // from steps 2-3 as printed. The result is the same root to the tolerance of the solver either way.
+    bool warm = false;
+    {
+      const double Wo = P[(size_t)WLOR * sp + pt], ro = P[(size_t)RHO * sp + pt], eo = P[(size_t)EPS * sp + pt], po = P[(size_t)PRESS * sp + pt];
+      const double mu0 = ro / (Wo * (ro * (1.0 + eo) + po));
+      if (mu0 > 0.0 && mu0 < mub) {                      // false for NaN / zero-initialised primitives
+        const double a = 0.99 * mu0, b = fmin(1.01 * mu0, mub);
+        const double fa_ = s.f(par, a), fb_ = s.f(par, b);
+        if (fa_ < 0.0 && fb_ > 0.0) {
+          mu = brent_root([&](double m) { return s.f(par, m); }, a, b, fa_, fb_, par.c2p_maxit, ok2);
+          warm = true;
+        }
+      }
+    }
+    if (!warm) {
+      const double mu_plus = brent_root([&](double m) { return s.fa(m); }, 0.0, mub, -1.0, s.fa(mub), par.c2p_maxit, ok1);   // step 2
+      const double f0 = s.f(par, 0.0), f1 = s.f(par, mu_plus);
+      if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; ok2 = fabs(f1) <= 1e-12; }   // R9: degenerate root at the bracket end
+      else mu = brent_root([&](double m) { return s.f(par, m); }, 0.0, mu_plus, f0, f1, par.c2p_maxit, ok2);                 // step 3
+    }
     s.f(par, mu);                                                                    // step 4
     if (!ok1 || !ok2) flag |= MHD_FLAG_NOCONV;
     W = s.W; rho = D / W; eps = s.eps_raw;
