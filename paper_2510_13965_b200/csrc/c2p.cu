@@ -161,9 +161,42 @@ __device__ __forceinline__ void cons_from_prim(const Sym3& gl, double rho, doubl
 
 // ------------------------------------------------------------------------------------------ root solves
 // State of the App. D master function; one instance per thread.
+// Tabulated EoS inside the mu iteration: pressure and clamped eps for (rho, eps_raw) at fixed Ye. Same interpolant and
+// same clamps as eos_eps_range + eos_eval, arranged for the iteration: one log10 per argument, the eps range compared in
+// log space (no pow unless the clamp acts), T and cs2 not evaluated, and the T cell of the previous evaluation tried
+// first (the interpolant is monotone along T, so whatever the search order the cell found is the same).
+__device__ __forceinline__ void tab_p_of_eps(const Par& q, TPos y, double rho, double eps_raw, int& hint, double& p, double& eps) {
+  const TPos r = tab_locate(log10(rho), q.lr0, q.dlr, q.n_rho);
+  const double e_min = tab_col(q, q.tab_loge, r, y, 0), e_max = tab_col(q, q.tab_loge, r, y, q.n_T - 1);
+  const double le = log10(eps_raw + q.tab_eps_shift);
+  TPos t;
+  if (!(le > e_min)) { t.i = 0; t.w = 0.0; eps = pow(10.0, e_min) - q.tab_eps_shift; }
+  else if (le >= e_max) { t.i = q.n_T - 2; t.w = 1.0; eps = pow(10.0, e_max) - q.tab_eps_shift; }
+  else {
+    eps = eps_raw;
+    int lo = 0, hi = q.n_T - 1;
+    double e_lo = e_min, e_hi = e_max;
+    if (hint >= 0 && hint < q.n_T - 1) {               // the cell of the last evaluation, then its neighbours, then bisection
+      const double a = tab_col(q, q.tab_loge, r, y, hint), b = tab_col(q, q.tab_loge, r, y, hint + 1);
+      if (le >= a) { lo = hint; e_lo = a; if (le < b) { hi = hint + 1; e_hi = b; } else { lo = hint + 1; e_lo = b; } }
+      else { hi = hint; e_hi = a; }
+    }
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      const double em = tab_col(q, q.tab_loge, r, y, mid);
+      if (le >= em) { lo = mid; e_lo = em; } else { hi = mid; e_hi = em; }
+    }
+    t.i = lo; t.w = (le - e_lo) / (e_hi - e_lo);
+    hint = lo;
+  }
+  p = pow(10.0, tab_tri(q, q.tab_logp, r, t, y));
+}
+
 struct Master {
   double D, q, r2, B2, rB2, B2rp2, ye, h0, v02, rho_lo, rho_hi;
   double W, eps_raw;   // by-products of the last evaluation
+  TPos ypos;           // table position of Ye (fixed during the solve)
+  int t_hint;          // T cell of the last table evaluation
   __device__ __forceinline__ double x_of(double mu) const { return 1.0 / (1.0 + mu * B2); }          // (D5)
   __device__ __forceinline__ double rbar2(double mu) const {                                          // (D4)
     const double x = x_of(mu);
@@ -180,11 +213,15 @@ struct Master {
     double rho = D * iW;
     rho = fmax(fmin(rho_hi, rho), rho_lo);
     eps_raw = W * ((qbar - mu * rb2) + v2 / (1.0 + iW));                                             // (D12): W^2/(1+W) = W/(1+1/W)
-    double emin, emax;
-    eos_eps_range(par, rho, ye, emin, emax);
-    const double eps = fmax(fmin(emax, eps_raw), emin);
-    const Eos e = eos_eval(par, rho, eps, ye);
-    const double a = e.p / (rho * (1.0 + eps));
+    double eps, p;
+    if (par.eos_kind == 2) tab_p_of_eps(par, ypos, rho, eps_raw, t_hint, p, eps);
+    else {
+      double emin, emax;
+      eos_eps_range(par, rho, ye, emin, emax);
+      eps = fmax(fmin(emax, eps_raw), emin);
+      p = eos_eval(par, rho, eps, ye).p;
+    }
+    const double a = p / (rho * (1.0 + eps));
     const double nuA = (1.0 + a) * (1.0 + eps) * iW;
     const double nuB = (1.0 + a) * (1.0 + qbar - mu * rb2);
     return mu - 1.0 / (fmax(nuA, nuB) + mu * rb2);
@@ -225,6 +262,8 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
     sym_apply(gu, rl, ru);
     sym_apply(gl, Bs, Bsl);
     s.ye = fmax(fmin(ye, par.ye_max), par.ye_min);
+    s.t_hint = -1;
+    if (par.eos_kind == 2) s.ypos = tab_locate(s.ye, par.ye0, par.dye, par.n_ye);
     s.r2 = ru[0] * rl[0] + ru[1] * rl[1] + ru[2] * rl[2];                            // (D2)
     s.B2 = Bs[0] * Bsl[0] + Bs[1] * Bsl[1] + Bs[2] * Bsl[2];
     const double rB = rl[0] * Bs[0] + rl[1] * Bs[1] + rl[2] * Bs[2];
@@ -238,18 +277,23 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
     const double mub = 1.0 / s.h0;
     double mu = 0.0;
     // Warm start: the primitive slot still holds the solution of the previous stage, which for a time-stepped state lies
-    // within ~1e-3 of the new one. mu = 1 / (W h) of it, +-1 %, is tried as the bracket of step 3; it is used only if f
-    // changes sign on it (the root of f on (0, mu_+] is unique, and f grows beyond mu_+), otherwise the solve starts cold
+    // within ~1e-3 of the new one. mu0 = 1 / (W h) of it and a second point one doubled Newton step away are tried as the
+    // bracket of step 3; they are used only if f changes sign between them (the root of f on (0, mu_+] is unique, and f grows beyond mu_+), otherwise the solve starts cold
     // from steps 2-3 as printed. The result is the same root to the tolerance of the solver either way.
     bool warm = false;
     {
       const double Wo = P[(size_t)WLOR * sp + pt], ro = P[(size_t)RHO * sp + pt], eo = P[(size_t)EPS * sp + pt], po = P[(size_t)PRESS * sp + pt];
       const double mu0 = ro / (Wo * (ro * (1.0 + eo) + po));
       if (mu0 > 0.0 && mu0 < mub) {                      // false for NaN / zero-initialised primitives
-        const double a = 0.99 * mu0, b = fmin(1.01 * mu0, mub);
-        const double fa_ = s.f(par, a), fb_ = s.f(par, b);
-        if (fa_ < 0.0 && fb_ > 0.0) {
-          mu = brent_root([&](double m) { return s.f(par, m); }, a, b, fa_, fb_, par.c2p_maxit, ok2);
+        // second point by a doubled Newton step with f' ~ 1 (f = mu - 1 / (nu + mu rbar^2), nu varies slowly): it
+        // overshoots the root, so the two points bracket it with a width of ~2 |f(mu0)|
+        const double fa_ = s.f(par, mu0);
+        const double b = fmin(fmax(mu0 - 2.0 * fa_, 0.5 * mu0), mub);
+        const bool hit = fa_ == 0.0 || b == mu0;        // the step is below one ulp: mu0 is the root to solver tolerance
+        const double fb_ = hit ? 0.0 : s.f(par, b);
+        if (hit) { mu = mu0; warm = true; }
+        else if ((fa_ < 0.0) != (fb_ < 0.0)) {
+          mu = brent_root([&](double m) { return s.f(par, m); }, mu0, b, fa_, fb_, par.c2p_maxit, ok2);
           warm = true;
         }
       }
