@@ -147,7 +147,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c1")
+    ap.add_argument("--workload", default="c4", help="c4 (BASELINE configs[3], the 256^3 workload the metric is quoted on), c1, c3, c5, c5crop")
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=40, help="sample size of the oracle legs")
@@ -259,7 +259,7 @@ def main():
         pass
     hbm_peak, hbm_src = (peaks["hbm_gbs"], "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
     fp64_peak = binding.mhd_probe_fp64_flops(patch.stream()) / 1e12
-    oc = json.load(open(os.path.join(ROOT, "tests", "golden", "op_counts.json")))["c5" if m1 else "c1"]
+    oc = json.load(open(os.path.join(ROOT, "tests", "golden", "op_counts.json")))[args.workload[:2]]
     pts_per_zone = patch.npts / zones
     # algorithmic flops per zone and launch of each kernel class (the oracle's count of the step(s) the kernel performs)
     alg_flops = {"fill_ghosts": 0.0, "con2prim": oc["con2prim_per_point"]["flops"] * pts_per_zone,

@@ -71,7 +71,8 @@ def count(cfg):
 
 
 def main():
-    res = {"c1": count(synth.config1(n=16)), "c5": count(synth.config5(n=16, crop_on_star=True))}
+    res = {"c1": count(synth.config1(n=16)), "c3": count(synth.config3(n=16)), "c4": count(synth.config4(n=16)),
+           "c5": count(synth.config5(n=16, crop_on_star=True))}
     path = os.path.join(ROOT, "tests", "golden", "op_counts.json")
     with open(path, "w") as f:
         json.dump(res, f, indent=1, sort_keys=True)
