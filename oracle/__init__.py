@@ -116,6 +116,7 @@ def _load(counting):
         L.orc_m1_rhs.argtypes = [vp, vp, vp, vp, vp]
         L.orc_m1_implicit.argtypes = [vp, vp, vp, vp, vp, f64, vp]
         L.orc_m1_backreaction.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_m1_gravity.argtypes = [vp, vp, vp, vp, vp]
         L.orc_evolve_imex.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, f64, i32]
     return _libs[counting]
 
@@ -286,6 +287,12 @@ def _m1_backreaction(self, U, P, R, K):
     return K
 
 
+def _m1_gravity(self, U, P, V, K):
+    """adds the radiation terms of the CCZ4 matter sources (R6) to K in place"""
+    lib().orc_m1_gravity(self.h, _ptr(U), _ptr(P), _ptr(V), _ptr(K))
+    return K
+
+
 def _evolve_imex(self, U, V, bc, a_expl, w_expl, a_impl, w_impl, dt, n_steps):
     P = np.zeros((NPRIM,) + self.shape)
     flags = np.zeros(self.shape, dtype=np.uint8)
@@ -299,4 +306,5 @@ Oracle.m1_implicit_point = _m1_implicit_point
 Oracle.m1_rhs = _m1_rhs
 Oracle.m1_implicit = _m1_implicit
 Oracle.m1_backreaction = _m1_backreaction
+Oracle.m1_gravity = _m1_gravity
 Oracle.evolve_imex = _evolve_imex

@@ -140,6 +140,7 @@ uint8_t m1_implicit_point(const Params& par, int species, const double Vstar[5],
 void m1_rhs(const Params& par, const Grid& g, const double* U, const double* P, const double* V, double* KV);          // a11: explicit part
 void m1_implicit(const Params& par, const Grid& g, const double* U, const double* P, double* V, double* R, double adt, uint8_t* flags);  // a12
 void m1_backreaction(const Params& par, const Grid& g, const double* U, const double* P, const double* R, double* K);  // a8 (M1 part)
+void m1_gravity(const Params& par, const Grid& g, const double* U, const double* P, const double* V, double* K);       // a4 (M1 part, R6)
 void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double* P, uint8_t* flags, const int bc[6], int stages,
                  const double* a_expl, const double* w_expl, const double* a_impl, const double* w_impl, double dt, int n_steps);
 

@@ -100,6 +100,7 @@ void orc_m1_implicit(void* hh, const double* U, const double* P, double* V, doub
   Handle* h = (Handle*)hh; m1_implicit(h->par, h->grid, U, P, V, R, adt, flags);
 }
 void orc_m1_backreaction(void* hh, const double* U, const double* P, const double* R, double* K) { Handle* h = (Handle*)hh; m1_backreaction(h->par, h->grid, U, P, R, K); }
+void orc_m1_gravity(void* hh, const double* U, const double* P, const double* V, double* K) { Handle* h = (Handle*)hh; m1_gravity(h->par, h->grid, U, P, V, K); }
 void orc_evolve_imex(void* hh, double* U, double* V, double* P, uint8_t* flags, const int* bc, int stages, const double* ae, const double* we,
                      const double* ai, const double* wi, double dt, int n_steps) {
   Handle* h = (Handle*)hh;

@@ -198,6 +198,43 @@ void m1_backreaction(const Params& par, const Grid& G, const double* U, const do
   }
 }
 
+// a4 with M1 on (R6, second half): the radiation energy density, momentum density and stresses of all species are added to
+// the matter sources of the CCZ4 equations. They enter Eqs. (14), (16), (17), (19) linearly:
+//   d_t K^      += alpha 4 pi G (E + S),            S = gamma^ij P_ij
+//   d_t Theta   -= alpha 8 pi G E
+//   d_t A~_ij   -= alpha 8 pi G chi [P_ij - gamma~_ij gamma~^kl P_kl / 3]
+//   d_t Gamma^^i -= 16 pi G alpha gamma~^ij F_j
+void m1_gravity(const Params& par, const Grid& G, const double* U, const double* P, const double* V, double* K) {
+  const size_t n = G.npts();
+  const int ng = G.ng;
+  const double G8 = 8.0 * 3.14159265358979323846 * par.grav_G;
+  if (G8 == 0.0) return;
+  for (int kk = ng; kk < G.nz + ng; ++kk) for (int jj = ng; jj < G.ny + ng; ++jj) for (int ii = ng; ii < G.nx + ng; ++ii) {
+    const size_t p = G.idx(ii, jj, kk);
+    GeoPt q;
+    load_geo(G, U, P, p, q);
+    double E = 0.0, F[3] = {0, 0, 0}, Pij[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    for (int s = 0; s < NSPECIES; ++s) {
+      const double Es = V[(size_t)(5 * s + 1) * n + p] / q.sg;
+      const double Fs[3] = {V[(size_t)(5 * s + 2) * n + p] / q.sg, V[(size_t)(5 * s + 3) * n + p] / q.sg, V[(size_t)(5 * s + 4) * n + p] / q.sg};
+      const M1Closure c = m1_closure_point(Es, Fs, q.vu, q.W, q.gl, q.gu);
+      E += Es;
+      for (int i = 0; i < 3; ++i) { F[i] += Fs[i]; for (int j = 0; j < 3; ++j) Pij[i][j] += c.P[i][j]; }
+    }
+    double S = 0.0;
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) S += q.gu[i][j] * Pij[i][j];
+    K[(size_t)KHAT * n + p] += q.al * 0.5 * G8 * (E + S);
+    K[(size_t)THETA * n + p] -= q.al * G8 * E;
+    for (int i = 0; i < 3; ++i) for (int j = i; j < 3; ++j)
+      K[(size_t)(AXX + SYMP[i][j]) * n + p] -= q.al * G8 * q.chi * (Pij[i][j] - q.gt[i][j] * (S / q.chi) / 3.0);
+    for (int i = 0; i < 3; ++i) {
+      double Fu = 0.0;                                   // gamma~^ij F_j = gamma^ij F_j / chi
+      for (int j = 0; j < 3; ++j) Fu += q.gu[i][j] / q.chi * F[j];
+      K[(size_t)(GAMX + i) * n + p] -= 2.0 * q.al * G8 * Fu;
+    }
+  }
+}
+
 void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double* P, uint8_t* flags, const int bc[6], int stages,
                  const double* ae, const double* we, const double* ai, const double* wi, double dt, int n_steps) {
   const size_t nu = (size_t)NSTATE * g.npts(), nv = (size_t)NM1 * g.npts();
@@ -224,6 +261,7 @@ void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double*
       m1_implicit(par, g, U, P, V, R[s].data(), ai[(size_t)s * stages + s] * dt, flags);   // (C4)
       rhs(par, g, U, P, K[s].data());
       m1_backreaction(par, g, U, P, R[s].data(), K[s].data());
+      m1_gravity(par, g, U, P, V, K[s].data());
       m1_rhs(par, g, U, P, V, KV[s].data());
     }
     rk_combine(g, NSTATE, U, U0.data(), stages, Kp.data(), we, dt);

@@ -211,3 +211,56 @@ def test_odd_even_switch_fires_on_a_zigzag_only(oracle_mod):
         o = oracle_mod.Oracle(synth.default_params(m1_kappa0=1e6, m1_odd_even=oe), n, n, n, ng, dx)
         res.append(o.m1_rhs(U, P, V)[1][I])
     assert np.array_equal(res[0], res[1])
+
+
+def test_radiation_gravitates_like_an_equal_fluid(oracle_mod):
+    """R6, second half: radiation that is isotropic in the frame of a fluid moving with v^i (H = 0: the closure is exact there)
+    has the stress-energy of a perfect fluid with p = e / 3 moving with the same v^i. The matter sources of Eqs. (14), (16),
+    (17), (19) are linear in T^ab, so  rhs(fluid A + radiation) - rhs(fluid A) = rhs(fluid R) - rhs(vacuum)  to rounding, with
+    fluid R: Gamma - 1 = (1 + eps_R) / (3 eps_R). Spacetime: the perturbed one of config 1 (non-trivial alpha, chi, gamma~_ij)."""
+    cfg = synth.config1(n=8, gauge_perturbation=True)
+    n = cfg["n"]
+    vu = (0.2, -0.1, 0.15)
+
+    def spacetime_rhs(rho, eps, gamma, moving, V=None, grav_G=1.0):
+        par = synth.default_params(eos_gamma=gamma, grav_G=grav_G)
+        o = oracle_mod.Oracle(par, n[0], n[1], n[2], cfg["ng"], cfg["dx"])
+        U, P = cfg["U"].copy(), np.zeros_like(cfg["P"])
+        U[28:32] = 0.0                                   # no magnetic field, no cleaning scalar
+        P[synth.RHO], P[synth.EPS], P[synth.YE] = rho, eps, 0.3
+        for i in range(3):
+            P[synth.VX + i] = vu[i] if moving else 0.0
+        o.prim2con(U, P)
+        Pc, F = o.con2prim(U)
+        K = o.rhs(U, Pc, "ccz4")
+        if V is not None:
+            o.m1_gravity(U, Pc, V, K)
+        return K[:22, 3:-3, 3:-3, 3:-3], U, Pc
+
+    X = synth.mesh(n[0], n[1], n[2], cfg["ng"], cfg["dx"])[0]
+    J = 4e-4 * (1.0 + 0.2 * np.sin(2 * np.pi * X / (n[0] * cfg["dx"])))      # comoving energy density of the radiation
+    KA, U, Pc = spacetime_rhs(1e-3, 0.1, 2.0, True)
+    chi = U[synth.CHI]
+    gl = [[U[synth.SYM[i][j]] / chi for j in range(3)] for i in range(3)]
+    vl = [sum(gl[i][j] * vu[j] for j in range(3)) for i in range(3)]
+    W2 = 1.0 / (1.0 - sum(vl[i] * vu[i] for i in range(3)))
+    assert np.abs(Pc[synth.WLOR] ** 2 / W2 - 1).max() < 1e-12
+    E = 4.0 / 3.0 * J * W2 - J / 3.0
+    sg = chi ** -1.5
+    V = np.zeros((15,) + X.shape)
+    for s, w in enumerate((0.5, 0.3, 0.2)):              # split over the three species
+        V[5 * s] = 1e-30
+        V[5 * s + 1] = sg * w * E
+        for i in range(3):
+            V[5 * s + 2 + i] = sg * w * 4.0 / 3.0 * J * W2 * vl[i]
+    KAR, _, _ = spacetime_rhs(1e-3, 0.1, 2.0, True, V)
+    eps_R = 500.0                                        # below eps_max = 1e3 of the error policy
+    KR, _, _ = spacetime_rhs(J / (1.0 + eps_R), eps_R, 1.0 + (1.0 + eps_R) / (3.0 * eps_R), True)
+    K0, _, _ = spacetime_rhs(1e-3, 0.1, 2.0, False, grav_G=0.0)   # geometry alone: matter decoupled (R29)
+    lhs, rhs_ = KAR - KA, KR - K0
+    scale = np.abs(rhs_).reshape(22, -1).max(axis=1)
+    live = scale > 1e-12
+    assert live.sum() >= 11                              # K^, Theta, six A~_ij, three Gamma^^i
+    err = np.abs(lhs - rhs_).reshape(22, -1).max(axis=1)
+    assert np.all(err[live] < 1e-8 * scale[live]), (err / np.maximum(scale, 1e-300), scale)
+    assert np.all(err[~live] < 1e-14)
