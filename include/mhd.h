@@ -180,9 +180,12 @@ int mhd_m1_rhs(mhd_patch *p, int slot_V, int slot_KV, void *cuda_stream);
 /* a8 (M1 part) — neutrino back-reaction on the fluid: slot_K[taubar, Sbar_i] -= sum_species slot_R[Ebar, Fbar_i],
  * slot_K[DYebar] -= m_b (R[Nbar]_nue - R[Nbar]_anti-nue), interior. */
 int mhd_m1_backreaction(mhd_patch *p, int slot_R, int slot_K, void *cuda_stream);
+/* a4 (M1 part, reading R6) — radiation E, F_i, P_ij of the three species added to the matter sources of the CCZ4 equations
+ * (Eqs. 14, 16, 17, 19) in slot_K, interior. P_ij is taken from MHD_SLOT_M1WORK: call after mhd_m1_rhs on the same slot_V. */
+int mhd_m1_gravity(mhd_patch *p, int slot_V, int slot_K, void *cuda_stream);
 /* n_steps full IMEX steps (Eq. 53, App. C steps C3-C4) of the coupled system, device resident; the tableau must carry
  * a_impl (row-major, lower triangular incl. diagonal) and w_impl. Per stage: combine -> fill -> con2prim -> implicit solve ->
- * rhs + back-reaction -> M1 explicit part. */
+ * M1 explicit part -> rhs + back-reaction + radiation in the CCZ4 sources. */
 int mhd_advance_imex(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
 
 /* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */

@@ -56,7 +56,7 @@ class mhd_status(ctypes.Structure):
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
-           "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_advance_imex"]
+           "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex"]
 NKERNELS = 12
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
                   "m1_point", "m1_div", "m1_implicit"]
@@ -92,6 +92,7 @@ def lib():
         L.mhd_m1_implicit.argtypes = [_p, _i, _i, _d, _p]
         L.mhd_m1_rhs.argtypes = [_p, _i, _i, _p]
         L.mhd_m1_backreaction.argtypes = [_p, _i, _i, _p]
+        L.mhd_m1_gravity.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
         if L.mhd_desc_sizeof() != ctypes.sizeof(mhd_patch_desc):
@@ -210,6 +211,10 @@ def mhd_m1_backreaction(h, slot_R, slot_K, stream=None):
     _check(lib().mhd_m1_backreaction(h, slot_R, slot_K, stream))
 
 
+def mhd_m1_gravity(h, slot_V, slot_K, stream=None):
+    _check(lib().mhd_m1_gravity(h, slot_V, slot_K, stream))
+
+
 def mhd_advance_imex(h, tableau, bc, dt, n_steps, stream=None):
     _check(lib().mhd_advance_imex(h, ctypes.byref(tableau), _bc(bc), dt, n_steps, stream))
 
@@ -284,6 +289,10 @@ class Patch:
 
     def m1_backreaction(self, j=1):
         mhd_m1_backreaction(self.h, SLOT_R1 + j - 1, SLOT_K1 + j - 1, self.stream())
+
+    def m1_gravity(self, j=1):
+        """radiation terms of the CCZ4 matter sources added to K_j (after m1_rhs on the same V)"""
+        mhd_m1_gravity(self.h, SLOT_V, SLOT_K1 + j - 1, self.stream())
 
     def advance_imex(self, tableau, bc, dt, n_steps):
         mhd_advance_imex(self.h, tableau, bc, dt, n_steps, self.stream())

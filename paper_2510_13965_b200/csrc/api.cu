@@ -280,6 +280,16 @@ int mhd_m1_backreaction(mhd_patch* p, int slot_R, int slot_K, void* stream) {
          == cudaSuccess ? MHD_OK : MHD_E_CUDA;
 }
 
+int mhd_m1_gravity(mhd_patch* p, int slot_V, int slot_K, void* stream) {
+  if (!p || !is_m1_slot(slot_V) || !is_state_slot(slot_K)) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  if (!slot_ok(p, slot_V) || !slot_ok(p, slot_K) || !slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_M1WORK)) return MHD_E_UNBOUND;
+  Timed tm(p, 11, (cudaStream_t)stream);
+  return launch_m1_gravity(p->dims, p->par, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, dptr(p, slot_V), p->slot[slot_V].stride,
+                           dptr(p, MHD_SLOT_M1WORK), p->slot[MHD_SLOT_M1WORK].stride, dptr(p, slot_K), p->slot[slot_K].stride, (cudaStream_t)stream)
+         == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
 // V <- V0 + dt (sum_j ce[j] KV_j + sum_j ci[j] R_j), j < nj
 static int m1_combine(mhd_patch* p, int nj, const double* ce, const double* ci, double dt, cudaStream_t s) {
   const double* Kp[MHD_MAX_STAGES];
@@ -326,9 +336,10 @@ int mhd_advance_imex(mhd_patch* p, const mhd_tableau* t, const int bc[6], double
         CK(mhd_fill_ghosts(p, MHD_SLOT_V, bc, s));
       }
       CK(mhd_m1_implicit(p, MHD_SLOT_V, MHD_SLOT_R1 + st, t->a_impl[(size_t)st * q + st] * dt, s));   // (C4)
+      CK(mhd_m1_rhs(p, MHD_SLOT_V, MHD_SLOT_KV1 + st, s));                            // also leaves P_ij of V^(i) in the M1 work slot
       CK(mhd_rhs(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st, s));
       CK(mhd_m1_backreaction(p, MHD_SLOT_R1 + st, MHD_SLOT_K1 + st, s));
-      CK(mhd_m1_rhs(p, MHD_SLOT_V, MHD_SLOT_KV1 + st, s));
+      CK(mhd_m1_gravity(p, MHD_SLOT_V, MHD_SLOT_K1 + st, s));
     }
     CK(mhd_rk_stage(p, t, q, dt, s));
     CK(m1_combine(p, q, t->w_expl, t->w_impl, dt, s));

@@ -488,3 +488,53 @@ cudaError_t launch_m1_backreact(const Dims& d, const Par& par, const double* R, 
 }
 
 }  // namespace mhd
+
+// ---------------------------------------------------------------------------------------------------------------
+// a4 with M1 on (R6, second half): E, F_i, P_ij of the three species added to the matter sources of Eqs. (14), (16), (17),
+// (19), which are linear in them. P_ij is read from the M1 work slot (written by k_m1_point for the same V).
+namespace mhd {
+__global__ void __launch_bounds__(128) k_m1_gravity(const __grid_constant__ Dims d, double G8, const double* __restrict__ U, size_t su,
+                                                    const double* __restrict__ V, size_t sv, const double* __restrict__ Wk, size_t sw,
+                                                    double* __restrict__ K, size_t sk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.nx) return;
+  const size_t pt = (size_t)(blockIdx.z + d.ng) * d.sz + (size_t)(blockIdx.y + d.ng) * d.sy + (i + d.ng);
+  double g[6], gi[6];
+#pragma unroll
+  for (int a = 0; a < 6; ++a) g[a] = __ldg(U + (size_t)(GXX + a) * su + pt);
+  const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
+  {
+    const double idet = 1.0 / (g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]));
+    gi[0] = (g[3] * g[5] - g[4] * g[4]) * idet; gi[1] = (g[2] * g[4] - g[1] * g[5]) * idet; gi[2] = (g[1] * g[4] - g[2] * g[3]) * idet;
+    gi[3] = (g[0] * g[5] - g[2] * g[2]) * idet; gi[4] = (g[1] * g[2] - g[0] * g[4]) * idet; gi[5] = (g[0] * g[3] - g[1] * g[1]) * idet;
+  }
+  const double isg = chi * sqrt(chi);
+  double E = 0.0, F[3] = {0.0, 0.0, 0.0}, Pl[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    E += __ldg(V + (size_t)(5 * s + 1) * sv + pt) * isg;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) F[a] += __ldg(V + (size_t)(5 * s + 2 + a) * sv + pt) * isg;
+#pragma unroll
+    for (int a = 0; a < 6; ++a) Pl[a] += __ldg(Wk + (size_t)(M1W * s + 19 + a) * sw + pt);
+  }
+  // gamma~^kl P_kl  (S = gamma^kl P_kl = chi times it)
+  const double trt = gi[0] * Pl[0] + gi[3] * Pl[3] + gi[5] * Pl[5] + 2.0 * (gi[1] * Pl[1] + gi[2] * Pl[2] + gi[4] * Pl[4]);
+  K[(size_t)KHAT * sk + pt] += al * 0.5 * G8 * (E + chi * trt);
+  K[(size_t)THETA * sk + pt] -= al * G8 * E;
+#pragma unroll
+  for (int a = 0; a < 6; ++a) K[(size_t)(AXX + a) * sk + pt] -= al * G8 * chi * (Pl[a] - g[a] * trt * (1.0 / 3.0));
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+    K[(size_t)(GAMX + a) * sk + pt] -= 2.0 * al * G8 * (gi[sy(a, 0)] * F[0] + gi[sy(a, 1)] * F[1] + gi[sy(a, 2)] * F[2]);
+}
+
+cudaError_t launch_m1_gravity(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
+                              double* K, size_t sk, cudaStream_t s) {
+  const double G8 = 8.0 * 3.14159265358979323846 * par.grav_G;
+  if (G8 == 0.0) return cudaSuccess;
+  dim3 grid((d.nx + 127) / 128, d.ny, d.nz);
+  k_m1_gravity<<<grid, 128, 0, s>>>(d, G8, U, su, V, sv, Wk, sw, K, sk);
+  return cudaGetLastError();
+}
+}  // namespace mhd

@@ -79,5 +79,7 @@ cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t
                           double* KV, size_t sk, cudaStream_t s);
 cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* V, size_t sv,
                                double* R, size_t sr, double adt, uint8_t* flags, cudaStream_t s);
+cudaError_t launch_m1_gravity(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
+                              double* K, size_t sk, cudaStream_t s);
 cudaError_t launch_m1_backreact(const Dims& d, const Par& par, const double* R, size_t sr, double* K, size_t sk, cudaStream_t s);
 }  // namespace mhd

@@ -406,6 +406,7 @@ def test_config5_m1_pieces_parity(oracle_mod, kappa0):
     KVo = o.m1_rhs(Uo, Po, Vo)
     Ko = o.rhs(Uo, Po)
     o.m1_backreaction(Uo, Po, Ro, Ko)
+    o.m1_gravity(Uo, Po, Vo, Ko)
     patch.upload(U=U)
     patch.V.copy_(patch.torch.as_tensor(V))
     patch.fill_ghosts(cfg["bc"])
@@ -427,6 +428,7 @@ def test_config5_m1_pieces_parity(oracle_mod, kappa0):
     assert np.all(num / den < 1e-11), num / den
     Kg = patch.rhs(1)
     patch.m1_backreaction(1)
+    patch.m1_gravity(1)
     rk, dk = _rel(Kg.cpu().numpy(), Ko)
     assert np.all(rk[dk > 0] < 1e-11), rk
     patch.close()
