@@ -69,14 +69,15 @@ __device__ __forceinline__ TPos tab_T_of_loge(const Par& q, TPos r, TPos y, doub
   return o;
 }
 
+template <int KIND>
 __device__ __forceinline__ Eos eos_eval(const Par& q, double rho, double eps, double ye) {
   Eos o;
-  if (q.eos_kind == 0) {
+  if (KIND == 0) {
     o.p = (q.eos_gamma - 1.0) * rho * eps;
     o.T = o.p / rho;
     const double h = 1.0 + eps + o.p / rho;
     o.cs2 = q.eos_gamma * o.p / (rho * h);
-  } else if (q.eos_kind == 1) {
+  } else if (KIND == 1) {
     double pc, ec, G;
     pp_cold(q, rho, pc, ec, G);
     const double gth = q.eos_gamma_th - 1.0;
@@ -95,9 +96,10 @@ __device__ __forceinline__ Eos eos_eval(const Par& q, double rho, double eps, do
   }
   return o;
 }
+template <int KIND>
 __device__ __forceinline__ void eos_eps_range(const Par& q, double rho, double ye, double& emin, double& emax) {
-  if (q.eos_kind == 0) { emin = q.eps_min; emax = q.eps_max; }
-  else if (q.eos_kind == 1) {
+  if (KIND == 0) { emin = q.eps_min; emax = q.eps_max; }
+  else if (KIND == 1) {
     double pc, ec, G;
     pp_cold(q, rho, pc, ec, G);
     emin = fmax(q.eps_min, ec); emax = q.eps_max;
@@ -192,6 +194,7 @@ __device__ __forceinline__ void tab_p_of_eps(const Par& q, TPos y, double rho, d
   p = pow(10.0, tab_tri(q, q.tab_logp, r, t, y));
 }
 
+template <int KIND>
 struct Master {
   double D, q, r2, B2, rB2, B2rp2, ye, h0, v02, rho_lo, rho_hi;
   double W, eps_raw;   // by-products of the last evaluation
@@ -214,12 +217,12 @@ struct Master {
     rho = fmax(fmin(rho_hi, rho), rho_lo);
     eps_raw = W * ((qbar - mu * rb2) + v2 / (1.0 + iW));                                             // (D12): W^2/(1+W) = W/(1+1/W)
     double eps, p;
-    if (par.eos_kind == 2) tab_p_of_eps(par, ypos, rho, eps_raw, t_hint, p, eps);
+    if (KIND == 2) tab_p_of_eps(par, ypos, rho, eps_raw, t_hint, p, eps);
     else {
       double emin, emax;
-      eos_eps_range(par, rho, ye, emin, emax);
+      eos_eps_range<KIND>(par, rho, ye, emin, emax);
       eps = fmax(fmin(emax, eps_raw), emin);
-      p = eos_eval(par, rho, eps, ye).p;
+      p = eos_eval<KIND>(par, rho, eps, ye).p;
     }
     const double a = p / (rho * (1.0 + eps));
     const double nuA = (1.0 + a) * (1.0 + eps) * iW;
@@ -229,6 +232,7 @@ struct Master {
 };
 
 // ------------------------------------------------------------------------------------------ kernels
+template <int KIND>
 __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dims d, const __grid_constant__ Par par,
                                                   double* __restrict__ U, size_t su, double* __restrict__ P, size_t sp,
                                                   uint8_t* __restrict__ flags) {
@@ -253,7 +257,7 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
   if (!atmo) {
     const double tau = u(TAUBAR) * isg;
     const double Sl[3] = {u(SXBAR) * isg, u(SYBAR) * isg, u(SZBAR) * isg};
-    Master s;
+    Master<KIND> s;
     const double iD = 1.0 / D, isD = 1.0 / sqrt(D);
     s.D = D; s.q = tau * iD;                                                         // (D1)
     const double rl[3] = {Sl[0] * iD, Sl[1] * iD, Sl[2] * iD};
@@ -263,15 +267,15 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
     sym_apply(gl, Bs, Bsl);
     s.ye = fmax(fmin(ye, par.ye_max), par.ye_min);
     s.t_hint = -1;
-    if (par.eos_kind == 2) s.ypos = tab_locate(s.ye, par.ye0, par.dye, par.n_ye);
+    if (KIND == 2) s.ypos = tab_locate(s.ye, par.ye0, par.dye, par.n_ye);
     s.r2 = ru[0] * rl[0] + ru[1] * rl[1] + ru[2] * rl[2];                            // (D2)
     s.B2 = Bs[0] * Bsl[0] + Bs[1] * Bsl[1] + Bs[2] * Bsl[2];
     const double rB = rl[0] * Bs[0] + rl[1] * Bs[1] + rl[2] * Bs[2];
     s.rB2 = rB * rB;
     s.B2rp2 = s.B2 * s.r2 - s.rB2;
-    s.h0 = par.eos_kind == 2 ? par.tab_h0 : 1.0;
+    s.h0 = KIND == 2 ? par.tab_h0 : 1.0;
     s.v02 = s.r2 / (s.h0 * s.h0 + s.r2);
-    if (par.eos_kind == 2) { s.rho_lo = pow(10.0, par.lr0); s.rho_hi = pow(10.0, par.lr0 + par.dlr * (par.n_rho - 1)); }
+    if (KIND == 2) { s.rho_lo = pow(10.0, par.lr0); s.rho_hi = pow(10.0, par.lr0 + par.dlr * (par.n_rho - 1)); }
     else { s.rho_lo = 0.0; s.rho_hi = par.rho_max; }
     bool ok1 = true, ok2 = true;
     const double mub = 1.0 / s.h0;
@@ -316,7 +320,7 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
       const bool allowed = (rho < par.rho_low) || bh;
       if (rho > par.rho_max) flag |= MHD_FLAG_FATAL;                                 // rule 2
       double emin, emax;
-      eos_eps_range(par, fmax(fmin(s.rho_hi, rho), s.rho_lo), s.ye, emin, emax);
+      eos_eps_range<KIND>(par, fmax(fmin(s.rho_hi, rho), s.rho_lo), s.ye, emin, emax);
       if (eps < emin) { eps = emin; flag |= MHD_FLAG_EPS_LO; changed = true; }       // rule 3
       else if (eps > emax) { eps = emax; changed = true; flag |= allowed ? MHD_FLAG_EPS_HI : (MHD_FLAG_EPS_HI | MHD_FLAG_FATAL); }   // rule 4
       if (W > par.w_max) {                                                           // rule 5
@@ -338,12 +342,12 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
   if (atmo) {
     flag |= MHD_FLAG_ATMO;
     rho = par.rho_atmo; W = 1.0; v[0] = v[1] = v[2] = 0.0; ye = par.ye_atmo;
-    if (par.eos_kind == 2) eps = eos_eps_of_T(par, rho, par.T_atmo, ye);
-    else if (par.eos_kind == 1) { double emin, emax; eos_eps_range(par, rho, ye, emin, emax); eps = emin + par.eps_atmo; }
+    if (KIND == 2) eps = eos_eps_of_T(par, rho, par.T_atmo, ye);
+    else if (KIND == 1) { double emin, emax; eos_eps_range<KIND>(par, rho, ye, emin, emax); eps = emin + par.eps_atmo; }
     else eps = par.eps_atmo;
     changed = true;
   }
-  const Eos e = eos_eval(par, rho, eps, ye);
+  const Eos e = eos_eval<KIND>(par, rho, eps, ye);
   P[(size_t)RHO * sp + pt] = rho; P[(size_t)YE * sp + pt] = ye; P[(size_t)EPS * sp + pt] = eps; P[(size_t)PRESS * sp + pt] = e.p;
   P[(size_t)VX * sp + pt] = v[0]; P[(size_t)VY * sp + pt] = v[1]; P[(size_t)VZ * sp + pt] = v[2];
   P[(size_t)WLOR * sp + pt] = W; P[(size_t)TEMP * sp + pt] = e.T; P[(size_t)CS2 * sp + pt] = e.cs2;
@@ -356,6 +360,7 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
   }
 }
 
+template <int KIND>
 __global__ void __launch_bounds__(128) k_prim2con(const __grid_constant__ Dims d, const __grid_constant__ Par par,
                                                   double* __restrict__ U, size_t su, double* __restrict__ P, size_t sp) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -369,7 +374,7 @@ __global__ void __launch_bounds__(128) k_prim2con(const __grid_constant__ Dims d
   const double rho = pr(RHO), eps = pr(EPS), ye = pr(YE);
   const double v[3] = {pr(VX), pr(VY), pr(VZ)};
   const double B[3] = {u(BXBAR) * isg, u(BYBAR) * isg, u(BZBAR) * isg};
-  const Eos e = eos_eval(par, rho, eps, ye);
+  const Eos e = eos_eval<KIND>(par, rho, eps, ye);
   double D, tau, S[3], W;
   cons_from_prim(gl, rho, eps, e.p, v, B, D, tau, S, W);
   pr(PRESS) = e.p; pr(TEMP) = e.T; pr(CS2) = e.cs2; pr(WLOR) = W;
@@ -378,11 +383,17 @@ __global__ void __launch_bounds__(128) k_prim2con(const __grid_constant__ Dims d
 }
 
 cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, cudaStream_t s) {
-  k_con2prim<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, flags);
+  const unsigned nb = (unsigned)((d.npts + 127) / 128);
+  if (par.eos_kind == 0) k_con2prim<0><<<nb, 128, 0, s>>>(d, par, U, su, P, sp, flags);
+  else if (par.eos_kind == 1) k_con2prim<1><<<nb, 128, 0, s>>>(d, par, U, su, P, sp, flags);
+  else k_con2prim<2><<<nb, 128, 0, s>>>(d, par, U, su, P, sp, flags);
   return cudaGetLastError();
 }
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s) {
-  k_prim2con<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp);
+  const unsigned nb = (unsigned)((d.npts + 127) / 128);
+  if (par.eos_kind == 0) k_prim2con<0><<<nb, 128, 0, s>>>(d, par, U, su, P, sp);
+  else if (par.eos_kind == 1) k_prim2con<1><<<nb, 128, 0, s>>>(d, par, U, su, P, sp);
+  else k_prim2con<2><<<nb, 128, 0, s>>>(d, par, U, su, P, sp);
   return cudaGetLastError();
 }
 
