@@ -264,6 +264,9 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     unsigned mask = 0;
 #pragma unroll
     for (int n = 0; n < SEG + 6; ++n) { fc[n] = __ldg(f + node(n)); uc[n] = __ldg(u + node(n)); }
+    double kold[SEG];                                          // K is read-modify-write: fetched with the column, not after the arithmetic
+#pragma unroll
+    for (int m = 1; m <= SEG; ++m) kold[m - 1] = (active && c0 + m - 1 < nline) ? k[base + (long long)(g0 + m + 2) * ls] : 0.0;
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
       acc[m] = flux_hat2(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
@@ -279,7 +282,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     for (int m = 1; m <= SEG; ++m)
       if (active && c0 + m - 1 < nline) {
         const long long pt = base + (long long)(g0 + m + 2) * ls;       // zone c0 + m - 1
-        k[pt] -= (acc[m] - acc[m - 1]) * hih;                           // Eq. (64)
+        k[pt] = kold[m - 1] - (acc[m] - acc[m - 1]) * hih;              // Eq. (64)
       }
   }
 }
@@ -310,8 +313,10 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   }
   const double hih = 0.5 / d.dx;
   const bool store = lane < 31 && zone < d.nx;
-  double acc[10];
+  double acc[10], kold[10];
   unsigned mask = 0;
+#pragma unroll
+  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + base + zone + d.ng] : 0.0;   // read-modify-write: fetched up front
   double fw[6], uw[6];
 #pragma unroll
   for (int n = 0; n < 6; ++n) { fw[n] = __ldg(Wk + node(n)); uw[n] = __ldg(U + (size_t)DBAR * su + node(n)); }
@@ -338,7 +343,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
     if (mask & (1u << (2 * a))) fl += q.corr[(2 * a) * 32 + lane];
     if (mask & (1u << (2 * a + 1))) fl += q.corr[(2 * a + 1) * 32 + lane];
     const double fr = __shfl_down_sync(FULL, fl, 1);           // F^ at zone + 1/2
-    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] -= (fr - fl) * hih;
+    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] = kold[a] - (fr - fl) * hih;
   }
 }
 
