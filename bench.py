@@ -274,6 +274,10 @@ def main():
     alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "ccz4_algebra": 22 + 10 + 5 + 32, "adv_ko": 22 * 3, "recon_x": 21 + 20,
                    "recon_y": 21 + 20, "recon_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33,
                    "m1_point": 21 + 15 + 75, "m1_div": 15 + 75 + 22 + 15, "m1_implicit": 21 + 15 + 30}
+    # measured DRAM traffic per zone and launch, bytes: dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture
+    # profiles/r1g_ncu_full_c4_128.md (128^3; per-zone figures carry over to 256^3, the tiles are the same)
+    ncu_traffic = {"ccz4_algebra": 592.9, "adv_ko": 634.2, "point_flux": 546.8, "recon_x": 332.2, "recon_y": 355.3, "recon_z": 359.7,
+                   "rk_combine": 802.8, "con2prim": 259.7, "fill_ghosts": 79.3}
     total_kernel_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
@@ -285,7 +289,9 @@ def main():
     step_tflops = F_alg * value / world / 1e12
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
                 "peak_source": "measured: FP64 DFMA probe of the library (mhd_probe_fp64_flops); nominal 37.2",
-                "traffic": None, "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
+                "traffic": ncu_traffic[dom] * zones if dom in ncu_traffic else None,
+                "traffic_source": "bytes per launch = ncu dram bytes per zone (profiles/r1g, 128^3 capture) x zones of this run",
+                "alg_bytes": alg_doubles[dom] * 8.0 * zones, "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
                 "share_of_step": dom_ms / total_kernel_ms if total_kernel_ms else None,
                 "alg_flops_per_zone": alg_flops[dom],
                 "hbm": {"achieved_gbs": alg_doubles[dom] * 8.0 * zones / sec_per_launch / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src},
