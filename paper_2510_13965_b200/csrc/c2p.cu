@@ -90,8 +90,8 @@ __device__ __forceinline__ Eos eos_eval(const Par& q, double rho, double eps, do
     const TPos r = tab_locate(log10(rho), q.lr0, q.dlr, q.n_rho);
     const TPos y = tab_locate(ye, q.ye0, q.dye, q.n_ye);
     const TPos t = tab_T_of_loge(q, r, y, log10(eps + q.tab_eps_shift));
-    o.p = pow(10.0, tab_tri(q, q.tab_logp, r, t, y));
-    o.T = pow(10.0, q.lT0 + ((double)t.i + t.w) * q.dlT);
+    o.p = exp10(tab_tri(q, q.tab_logp, r, t, y));
+    o.T = exp10(q.lT0 + ((double)t.i + t.w) * q.dlT);
     o.cs2 = tab_tri(q, q.tab_cs2, r, t, y);
   }
   return o;
@@ -106,15 +106,15 @@ __device__ __forceinline__ void eos_eps_range(const Par& q, double rho, double y
   } else {
     const TPos r = tab_locate(log10(rho), q.lr0, q.dlr, q.n_rho);
     const TPos y = tab_locate(ye, q.ye0, q.dye, q.n_ye);
-    emin = pow(10.0, tab_col(q, q.tab_loge, r, y, 0)) - q.tab_eps_shift;
-    emax = pow(10.0, tab_col(q, q.tab_loge, r, y, q.n_T - 1)) - q.tab_eps_shift;
+    emin = exp10(tab_col(q, q.tab_loge, r, y, 0)) - q.tab_eps_shift;
+    emax = exp10(tab_col(q, q.tab_loge, r, y, q.n_T - 1)) - q.tab_eps_shift;
   }
 }
 __device__ __forceinline__ double eos_eps_of_T(const Par& q, double rho, double T, double ye) {
   const TPos r = tab_locate(log10(rho), q.lr0, q.dlr, q.n_rho);
   const TPos y = tab_locate(ye, q.ye0, q.dye, q.n_ye);
   const TPos t = tab_locate(log10(T), q.lT0, q.dlT, q.n_T);
-  return pow(10.0, tab_tri(q, q.tab_loge, r, t, y)) - q.tab_eps_shift;
+  return exp10(tab_tri(q, q.tab_loge, r, t, y)) - q.tab_eps_shift;
 }
 
 // ------------------------------------------------------------------------------------------ metric helpers
@@ -172,8 +172,8 @@ __device__ __forceinline__ void tab_p_of_eps(const Par& q, TPos y, double rho, d
   const double e_min = tab_col(q, q.tab_loge, r, y, 0), e_max = tab_col(q, q.tab_loge, r, y, q.n_T - 1);
   const double le = log10(eps_raw + q.tab_eps_shift);
   TPos t;
-  if (!(le > e_min)) { t.i = 0; t.w = 0.0; eps = pow(10.0, e_min) - q.tab_eps_shift; }
-  else if (le >= e_max) { t.i = q.n_T - 2; t.w = 1.0; eps = pow(10.0, e_max) - q.tab_eps_shift; }
+  if (!(le > e_min)) { t.i = 0; t.w = 0.0; eps = exp10(e_min) - q.tab_eps_shift; }
+  else if (le >= e_max) { t.i = q.n_T - 2; t.w = 1.0; eps = exp10(e_max) - q.tab_eps_shift; }
   else {
     eps = eps_raw;
     int lo = 0, hi = q.n_T - 1;
@@ -191,7 +191,7 @@ __device__ __forceinline__ void tab_p_of_eps(const Par& q, TPos y, double rho, d
     t.i = lo; t.w = (le - e_lo) / (e_hi - e_lo);
     hint = lo;
   }
-  p = pow(10.0, tab_tri(q, q.tab_logp, r, t, y));
+  p = exp10(tab_tri(q, q.tab_logp, r, t, y));
 }
 
 template <int KIND>
@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(128, 4) k_con2prim(const __grid_constant__ Dim
     s.B2rp2 = s.B2 * s.r2 - s.rB2;
     s.h0 = KIND == 2 ? par.tab_h0 : 1.0;
     s.v02 = s.r2 / (s.h0 * s.h0 + s.r2);
-    if (KIND == 2) { s.rho_lo = pow(10.0, par.lr0); s.rho_hi = pow(10.0, par.lr0 + par.dlr * (par.n_rho - 1)); }
+    if (KIND == 2) { s.rho_lo = exp10(par.lr0); s.rho_hi = exp10(par.lr0 + par.dlr * (par.n_rho - 1)); }
     else { s.rho_lo = 0.0; s.rho_hi = par.rho_max; }
     bool ok1 = true, ok2 = true;
     const double mub = 1.0 / s.h0;
