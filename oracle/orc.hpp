@@ -18,7 +18,9 @@
 // MP5 (Eq. 70 on smooth data, monotone on a step), RK (exp series).
 // PARITY UNPINNED: kappa_z/kappa_c/kappa_2 damping terms beyond "vanish with the
 // constraint" and a hand value; atmosphere / error-policy parameter values (R10);
-// outflow boundary order (R17).
+// outflow boundary order (R17); M1: the Phi / A blend of Eq. (77) beyond its limits, the E -> 0 and |F| > E fix-ups (R22),
+// the N equation's closure assumption (Eq. 37), the implicit tableau values (R1), the geometric sources of Eqs. (39)-(40)
+// beyond flat space (their algebra was checked against nabla_a T^ab_rad in SURVEY.md, not in a test).
 #pragma once
 #include <cstddef>
 #include <cstdint>
