@@ -19,8 +19,8 @@
 // PARITY UNPINNED: kappa_z/kappa_c/kappa_2 damping terms beyond "vanish with the
 // constraint" and a hand value; atmosphere / error-policy parameter values (R10);
 // outflow boundary order (R17); M1: the Phi / A blend of Eq. (77) beyond its limits, the E -> 0 and |F| > E fix-ups (R22),
-// the N equation's closure assumption (Eq. 37), the implicit tableau values (R1), the geometric sources of Eqs. (39)-(40)
-// beyond flat space (their algebra was checked against nabla_a T^ab_rad in SURVEY.md, not in a test).
+// the N equation's closure assumption (Eq. 37), the implicit tableau values (R1), the shift- and curvature-dependent geometric sources of
+// Eqs. (39)-(40) (d beta, A~_ij, K^ terms; the d alpha, d chi terms are pinned by the static beam in Schwarzschild).
 #pragma once
 #include <cstddef>
 #include <cstdint>

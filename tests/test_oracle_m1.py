@@ -264,3 +264,43 @@ def test_radiation_gravitates_like_an_equal_fluid(oracle_mod):
     err = np.abs(lhs - rhs_).reshape(22, -1).max(axis=1)
     assert np.all(err[live] < 1e-8 * scale[live]), (err / np.maximum(scale, 1e-300), scale)
     assert np.all(err[~live] < 1e-14)
+
+
+def test_static_radial_beam_in_schwarzschild(oracle_mod):
+    """Pin of the flux brackets AND the geometric sources of Eqs. (38)-(40) in a curved, static spacetime: radiation streaming
+    radially outwards in the Schwarzschild metric in isotropic coordinates (alpha = (1 - M/2r)/(1 + M/2r), gamma_ij = psi^4 delta_ij,
+    psi = 1 + M/2r) is stationary when  alpha^2 psi^6 r^2 F^r = const  (d_r (sqrt(-g) T^r_t) = 0),  E = |F| = psi^2 F^r (free
+    streaming) and N = alpha E (number flux alpha psi^6 r^2 N F^r / E = const; E = N x local energy ~ N / alpha): energy redshifts,
+    number does not.
+    The explicit part F_V of the oracle must then vanish at the order of its centred fluxes (second)."""
+    M, C = 1.0, 1e-3
+    res = {}
+    for n in (16, 32):
+        ng, L = 3, 4.0
+        dx = L / n
+        o = oracle_mod.Oracle(synth.default_params(m1_kappa0=0.0), n, n, n, ng, dx)
+        X, Y, Z = synth.mesh(n, n, n, ng, dx, x0=(4.0, -2.0, -2.0))
+        r = np.sqrt(X * X + Y * Y + Z * Z)
+        psi = 1.0 + M / (2 * r)
+        alpha = (1.0 - M / (2 * r)) / psi
+        U = synth._flat_state(X.shape)
+        U[synth.CHI], U[synth.ALPHA] = psi ** -4, alpha
+        P = np.zeros((10,) + X.shape)
+        P[synth.RHO], P[synth.WLOR], P[synth.TEMP] = 1e-10, 1.0, 1e-8
+        Fr = C / (alpha ** 2 * psi ** 6 * r * r)              # F^r
+        E = psi ** 2 * Fr
+        sg = psi ** 6
+        V = np.zeros((15,) + X.shape)
+        for s in range(3):
+            V[5 * s] = sg * E * alpha
+            V[5 * s + 1] = sg * E
+            for i, xi in enumerate((X, Y, Z)):
+                V[5 * s + 2 + i] = sg * psi ** 4 * Fr * xi / r    # F_i = gamma_ij F^j
+        KV = o.m1_rhs(U, P, V)
+        I = (slice(ng, -ng),) * 3
+        # scale of the individual terms that must cancel: alpha F^x sqrt(gamma) / r ~ flux / length
+        scaleE = np.abs(alpha * sg * Fr / r)[I].max()
+        res[n] = [np.abs(KV[f][I]).max() / scaleE for f in range(5)]
+    for f in range(5):
+        assert res[32][f] < 0.02, res                          # O(dx^2) of the cancelling terms (dx = 0.125, gradients ~ 1/r)
+        assert res[16][f] / res[32][f] > 3.0, (f, res)         # second-order convergence to the stationary state
