@@ -103,8 +103,17 @@ __device__ void closure_solve(double E, const double F[3], const Geo& q, Closure
   if (R0 >= 0.0) { c.xi = 0.0; return; }
   const double R1 = R(1.0);
   if (R1 <= 0.0) { c.xi = 1.0; return; }
+  // R(0) < 0 < R(1). For a fluid at rest xi = |F| / E exactly, for a moving one it is off by O(v): one evaluation there
+  // shrinks the bracket from [0, 1] to one side of it before Brent starts.
   bool ok;
-  c.xi = brent_root(R, 0.0, 1.0, R0, R1, 100, ok);
+  double a = 0.0, b = 1.0, Ra = R0, Rb = R1;
+  const double xg = sqrt(F2) / E;
+  if (xg > 0.0 && xg < 1.0) {
+    const double Rg = R(xg);
+    if (Rg == 0.0) { c.xi = xg; return; }
+    if (Rg < 0.0) { a = xg; Ra = Rg; } else { b = xg; Rb = Rg; }
+  }
+  c.xi = brent_root(R, a, b, Ra, Rb, 100, ok);
   R(c.xi);
 }
 
