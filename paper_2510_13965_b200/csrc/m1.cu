@@ -262,6 +262,9 @@ __global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims 
   for (int s = 0; s < 3; ++s) {
     const double* wk = Wk + (size_t)(M1W * s) * sw + pt;
     double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    double kold[5];                                      // flux part written above by this thread: fetched before the arithmetic
+#pragma unroll
+    for (int f = 1; f < 5; ++f) kold[f] = KV[(size_t)(5 * s + f) * sk + pt];
     // ---- geometric sources
     double Pl[6], ub[5];
 #pragma unroll
@@ -299,7 +302,7 @@ __global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims 
       acc[2 + a] += sF + 0.5 * al * ichi * Pdg;
     }
 #pragma unroll
-    for (int f = 1; f < 5; ++f) KV[(size_t)(5 * s + f) * sk + pt] += acc[f];
+    for (int f = 1; f < 5; ++f) KV[(size_t)(5 * s + f) * sk + pt] = kold[f] + acc[f];
   }
 }
 
