@@ -206,7 +206,7 @@ struct Master {
     return r2 * x * x + mu * x * (1.0 + x) * rB2;
   }
   __device__ __forceinline__ double fa(double mu) const { return mu * sqrt(h0 * h0 + rbar2(mu)) - 1.0; }   // (D3)
-  __device__ double f(const Par& par, double mu) {                                                    // (D6)-(D14)
+  __device__ __forceinline__ double f_body(const Par& par, double mu) {                                   // (D6)-(D14)
     const double x = x_of(mu);
     const double rb2 = rbar2(mu);
     const double qbar = q - 0.5 * B2 - 0.5 * mu * mu * x * x * B2rp2;
@@ -229,6 +229,10 @@ struct Master {
     const double nuB = (1.0 + a) * (1.0 + qbar - mu * rb2);
     return mu - 1.0 / (fmax(nuA, nuB) + mu * rb2);
   }
+  // the table version is evaluated from seven places and is ~700 instructions long: one out-of-line copy keeps the kernel
+  // inside the instruction cache (its top stall was no_instruction); the analytic EoS versions are short and stay inline
+  __device__ __noinline__ double f_out(const Par& par, double mu) { return f_body(par, mu); }
+  __device__ __forceinline__ double f(const Par& par, double mu) { return KIND == 2 ? f_out(par, mu) : f_body(par, mu); }
 };
 
 // ------------------------------------------------------------------------------------------ kernels
