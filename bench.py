@@ -160,6 +160,9 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2510_13965_b200 import binding, synth
+    from paper_2510_13965_b200 import build as _build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        _build.build()                  # refresh the in-tree library if a source is newer (seconds when up to date)
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))

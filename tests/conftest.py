@@ -18,3 +18,10 @@ def oracle_mod():
     import oracle
     oracle.build()
     return oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _library_is_built():
+    """Build (or refresh) libmhd_b200.so in-tree before any test: nvcc cross-compiles without a GPU, seconds when up to date."""
+    from paper_2510_13965_b200 import build
+    build.build()
