@@ -474,3 +474,16 @@ def test_con2prim_warm_start_is_the_same_root(oracle_mod):
         rp = _rel_vec(Pg, Po, [(4, 5, 6)])
         assert np.all(rp < 1e-12), (name, rp)
     patch.close()
+
+
+def test_hybrid_piecewise_polytrope_eos_parity(oracle_mod):
+    """eos_kind = 1 (Eqs. 30-31: three-piece cold polytrope + Gamma_th thermal part) through con2prim, the fluxes (c_s^2 of R13)
+    and the sources: one-stage parity on the all-terms-live instance of config 1; the density range straddles a piece boundary."""
+    cfg = synth.config1(n=24, gauge_perturbation=True)
+    cfg["params"].update(eos_kind=1, eos_gamma_th=1.8, n_pieces=3, pp_K=[30.0, 0.0, 0.0], pp_Gamma=[1.9, 2.4, 2.9],
+                         pp_rho=[1.0e-3, 5.0e-3, 1e300], eps_max=1e3)
+    cfg["P"][synth.EPS] = 0.25                     # above eps_cold everywhere: thermal part positive
+    _one_stage(oracle_mod, cfg)
+    (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 3)
+    assert np.array_equal(Fg, Fo)
+    assert np.all(_rel_vec(Ug, Uo, [(25, 26, 27), (28, 29, 30)]) < 1e-9) and np.all(_rel_vec(Pg, Po, [(4, 5, 6)]) < 1e-9)
