@@ -487,3 +487,35 @@ def test_hybrid_piecewise_polytrope_eos_parity(oracle_mod):
     (Ug, Pg, Fg), (Uo, Po, Fo) = _advance_both(oracle_mod, cfg, 3)
     assert np.array_equal(Fg, Fo)
     assert np.all(_rel_vec(Ug, Uo, [(25, 26, 27), (28, 29, 30)]) < 1e-9) and np.all(_rel_vec(Pg, Po, [(4, 5, 6)]) < 1e-9)
+
+
+def test_ssprk3_and_matter_dissipation(oracle_mod):
+    """The other explicit tableau of PAPER.md:400 (Shu-Osher SSP-RK3: two non-zero coefficients in its third row) and the optional
+    Kreiss-Oliger term on the matter fields (R16, k_adv_ko<false>): 4 steps against the oracle."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config1(n=16, gauge_perturbation=True)
+    cfg["params"].update(sigma_ko_matter=0.05)
+    o, patch, U, P = _setup(oracle_mod, cfg)
+    a, w = synth.tableau("ssprk3")
+    dt = 0.25 * cfg["dx"]
+    Uo = U.copy()
+    Po, Fo = o.evolve(Uo, cfg["bc"], a, w, dt, 4)
+    patch.upload(U=U)
+    patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, 4)
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    ru, _ = _rel(patch.U.cpu().numpy(), Uo, interior=False)
+    assert np.all(ru < 1e-9), ru
+    patch.close()
+    _one_stage(oracle_mod, cfg)
+
+
+@pytest.mark.parametrize("shape,bc", [((3, 3, 3), [0] * 6), ((3, 5, 4), [1, 1, 0, 0, 1, 0]), ((31, 3, 3), [0, 0, 1, 1, 1, 1])])
+def test_smallest_patches(oracle_mod, shape, bc):
+    """Degenerate sizes: the interior is as thin as the ghost width (every stencil reaches wrapped / copied data in every
+    direction, every tile is ragged)."""
+    cfg = synth.config1(n=32, gauge_perturbation=True)
+    nx, ny, nz = shape
+    cfg["U"] = np.ascontiguousarray(cfg["U"][:, :nz + 6, :ny + 6, :nx + 6])
+    cfg["P"] = np.ascontiguousarray(cfg["P"][:, :nz + 6, :ny + 6, :nx + 6])
+    cfg["n"], cfg["bc"] = shape, bc
+    _one_stage(oracle_mod, cfg)
