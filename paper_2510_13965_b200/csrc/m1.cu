@@ -3,7 +3,8 @@
 //                  brackets of Eqs. (38)-(40) in the three directions, the speed bound (B4)-(B5, reading R32), the
 //                  opacity sum kappa_a + kappa_s and P_ij, written to the M1 work slot (25 fields per species).
 //   k_m1_div       every interior zone: flux-limited advection-diffusion fluxes of Sec. III D (Eqs. 77-78, readings R20) at
-//                  the six faces from the work slot, the geometric sources of Eqs. (39)-(40) (reading R19) -> KV.
+//                  the two x faces from the work slot, the geometric sources of Eqs. (39)-(40) (reading R19) -> KV.
+//   k_m1_march     the y and z faces as a march (register window along the line), added to KV.
 //   k_m1_implicit  every grid point: the pointwise implicit solve of App. C — closure frozen at V* (R21), Newton on the
 //                  4x4 system (C13)-(C16) with the Jacobian (C28)-(C35), N from (C11); writes V^(i) and the stiff source R.
 //   k_m1_backreact K_fluid -= sum over species of R (l.256, l.312-316; R24).
@@ -207,8 +208,8 @@ __global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims 
   for (int s = 0; s < 3; ++s) {
     double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     const double* wk = Wk + (size_t)(M1W * s) * sw + pt;
-#pragma unroll
-    for (int dir = 0; dir < 3; ++dir) {
+    {                                                  // x faces here; the y and z faces are added by k_m1_march
+      constexpr int dir = 0;
       const long long ls = st[dir];
       const double* wl = wk + (size_t)(6 * dir + 5) * sw;
       const double* wkap = wk + (size_t)18 * sw;
@@ -477,6 +478,63 @@ __global__ void __launch_bounds__(128) k_m1_backreact(const __grid_constant__ Di
   K[(size_t)DYEBAR * sk + pt] -= mb * (__ldg(R + pt) - __ldg(R + (size_t)5 * sr + pt));
 }
 
+// y / z faces of Eq. (77) as a march: thread = (x column, segment of SEG zones along the line), every node value loaded once per
+// segment into a register window; KV (written by k_m1_div with the x faces and the sources) is read-modify-write, fetched early.
+template <int DIR, int SEG>
+__global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dims d, bool oe, const double* __restrict__ V, size_t sv,
+                                                     const double* __restrict__ Wk, size_t sw, double* __restrict__ KV, size_t sk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= d.nx) return;
+  const int nline = DIR == 1 ? d.ny : d.nz;
+  const int mline = nline + 2 * d.ng;
+  const long long ls = DIR == 1 ? d.sy : d.sz;
+  const int c0 = blockIdx.z * SEG;                           // first zone of the segment (interior index)
+  const int other = blockIdx.y + d.ng;
+  const long long base = (DIR == 1 ? (long long)other * d.sz : (long long)other * d.sy) + (i + d.ng);
+  const int g0 = c0 + d.ng - 2;                              // line index of node 0 of the window (zone c0 - 2)
+  auto node = [&](int n) { return base + (long long)min(g0 + n, mline - 1) * ls; };   // clamped: a ragged tail never reads past the field
+  const double h = DIR == 1 ? d.dy : d.dz, ih = 1.0 / h;
+#pragma unroll 1
+  for (int s = 0; s < 3; ++s) {
+    const double* wk = Wk + (size_t)(M1W * s) * sw;
+    // face m (m = 0..SEG) lies between window nodes m + 1 and m + 2
+    double lam[SEG + 1], A[SEG + 1];
+    {
+      const double* wl = wk + (size_t)(6 * DIR + 5) * sw;
+      const double* wkap = wk + (size_t)18 * sw;
+      double lp = __ldg(wl + node(1)), kp = __ldg(wkap + node(1));
+#pragma unroll
+      for (int m = 0; m <= SEG; ++m) {
+        const double ln = __ldg(wl + node(m + 2)), kn = __ldg(wkap + node(m + 2));
+        lam[m] = fmax(lp, ln);
+        const double kh = 0.5 * (kp + kn) * h;
+        A[m] = kh > 0.05 ? tanh(1.0 / kh) : 1.0;
+        lp = ln; kp = kn;
+      }
+    }
+#pragma unroll 1
+    for (int f = 0; f < 5; ++f) {
+      const double* u = V + (size_t)(5 * s + f) * sv;
+      const double* F = wk + (size_t)(6 * DIR + f) * sw;
+      double* kv = KV + (size_t)(5 * s + f) * sk;
+      double uw[SEG + 4], Fw[SEG + 2], kold[SEG];
+#pragma unroll
+      for (int n = 0; n < SEG + 4; ++n) uw[n] = __ldg(u + node(n));
+#pragma unroll
+      for (int n = 0; n < SEG + 2; ++n) Fw[n] = __ldg(F + node(n + 1));
+#pragma unroll
+      for (int z = 0; z < SEG; ++z) kold[z] = c0 + z < nline ? kv[base + (long long)(g0 + z + 2) * ls] : 0.0;
+      double prev = m1_face(uw[0], uw[1], uw[2], uw[3], Fw[0], Fw[1], lam[0], A[0], oe);
+#pragma unroll
+      for (int z = 0; z < SEG; ++z) {
+        const double cur = m1_face(uw[z + 1], uw[z + 2], uw[z + 3], uw[z + 4], Fw[z + 1], Fw[z + 2], lam[z + 1], A[z + 1], oe);
+        if (c0 + z < nline) kv[base + (long long)(g0 + z + 2) * ls] = kold[z] - (cur - prev) * ih;
+        prev = cur;
+      }
+    }
+  }
+}
+
 cudaError_t launch_m1_point(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, const double* V, size_t sv,
                             double* Wk, size_t sw, cudaStream_t s) {
   k_m1_point<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, V, sv, Wk, sw);
@@ -486,6 +544,9 @@ cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t
                           double* KV, size_t sk, cudaStream_t s) {
   dim3 grid((d.nx + 127) / 128, d.ny, d.nz);
   k_m1_div<<<grid, 128, 0, s>>>(d, par.m1_odd_even != 0, U, su, V, sv, Wk, sw, KV, sk);
+  constexpr int SEG = 6;
+  k_m1_march<1, SEG><<<dim3((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG), 128, 0, s>>>(d, par.m1_odd_even != 0, V, sv, Wk, sw, KV, sk);
+  k_m1_march<2, SEG><<<dim3((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG), 128, 0, s>>>(d, par.m1_odd_even != 0, V, sv, Wk, sw, KV, sk);
   return cudaGetLastError();
 }
 cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* V, size_t sv,
