@@ -281,6 +281,10 @@ def main():
     # profiles/r1g_ncu_full_c4_128.md (128^3; per-zone figures carry over to 256^3, the tiles are the same)
     ncu_traffic = {"ccz4_algebra": 592.9, "adv_ko": 634.2, "point_flux": 546.8, "recon_x": 332.2, "recon_y": 355.3, "recon_z": 359.7,
                    "rk_combine": 802.8, "con2prim": 259.7, "fill_ghosts": 79.3}
+    # FP64 pipe utilisation of each kernel in the same capture (sm__inst_executed_pipe_fp64, % of peak): the executed-instruction
+    # view beside the algorithmic-flop view (the oracle's count includes work a fused kernel shares, so "frac" reads high)
+    ncu_fp64_busy = {"ccz4_algebra": 0.38, "adv_ko": 0.36, "point_flux": 0.28, "recon_x": 0.18, "recon_y": 0.31, "recon_z": 0.31,
+                     "rk_combine": 0.03, "con2prim": 0.26, "fill_ghosts": 0.0}
     total_kernel_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
@@ -294,7 +298,8 @@ def main():
                 "peak_source": "measured: FP64 DFMA probe of the library (mhd_probe_fp64_flops); nominal 37.2",
                 "traffic": ncu_traffic[dom] * zones if dom in ncu_traffic else None,
                 "traffic_source": "bytes per launch = ncu dram bytes per zone (profiles/r1g, 128^3 capture) x zones of this run",
-                "alg_bytes": alg_doubles[dom] * 8.0 * zones, "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
+                "alg_bytes": alg_doubles[dom] * 8.0 * zones, "fp64_pipe_busy_ncu": ncu_fp64_busy.get(dom),
+                "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
                 "share_of_step": dom_ms / total_kernel_ms if total_kernel_ms else None,
                 "alg_flops_per_zone": alg_flops[dom],
                 "hbm": {"achieved_gbs": alg_doubles[dom] * 8.0 * zones / sec_per_launch / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src},
