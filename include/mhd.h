@@ -104,9 +104,13 @@ typedef struct {
   double ye_min, ye_max, ye_atmo, eps_atmo, T_atmo;
   int c2p_maxit;
   /* M1 (n_species = 3): synthetic grey opacities kappa_a = kappa_s = m1_kappa0 (rho / m1_rho0)^2 m1_species_scale[s],
-   * eta = kappa_a T^4 (BASELINE.json configs[4]); energy floor, Newton tolerance / cap of App. C, baryon mass of l.316 */
+   * eta = m1_arad kappa_a T^4 (BASELINE.json configs[4]: m1_arad = 1; it is the radiation constant in the units T is measured in);
+   * energy floor, Newton tolerance / cap of App. C, baryon mass of l.316 */
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
   int m1_maxit, m1_odd_even;       /* m1_odd_even != 0: the A := 1 switch against odd-even decoupling (l.565-570) */
+  double m1_arad;                  /* see above; 0 switches the emission off */
+  double m1_oe_guard;              /* reading R33: the switch also needs all three differences to exceed m1_oe_guard x the local
+                                      magnitude; 0 = the rule exactly as printed (two strict "< 0" tests) */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */

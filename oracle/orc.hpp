@@ -80,6 +80,8 @@ struct Params {
   // eta = kappa_a T^4 (BASELINE.json configs[4]); number opacities kappa_a^0 = kappa_a, eta^0 = eta (synthetic)
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
   int m1_maxit, m1_odd_even;   // m1_odd_even: apply the A := 1 switch of l.565-570
+  double m1_arad;              // eta = m1_arad kappa_a T^4 (radiation constant in the units of T; BASELINE: 1)
+  double m1_oe_guard;          // R33: relative size the three differences must exceed for the switch; 0 = the printed rule
 };
 
 // ---- stencils (Sec. III B)

@@ -1,5 +1,5 @@
 // ORACLE (test infrastructure) — conserved <-> primitive, Eq. (29) l.223-232 and
-// App. D l.1081-1162 (RePrimAnd-style recovery with two bracketed root solves, Brent).
+// App. D l.1081-1162 (RePrimAnd-style recovery with two bracketed root solves; the oracle solves both by bisection).
 #include <algorithm>
 #include <cfloat>
 #include <cmath>
@@ -41,35 +41,24 @@ void prim2con_point(const double gl[6], const double prim[NPRIM], const double B
   for (int i = 0; i < 3; ++i) S[i] = (h * W2 + B2) * vl[i] - Bv * Bl[i];
 }
 
-// Brent's method (zeroin) on [a,b] with f(a) f(b) <= 0, to ~2 ulp of the root (R9)
+// Root of f on [a, b] with f(a) f(b) <= 0 by plain bisection until the two ends are adjacent doubles (R9: App. D asks for a
+// bracketing solver, "Brent" at l.1114, l.1143; the root in the bracket is unique, so every convergent bracketing method
+// returns the same number to rounding — the oracle uses the simplest one). The end whose |f| is smaller is returned.
+// conv = false if maxit halvings were not enough.
 template <class F>
-static double brent(F&& f, double a, double b, double fa, double fb, int maxit, bool& conv) {
+static double bisect_root(F&& f, double a, double b, double fa, double fb, int maxit, bool& conv) {
   conv = true;
   if (fa == 0.0) return a;
   if (fb == 0.0) return b;
-  double c = a, fc = fa, d = b - a, e = d;
   for (int it = 0; it < maxit; ++it) {
-    if ((fb > 0.0) == (fc > 0.0)) { c = a; fc = fa; d = b - a; e = d; }
-    if (std::fabs(fc) < std::fabs(fb)) { a = b; b = c; c = a; fa = fb; fb = fc; fc = fa; }
-    const double tol = 2.0 * DBL_EPSILON * std::fabs(b);
-    const double m = 0.5 * (c - b);
-    if (std::fabs(m) <= tol || fb == 0.0) return b;
-    if (std::fabs(e) < tol || std::fabs(fa) <= std::fabs(fb)) { d = m; e = m; }
-    else {
-      double p, q, r, s = fb / fa;
-      if (a == c) { p = 2.0 * m * s; q = 1.0 - s; }
-      else { q = fa / fc; r = fb / fc; p = s * (2.0 * m * q * (q - r) - (b - a) * (r - 1.0)); q = (q - 1.0) * (r - 1.0) * (s - 1.0); }
-      if (p > 0.0) q = -q; else p = -p;
-      s = e; e = d;
-      if (2.0 * p < 3.0 * m * q - std::fabs(tol * q) && p < std::fabs(0.5 * s * q)) d = p / q;
-      else { d = m; e = m; }
-    }
-    a = b; fa = fb;
-    if (std::fabs(d) > tol) b += d; else b += (m > 0.0 ? tol : -tol);
-    fb = f(b);
+    const double m = a + 0.5 * (b - a);
+    if (m == a || m == b) return std::fabs(fa) <= std::fabs(fb) ? a : b;
+    const double fm = f(m);
+    if (fm == 0.0) return m;
+    if ((fm > 0.0) == (fa > 0.0)) { a = m; fa = fm; } else { b = m; fb = fm; }
   }
   conv = false;
-  return b;
+  return std::fabs(fa) <= std::fabs(fb) ? a : b;
 }
 
 namespace {
@@ -152,14 +141,14 @@ uint8_t con2prim_point(const Params& par, const double gt[6], double chi, double
     // step 2: root of f_a on (0, 1/h0]
     bool c1 = true, c2 = true;
     const double mub = 1.0 / s.h0;
-    const double mu_plus = brent([&](double m) { return s.fa(m); }, 0.0, mub, -1.0, s.fa(mub), par.c2p_maxit, c1);
+    const double mu_plus = bisect_root([&](double m) { return s.fa(m); }, 0.0, mub, -1.0, s.fa(mub), std::max(par.c2p_maxit, 1100), c1);
     // step 3: root of f on (0, mu_plus]
     const double f0 = s.f(0.0), f1 = s.f(mu_plus);
     double mu;
     // no sign change: the root sits at the bracket end when the state is degenerate (eps clamped to its minimum gives
     // h = h0 and f(mu_plus) = 0 analytically, +-1e-16 numerically): that is a converged solve, not a failure (R9)
     if ((f0 > 0.0) == (f1 > 0.0) && f1 != 0.0 && f0 != 0.0) { mu = mu_plus; c2 = std::fabs(f1) <= 1e-12; }
-    else mu = brent([&](double m) { return s.f(m); }, 0.0, mu_plus, f0, f1, par.c2p_maxit, c2);
+    else mu = bisect_root([&](double m) { return s.f(m); }, 0.0, mu_plus, f0, f1, std::max(par.c2p_maxit, 1100), c2);
     s.f(mu);                                                // step 4: primitives at the root
     if (!c1 || !c2) flag |= FLAG_NOCONV;
     rho = D / s.W; W = s.W; eps = s.eps_raw;
@@ -218,6 +207,7 @@ uint8_t con2prim_point(const Params& par, const double gt[6], double chi, double
 
 void con2prim(const Params& par, const Grid& g, double* U, double* P, uint8_t* flags) {
   const size_t n = g.npts();
+#pragma omp parallel for schedule(dynamic, 512)
   for (size_t p = 0; p < n; ++p) {
     double gt[6], uc[10], prim[NPRIM];
     for (int a = 0; a < 6; ++a) gt[a] = U[(GXX + a) * n + p];
@@ -232,6 +222,7 @@ void con2prim(const Params& par, const Grid& g, double* U, double* P, uint8_t* f
 // and the densitised Dbar, DYebar, taubar, Sbar_i are written into U (Bbar^i, phibar and the metric are inputs).
 void prim2con(const Params& par, const Grid& g, double* U, double* P) {
   const size_t n = g.npts();
+#pragma omp parallel for schedule(dynamic, 512)
   for (size_t p = 0; p < n; ++p) {
     const double chi = U[CHI * n + p];
     const double isg = chi * std::sqrt(chi), sg = 1.0 / isg;

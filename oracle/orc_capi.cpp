@@ -16,7 +16,7 @@ bool set_scalar(Params& p, const std::string& k, double v) {
   D(sigma_ko_spacetime) D(sigma_ko_matter) D(c_b) D(kappa_b) D(mp5_alpha)
   D(rho_atmo) D(rho_cut) D(rho_low) D(alpha_bh) D(w_max) D(rho_max) D(eps_min) D(eps_max)
   D(ye_min) D(ye_max) D(ye_atmo) D(eps_atmo) D(T_atmo) I(c2p_maxit)
-  D(m1_kappa0) D(m1_rho0) D(m1_efloor) D(m1_tol) D(m1_mb) I(m1_maxit) I(m1_odd_even)
+  D(m1_kappa0) D(m1_rho0) D(m1_efloor) D(m1_tol) D(m1_mb) I(m1_maxit) I(m1_odd_even) D(m1_arad) D(m1_oe_guard)
   I(n_rho) I(n_T) I(n_ye) D(lr0) D(dlr) D(lT0) D(dlT) D(ye0) D(dye) D(tab_eps_shift) D(tab_h0)
 #undef D
 #undef I
@@ -24,7 +24,23 @@ bool set_scalar(Params& p, const std::string& k, double v) {
 }
 }  // namespace
 
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
 extern "C" {
+
+// thread count of the -fopenmp build (the outermost grid loops carry `#pragma omp parallel for`; the arithmetic of every point
+// is unchanged). Returns the count in effect: always 1 in the plain build.
+int orc_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+  return omp_get_max_threads();
+#else
+  (void)n;
+  return 1;
+#endif
+}
 
 void* orc_new() {
   Handle* h = new Handle();

@@ -31,6 +31,7 @@ void rhs_ccz4(const Params& par, const Grid& G, const double* U, const double* P
   const double hh[3] = {G.dx, G.dy, G.dz};
   const double PI = 3.14159265358979323846;
   const int ng = G.ng;
+#pragma omp parallel for schedule(dynamic)
   for (int kk = ng; kk < G.nz + ng; ++kk)
   for (int jj = ng; jj < G.ny + ng; ++jj)
   for (int ii = ng; ii < G.nx + ng; ++ii) {

@@ -2,75 +2,91 @@
 // tabulated p(rho,T,Ye), eps(rho,T,Ye) of l.248-250 with reading R26 (trilinear in
 // (log10 rho, log10 T, Ye) of log10 p and log10 eps; T from eps by exact inversion of the
 // interpolant along the monotone log T axis, clamped to the table).
+// Written the plain way on purpose (8-corner sums, walks over the node coordinates, continuity conditions spelled
+// out): the CUDA kernels use nested linear interpolation, index arithmetic and a hinted bisection instead, so a slip in
+// either shows up as a parity failure.
 #include <algorithm>
 #include <cmath>
 #include "orc.hpp"
 
 namespace orc {
 
-// continuity of eps_cold and p_cold across pieces, PAPER.md:246 (a_0 = 0)
+// Piecewise polytrope, PAPER.md:240-246 (Eq. 31): in piece i (rho_{i-1} <= rho < rho_i)
+//     p_cold = K_i rho^Gamma_i,     eps_cold = a_i + K_i rho^(Gamma_i - 1) / (Gamma_i - 1),
+// with K_0 given, a_0 = 0, and K_i, a_i (i > 0) fixed by demanding that p_cold and eps_cold are continuous at the
+// dividing density rho_{i-1} (l.246). Written out, the two continuity conditions at rb = rho_{i-1} read
+//     K_i rb^Gamma_i = p_left,                                where p_left = K_{i-1} rb^Gamma_{i-1},
+//     a_i + p_left / ((Gamma_i - 1) rb) = eps_left,            where eps_left = a_{i-1} + p_left / ((Gamma_{i-1} - 1) rb),
+// (using K rho^(Gamma-1) = p_cold / rho on both sides of the second one).
 void eos_init(Params& par) {
   if (par.eos_kind != 1) return;
   par.pp_a[0] = 0.0;
   for (int i = 1; i < par.n_pieces; ++i) {
-    const double rb = par.pp_rho[i - 1];   // boundary between piece i-1 and i
-    // K_i from p continuity: K_{i-1} rb^G_{i-1} = K_i rb^G_i
-    par.pp_K[i] = par.pp_K[i - 1] * std::pow(rb, par.pp_Gamma[i - 1] - par.pp_Gamma[i]);
-    const double em = par.pp_a[i - 1] + par.pp_K[i - 1] / (par.pp_Gamma[i - 1] - 1.0) * std::pow(rb, par.pp_Gamma[i - 1] - 1.0);
-    par.pp_a[i] = em - par.pp_K[i] / (par.pp_Gamma[i] - 1.0) * std::pow(rb, par.pp_Gamma[i] - 1.0);
+    const double rb = par.pp_rho[i - 1];
+    const double p_left = par.pp_K[i - 1] * std::exp(par.pp_Gamma[i - 1] * std::log(rb));
+    const double eps_left = par.pp_a[i - 1] + p_left / ((par.pp_Gamma[i - 1] - 1.0) * rb);
+    par.pp_K[i] = p_left / std::exp(par.pp_Gamma[i] * std::log(rb));
+    par.pp_a[i] = eps_left - p_left / ((par.pp_Gamma[i] - 1.0) * rb);
   }
 }
 
-static int pp_piece(const Params& par, double rho) {
-  int i = 0;
-  while (i < par.n_pieces - 1 && rho >= par.pp_rho[i]) ++i;
-  return i;
-}
+// cold pressure, cold specific internal energy and exponent of the piece that contains rho
 static void pp_cold(const Params& par, double rho, double& pc, double& ec, double& G) {
-  const int i = pp_piece(par, rho);
-  G = par.pp_Gamma[i];
-  const double x = par.pp_K[i] * std::pow(rho, G - 1.0);   // K rho^(G-1) = p_cold / rho
-  pc = x * rho;                                            // Eq. (31)
-  ec = par.pp_a[i] + x / (G - 1.0);
+  int piece = par.n_pieces - 1;                              // the last piece is unbounded above
+  for (int i = par.n_pieces - 2; i >= 0; --i)                // walk down while rho lies below the dividing density
+    if (rho < par.pp_rho[i]) piece = i;
+  G = par.pp_Gamma[piece];
+  pc = par.pp_K[piece] * std::pow(rho, G);                   // Eq. (31)
+  ec = par.pp_a[piece] + pc / ((G - 1.0) * rho);
 }
 
-// ---- table helpers ------------------------------------------------------------------
+// ---- table (R26): values on the nodes x_i = x0 + i dx of the three axes (log10 rho, log10 T, Ye), rho fastest -------------
+static double tab_node(const Params& par, const double* q, int ir, int it, int iy) {
+  return q[((size_t)iy * par.n_T + it) * par.n_rho + ir];
+}
+// cell [x_i, x_{i+1}] holding x and the weight of its upper node; x is clamped to the table first. Found by walking along
+// the node coordinates themselves.
 struct TabPos { int i; double w; };
 static TabPos tab_locate(double x, double x0, double dx, int n) {
-  double s = (x - x0) / dx;
-  if (s < 0.0) s = 0.0;
-  if (s > (double)(n - 1)) s = (double)(n - 1);
-  int i = (int)s;
-  if (i > n - 2) i = n - 2;
-  return {i, s - (double)i};
+  const double xlast = x0 + (n - 1) * dx;
+  if (x <= x0) return {0, 0.0};
+  if (x >= xlast) return {n - 2, 1.0};
+  int i = 0;
+  while (i < n - 2 && x >= x0 + (i + 1) * dx) ++i;
+  double w = (x - (x0 + i * dx)) / dx;
+  if (w < 0.0) w = 0.0;
+  if (w > 1.0) w = 1.0;
+  return {i, w};
 }
-static size_t tab_idx(const Params& par, int ir, int it, int iy) {
-  return ((size_t)iy * par.n_T + it) * par.n_rho + ir;     // rho fastest
-}
-// bilinear (in log rho, Ye) value of table q at T-node it
-static double tab_column(const Params& par, const double* q, TabPos r, TabPos y, int it) {
-  const double a = q[tab_idx(par, r.i, it, y.i)], b = q[tab_idx(par, r.i + 1, it, y.i)];
-  const double c = q[tab_idx(par, r.i, it, y.i + 1)], d = q[tab_idx(par, r.i + 1, it, y.i + 1)];
-  const double lo = a + r.w * (b - a), hi = c + r.w * (d - c);
-  return lo + y.w * (hi - lo);
-}
+// PAPER.md:250 "linear interpolation": the trilinear interpolant is the sum over the 8 corners of the cell, each weighted by
+// the product of its three one-dimensional weights
 static double tab_interp(const Params& par, const double* q, TabPos r, TabPos t, TabPos y) {
-  const double lo = tab_column(par, q, r, y, t.i), hi = tab_column(par, q, r, y, t.i + 1);
-  return lo + t.w * (hi - lo);
+  double sum = 0.0;
+  for (int cy = 0; cy < 2; ++cy)
+    for (int ct = 0; ct < 2; ++ct)
+      for (int cr = 0; cr < 2; ++cr) {
+        const double w = (cr ? r.w : 1.0 - r.w) * (ct ? t.w : 1.0 - t.w) * (cy ? y.w : 1.0 - y.w);
+        sum += w * tab_node(par, q, r.i + cr, t.i + ct, y.i + cy);
+      }
+  return sum;
 }
-// invert log10(eps+shift) -> position on the log T axis (clamped to the table)
+// the interpolant on the T node `it` (weight 1 on that node): the 4-corner sum in (log10 rho, Ye)
+static double tab_column(const Params& par, const double* q, TabPos r, TabPos y, int it) {
+  const TabPos on_node = {it < par.n_T - 1 ? it : it - 1, it < par.n_T - 1 ? 0.0 : 1.0};
+  return tab_interp(par, q, r, on_node, y);
+}
+// T from eps at fixed (rho, Ye): the interpolant is piecewise linear and increasing along the log10 T axis, so its inverse
+// is found by walking up the T nodes until the column value exceeds log10(eps + shift) (coarse strides of 16 nodes first,
+// then node by node), and solving the linear interpolation in that cell. Below / above the table: clamped (l.1145).
 static TabPos tab_T_from_loge(const Params& par, TabPos r, TabPos y, double le) {
-  int lo = 0, hi = par.n_T - 1;
-  const double elo = tab_column(par, par.tab_loge, r, y, lo), ehi = tab_column(par, par.tab_loge, r, y, hi);
-  if (le <= elo) return {0, 0.0};
-  if (le >= ehi) return {par.n_T - 2, 1.0};
-  double e_lo = elo, e_hi = ehi;
-  while (hi - lo > 1) {               // bisection on the node index; column is monotone in T
-    const int mid = (lo + hi) / 2;
-    const double em = tab_column(par, par.tab_loge, r, y, mid);
-    if (le >= em) { lo = mid; e_lo = em; } else { hi = mid; e_hi = em; }
-  }
-  return {lo, (le - e_lo) / (e_hi - e_lo)};
+  const int last = par.n_T - 1;
+  if (le <= tab_column(par, par.tab_loge, r, y, 0)) return {0, 0.0};
+  if (le >= tab_column(par, par.tab_loge, r, y, last)) return {last - 1, 1.0};
+  int it = 0;
+  while (it + 16 < last && le >= tab_column(par, par.tab_loge, r, y, it + 16)) it += 16;
+  while (it + 1 < last && le >= tab_column(par, par.tab_loge, r, y, it + 1)) ++it;
+  const double e_lo = tab_column(par, par.tab_loge, r, y, it), e_hi = tab_column(par, par.tab_loge, r, y, it + 1);
+  return {it, (le - e_lo) / (e_hi - e_lo)};
 }
 
 EosOut eos_from_rho_eps(const Params& par, double rho, double eps, double ye) {

@@ -114,8 +114,9 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
   for (int d = 0; d < 3 && (parts & 1); ++d) {
     const int d1_ = (d + 1) % 3, d2_ = (d + 2) % 3;
     const int Md = M[d];
-    std::vector<double> Fp(10 * Md), Uc(10 * Md), sp(Md), Fhat(10 * (Md + 1));
+#pragma omp parallel for schedule(dynamic)
     for (int b = ng; b < N[d2_] + ng; ++b) for (int a = ng; a < N[d1_] + ng; ++a) {
+      std::vector<double> Fp(10 * Md), Uc(10 * Md), sp(Md), Fhat(10 * (Md + 1));
       int c[3];
       c[d1_] = a; c[d2_] = b; c[d] = 0;
       const size_t base = G.idx(c[0], c[1], c[2]);
@@ -150,6 +151,7 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
 
   // ---- sources of Eq. (32) (+ KO on matter fields if sigma_ko_matter != 0, R16)
   if (parts & 2)
+#pragma omp parallel for schedule(dynamic)
   for (int kk = ng; kk < G.nz + ng; ++kk) for (int jj = ng; jj < G.ny + ng; ++jj) for (int ii = ng; ii < G.nx + ng; ++ii) {
     const size_t p = G.idx(ii, jj, kk);
     auto Fd = [&](int f) { return U + (size_t)f * n + p; };

@@ -140,7 +140,7 @@ void m1_opacities(const Params& par, int species, double rho, double T, double& 
   const double x = rho / par.m1_rho0;
   ka = par.m1_kappa0 * x * x * par.m1_species_scale[species];
   ks = ka;
-  eta = ka * T * T * T * T;
+  eta = par.m1_arad * ka * T * T * T * T;
 }
 
 namespace {

@@ -79,8 +79,9 @@ void m1_rhs(const Params& par, const Grid& G, const double* U, const double* P, 
       KV[(size_t)f * n + G.idx(ii, jj, kk)] = 0.0;
   for (int s = 0; s < NSPECIES; ++s) for (int d = 0; d < 3; ++d) {
     const int d1_ = (d + 1) % 3, d2_ = (d + 2) % 3, Md = M[d];
-    std::vector<double> Fp(5 * Md), Uc(5 * Md), lam(Md), kap(Md), Fhat(5 * (Md + 1));
+#pragma omp parallel for schedule(dynamic)
     for (int b = ng; b < N[d2_] + ng; ++b) for (int a = ng; a < N[d1_] + ng; ++a) {
+      std::vector<double> Fp(5 * Md), Uc(5 * Md), lam(Md), kap(Md), Fhat(5 * (Md + 1));
       int c[3];
       c[d1_] = a; c[d2_] = b; c[d] = 0;
       const size_t base = G.idx(c[0], c[1], c[2]);
@@ -106,9 +107,11 @@ void m1_rhs(const Params& par, const Grid& G, const double* U, const double* P, 
           const double dm = u[i] - u[i - 1], d0 = u[i + 1] - u[i], dp = u[i + 2] - u[i + 1];
           const double Phi = d0 == 0.0 ? 1.0 : std::max(0.0, std::min(1.0, std::min(2.0 * dm / d0, 2.0 * dp / d0)));   // Eq. (78), R20
           double A = A0;
-          // odd-even decoupling, l.565-570. R33: the three differences must all exceed 1e-10 of the local magnitude —
-          // a zigzag of rounding noise on a flat profile is not an oscillation (and would make the switch irreproducible)
-          const double tiny = 1e-10 * std::max(std::max(std::fabs(u[i - 1]), std::fabs(u[i])), std::max(std::fabs(u[i + 1]), std::fabs(u[i + 2])));
+          // odd-even decoupling, l.565-570, as printed: A := 1 when (u_i - u_{i-1})(u_{i+1} - u_i) < 0 and
+          // (u_{i+1} - u_i)(u_{i+2} - u_{i+1}) < 0. Reading R33 (a DEPARTURE from the printed rule, off when m1_oe_guard = 0):
+          // the three differences must also exceed m1_oe_guard x the local magnitude, so that a zigzag of rounding noise on a
+          // flat profile does not count as an oscillation
+          const double tiny = par.m1_oe_guard * std::max(std::max(std::fabs(u[i - 1]), std::fabs(u[i])), std::max(std::fabs(u[i + 1]), std::fabs(u[i + 2])));
           if (par.m1_odd_even && dm * d0 < 0.0 && d0 * dp < 0.0 && std::min(std::min(std::fabs(dm), std::fabs(d0)), std::fabs(dp)) > tiny) A = 1.0;
           const double FHO = 0.5 * (F[i] + F[i + 1]);
           const double FLO = FHO - 0.5 * l * d0;                    // R20
@@ -121,6 +124,7 @@ void m1_rhs(const Params& par, const Grid& G, const double* U, const double* P, 
     }
   }
   // geometric sources of Eqs. (39)-(40)
+#pragma omp parallel for schedule(dynamic)
   for (int kk = ng; kk < G.nz + ng; ++kk) for (int jj = ng; jj < G.ny + ng; ++jj) for (int ii = ng; ii < G.nx + ng; ++ii) {
     const size_t p = G.idx(ii, jj, kk);
     auto Fd = [&](int f) { return U + (size_t)f * n + p; };
@@ -169,6 +173,7 @@ void m1_rhs(const Params& par, const Grid& G, const double* U, const double* P, 
 // a12 over the patch (every point incl. ghosts): V holds V* on entry (densitised), V^(i) on exit; R = densitised stiff source
 void m1_implicit(const Params& par, const Grid& G, const double* U, const double* P, double* V, double* R, double adt, uint8_t* flags) {
   const size_t n = G.npts();
+#pragma omp parallel for schedule(dynamic, 512)
   for (size_t p = 0; p < n; ++p) {
     GeoPt q;
     load_geo(G, U, P, p, q);
@@ -209,6 +214,7 @@ void m1_gravity(const Params& par, const Grid& G, const double* U, const double*
   const int ng = G.ng;
   const double G8 = 8.0 * 3.14159265358979323846 * par.grav_G;
   if (G8 == 0.0) return;
+#pragma omp parallel for schedule(dynamic)
   for (int kk = ng; kk < G.nz + ng; ++kk) for (int jj = ng; jj < G.ny + ng; ++jj) for (int ii = ng; ii < G.nx + ng; ++ii) {
     const size_t p = G.idx(ii, jj, kk);
     GeoPt q;

@@ -41,6 +41,7 @@ class mhd_patch_desc(ctypes.Structure):
         ("c2p_maxit", _i),
         ("m1_kappa0", _d), ("m1_rho0", _d), ("m1_species_scale", _d * 3), ("m1_efloor", _d), ("m1_tol", _d), ("m1_mb", _d),
         ("m1_maxit", _i), ("m1_odd_even", _i),
+        ("m1_arad", _d), ("m1_oe_guard", _d),
     ]
 
 

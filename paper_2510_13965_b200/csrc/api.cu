@@ -126,7 +126,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.m1_kappa0 = desc->m1_kappa0; q.m1_rho0 = desc->m1_rho0 > 0.0 ? desc->m1_rho0 : 1.0; q.m1_efloor = desc->m1_efloor;
   q.m1_tol = desc->m1_tol > 0.0 ? desc->m1_tol : 1e-13; q.m1_mb = desc->m1_mb; q.m1_maxit = desc->m1_maxit > 0 ? desc->m1_maxit : 30;
   for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
-  q.m1_odd_even = desc->m1_odd_even;
+  q.m1_odd_even = desc->m1_odd_even; q.m1_arad = desc->m1_arad; q.m1_oe_guard = desc->m1_oe_guard;
   p->d_counts = nullptr;
   if (cudaMalloc(&p->d_counts, 8 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   *out = p;

@@ -123,7 +123,7 @@ __device__ __forceinline__ void opacities(const Par& par, int s, double rho, dou
   ka = par.m1_kappa0 * x * x * par.m1_species_scale[s];
   ks = ka;
   const double T2 = T * T;
-  eta = ka * T2 * T2;
+  eta = par.m1_arad * ka * T2 * T2;
 }
 
 }  // namespace
@@ -182,12 +182,12 @@ __global__ void __launch_bounds__(128, 3) k_m1_point(const __grid_constant__ Dim
 // ---------------------------------------------------------------------------------------------------------------
 namespace {
 // F^_{i+1/2} of Eq. (77) from u_{i-1..i+2}, the fluxes at i, i+1, lambda_{i+1/2} and A_{i+1/2}
-__device__ __forceinline__ double m1_face(double um, double u0, double up, double upp, double F0, double F1, double lam, double A0, bool oe) {
+__device__ __forceinline__ double m1_face(double um, double u0, double up, double upp, double F0, double F1, double lam, double A0, double oe) {
   const double dm = u0 - um, d0 = up - u0, dp = upp - up;
   const double r2 = 2.0 / d0;                                                                           // one reciprocal per face and field
   const double Phi = d0 == 0.0 ? 1.0 : fmax(0.0, fmin(1.0, fmin(dm * r2, dp * r2)));                    // Eq. (78), R20
-  const double tiny = 1e-10 * fmax(fmax(fabs(um), fabs(u0)), fmax(fabs(up), fabs(upp)));                // R33
-  const double A = (oe && dm * d0 < 0.0 && d0 * dp < 0.0 && fmin(fmin(fabs(dm), fabs(d0)), fabs(dp)) > tiny) ? 1.0 : A0;   // l.565-570
+  const double tiny = oe * fmax(fmax(fabs(um), fabs(u0)), fmax(fabs(up), fabs(upp)));                   // R33 (oe = 0: the printed rule; oe < 0: switch off)
+  const double A = (oe >= 0.0 && dm * d0 < 0.0 && d0 * dp < 0.0 && fmin(fmin(fabs(dm), fabs(d0)), fabs(dp)) > tiny) ? 1.0 : A0;   // l.565-570
   const double FHO = 0.5 * (F0 + F1);
   return FHO - A * (1.0 - Phi) * (0.5 * lam * d0);                                                      // F^HO - F^LO = lambda d0 / 2
 }
@@ -196,7 +196,7 @@ __device__ __forceinline__ double d1c(const double* __restrict__ u, long long s,
 }
 }  // namespace
 
-__global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims d, bool oe, const double* __restrict__ U, size_t su,
+__global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims d, double oe, const double* __restrict__ U, size_t su,
                                                 const double* __restrict__ V, size_t sv, const double* __restrict__ Wk, size_t sw,
                                                 double* __restrict__ KV, size_t sk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -481,7 +481,7 @@ __global__ void __launch_bounds__(128) k_m1_backreact(const __grid_constant__ Di
 // y / z faces of Eq. (77) as a march: thread = (x column, segment of SEG zones along the line), every node value loaded once per
 // segment into a register window; KV (written by k_m1_div with the x faces and the sources) is read-modify-write, fetched early.
 template <int DIR, int SEG>
-__global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dims d, bool oe, const double* __restrict__ V, size_t sv,
+__global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dims d, double oe, const double* __restrict__ V, size_t sv,
                                                      const double* __restrict__ Wk, size_t sw, double* __restrict__ KV, size_t sk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= d.nx) return;
@@ -543,10 +543,11 @@ cudaError_t launch_m1_point(const Dims& d, const Par& par, const double* U, size
 cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
                           double* KV, size_t sk, cudaStream_t s) {
   dim3 grid((d.nx + 127) / 128, d.ny, d.nz);
-  k_m1_div<<<grid, 128, 0, s>>>(d, par.m1_odd_even != 0, U, su, V, sv, Wk, sw, KV, sk);
+  const double oe = par.m1_odd_even != 0 ? par.m1_oe_guard : -1.0;
+  k_m1_div<<<grid, 128, 0, s>>>(d, oe, U, su, V, sv, Wk, sw, KV, sk);
   constexpr int SEG = 6;
-  k_m1_march<1, SEG><<<dim3((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG), 128, 0, s>>>(d, par.m1_odd_even != 0, V, sv, Wk, sw, KV, sk);
-  k_m1_march<2, SEG><<<dim3((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG), 128, 0, s>>>(d, par.m1_odd_even != 0, V, sv, Wk, sw, KV, sk);
+  k_m1_march<1, SEG><<<dim3((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG), 128, 0, s>>>(d, oe, V, sv, Wk, sw, KV, sk);
+  k_m1_march<2, SEG><<<dim3((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG), 128, 0, s>>>(d, oe, V, sv, Wk, sw, KV, sk);
   return cudaGetLastError();
 }
 cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* V, size_t sv,

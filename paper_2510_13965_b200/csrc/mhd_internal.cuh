@@ -37,6 +37,7 @@ struct Par {
   int c2p_maxit;
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
   int m1_maxit, m1_odd_even;
+  double m1_arad, m1_oe_guard;
 };
 
 struct Slot {

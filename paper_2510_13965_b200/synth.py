@@ -69,19 +69,21 @@ def tableau(name):
 
 
 def imex_tableau(name="imex332"):
-    """IMEX pair (a_expl, w_expl, a_impl, w_impl) in the form of PAPER.md Eqs. (53)-(55). The paper's Tables I, II have no
-    body (R1), so the implicit tableau is caller data; this 3-stage, 2nd-order, L-stable pair satisfies every condition the
-    paper states (sum w = 1, sum w c = sum w c~ = sum w~ c = sum w~ c~ = 1/2, DIRK, R(-inf) = 0)."""
+    """IMEX pair (a_expl, w_expl, a_impl, w_impl) in the form of PAPER.md Eqs. (53)-(55) for IMEX(3,3,2) (l.408-410): the explicit
+    half IS the Shu-Osher SSP-RK(3,3) the paper names (tableau('ssprk3')). The body of the paper's Table II (I32L(3,2)) is
+    missing (R1), so the implicit half is caller data; the default is the 3-stage, 2nd-order, L-stable DIRK with constant
+    diagonal g = 1 - 1/sqrt(2) and the same weights as the explicit half (the published IMEX-SSP3(3,3,2) pairing): it meets
+    every condition the paper states (sum w = 1, sum w c = sum w c~ = sum w~ c = sum w~ c~ = 1/2, DIRK, c_i = sum_j a_ij,
+    R(-inf) = 0); `tests/test_oracle_m1.py::test_imex_tableau_conditions` checks them."""
     if name != "imex332":
         raise ValueError(name)
-    ae = np.zeros((3, 3))
-    ae[1, 0] = 0.5
-    ae[2, 0] = ae[2, 1] = 0.5
-    we = np.array([1 / 3, 1 / 3, 1 / 3])
+    ae, we = tableau("ssprk3")
+    g = 1.0 - 1.0 / math.sqrt(2.0)
     ai = np.zeros((3, 3))
-    ai[0, 0] = ai[1, 1] = 0.25
-    ai[2, 0] = ai[2, 1] = ai[2, 2] = 1 / 3
-    wi = np.array([1 / 3, 1 / 3, 1 / 3])
+    ai[0, 0] = ai[1, 1] = ai[2, 2] = g
+    ai[1, 0] = 1.0 - 2.0 * g
+    ai[2, 0] = 0.5 - g
+    wi = we.copy()
     return ae, we, ai, wi
 
 
@@ -97,7 +99,7 @@ def default_params(**over):
         rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, alpha_bh=0.1, w_max=100.0, rho_max=1.0,
         eps_min=0.0, eps_max=1e3, ye_min=0.0, ye_max=1.0, ye_atmo=0.3, eps_atmo=1e-8, T_atmo=0.1,
         c2p_maxit=100,
-        m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30, m1_odd_even=1,
+        m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30, m1_odd_even=1, m1_arad=1.0, m1_oe_guard=1e-10,
     )
     p.update(over)
     return p
@@ -407,6 +409,58 @@ def tov_fields(prof, rb):
     return rho, p, alpha, psi, dpdr
 
 
+def tov_profile_barotrope(key, p_of_rho, e_of_rho, dpdrho, rho_c, rho_surf, dr=2.0e-3):
+    """The same TOV equations as tov_profile for a general barotrope p(rho), e(rho) (total energy density), integrated in
+    (m, rho, nu, ln(rbar/r)) with d rho/dr = (dp/dr) / (dp/drho) from the centre down to rho = rho_surf (the stellar surface of
+    the synthetic star: the density below which the patch holds atmosphere). Initial data only; `key` caches the result."""
+    if key in _TOV_CACHE:
+        return _TOV_CACHE[key]
+
+    def rhs(r, y):
+        m, rho, nu, lq = y
+        if r == 0.0:
+            return np.array([0.0, 0.0, 0.0, 0.0])
+        rho = max(rho, 0.5 * rho_surf)
+        p, e = p_of_rho(rho), e_of_rho(rho)
+        a = (m + 4.0 * math.pi * r ** 3 * p) / (r * (r - 2.0 * m))
+        return np.array([4.0 * math.pi * r * r * e, -(e + p) * a / dpdrho(rho), a, (1.0 / math.sqrt(1.0 - 2.0 * m / r) - 1.0) / r])
+
+    y = np.array([0.0, rho_c, 0.0, 0.0])
+    r = 0.0
+    rs, ys = [r], [y.copy()]
+    while r < 100.0:
+        k1 = rhs(r, y)
+        k2 = rhs(r + 0.5 * dr, y + 0.5 * dr * k1)
+        k3 = rhs(r + 0.5 * dr, y + 0.5 * dr * k2)
+        k4 = rhs(r + dr, y + dr * k3)
+        yn = y + dr / 6.0 * (k1 + 2 * k2 + 2 * k3 + k4)
+        if yn[1] <= rho_surf:                    # last partial step to the surface by linear interpolation in rho
+            f = (y[1] - rho_surf) / (y[1] - yn[1])
+            yn = y + f * (yn - y)
+            r += f * dr
+            yn[1] = rho_surf
+            rs.append(r)
+            ys.append(yn)
+            break
+        r += dr
+        y = yn
+        rs.append(r)
+        ys.append(y.copy())
+    rs, ys = np.array(rs), np.array(ys)
+    M, R = ys[-1, 0], rs[-1]
+    Rbar = 0.5 * (R - M + math.sqrt(R * R - 2.0 * M * R))
+    lq = ys[:, 3] + (math.log(Rbar / R) - ys[-1, 3])
+    rbar = rs * np.exp(lq)
+    nu = ys[:, 2] + (0.5 * math.log(1.0 - 2.0 * M / R) - ys[-1, 2])
+    rho = ys[:, 1]
+    p = np.array([p_of_rho(x) for x in rho])
+    psi = np.sqrt(np.where(rbar > 0, rs / np.where(rbar > 0, rbar, 1.0), np.exp(-lq[0])))
+    psi[0] = math.exp(-0.5 * lq[0])
+    out = dict(rbar=rbar, rho=rho, p=p, alpha=np.exp(nu), psi=psi, M=M, R=R, Rbar=Rbar)
+    _TOV_CACHE[key] = out
+    return out
+
+
 # ---- config 3: static magnetised TOV star (BASELINE.json configs[2]) --------------------------------------
 def config3(n=128, half_width=16.0, ng=NG, b_scale=1e-4, seed=SEED_BASE + 3):
     """Polytrope K=100, Gamma=2, rho_c=1.28e-3 (M ~ 1.4) on an n^3 patch of the given half width, outflow boundaries.
@@ -484,41 +538,69 @@ def make_table(n_rho=180, n_T=120, n_ye=50):
     return tab
 
 
+def config4_thermal(rho, rho_c, T_star, T_floor=0.2):
+    """Temperature [MeV] and electron fraction of the synthetic hot star as functions of density (input recipe): T falls from
+    T_star at the centre to T_floor (inside the table, above its lower edge) like rho^(Gamma-1), Ye from 0.3 to 0.1."""
+    x = np.maximum(rho, 0.0) / rho_c
+    return T_floor + (T_star - T_floor) * x ** 1.5, 0.1 + 0.2 * x ** 0.25
+
+
 def config4(n=256, ng=NG, seed=SEED_BASE + 4, table_shape=(180, 120, 50), T_star=10.0, v_eq=0.2, b_scale=1e-4):
     """Hot, rigidly rotating, magnetised star on an n^3 patch with the tabulated EoS (eos_kind = 2).
-    Cold part p = K rho^2.5 with K = 2800 (gives p_c close to the Gamma = 2, K = 100 polytrope at rho_c = 1.28e-3);
-    TOV-like profile of that cold EoS in isotropic coordinates; uniform temperature T_star inside, T_atmo outside;
+    Cold part p = K rho^2.5 with K = 2800 (gives p_c close to the Gamma = 2, K = 100 polytrope at rho_c = 1.28e-3); thermal part
+    with T(rho), Ye(rho) of config4_thermal (T_star at the centre). The star is the TOV solution of THAT hot barotrope
+    p(rho) = p_table(rho, T(rho), Ye(rho)) in isotropic coordinates, so the thermal pressure is in hydrostatic balance (a cold
+    profile with a uniform temperature painted on is not: its surface layers, where the thermal pressure dominates, blow off
+    and shock-heat past the table's eps_max, which the error policy of PAPER.md:1158-1162 treats as fatal);
     rigid rotation about z with Omega such that v = v_eq at the equator; poloidal field as in config 3; density
     multiplied by (1 + 1e-3 U(-1,1)) cell by cell (seeded). The patch width is Rbar / 0.46 (half width Rbar / 0.92), so that about 41 %
     of the cells are star."""
     Kc, Gc, rho_c = 2800.0, 2.5, 1.28e-3
     tab = make_table(*table_shape)
-    prof = tov_profile(Kc, Gc, rho_c)
+    # rho_low (R10, the "low-density region" of PAPER.md:1160-1162 where eps / v / Ye excursions are repaired instead of being
+    # fatal) = 10 x the surface density of the synthetic star: the three-decade jump to the atmosphere makes the ratio
+    # Dbar Ye / Dbar of the cells the surface spills into leave the table's Ye range
+    par = default_params(eos_kind=2, rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-6, T_atmo=0.1, ye_min=0.05, ye_max=0.6,
+                         ye_atmo=0.3, rho_max=10.0 ** (tab["lr0"] + tab["dlr"] * (tab["n_rho"] - 1)), eps_max=1e3)
+    rho_surf = 1e3 * par["rho_atmo"]
+
+    def p_of_rho(r):
+        T, ye = config4_thermal(r, rho_c, T_star)
+        return float(table_eos_analytic(r, T, ye, K=Kc, Gamma=Gc)[0])
+
+    def e_of_rho(r):
+        T, ye = config4_thermal(r, rho_c, T_star)
+        return float(r * (1.0 + table_eos_analytic(r, T, ye, K=Kc, Gamma=Gc)[1]))
+
+    def dpdrho(r):
+        h = 1e-6 * r
+        return (p_of_rho(r + h) - p_of_rho(r - h)) / (2.0 * h)
+
+    prof = tov_profile_barotrope(("c4hot", Kc, Gc, rho_c, T_star, rho_surf), p_of_rho, e_of_rho, dpdrho, rho_c, rho_surf)
     half = prof["Rbar"] / 0.92
     dx = 2.0 * half / n
     x0 = -half + 0.5 * dx
     X, Y, Z = mesh(n, n, n, ng, dx, x0=(x0, x0, x0))
     rb = np.sqrt(X * X + Y * Y + Z * Z)
     rho, p, alpha, psi, dpdr = tov_fields(prof, rb)
-    par = default_params(eos_kind=2, rho_atmo=1e-10, rho_cut=1.01e-10, rho_low=1e-8, T_atmo=0.1, ye_min=0.05, ye_max=0.6,
-                         ye_atmo=0.3, rho_max=10.0 ** (tab["lr0"] + tab["dlr"] * (tab["n_rho"] - 1)), eps_max=1e3)
     U = _flat_state(X.shape)
     U[CHI] = psi ** -4
     U[ALPHA] = alpha
     rng = SplitMix64(seed)
     noise = np.array([rng.uniform(-1.0, 1.0) for _ in range(4096)])
     idx = (np.arange(X.size, dtype=np.int64) * 2654435761 % 4096).reshape(X.shape)        # cheap seeded scatter of 4096 draws
-    star = rho > 1e3 * par["rho_atmo"]
+    star = rho >= rho_surf
     P = np.zeros((NPRIM,) + X.shape)
     P[RHO] = np.where(star, rho * (1.0 + 1e-3 * noise[idx]), par["rho_atmo"])
-    P[YE] = np.where(star, 0.1 + 0.2 * np.exp(-(rb / prof["Rbar"]) ** 2), par["ye_atmo"])
-    Tf = np.where(star, T_star, par["T_atmo"])
-    P[EPS] = table_eos_analytic(P[RHO], Tf, P[YE])[1]
+    Ts, yes = config4_thermal(rho, rho_c, T_star)
+    P[YE] = np.where(star, yes, par["ye_atmo"])
+    Tf = np.where(star, Ts, par["T_atmo"])
+    P[EPS] = table_eos_analytic(P[RHO], Tf, P[YE], K=Kc, Gamma=Gc)[1]
     # atmosphere eps must be what the EoS returns for T_atmo through the table (interpolated), the kernels reset it anyway
     omega = v_eq / prof["Rbar"]
     P[VX] = np.where(star, -omega * Y, 0.0)
     P[VX + 1] = np.where(star, omega * X, 0.0)
-    pmax = Kc * rho_c ** Gc
+    pmax = p_of_rho(rho_c)
     on = p > 0.04 * pmax
     Ab = np.where(on, p - 0.04 * pmax, 0.0)
     dAb = np.where(on, dpdr, 0.0) / np.maximum(rb, 1e-300)

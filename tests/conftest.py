@@ -17,6 +17,9 @@ def pytest_configure(config):
 def oracle_mod():
     import oracle
     oracle.build()
+    # the -fopenmp build of the same sources (outermost grid loops only; per-point arithmetic and results unchanged) keeps the
+    # suite to minutes; ORACLE_THREADS=1 runs the plain single-threaded build
+    oracle.use_threads(int(os.environ.get("ORACLE_THREADS", os.cpu_count() or 1)))
     return oracle
 
 

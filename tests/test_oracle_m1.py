@@ -168,15 +168,29 @@ def test_m1_rhs_constant_state_and_diffusion_limit(oracle_mod):
 
 
 def test_imex_tableau_conditions():
-    """R1: the conditions PAPER.md:389-408 states for the IMEX pair."""
+    """R1: the conditions PAPER.md:389-410 states for IMEX(3,3,2): the explicit half is the Shu-Osher SSP-RK(3,3) (its weights are
+    Eq. 59 at theta = 1), the implicit half is a DIRK with c_i = sum_j a_ij (Eq. 55), second order incl. the mixed conditions,
+    L-stable. Catches: a non-SSP explicit half (the round-1 tableau), a wrong sign in a_21, a diagonal that is not L-stable."""
     ae, we, ai, wi = synth.imex_tableau()
+    a3, w3 = synth.tableau("ssprk3")
+    assert np.array_equal(ae, a3) and np.array_equal(we, w3)
+    assert np.allclose(ae.sum(axis=1), [0.0, 1.0, 0.5])
+    b = lambda th: np.array([th - 5.0 / 6.0 * th * th, th * th / 6.0, 4.0 * th * th / 6.0])      # Eq. (59)
+    assert np.allclose(b(1.0), we, atol=1e-15)
+    # explicit half: third order
     ce, ci = ae.sum(axis=1), ai.sum(axis=1)
+    assert abs(we @ ce ** 2 - 1 / 3) < 1e-15 and abs(we @ (ae @ ce) - 1 / 6) < 1e-15
     assert np.allclose(np.triu(ae), 0) and np.allclose(np.triu(ai, 1), 0)
     assert abs(we.sum() - 1) < 1e-15 and abs(wi.sum() - 1) < 1e-15
     for w in (we, wi):
         for c in (ce, ci):
             assert abs(w @ c - 0.5) < 1e-15
     assert abs(1.0 - wi @ np.linalg.solve(ai, np.ones(3))) < 1e-14      # R(-inf) = 0: L-stable
+    # A-stability on the imaginary axis: |R(iy)| <= 1
+    for y in np.linspace(0.0, 50.0, 201):
+        z = 1j * y
+        R = 1.0 + z * (wi @ np.linalg.solve(np.eye(3) - z * ai, np.ones(3)))
+        assert abs(R) <= 1.0 + 1e-12
 
 
 def test_odd_even_switch_fires_on_a_zigzag_only(oracle_mod):
