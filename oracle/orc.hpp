@@ -11,16 +11,19 @@
 // Citations are "PAPER.md:<line>" plus the equation they fall in. Readings of
 // silent / garbled passages are the R-numbers of DESIGN.md.
 //
-// Parity pins (tests/test_oracle_*.py): stencils (polynomial exactness + leading
-// error constants), CCZ4 (flat space = 0; manufactured wavy-Minkowski exact solution,
-// also with a Killing Z-vector), GRMHD (boosted magnetised fluid in wavy Minkowski;
-// TOV equilibrium; SRMHD Alfven wave; Riemann monotonicity), con2prim (round trip),
-// MP5 (Eq. 70 on smooth data, monotone on a step), RK (exp series).
-// PARITY UNPINNED: kappa_z/kappa_c/kappa_2 damping terms beyond "vanish with the
-// constraint" and a hand value; atmosphere / error-policy parameter values (R10);
-// outflow boundary order (R17); M1: the Phi / A blend of Eq. (77) beyond its limits, the E -> 0 and |F| > E fix-ups (R22),
-// the N equation's closure assumption (Eq. 37), the implicit tableau values (R1), the shift- and curvature-dependent geometric sources of
-// Eqs. (39)-(40) (d beta, A~_ij, K^ terms; the d alpha, d chi terms are pinned by the static beam in Schwarzschild).
+// Parity pins (tests/test_oracle_*.py): stencils (polynomial exactness + leading error constants), CCZ4 (flat space = 0;
+// manufactured wavy-Minkowski exact solution, also with a Killing Z-vector; every algebraic term incl. the kappa_z, kappa_c,
+// kappa_2 dampings by hand values on a uniform state), GRMHD (boosted magnetised fluid in wavy Minkowski; TOV equilibrium;
+// SRMHD Alfven wave; Riemann monotonicity), con2prim (round trip; textbook hydro limit; the degenerate root h = h0), EoS
+// (piecewise-polytrope constants in closed form; table lookup and T inversion against scipy's multilinear interpolator), MP5
+// (Eq. 70 on smooth data, monotone on a step), RK (exp series, dense-output weights), M1 (closure exact in the thick and thin
+// limits; App. C forms = Sec. II C forms; Jacobian vs finite differences; implicit-solve limits; (C11)-(C12) in a moving
+// fluid; fix-up branches; Schwarzschild beam; isotropic radiation and a null beam in wavy Minkowski = flux brackets and all
+// geometric sources of Eqs. 38-40 incl. R19 and the number flux; one hand-computed face of Eq. 77; odd-even switch as printed
+// and with the R33 guard).
+// PARITY UNPINNED (readings of passages the paper leaves open; nothing in the paper or the mathematics fixes them): the values
+// of the implicit tableau (R1: Table II has no body), the error-policy parameter values (R10), the outflow boundary order
+// (R17), the choice of (log10 rho, log10 T, Ye) / (log10 p, log10 eps) as the table's interpolation variables (R26).
 #pragma once
 #include <cstddef>
 #include <cstdint>

@@ -2,8 +2,7 @@
 // characteristic speeds (App. B, Eqs. B4-B5), flux-limited advection-diffusion fluxes (Sec. III D, Eqs. 77-78),
 // geometric sources of Eqs. (39)-(40), pointwise implicit stiff solve (App. C, Eqs. C10-C35) and the IMEX stage driver
 // (Eq. 53, App. C steps C3-C4). Readings R19-R24 of DESIGN.md.
-// PARITY UNPINNED: the Phi / A blend of Eq. (77) beyond its limits (constant state, kappa dx -> infinity), the E -> 0 and
-// F_k F^k > E^2 fix-ups (R22), the N equation's closure assumption (Eq. 37), the implicit tableau values (R1).
+// PARITY UNPINNED: the implicit tableau values (R1) only; see orc.hpp for the list of pins.
 #include <algorithm>
 #include <cmath>
 #include <cstring>

@@ -113,3 +113,38 @@ def fluid(t, X, Y, Z):
     v = [u[..., i + 1] / W + beta[i] / alpha for i in range(3)]
     B = [W * b[..., i + 1] - alpha * b[..., 0] * u[..., i + 1] for i in range(3)]
     return a, v, W, B
+
+
+# ---- radiation fields with a uniform stress-energy tensor in the inertial frame -------------------------
+def radiation(t, X, Y, Z, TMN, NM):
+    """Densitised M1 fields (Nbar, Ebar, Fbar_i) on the wavy slice at time t of a radiation field whose stress-energy tensor
+    T^MN and number current N^M are CONSTANT in the inertial frame (so nabla_a T^ab = 0 and nabla_a N^a = 0 hold exactly):
+    E = n_a n_b T^ab = alpha^2 T^tt, F_i = -n_a gamma_ib T^ab = alpha g_i_nu T^t_nu, N = -n_a N^a = alpha N^t (Eq. 35)."""
+    a = adm(t, X, Y, Z)
+    J = a["J"]
+    shape = X.shape
+    Jm = np.zeros(shape + (4, 4))
+    for M in range(4):
+        for mu in range(4):
+            Jm[..., M, mu] = J[M][mu]
+    Ji = np.linalg.inv(Jm)                                # (J^-1)^mu_M
+    T = np.einsum("...mM,...nN,MN->...mn", Ji, Ji, TMN)   # T^mu_nu in wavy coordinates
+    Nu = np.einsum("...mM,M->...m", Ji, NM)
+    g = np.einsum("M,...Mm,...Mn->...mn", np.diag(ETA), Jm, Jm)
+    alpha = a["alpha"]
+    sg = np.sqrt(a["det"])
+    E = alpha ** 2 * T[..., 0, 0]
+    F = [alpha * np.einsum("...n,...n->...", g[..., i + 1, :], T[..., 0, :]) for i in range(3)]
+    return np.stack([sg * alpha * Nu[..., 0], sg * E] + [sg * f for f in F])
+
+
+def isotropic_radiation(J0, n0):
+    """T^MN = 4/3 J u^M u^N + J/3 eta^MN, N^M = n u^M: radiation isotropic in the frame of the uniform fluid of `fluid`."""
+    return 4.0 / 3.0 * J0 * np.outer(UM, UM) + J0 / 3.0 * ETA, n0 * UM
+
+
+def null_beam(e0, n0, direction):
+    """T^MN = e k^M k^N, N^M = n k^M with k = (1, unit vector): a single beam of free-streaming radiation."""
+    d = np.asarray(direction, dtype=float)
+    k = np.concatenate([[1.0], d / np.linalg.norm(d)])
+    return e0 * np.outer(k, k), n0 * k
