@@ -96,7 +96,8 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
-  if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2)) return MHD_E_ARG;
+  if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2 ||
+                              !(desc->dlr > 0.0 && desc->dlT > 0.0 && desc->dye > 0.0))) return MHD_E_ARG;
   mhd_patch* p = new (std::nothrow) mhd_patch();
   if (!p) return MHD_E_ARG;
   p->desc = *desc;
@@ -114,6 +115,10 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.n_rho = desc->n_rho; q.n_T = desc->n_T; q.n_ye = desc->n_ye;
   q.lr0 = desc->lr0; q.dlr = desc->dlr; q.lT0 = desc->lT0; q.dlT = desc->dlT; q.ye0 = desc->ye0; q.dye = desc->dye;
   q.tab_eps_shift = desc->tab_eps_shift; q.tab_h0 = desc->tab_h0;
+  if (q.eos_kind == 2) {
+    q.idlr = 1.0 / q.dlr; q.idlT = 1.0 / q.dlT; q.idye = 1.0 / q.dye;
+    q.tab_rho_lo = pow(10.0, q.lr0); q.tab_rho_hi = pow(10.0, q.lr0 + q.dlr * (q.n_rho - 1));
+  }
   q.kappa_z = desc->kappa_z; q.kappa_c = desc->kappa_c; q.kappa_2 = desc->kappa_2; q.eta_shift = desc->eta_shift;
   q.f_alpha = desc->f_alpha; q.f_beta = desc->f_beta; q.grav_G = desc->grav_G;
   for (int i = 0; i < 3; ++i) q.beta0[i] = desc->beta0[i];
@@ -128,7 +133,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
   q.m1_odd_even = desc->m1_odd_even; q.m1_arad = desc->m1_arad; q.m1_oe_guard = desc->m1_oe_guard;
   p->d_counts = nullptr;
-  if (cudaMalloc(&p->d_counts, 8 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
+  if (cudaMalloc(&p->d_counts, 16 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   *out = p;
   return MHD_OK;
 }
@@ -163,7 +168,7 @@ int mhd_con2prim(mhd_patch* p, int slot_state, int slot_prim, int slot_flags, vo
   if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_flags)) return MHD_E_UNBOUND;
   Timed tm(p, 1, (cudaStream_t)stream);
   return launch_con2prim(p->dims, p->par, dptr(p, slot_state), p->slot[slot_state].stride, dptr(p, slot_prim), p->slot[slot_prim].stride,
-                         (uint8_t*)p->slot[slot_flags].ptr, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+                         (uint8_t*)p->slot[slot_flags].ptr, (double*)(p->d_counts + 8), (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
 }
 
 int mhd_prim2con(mhd_patch* p, int slot_state, int slot_prim, void* stream) {

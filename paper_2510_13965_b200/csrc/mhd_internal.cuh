@@ -29,6 +29,7 @@ struct Par {
   const double *tab_logp, *tab_loge, *tab_cs2;
   int n_rho, n_T, n_ye;
   double lr0, dlr, lT0, dlT, ye0, dye, tab_eps_shift, tab_h0;
+  double idlr, idlT, idye, tab_rho_lo, tab_rho_hi;   // derived at create time: reciprocal spacings, density range of the table
   double kappa_z, kappa_c, kappa_2, eta_shift, f_alpha, f_beta, beta0[3], grav_G;
   double sigma_ko_spacetime, sigma_ko_matter;
   double c_b, kappa_b, mp5_alpha;
@@ -52,7 +53,7 @@ struct mhd_patch {
   mhd::Dims dims;
   mhd::Par par;
   mhd::Slot slot[MHD_NSLOTS];
-  unsigned long long* d_counts;   // 8 counters for mhd_patch_status
+  unsigned long long* d_counts;   // device scratch: 8 counters for mhd_patch_status, then 8 doubles (EoS part of the atmosphere state)
   // optional per-kernel timing (mhd_patch_profile)
   bool profiling = false;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -63,7 +64,7 @@ struct mhd_patch {
 namespace mhd {
 // kernel launchers (one per translation unit); all return cudaGetLastError()
 cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], cudaStream_t s);
-cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, cudaStream_t s);
+cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, double* atmo, cudaStream_t s);
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
 cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, cudaStream_t s);
