@@ -55,7 +55,10 @@ enum {
   MHD_SLOT_M1WORK,                        /* scratch of mhd_m1_rhs                           (MHD_NM1WORK fields) */
   MHD_SLOT_KV1,                           /* explicit parts F_V(U^(j)): MHD_SLOT_KV1 + j - 1 (MHD_NM1 fields)     */
   MHD_SLOT_R1 = MHD_SLOT_KV1 + MHD_MAX_STAGES,   /* stiff sources R_V(U^(j)): MHD_SLOT_R1 + j - 1 (MHD_NM1 fields) */
-  MHD_NSLOTS = MHD_SLOT_R1 + MHD_MAX_STAGES
+  MHD_SLOT_U1 = MHD_SLOT_R1 + MHD_MAX_STAGES,    /* optional third state buffer (MHD_NSTATE fields): lets mhd_advance fuse the RK combine
+                                                    into the right-hand-side kernels (the new stage state cannot overwrite the one
+                                                    whose stencils are being read); unbound = separate combine kernel */
+  MHD_NSLOTS = MHD_SLOT_U1 + 1
 };
 
 /* flag bits: error policy of PAPER.md:1157-1162 */
@@ -164,7 +167,9 @@ int mhd_rhs(mhd_patch *p, int slot_state, int slot_prim, int slot_rhs, void *cud
 int mhd_rk_stage(mhd_patch *p, const mhd_tableau *t, int stage, double dt, void *cuda_stream);
 
 /* n_steps full RK steps, device resident: per stage fill -> con2prim -> rhs(K_stage) -> rk_stage; the state is
- * left with ghosts filled and primitives/flags consistent. Asynchronous. */
+ * left with ghosts filled and primitives/flags consistent. Asynchronous. With MHD_SLOT_U1 bound the combine of Eq. (53) is
+ * computed by the last right-hand-side kernel that touches each field (same arithmetic, one pass less over K and U per
+ * stage; K_s of the last stage is then not stored); the buffers bound to U, U0, U1 are all overwritten, the result is in U. */
 int mhd_advance(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
 
 /* Same, end to end with HOST buffers: copies host_U (MHD_NSTATE fields, packed, field_stride = MX*MY*MZ) to

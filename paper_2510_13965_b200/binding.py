@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
 SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
 NM1, NM1WORK = 15, 75
-SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1 = 13, 14, 15, 16, 24
+SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1, SLOT_U1 = 13, 14, 15, 16, 24, 32
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p
@@ -244,7 +244,7 @@ def mhd_probe_fp64_flops(stream=None):
 class Patch:
     """Owns the torch device tensors of one patch and binds them to the library's slots."""
 
-    def __init__(self, params, n, ng, dx, stages=4, table=None, device="cuda:0", m1=False):
+    def __init__(self, params, n, ng, dx, stages=4, table=None, device="cuda:0", m1=False, fused=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libmhd_b200 needs a CUDA device; there is no CPU fallback")
@@ -271,6 +271,11 @@ class Patch:
         for slot, t in [(SLOT_U, self.U), (SLOT_U0, self.U0), (SLOT_P, self.P), (SLOT_FLAGS, self.flags), (SLOT_WORK, self.work)] + \
                        [(SLOT_K1 + j, k) for j, k in enumerate(self.K)]:
             mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
+        self.U1 = None
+        if fused and not m1:                                # third state buffer: mhd_advance then fuses the RK combine into the RHS kernels (measured slower on B200
+                                                            # with the present latency-bound k_adv_ko / k_recon_march: 111.9 vs 107.5 ms per step at c4_256; off by default)
+            self.U1 = z(NSTATE)
+            mhd_patch_bind(self.h, SLOT_U1, self.U1.data_ptr(), self.npts)
         if m1:                                              # grey M1, 3 species: V, V^n, per-stage explicit parts and stiff sources
             self.V, self.V0, self.m1work = z(NM1), z(NM1), z(NM1WORK)
             self.KV = [z(NM1) for _ in range(stages)]

@@ -17,8 +17,8 @@ int slot_fields(int slot) {
   return MHD_NSTATE;
 }
 bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLOTS && p->slot[slot].ptr != nullptr; }
-bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || (slot >= MHD_SLOT_K1 && slot < MHD_SLOT_K1 + MHD_MAX_STAGES); }
-bool is_m1_slot(int slot) { return slot >= MHD_SLOT_V && slot < MHD_NSLOTS && slot != MHD_SLOT_M1WORK; }
+bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || slot == MHD_SLOT_U1 || (slot >= MHD_SLOT_K1 && slot < MHD_SLOT_K1 + MHD_MAX_STAGES); }
+bool is_m1_slot(int slot) { return slot >= MHD_SLOT_V && slot < MHD_SLOT_U1 && slot != MHD_SLOT_M1WORK; }
 double* dptr(const mhd_patch* p, int slot) { return (double*)p->slot[slot].ptr; }
 
 // piecewise-polytrope continuity constants: K_i, a_i for i > 0
@@ -49,6 +49,63 @@ struct Timed {
   }
 };
 
+// a3-a8: the kernels of one right-hand-side evaluation; fz (optional) fuses the RK combine into the last kernel that touches each field
+int rhs_impl(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, const Fuse& fz, cudaStream_t s) {
+  double* Wk = dptr(p, MHD_SLOT_WORK);
+  const size_t sw = p->slot[MHD_SLOT_WORK].stride;
+  const double* U = dptr(p, slot_state);
+  const double* P = dptr(p, slot_prim);
+  double* K = dptr(p, slot_rhs);
+  const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
+  { Timed tm(p, 2, s); if (launch_ccz4_algebra(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
+  { Timed tm(p, 8, s); if (launch_adv_ko(p->dims, p->par, U, su, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA; }
+  { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
+  for (int dir = 0; dir < 3; ++dir) {
+    Timed tm(p, 3 + dir, s);
+    if (launch_recon(dir, p->dims, p->par, U, su, Wk, sw, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA;
+  }
+  return MHD_OK;
+}
+
+
+// n_steps full RK steps, the combine of Eq. (53) fused into the right-hand-side kernels (needs the third state buffer MHD_SLOT_U1).
+// Three buffers rotate: one holds U^n for the whole step, each stage differentiates `cur` and writes the next stage state into the
+// buffer that is neither `cur` nor U^n. Nothing is copied except, once per call, the result into the buffer bound to MHD_SLOT_U.
+int stage_sequence_fused(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, cudaStream_t s) {
+  const Slot buf[3] = {p->slot[MHD_SLOT_U], p->slot[MHD_SLOT_U0], p->slot[MHD_SLOT_U1]};
+  auto done = [&](int code) { p->slot[MHD_SLOT_U] = buf[0]; return code; };
+  const int q = t->stages;
+  for (int j = 0; j < q; ++j) if (!slot_ok(p, MHD_SLOT_K1 + j)) return MHD_E_UNBOUND;
+  int rc, cur = 0;
+  for (int step = 0; step < n_steps; ++step) {
+    const int u0 = cur;                                      // U^n = the state entering the step, after the ghost fill and con2prim of stage 1 (R31)
+    for (int st = 1; st <= q; ++st) {
+      p->slot[MHD_SLOT_U] = buf[cur];
+      if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return done(rc);
+      if ((rc = mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s)) != MHD_OK) return done(rc);
+      int w = 0;
+      while (w == cur || w == u0) ++w;
+      const double* coef = st < q ? t->a_expl + (size_t)st * q : t->w_expl;      // row of U^(st+1), or the weights
+      Fuse fz;
+      fz.Uout = (double*)buf[w].ptr; fz.so = buf[w].stride;
+      fz.U0 = (const double*)buf[u0].ptr; fz.s0 = buf[u0].stride;
+      fz.cself = dt * coef[st - 1];
+      fz.write_k = st < q;                                   // K_q has no later reader
+      for (int j = 0; j < st - 1; ++j)
+        if (coef[j] != 0.0) { fz.Kp[fz.nk] = dptr(p, MHD_SLOT_K1 + j); fz.skp[fz.nk] = p->slot[MHD_SLOT_K1 + j].stride; fz.cp[fz.nk] = dt * coef[j]; ++fz.nk; }
+      if ((rc = rhs_impl(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_K1 + st - 1, fz, s)) != MHD_OK) return done(rc);
+      cur = w;
+    }
+  }
+  if (cur != 0) {                                            // result lives in another buffer: copy it home (once per call)
+    Timed tm(p, 6, s);
+    if (launch_copy_fields(p->dims, MHD_NSTATE, (double*)buf[0].ptr, buf[0].stride, (const double*)buf[cur].ptr, buf[cur].stride, s) != cudaSuccess) return done(MHD_E_CUDA);
+  }
+  p->slot[MHD_SLOT_U] = buf[0];
+  if ((rc = mhd_fill_ghosts(p, MHD_SLOT_U, bc, s)) != MHD_OK) return rc;
+  return mhd_con2prim(p, MHD_SLOT_U, MHD_SLOT_P, MHD_SLOT_FLAGS, s);
+}
+
 // n_steps full RK steps. "U0 <- U" at the start of a step is a swap of the two slot pointers, not a copy: the first
 // combine of the step rewrites the whole interior of the new U buffer and the ghost fill that follows rewrites every
 // ghost cell, so nothing of its old content survives. After an odd number of steps the result is copied back into the
@@ -56,6 +113,8 @@ struct Timed {
 int stage_sequence(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, cudaStream_t s) {
   int rc;
   if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_U0)) return MHD_E_UNBOUND;
+  if (slot_ok(p, MHD_SLOT_U1) && slot_ok(p, MHD_SLOT_P) && slot_ok(p, MHD_SLOT_FLAGS) && slot_ok(p, MHD_SLOT_WORK) && n_steps > 0)
+    return stage_sequence_fused(p, t, bc, dt, n_steps, s);
   bool swapped = false;
   auto swap_u = [&]() { Slot tmp = p->slot[MHD_SLOT_U]; p->slot[MHD_SLOT_U] = p->slot[MHD_SLOT_U0]; p->slot[MHD_SLOT_U0] = tmp; swapped = !swapped; };
   auto fail = [&](int code) { if (swapped) swap_u(); return code; };
@@ -181,21 +240,7 @@ int mhd_prim2con(mhd_patch* p, int slot_state, int slot_prim, void* stream) {
 int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* stream) {
   if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || !is_state_slot(slot_rhs) || slot_rhs == slot_state) return MHD_E_ARG;
   if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_rhs) || !slot_ok(p, MHD_SLOT_WORK)) return MHD_E_UNBOUND;
-  cudaStream_t s = (cudaStream_t)stream;
-  double* Wk = dptr(p, MHD_SLOT_WORK);
-  const size_t sw = p->slot[MHD_SLOT_WORK].stride;
-  const double* U = dptr(p, slot_state);
-  const double* P = dptr(p, slot_prim);
-  double* K = dptr(p, slot_rhs);
-  const size_t su = p->slot[slot_state].stride, sp = p->slot[slot_prim].stride, sk = p->slot[slot_rhs].stride;
-  { Timed tm(p, 2, s); if (launch_ccz4_algebra(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
-  { Timed tm(p, 8, s); if (launch_adv_ko(p->dims, p->par, U, su, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
-  { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
-  for (int dir = 0; dir < 3; ++dir) {
-    Timed tm(p, 3 + dir, s);
-    if (launch_recon(dir, p->dims, p->par, U, su, Wk, sw, K, sk, s) != cudaSuccess) return MHD_E_CUDA;
-  }
-  return MHD_OK;
+  return rhs_impl(p, slot_state, slot_prim, slot_rhs, Fuse(), (cudaStream_t)stream);
 }
 
 int mhd_rk_stage(mhd_patch* p, const mhd_tableau* t, int stage, double dt, void* stream) {

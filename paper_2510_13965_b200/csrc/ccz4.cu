@@ -514,9 +514,10 @@ __device__ __forceinline__ double adv_ko_axis(double um3, double um2, double um1
   return fma(cko + fabs(cbh), q, cbh * a);
 }
 
-template <bool ADV, int AZ, int MINB>
+template <bool ADV, int AZ, int MINB, bool FUSED>
 __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Dims d, double sigma, int f0, int nf,
-                                                      const double* __restrict__ U, size_t su, double* __restrict__ K, size_t sk) {
+                                                      const double* __restrict__ U, size_t su, double* __restrict__ K, size_t sk,
+                                                      const __grid_constant__ Fuse fz) {
   const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k0 = blockIdx.z * AZ;
   if (i >= d.nx || j >= d.ny) return;
   const int nzl = min(AZ, d.nz - k0);
@@ -539,6 +540,9 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
     double kold[AZ];    // K is read-modify-write: its loads are issued with the stencil loads, not after the arithmetic
 #pragma unroll
     for (int kk = 0; kk < AZ; ++kk) kold[kk] = kk < nzl ? ko[kk * sz] : 0.0;
+    double pre[AZ];     // U0 + earlier stages of the fused RK combine, fetched with the rest
+#pragma unroll
+    for (int kk = 0; kk < AZ; ++kk) pre[kk] = (FUSED && kk < nzl) ? fused_fetch(fz, f, base + kk * sz) : 0.0;
 #pragma unroll
     for (int kk = 0; kk < AZ; ++kk) {
       if (kk < nzl) {
@@ -547,7 +551,7 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
         double acc = adv_ko_axis<ADV>(w[kk], w[kk + 1], w[kk + 2], u0, w[kk + 4], w[kk + 5], w[kk + 6], cb[kk][2], cko[2]);
         acc += adv_ko_axis<ADV>(__ldg(c - 3), __ldg(c - 2), __ldg(c - 1), u0, __ldg(c + 1), __ldg(c + 2), __ldg(c + 3), cb[kk][0], cko[0]);
         acc += adv_ko_axis<ADV>(__ldg(c - 3 * sy), __ldg(c - 2 * sy), __ldg(c - sy), u0, __ldg(c + sy), __ldg(c + 2 * sy), __ldg(c + 3 * sy), cb[kk][1], cko[1]);
-        ko[kk * sz] = kold[kk] + acc;
+        if (FUSED) fused_store(fz, f, base + kk * sz, pre[kk], kold[kk] + acc, ko + kk * sz); else ko[kk * sz] = kold[kk] + acc;
       }
     }
   }
@@ -571,12 +575,13 @@ cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, cudaStream_t s) {
+cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
   constexpr int AZ = 4;
   dim3 ablock(32, 8), agrid((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + AZ - 1) / AZ);
-  k_adv_ko<true, AZ, 3><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk);
-  if (par.sigma_ko_matter != 0.0)                                          // R16: optional KO on the matter fields
-    k_adv_ko<false, AZ, 4><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk);
+  if (fz.Uout) k_adv_ko<true, AZ, 2, true><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk, fz);   // last kernel to touch the spacetime K
+  else k_adv_ko<true, AZ, 3, false><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk, fz);
+  if (par.sigma_ko_matter != 0.0)                                          // R16: optional KO on the matter fields (the fluid K is finished by flux.cu)
+    k_adv_ko<false, AZ, 4, false><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_matter, DBAR, 10, U, su, K, sk, fz);
   return cudaGetLastError();
 }
 

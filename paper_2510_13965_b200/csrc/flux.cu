@@ -219,9 +219,10 @@ namespace {
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int RW = 4;    // warps per CTA of the reconstruction kernels
 
-template <int DIR, int SEG>
+template <int DIR, int SEG, bool FUSED>
 __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
-                                                            const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
+                                                            const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk,
+                                                            const __grid_constant__ Fuse fz) {
   __shared__ double q_v[RW][5 * QCAP];
   __shared__ int q_tag[RW][QCAP];
   __shared__ double q_corr[RW][2 * (SEG + 1) * 32];
@@ -267,6 +268,9 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     double kold[SEG];                                          // K is read-modify-write: fetched with the column, not after the arithmetic
 #pragma unroll
     for (int m = 1; m <= SEG; ++m) kold[m - 1] = (active && c0 + m - 1 < nline) ? k[base + (long long)(g0 + m + 2) * ls] : 0.0;
+    double pre[SEG];                                           // U0 + earlier stages of the fused RK combine (z pass only), fetched with the rest
+#pragma unroll
+    for (int m = 1; m <= SEG; ++m) pre[m - 1] = (FUSED && active && c0 + m - 1 < nline) ? fused_fetch(fz, DBAR + a, (size_t)(base + (long long)(g0 + m + 2) * ls)) : 0.0;
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
       acc[m] = flux_hat2(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
@@ -282,7 +286,8 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     for (int m = 1; m <= SEG; ++m)
       if (active && c0 + m - 1 < nline) {
         const long long pt = base + (long long)(g0 + m + 2) * ls;       // zone c0 + m - 1
-        k[pt] = kold[m - 1] - (acc[m] - acc[m - 1]) * hih;              // Eq. (64)
+        const double knew = kold[m - 1] - (acc[m] - acc[m - 1]) * hih;          // Eq. (64)
+        if (FUSED) fused_store(fz, DBAR + a, (size_t)pt, pre[m - 1], knew, k + pt); else k[pt] = knew;
       }
   }
 }
@@ -350,26 +355,27 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
 }  // namespace
 
 template <int SEG>
-static void launch_march(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
+static void launch_march(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
   if (dir == 1) {
     dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.nz, (d.ny + SEG - 1) / SEG);
-    k_recon_march<1, SEG><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  } else {
+    k_recon_march<1, SEG, false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
+  } else {                                                                    // z is the last pass over the fluid K: the RK combine rides on it
     dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.ny, (d.nz + SEG - 1) / SEG);
-    k_recon_march<2, SEG><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+    if (fz.Uout) k_recon_march<2, SEG, true><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
+    else k_recon_march<2, SEG, false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
   }
 }
 
-cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s) {
+cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
   static int seg = 0;
   if (seg == 0) { const char* v = getenv("MHD_RECON_SEG"); seg = v ? atoi(v) : 6; }
   if (dir == 0) {
     dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
     k_recon_x<<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  } else if (seg == 4) launch_march<4>(dir, d, par, U, su, Wk, sw, K, sk, s);
-  else if (seg == 6) launch_march<6>(dir, d, par, U, su, Wk, sw, K, sk, s);
-  else if (seg == 12) launch_march<12>(dir, d, par, U, su, Wk, sw, K, sk, s);
-  else launch_march<8>(dir, d, par, U, su, Wk, sw, K, sk, s);
+  } else if (seg == 4) launch_march<4>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else if (seg == 6) launch_march<6>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else if (seg == 12) launch_march<12>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else launch_march<8>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
   return cudaGetLastError();
 }
 

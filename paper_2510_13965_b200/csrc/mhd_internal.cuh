@@ -46,6 +46,33 @@ struct Slot {
   size_t stride = 0;
 };
 
+// Explicit RK combine (Eq. 53) fused into the last kernel that touches a field of K_i (k_adv_ko for the 22 spacetime fields,
+// k_recon_march<z> for the 10 fluid fields):  Uout = U0 + sum_m cp[m] Kp[m] + cself K_i,  with cp, cself already multiplied by dt.
+// Uout must not be the state the stencils read. K_i itself is written only if write_k (the last stage has no later reader).
+struct Fuse {
+  double* Uout = nullptr; size_t so = 0;          // nullptr: no fused combine (K_i is written)
+  const double* U0 = nullptr; size_t s0 = 0;
+  const double* Kp[MHD_MAX_STAGES - 1] = {}; size_t skp[MHD_MAX_STAGES - 1] = {}; double cp[MHD_MAX_STAGES - 1] = {};
+  int nk = 0;
+  double cself = 0.0;
+  int write_k = 1;
+};
+// Two halves, so that the loads are issued with the stencil loads of the kernel and not after its arithmetic:
+// fused_fetch returns U0 + sum_m cp[m] Kp[m] at the point, fused_store adds cself K_i and writes.
+__device__ __forceinline__ double fused_fetch(const Fuse& fz, int field, size_t pt) {
+  if (!fz.Uout) return 0.0;
+  double acc = __ldg(fz.U0 + (size_t)field * fz.s0 + pt);
+  for (int m = 0; m < fz.nk; ++m) acc = fma(fz.cp[m], __ldg(fz.Kp[m] + (size_t)field * fz.skp[m] + pt), acc);
+  return acc;
+}
+__device__ __forceinline__ void fused_store(const Fuse& fz, int field, size_t pt, double fetched, double knew, double* kdst) {
+  if (fz.Uout) {
+    fz.Uout[(size_t)field * fz.so + pt] = fma(fz.cself, knew, fetched);
+    if (!fz.write_k) return;
+  }
+  *kdst = knew;
+}
+
 }  // namespace mhd
 
 struct mhd_patch {
@@ -67,9 +94,9 @@ cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfie
 cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, double* atmo, cudaStream_t s);
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
-cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, const Fuse& fz, cudaStream_t s);
 cudaError_t launch_point_flux(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* Wk, size_t sw, cudaStream_t s);
-cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, const Fuse& fz, cudaStream_t s);
 cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
                               int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s);
 cudaError_t launch_copy_fields(const Dims& d, int nfields, double* dst, size_t sd, const double* src, size_t ss, cudaStream_t s);

@@ -656,3 +656,33 @@ def test_flags_next_to_the_thresholds(oracle_mod):
         assert 0 < int(((Fo & bit) != 0).sum()) < Fo.size, bit
     assert np.all(_rel(patch.P.cpu().numpy(), Po, interior=False)[0] < 1e-12)
     patch.close()
+
+
+@pytest.mark.parametrize("rk", ["rk4", "ssprk3"])
+def test_fused_and_separate_combine_agree(oracle_mod, rk):
+    """mhd_advance with the third state buffer bound computes Eq. (53) inside the last right-hand-side kernels (k_adv_ko,
+    k_recon_march<z>) and rotates three state buffers; without it, it runs mhd_rk_stage as a separate kernel. Same arithmetic up to the
+    order of the sum: both must match the oracle (<= 1e-9 after the steps) and each other (<= 1e-11). Odd step counts leave the
+    result in a rotated buffer (the copy home is exercised); SSP-RK3 has two non-zero coefficients in its third row."""
+    from paper_2510_13965_b200 import binding
+    cfg = synth.config1(n=16, gauge_perturbation=True)
+    n = cfg["n"]
+    o = oracle_mod.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"])
+    U, P = cfg["U"].copy(), cfg["P"].copy()
+    o.prim2con(U, P)
+    a, w = synth.tableau(rk)
+    dt = 0.25 * cfg["dx"]
+    for steps in (1, 2, 3):
+        Uo = U.copy()
+        Po, Fo = o.evolve(Uo, cfg["bc"], a, w, dt, steps)
+        res = []
+        for fused in (True, False):
+            patch = binding.Patch(cfg["params"], n, cfg["ng"], cfg["dx"], stages=len(w), fused=fused)
+            patch.upload(U=U)
+            patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, steps)
+            res.append((patch.U.cpu().numpy(), patch.P.cpu().numpy(), patch.flags.cpu().numpy()[0]))
+            patch.close()
+        for Ug, Pg, Fg in res:
+            assert np.array_equal(Fg, Fo)
+            assert np.all(_rel(Ug, Uo, interior=False)[0] < 1e-9) and np.all(_rel(Pg, Po, interior=False)[0] < 1e-9)
+        assert np.all(_rel(res[0][0], res[1][0], interior=False)[0] < 1e-11)
