@@ -8,7 +8,7 @@
 // Two kernels:
 //   k_ccz4_algebra  everything that needs the radius-2 centred derivatives (Eqs. 60-62). A CTA of 256 threads owns a
 //                   16x4x4 tile, one point per thread. The 16 fields that are differentiated are staged one at a time
-//                   through a 3-deep shared-memory ring of 20x8x8 tiles (tile + halo 2) filled with cp.async, so
+//                   through a 3-deep shared-memory ring of 22x8x8 tiles (tile + halo) filled by the copy engine (TMA), so
 //                   every stencil operand is an LDS with a compile-time offset and the copy of field f+2 overlaps the
 //                   arithmetic on field f. Phase 1 turns each tile into derivatives, contracts second derivatives at
 //                   once (gamma~^mn d_m d_n gamma~_ab, gamma~^jk d_j d_k beta^c, d_j d_k beta^k) and parks the 72
@@ -21,7 +21,10 @@
 //
 // All stencils are evaluated on differences (note N1 of DESIGN.md): algebraically identical to the printed
 // coefficients, exact zeros in flat space, no cancellation noise.
+#include <cuda.h>
+#include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
 #include "mhd_internal.cuh"
 
 namespace mhd {
@@ -32,7 +35,11 @@ __device__ __forceinline__ constexpr int sym(int i, int j) { return i <= j ? (i 
 
 // ------------------------------------------------------------------------------------------------ tile geometry
 constexpr int TX = 16, TY = 4, RH = 2;                                // the tile depth TZ is a template parameter of the kernel
-constexpr int SX = TX + 2 * RH, SY = TY + 2 * RH;                     // 20 x 8 x (TZ + 4)
+// x halo of the shared tile: 3 to the left although the stencil radius is 2. A cp.async.bulk.tensor box must start on a 16-byte boundary
+// of global memory (measured on sm_100a: an odd x origin of 8-byte elements raises "illegal instruction"); with ng = 3 ghost points and
+// TX even the box that starts 3 points left of the tile does, and 22 x 8 bytes is a whole number of 16-byte units.
+constexpr int XL = 3;
+constexpr int SX = TX + XL + RH + 1, SY = TY + 2 * RH;                // 22 x 8 x (TZ + 4)
 constexpr int NBUF = 3;
 constexpr int OX = 1, OY = SX, OZ = SX * SY;                          // shared-memory strides
 
@@ -44,7 +51,7 @@ enum {
   S_DBE = 24,     //  9: d_a beta^c at S_DBE + 3 a + c
   NSCR = 33
 };
-template <int TZ> constexpr size_t smem_bytes() { return (size_t)(NBUF * SX * SY * (TZ + 2 * RH) + NSCR * TX * TY * TZ) * sizeof(double); }
+template <int TZ> constexpr size_t smem_bytes() { return (size_t)(NBUF * SX * SY * (TZ + 2 * RH) + NSCR * TX * TY * TZ) * sizeof(double) + 128; }   // + mbarriers
 
 __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -53,6 +60,31 @@ __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// ---- TMA: one cp.async.bulk.tensor per field and tile (a 22 x 8 x (TZ+4) box of the 4-D tensor (x, y, z, field); coordinates past
+// the end of the array are zero-filled by the copy engine: those points belong to ragged tiles and are masked), completion on an mbarrier
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(double* smem, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];\n"
+               ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"((uint64_t)map), "r"((unsigned)__cvta_generic_to_shared(bar)),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 
 // unscaled Eq. (60): 12 h D u
 template <int O>
@@ -85,15 +117,17 @@ __device__ __forceinline__ void second(const double* s, const Scale& sc, double 
 // order in which the differentiated fields pass through the ring
 __device__ constexpr int FORDER[16] = {GXX, GXY, GXZ, GYY, GYZ, GZZ, GAMX, GAMY, GAMZ, CHI, ALPHA, BETAX, BETAY, BETAZ, KHAT, THETA};
 
-template <int TZ>
+template <int TZ, bool TMA>
 __global__ void __launch_bounds__(TX * TY * TZ, 1)
 k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
-               const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk) {
-  constexpr int SZ = TZ + 2 * RH, TILE = SX * SY * SZ, NT = TX * TY * TZ, NLD = (TILE + NT - 1) / NT;
-  extern __shared__ __align__(16) double smem[];
+               const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk, const __grid_constant__ CUtensorMap tmap) {
+  constexpr int SZ = TZ + 2 * RH, TILE = SX * SY * SZ, NT = TX * TY * TZ, NLD = TMA ? 1 : (TILE + NT - 1) / NT;
+  static_assert((TILE * sizeof(double)) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
+  extern __shared__ __align__(128) double smem[];
   double* ring = smem;
   const int tid = threadIdx.x;
   double* scr = smem + NBUF * TILE + tid;
+  uint64_t* full = (uint64_t*)(smem + NBUF * TILE + NSCR * NT);   // NBUF mbarriers (TMA path)
 #define SCR(slot) scr[(slot) * NT]
   const int tx = tid % TX, ty = (tid / TX) % TY, tz = tid / (TX * TY);
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, k0 = blockIdx.z * TZ;
@@ -102,21 +136,37 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
   // centre point (clamped for the threads of a ragged tile: they take part in the copies and barriers only)
   const size_t pt = (size_t)(min(k, d.nz - 1) + d.ng) * d.sz + (size_t)(min(j, d.ny - 1) + d.ng) * d.sy + (min(i, d.nx - 1) + d.ng);
 
-  // global offsets of the NLD tile elements this thread copies (clamped into the ghosted array)
+  // cp.async path: global offsets of the NLD tile elements this thread copies (clamped into the ghosted array)
   int goff[NLD];
+  if (!TMA) {
 #pragma unroll
-  for (int m = 0; m < NLD; ++m) {
-    const int e = min(tid + m * NT, TILE - 1);
-    const int x = e % SX, y = (e / SX) % SY, z = e / (SX * SY);
-    const int gx = min(i0 + x - RH + d.ng, d.mx - 1), gy = min(j0 + y - RH + d.ng, d.my - 1), gz = min(k0 + z - RH + d.ng, d.mz - 1);
-    goff[m] = (int)(gz * d.sz + gy * d.sy + gx);
+    for (int m = 0; m < NLD; ++m) {
+      const int e = min(tid + m * NT, TILE - 1);
+      const int x = e % SX, y = (e / SX) % SY, z = e / (SX * SY);
+      const int gx = min(i0 + x - XL + d.ng, d.mx - 1), gy = min(j0 + y - RH + d.ng, d.my - 1), gz = min(k0 + z - RH + d.ng, d.mz - 1);
+      goff[m] = (int)(gz * d.sz + gy * d.sy + gx);
+    }
+  } else {
+    if (tid == 0) {
+#pragma unroll
+      for (int b = 0; b < NBUF; ++b) mbar_init(full + b, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
   }
   auto issue = [&](int f, int buf) {
-    const double* src = U + (size_t)f * su;
-    double* dst = ring + buf * TILE + tid;
+    if (TMA) {                                           // one thread arms the barrier and hands the box to the copy engine
+      if (tid == 0) {
+        mbar_expect_tx(full + buf, TILE * (unsigned)sizeof(double));
+        tma_load_4d(ring + buf * TILE, &tmap, full + buf, i0 - XL + d.ng, j0 - RH + d.ng, k0 - RH + d.ng, f);
+      }
+    } else {
+      const double* src = U + (size_t)f * su;
+      double* dst = ring + buf * TILE + tid;
 #pragma unroll
-    for (int m = 0; m < NLD; ++m) if (TILE % NT == 0 || tid + m * NT < TILE) cp_async8(dst + m * NT, src + goff[m]);
-    cp_commit();
+      for (int m = 0; m < NLD; ++m) if (TILE % NT == 0 || tid + m * NT < TILE) cp_async8(dst + m * NT, src + goff[m]);
+      cp_commit();
+    }
   };
   issue(FORDER[0], 0);
   issue(FORDER[1], 1);
@@ -148,7 +198,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 #define GI(i, j) gi[sym(i, j)]
 
   // ================================================================= phase 1: derivatives, field by field
-  const int ctr = ((tz + RH) * SY + (ty + RH)) * SX + (tx + RH);
+  const int ctr = ((tz + RH) * SY + (ty + RH)) * SX + (tx + XL);
   const double chi = F(CHI), al = F(ALPHA);
   double be[3] = {0, 0, 0}, Gh[3] = {0, 0, 0}, Kh = 0.0, Th = 0.0;
   double Racc[6] = {0, 0, 0, 0, 0, 0};   // part of chi (R^_ab + R^chi_ab) that is linear in second derivatives and in d Gamma^
@@ -156,9 +206,15 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
   double dchi[3] = {0, 0, 0}, dal[3] = {0, 0, 0};
 #pragma unroll
   for (int n = 0; n < 16; ++n) {
-    if (n + 1 < 16) cp_wait<1>(); else cp_wait<0>();
-    __syncthreads();
-    if (n + 2 < 16) issue(FORDER[n + 2], (n + 2) % NBUF);
+    if (TMA) {
+      __syncthreads();                                   // everybody is done reading the buffer the next copy overwrites
+      if (n + 2 < 16) issue(FORDER[n + 2], (n + 2) % NBUF);
+      mbar_wait(full + n % NBUF, (n / NBUF) & 1);        // field n has landed (the barrier of a buffer completes once per use)
+    } else {
+      if (n + 1 < 16) cp_wait<1>(); else cp_wait<0>();
+      __syncthreads();
+      if (n + 2 < 16) issue(FORDER[n + 2], (n + 2) % NBUF);
+    }
     const double* s = ring + (n % NBUF) * TILE + ctr;
     double d1[3];
     first(s, sc, d1);
@@ -558,21 +614,64 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
 }
 }  // namespace
 
+// Tensor map of a state slot as a 4-D tensor (x, y, z, field) of doubles with a 22 x 8 x (TZ+4) x 1 box. Legal when the row pitch and the
+// field stride are multiples of 16 bytes (MX even, stride even), the base is 16-byte aligned and the box origin i0 - XL + ng is even
+// (ng odd); otherwise the cp.async path is used.
+static bool make_tensor_map(const Dims& d, const double* U, size_t su, int tz, CUtensorMap* out) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                               const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) encode = (EncodeFn)fn;
+    const char* v = getenv("MHD_CCZ4_TMA");
+    if (v && atoi(v) == 0) encode = nullptr;
+  }
+  if (!encode || (d.mx & 1) || (su & 1) || ((uintptr_t)U & 15) || ((d.ng - XL) & 1)) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)d.mx, (cuuint64_t)d.my, (cuuint64_t)d.mz, (cuuint64_t)MHD_NSTATE};
+  const cuuint64_t strides[3] = {(cuuint64_t)d.mx * 8, (cuuint64_t)d.sz * 8, (cuuint64_t)su * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)SX, (cuuint32_t)SY, (cuuint32_t)(tz + 2 * RH), 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int TZ>
+static cudaError_t launch_algebra_tz(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
+  // the opt-in to > 48 KB of dynamic shared memory is per device and per instantiation
+  static int attr_set[64][2] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  CUtensorMap map;
+  const bool tma = make_tensor_map(d, U, su, TZ, &map);
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  if (!attr_set[dev][tma]) {
+    e = tma ? cudaFuncSetAttribute(k_ccz4_algebra<TZ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<TZ>())
+            : cudaFuncSetAttribute(k_ccz4_algebra<TZ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<TZ>());
+    if (e != cudaSuccess) return e;
+    attr_set[dev][tma] = 1;                              // only after the attribute call succeeded
+  }
+  const dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
+  if (tma) k_ccz4_algebra<TZ, true><<<grid, TX * TY * TZ, smem_bytes<TZ>(), s>>>(d, par, U, su, P, sp, K, sk, map);
+  else {
+    memset(&map, 0, sizeof(map));
+    k_ccz4_algebra<TZ, false><<<grid, TX * TY * TZ, smem_bytes<TZ>(), s>>>(d, par, U, su, P, sp, K, sk, map);
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess && getenv("MHD_DEBUG")) fprintf(stderr, "libmhd_b200: k_ccz4_algebra<%d, %d> launch: %s\n", TZ, (int)tma, cudaGetErrorString(e));
+  return e;
+}
+
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
   static int tz = 0;
-  if (tz == 0) {
-    const char* v = getenv("MHD_CCZ4_TZ");
-    tz = v ? atoi(v) : 4;
-    cudaError_t e = cudaFuncSetAttribute(k_ccz4_algebra<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<4>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ccz4_algebra<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<5>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ccz4_algebra<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<6>());
-    if (e != cudaSuccess) return e;
-  }
-  auto grid = [&](int TZ) { return dim3((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ); };
-  if (tz == 6) k_ccz4_algebra<6><<<grid(6), TX * TY * 6, smem_bytes<6>(), s>>>(d, par, U, su, P, sp, K, sk);
-  else if (tz == 5) k_ccz4_algebra<5><<<grid(5), TX * TY * 5, smem_bytes<5>(), s>>>(d, par, U, su, P, sp, K, sk);
-  else k_ccz4_algebra<4><<<grid(4), TX * TY * 4, smem_bytes<4>(), s>>>(d, par, U, su, P, sp, K, sk);
-  return cudaGetLastError();
+  if (tz == 0) { const char* v = getenv("MHD_CCZ4_TZ"); tz = v ? atoi(v) : 4; }
+  if (tz == 6) return launch_algebra_tz<6>(d, par, U, su, P, sp, K, sk, s);
+  if (tz == 5) return launch_algebra_tz<5>(d, par, U, su, P, sp, K, sk, s);
+  return launch_algebra_tz<4>(d, par, U, su, P, sp, K, sk, s);
 }
 
 cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
