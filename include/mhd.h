@@ -114,6 +114,12 @@ typedef struct {
   double m1_arad;                  /* see above; 0 switches the emission off */
   double m1_oe_guard;              /* reading R33: the switch also needs all three differences to exceed m1_oe_guard x the local
                                       magnitude; 0 = the rule exactly as printed (two strict "< 0" tests) */
+  /* SURVEY 8(f) rows */
+  int recon_kind;                  /* the reconstruction R of Eq. (66): 0 MP5 (Eqs. 70-76, the paper's default), 1 WENO5 (PAPER.md:486-488,
+                                      ref. [63]: linear weights 1/10, 6/10, 3/10, exponent 2) */
+  double weno_eps;                 /* recon_kind 1: the epsilon added to the smoothness indicators (ref. [63]: 1e-6); must be > 0 */
+  double les_C_M;                  /* App. A, Eq. (A11): coefficient C_M of the sub-grid-scale tensor of the induction equation (the paper's
+                                      production value is 8); 0 = LES terms off */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */

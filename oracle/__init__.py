@@ -130,6 +130,8 @@ def _load(counting):
         L.orc_dko.restype = f64
         L.orc_mp5.argtypes = [f64] * 6
         L.orc_mp5.restype = f64
+        L.orc_weno5.argtypes = [f64] * 6
+        L.orc_weno5.restype = f64
         L.orc_eos.argtypes = [vp, f64, f64, f64, vp]
         L.orc_eos_eps_from_T.argtypes = [vp, f64, f64, f64]
         L.orc_eos_eps_from_T.restype = f64

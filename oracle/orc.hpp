@@ -85,6 +85,10 @@ struct Params {
   int m1_maxit, m1_odd_even;   // m1_odd_even: apply the A := 1 switch of l.565-570
   double m1_arad;              // eta = m1_arad kappa_a T^4 (radiation constant in the units of T; BASELINE: 1)
   double m1_oe_guard;          // R33: relative size the three differences must exceed for the switch; 0 = the printed rule
+  // SURVEY 8(f) rows
+  int recon_kind;              // R of Eq. (66): 0 MP5 (default), 1 WENO5 (l.486-488)
+  double weno_eps;             // the epsilon of [63] Eq. (2.16) (their 1e-6); R37
+  double les_C_M;              // App. A: coefficient of the SGS tensor of the induction equation (paper: 8); 0 = off
 };
 
 // ---- stencils (Sec. III B)
@@ -94,6 +98,8 @@ double d11(const double* u, long s1, double h1, long s2, double h2);  // Eq. (61
 double dadv(const double* u, long s, double h, double beta);  // l.454-456
 double dko(const double* u, long s, double h, double sigma);  // l.460
 double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alpha);  // Eqs. (70)-(76)
+double weno5(double fm2, double fm1, double f0, double fp1, double fp2, double eps);   // l.486-488, refs. [61], [63]
+double reconstruct(const Params& par, double fm2, double fm1, double f0, double fp1, double fp2);   // R of Eq. (66)
 
 // ---- EoS
 struct EosOut { double p, T, cs2; };

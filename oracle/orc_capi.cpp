@@ -17,6 +17,7 @@ bool set_scalar(Params& p, const std::string& k, double v) {
   D(rho_atmo) D(rho_cut) D(rho_low) D(alpha_bh) D(w_max) D(rho_max) D(eps_min) D(eps_max)
   D(ye_min) D(ye_max) D(ye_atmo) D(eps_atmo) D(T_atmo) I(c2p_maxit)
   D(m1_kappa0) D(m1_rho0) D(m1_efloor) D(m1_tol) D(m1_mb) I(m1_maxit) I(m1_odd_even) D(m1_arad) D(m1_oe_guard)
+  I(recon_kind) D(weno_eps) D(les_C_M)
   I(n_rho) I(n_T) I(n_ye) D(lr0) D(dlr) D(lT0) D(dlT) D(ye0) D(dye) D(tab_eps_shift) D(tab_h0)
 #undef D
 #undef I
@@ -130,6 +131,7 @@ double orc_d11(const double* u, long s1, double h1, long s2, double h2) { return
 double orc_dadv(const double* u, long s, double h, double beta) { return dadv(u, s, h, beta); }
 double orc_dko(const double* u, long s, double h, double sigma) { return dko(u, s, h, sigma); }
 double orc_mp5(double a, double b, double c, double d, double e, double alpha) { return mp5(a, b, c, d, e, alpha); }
+double orc_weno5(double a, double b, double c, double d, double e, double eps) { return weno5(a, b, c, d, e, eps); }
 void orc_eos(void* hh, double rho, double eps, double ye, double* out3) {
   const EosOut e = eos_from_rho_eps(((Handle*)hh)->par, rho, eps, ye);
   out3[0] = e.p; out3[1] = e.T; out3[2] = e.cs2;

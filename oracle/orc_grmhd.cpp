@@ -138,8 +138,8 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
             fpl[m] = 0.5 * (Fp[f * Md + j] + lam * Uc[f * Md + j]);
             fmi[m] = 0.5 * (Fp[f * Md + j] - lam * Uc[f * Md + j]);
           }
-          const double FL = mp5(fpl[0], fpl[1], fpl[2], fpl[3], fpl[4], par.mp5_alpha);   // Eq. (67)
-          const double FR = mp5(fmi[5], fmi[4], fmi[3], fmi[2], fmi[1], par.mp5_alpha);   // Eq. (68)
+          const double FL = reconstruct(par, fpl[0], fpl[1], fpl[2], fpl[3], fpl[4]);   // Eq. (67)
+          const double FR = reconstruct(par, fmi[5], fmi[4], fmi[3], fmi[2], fmi[1]);   // Eq. (68)
           Fhat[f * (Md + 1) + i] = FL + FR;                                               // Eq. (69)
         }
       }

@@ -75,4 +75,26 @@ double mp5(double fm2, double fm1, double f0, double fp1, double fp2, double alp
   return median3(fmin, fhi, fmax);
 }
 
+// WENO5 (the second reconstruction the paper names, refs. [61] Shu 1998, [63] Jiang & Shu 1996; the formulas are
+// not printed in the paper, this is the textbook scheme of [63] Sec. 3 written out): three third-order candidate values of the
+// interface i+1/2, the smoothness indicators IS_k of [63] Eq. (3.1)-(3.3), linear weights (1/10, 6/10, 3/10), exponent 2.
+double weno5(double fm2, double fm1, double f0, double fp1, double fp2, double eps) {
+  const double q0 = (2.0 * fm2 - 7.0 * fm1 + 11.0 * f0) / 6.0;
+  const double q1 = (-fm1 + 5.0 * f0 + 2.0 * fp1) / 6.0;
+  const double q2 = (2.0 * f0 + 5.0 * fp1 - fp2) / 6.0;
+  const double b0 = 13.0 / 12.0 * (fm2 - 2.0 * fm1 + f0) * (fm2 - 2.0 * fm1 + f0) + 0.25 * (fm2 - 4.0 * fm1 + 3.0 * f0) * (fm2 - 4.0 * fm1 + 3.0 * f0);
+  const double b1 = 13.0 / 12.0 * (fm1 - 2.0 * f0 + fp1) * (fm1 - 2.0 * f0 + fp1) + 0.25 * (fm1 - fp1) * (fm1 - fp1);
+  const double b2 = 13.0 / 12.0 * (f0 - 2.0 * fp1 + fp2) * (f0 - 2.0 * fp1 + fp2) + 0.25 * (3.0 * f0 - 4.0 * fp1 + fp2) * (3.0 * f0 - 4.0 * fp1 + fp2);
+  const double a0 = 0.1 / ((eps + b0) * (eps + b0));
+  const double a1 = 0.6 / ((eps + b1) * (eps + b1));
+  const double a2 = 0.3 / ((eps + b2) * (eps + b2));
+  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+}
+
+// the reconstruction R of Eq. (66) selected by recon_kind: 0 = MP5 (default, Eqs. 70-76), 1 = WENO5
+double reconstruct(const Params& par, double fm2, double fm1, double f0, double fp1, double fp2) {
+  if (par.recon_kind == 1) return weno5(fm2, fm1, f0, fp1, fp2, par.weno_eps);
+  return mp5(fm2, fm1, f0, fp1, fp2, par.mp5_alpha);
+}
+
 }  // namespace orc

@@ -42,6 +42,7 @@ class mhd_patch_desc(ctypes.Structure):
         ("m1_kappa0", _d), ("m1_rho0", _d), ("m1_species_scale", _d * 3), ("m1_efloor", _d), ("m1_tol", _d), ("m1_mb", _d),
         ("m1_maxit", _i), ("m1_odd_even", _i),
         ("m1_arad", _d), ("m1_oe_guard", _d),
+        ("recon_kind", _i), ("weno_eps", _d), ("les_C_M", _d),
     ]
 
 
@@ -125,7 +126,7 @@ def make_desc(params, nx, ny, nz, ng, dx, dy=None, dz=None, table_ptrs=None, tab
             arr = getattr(d, k)
             for i, x in enumerate(v):
                 arr[i] = float(x)
-        elif k in ("eos_kind", "n_pieces", "c2p_maxit", "m1_maxit", "m1_odd_even"):
+        elif k in ("eos_kind", "n_pieces", "c2p_maxit", "m1_maxit", "m1_odd_even", "recon_kind"):
             setattr(d, k, int(v))
         else:
             setattr(d, k, float(v))

@@ -154,6 +154,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
   if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
+  if (desc->recon_kind < 0 || desc->recon_kind > 1 || (desc->recon_kind == 1 && !(desc->weno_eps > 0.0))) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
   if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2 ||
                               !(desc->dlr > 0.0 && desc->dlT > 0.0 && desc->dye > 0.0))) return MHD_E_ARG;
@@ -191,6 +192,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.m1_tol = desc->m1_tol > 0.0 ? desc->m1_tol : 1e-13; q.m1_mb = desc->m1_mb; q.m1_maxit = desc->m1_maxit > 0 ? desc->m1_maxit : 30;
   for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
   q.m1_odd_even = desc->m1_odd_even; q.m1_arad = desc->m1_arad; q.m1_oe_guard = desc->m1_oe_guard;
+  q.recon_kind = desc->recon_kind; q.weno_eps = desc->weno_eps; q.les_C_M = desc->les_C_M;
   p->d_counts = nullptr;
   if (cudaMalloc(&p->d_counts, 16 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   *out = p;

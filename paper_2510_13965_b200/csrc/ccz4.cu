@@ -34,14 +34,14 @@ namespace {
 __device__ __forceinline__ constexpr int sym(int i, int j) { return i <= j ? (i * (5 - i)) / 2 + j : (j * (5 - j)) / 2 + i; }   // (0,0)=0 (0,1)=1 (0,2)=2 (1,1)=3 (1,2)=4 (2,2)=5
 
 // ------------------------------------------------------------------------------------------------ tile geometry
-constexpr int TX = 16, TY = 4, RH = 2;                                // the tile depth TZ is a template parameter of the kernel
+constexpr int TX = 16, RH = 2;                                        // the tile extents TY, TZ are template parameters of the kernel
 // x halo of the shared tile: 3 to the left although the stencil radius is 2. A cp.async.bulk.tensor box must start on a 16-byte boundary
 // of global memory (measured on sm_100a: an odd x origin of 8-byte elements raises "illegal instruction"); with ng = 3 ghost points and
 // TX even the box that starts 3 points left of the tile does, and 22 x 8 bytes is a whole number of 16-byte units.
 constexpr int XL = 3;
-constexpr int SX = TX + XL + RH + 1, SY = TY + 2 * RH;                // 22 x 8 x (TZ + 4)
+constexpr int SX = TX + XL + RH + 1;                                  // shared tile: 22 x (TY + 4) x (TZ + 4)
 constexpr int NBUF = 3;
-constexpr int OX = 1, OY = SX, OZ = SX * SY;                          // shared-memory strides
+constexpr int OX = 1, OY = SX;                                        // shared-memory strides (z: SX * (TY + 4))
 
 // scratch slots (per thread): only what the pointwise algebra needs more than once. Second derivatives, d Gamma^, d K^ and
 // d Theta enter the right-hand side linearly and are folded into register accumulators the moment they are computed.
@@ -51,7 +51,7 @@ enum {
   S_DBE = 24,     //  9: d_a beta^c at S_DBE + 3 a + c
   NSCR = 33
 };
-template <int TZ> constexpr size_t smem_bytes() { return (size_t)(NBUF * SX * SY * (TZ + 2 * RH) + NSCR * TX * TY * TZ) * sizeof(double) + 128; }   // + mbarriers
+template <int TY, int TZ> constexpr size_t smem_bytes() { return (size_t)(NBUF * ((SX * (TY + 2 * RH) * (TZ + 2 * RH) + 15) & ~15) + NSCR * TX * TY * TZ) * sizeof(double) + 128; }   // + mbarriers
 
 __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -102,10 +102,12 @@ __device__ __forceinline__ double d11u(const double* s) {
 
 struct Scale { double i12h[3], i12h2[3], i144[3]; };   // i144: xy, xz, yz
 
+template <int OZ>
 __device__ __forceinline__ void first(const double* s, const Scale& sc, double o[3]) {
   o[0] = d1u<OX>(s) * sc.i12h[0]; o[1] = d1u<OY>(s) * sc.i12h[1]; o[2] = d1u<OZ>(s) * sc.i12h[2];
 }
 // second derivatives in sym order xx, xy, xz, yy, yz, zz
+template <int OZ>
 __device__ __forceinline__ void second(const double* s, const Scale& sc, double o[6]) {
   const double u0 = s[0];
   o[0] = d2u<OX>(s, u0) * sc.i12h2[0]; o[3] = d2u<OY>(s, u0) * sc.i12h2[1]; o[5] = d2u<OZ>(s, u0) * sc.i12h2[2];
@@ -117,17 +119,18 @@ __device__ __forceinline__ void second(const double* s, const Scale& sc, double 
 // order in which the differentiated fields pass through the ring
 __device__ constexpr int FORDER[16] = {GXX, GXY, GXZ, GYY, GYZ, GZZ, GAMX, GAMY, GAMZ, CHI, ALPHA, BETAX, BETAY, BETAZ, KHAT, THETA};
 
-template <int TZ, bool TMA>
-__global__ void __launch_bounds__(TX * TY * TZ, 1)
+template <int TY, int TZ, bool TMA>
+__global__ void __launch_bounds__(TX * TY * TZ, (TX * TY * TZ <= 64 ? 4 : TX * TY * TZ <= 128 ? 2 : 1))
 k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                const double* __restrict__ P, size_t sp, double* __restrict__ K, size_t sk, const __grid_constant__ CUtensorMap tmap) {
+  constexpr int SY = TY + 2 * RH, OZ = SX * SY;
   constexpr int SZ = TZ + 2 * RH, TILE = SX * SY * SZ, NT = TX * TY * TZ, NLD = TMA ? 1 : (TILE + NT - 1) / NT;
-  static_assert((TILE * sizeof(double)) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
+  constexpr int TILEP = (TILE + 15) & ~15;             // buffer stride: TMA destination tiles must stay 128-byte aligned
   extern __shared__ __align__(128) double smem[];
   double* ring = smem;
   const int tid = threadIdx.x;
-  double* scr = smem + NBUF * TILE + tid;
-  uint64_t* full = (uint64_t*)(smem + NBUF * TILE + NSCR * NT);   // NBUF mbarriers (TMA path)
+  double* scr = smem + NBUF * TILEP + tid;
+  uint64_t* full = (uint64_t*)(smem + NBUF * TILEP + NSCR * NT);   // NBUF mbarriers (TMA path)
 #define SCR(slot) scr[(slot) * NT]
   const int tx = tid % TX, ty = (tid / TX) % TY, tz = tid / (TX * TY);
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY, k0 = blockIdx.z * TZ;
@@ -158,11 +161,11 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
     if (TMA) {                                           // one thread arms the barrier and hands the box to the copy engine
       if (tid == 0) {
         mbar_expect_tx(full + buf, TILE * (unsigned)sizeof(double));
-        tma_load_4d(ring + buf * TILE, &tmap, full + buf, i0 - XL + d.ng, j0 - RH + d.ng, k0 - RH + d.ng, f);
+        tma_load_4d(ring + buf * TILEP, &tmap, full + buf, i0 - XL + d.ng, j0 - RH + d.ng, k0 - RH + d.ng, f);
       }
     } else {
       const double* src = U + (size_t)f * su;
-      double* dst = ring + buf * TILE + tid;
+      double* dst = ring + buf * TILEP + tid;
 #pragma unroll
       for (int m = 0; m < NLD; ++m) if (TILE % NT == 0 || tid + m * NT < TILE) cp_async8(dst + m * NT, src + goff[m]);
       cp_commit();
@@ -215,12 +218,12 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
       __syncthreads();
       if (n + 2 < 16) issue(FORDER[n + 2], (n + 2) % NBUF);
     }
-    const double* s = ring + (n % NBUF) * TILE + ctr;
+    const double* s = ring + (n % NBUF) * TILEP + ctr;
     double d1[3];
-    first(s, sc, d1);
+    first<OZ>(s, sc, d1);
     if (n < 6) {                       // gamma~_ab, ab = n: -1/2 gamma~^mn d_m d_n gamma~_ab of Eq. (23)
       double dd[6];
-      second(s, sc, dd);
+      second<OZ>(s, sc, dd);
 #pragma unroll
       for (int c = 0; c < 3; ++c) SCR(S_DG + 6 * c + n) = d1[c];
       Racc[n] -= chi * (0.5 * (gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5]) + (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]));
@@ -233,7 +236,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
         for (int b = a; b < 3; ++b) Racc[sym(a, b)] += 0.5 * chi * (G_(c, a) * d1[b] + G_(c, b) * d1[a]);
     } else if (n == 9) {               // chi: 1/2 d_i d_j chi + 1/2 gamma~_ij gamma~^mn d_m d_n chi of Eq. (22)
       double dd[6];
-      second(s, sc, dd);
+      second<OZ>(s, sc, dd);
       const double lap = gi[0] * dd[0] + gi[3] * dd[3] + gi[5] * dd[5] + 2.0 * (gi[1] * dd[1] + gi[2] * dd[2] + gi[4] * dd[4]);
 #pragma unroll
       for (int a = 0; a < 3; ++a) dchi[a] = d1[a];
@@ -241,7 +244,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
       for (int a = 0; a < 6; ++a) Racc[a] += 0.5 * dd[a] + 0.5 * g[a] * lap;
     } else if (n == 10) {              // alpha
       double dd[6];
-      second(s, sc, dd);
+      second<OZ>(s, sc, dd);
 #pragma unroll
       for (int a = 0; a < 3; ++a) dal[a] = d1[a];
 #pragma unroll
@@ -249,7 +252,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
     } else if (n < 14) {               // beta^c, c = n - 11
       const int c = n - 11;
       double dd[6];
-      second(s, sc, dd);
+      second<OZ>(s, sc, dd);
       be[c] = s[0];
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
@@ -617,7 +620,7 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
 // Tensor map of a state slot as a 4-D tensor (x, y, z, field) of doubles with a 22 x 8 x (TZ+4) x 1 box. Legal when the row pitch and the
 // field stride are multiples of 16 bytes (MX even, stride even), the base is 16-byte aligned and the box origin i0 - XL + ng is even
 // (ng odd); otherwise the cp.async path is used.
-static bool make_tensor_map(const Dims& d, const double* U, size_t su, int tz, CUtensorMap* out) {
+static bool make_tensor_map(const Dims& d, const double* U, size_t su, int ty, int tz, CUtensorMap* out) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
   static EncodeFn encode = nullptr;
@@ -633,13 +636,13 @@ static bool make_tensor_map(const Dims& d, const double* U, size_t su, int tz, C
   if (!encode || (d.mx & 1) || (su & 1) || ((uintptr_t)U & 15) || ((d.ng - XL) & 1)) return false;
   const cuuint64_t dims[4] = {(cuuint64_t)d.mx, (cuuint64_t)d.my, (cuuint64_t)d.mz, (cuuint64_t)MHD_NSTATE};
   const cuuint64_t strides[3] = {(cuuint64_t)d.mx * 8, (cuuint64_t)d.sz * 8, (cuuint64_t)su * 8};
-  const cuuint32_t box[4] = {(cuuint32_t)SX, (cuuint32_t)SY, (cuuint32_t)(tz + 2 * RH), 1};
+  const cuuint32_t box[4] = {(cuuint32_t)SX, (cuuint32_t)(ty + 2 * RH), (cuuint32_t)(tz + 2 * RH), 1};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TZ>
+template <int TY, int TZ>
 static cudaError_t launch_algebra_tz(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
   // the opt-in to > 48 KB of dynamic shared memory is per device and per instantiation
   static int attr_set[64][2] = {};
@@ -647,31 +650,37 @@ static cudaError_t launch_algebra_tz(const Dims& d, const Par& par, const double
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   CUtensorMap map;
-  const bool tma = make_tensor_map(d, U, su, TZ, &map);
+  const bool tma = make_tensor_map(d, U, su, TY, TZ, &map);
   if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  constexpr int SMEM = (int)smem_bytes<TY, TZ>();
   if (!attr_set[dev][tma]) {
-    e = tma ? cudaFuncSetAttribute(k_ccz4_algebra<TZ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<TZ>())
-            : cudaFuncSetAttribute(k_ccz4_algebra<TZ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<TZ>());
+    e = tma ? cudaFuncSetAttribute(k_ccz4_algebra<TY, TZ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM)
+            : cudaFuncSetAttribute(k_ccz4_algebra<TY, TZ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
     if (e != cudaSuccess) return e;
     attr_set[dev][tma] = 1;                              // only after the attribute call succeeded
   }
   const dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, (d.nz + TZ - 1) / TZ);
-  if (tma) k_ccz4_algebra<TZ, true><<<grid, TX * TY * TZ, smem_bytes<TZ>(), s>>>(d, par, U, su, P, sp, K, sk, map);
+  if (tma) k_ccz4_algebra<TY, TZ, true><<<grid, TX * TY * TZ, SMEM, s>>>(d, par, U, su, P, sp, K, sk, map);
   else {
     memset(&map, 0, sizeof(map));
-    k_ccz4_algebra<TZ, false><<<grid, TX * TY * TZ, smem_bytes<TZ>(), s>>>(d, par, U, su, P, sp, K, sk, map);
+    k_ccz4_algebra<TY, TZ, false><<<grid, TX * TY * TZ, SMEM, s>>>(d, par, U, su, P, sp, K, sk, map);
   }
   e = cudaGetLastError();
-  if (e != cudaSuccess && getenv("MHD_DEBUG")) fprintf(stderr, "libmhd_b200: k_ccz4_algebra<%d, %d> launch: %s\n", TZ, (int)tma, cudaGetErrorString(e));
+  if (e != cudaSuccess && getenv("MHD_DEBUG")) fprintf(stderr, "libmhd_b200: k_ccz4_algebra<%d, %d, %d> launch: %s\n", TY, TZ, (int)tma, cudaGetErrorString(e));
   return e;
 }
 
+// Tile shapes (x extent 16): MHD_CCZ4_TILE = "TYxTZ". 4x2 = 128 threads, two CTAs per SM (default: the derivative phase of one CTA, bound by
+// shared-memory loads, overlaps the pointwise algebra of the other, bound by the FP64 pipe); 4x4 = 256 threads, one CTA per SM (round 1);
+// 2x2 and 4x1 = 64 threads, four CTAs per SM.
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s) {
-  static int tz = 0;
-  if (tz == 0) { const char* v = getenv("MHD_CCZ4_TZ"); tz = v ? atoi(v) : 4; }
-  if (tz == 6) return launch_algebra_tz<6>(d, par, U, su, P, sp, K, sk, s);
-  if (tz == 5) return launch_algebra_tz<5>(d, par, U, su, P, sp, K, sk, s);
-  return launch_algebra_tz<4>(d, par, U, su, P, sp, K, sk, s);
+  static int tile = 0;
+  if (tile == 0) { const char* v = getenv("MHD_CCZ4_TILE"); tile = v && strlen(v) == 3 ? (v[0] - '0') * 10 + (v[2] - '0') : 42; }
+  if (tile == 44) return launch_algebra_tz<4, 4>(d, par, U, su, P, sp, K, sk, s);
+  if (tile == 22) return launch_algebra_tz<2, 2>(d, par, U, su, P, sp, K, sk, s);
+  if (tile == 41) return launch_algebra_tz<4, 1>(d, par, U, su, P, sp, K, sk, s);
+  if (tile == 24) return launch_algebra_tz<2, 4>(d, par, U, su, P, sp, K, sk, s);
+  return launch_algebra_tz<4, 2>(d, par, U, su, P, sp, K, sk, s);
 }
 
 cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {

@@ -118,11 +118,36 @@ __device__ __forceinline__ void q_drain(LimQueue& q, int lane, double alpha) {
   if (q.count > 0) { q_process(q.v, q.tag, q.corr, 0, q.count, lane, alpha); q.count = 0; }
 }
 
+// WENO5, the second reconstruction named at PAPER.md:486-488 (Jiang & Shu, ref. [63]): candidate values, smoothness indicators,
+// linear weights (1/10, 6/10, 3/10), exponent 2, epsilon = weno_eps. One division per reconstruction; no branches, so no queue.
+__device__ __forceinline__ double weno5(double fm2, double fm1, double f0, double fp1, double fp2, double eps) {
+  const double q0 = (2.0 * fm2 - 7.0 * fm1 + 11.0 * f0) * (1.0 / 6.0);
+  const double q1 = (-fm1 + 5.0 * f0 + 2.0 * fp1) * (1.0 / 6.0);
+  const double q2 = (2.0 * f0 + 5.0 * fp1 - fp2) * (1.0 / 6.0);
+  const double c0 = fm2 - 2.0 * fm1 + f0, e0 = fm2 - 4.0 * fm1 + 3.0 * f0;
+  const double c1 = fm1 - 2.0 * f0 + fp1, e1 = fm1 - fp1;
+  const double c2 = f0 - 2.0 * fp1 + fp2, e2 = 3.0 * f0 - 4.0 * fp1 + fp2;
+  const double b0 = eps + ((13.0 / 12.0) * c0 * c0 + 0.25 * e0 * e0);
+  const double b1 = eps + ((13.0 / 12.0) * c1 * c1 + 0.25 * e1 * e1);
+  const double b2 = eps + ((13.0 / 12.0) * c2 * c2 + 0.25 * e2 * e2);
+  // a_k = d_k / b_k^2 over the common denominator (b0 b1 b2)^2: w_k = d_k (b_l b_m)^2 / sum
+  const double n0 = 0.1 * (b1 * b2) * (b1 * b2), n1 = 0.6 * (b0 * b2) * (b0 * b2), n2 = 0.3 * (b0 * b1) * (b0 * b1);
+  return (n0 * q0 + n1 * q1 + n2 * q2) / (n0 + n1 + n2);
+}
+
 // Eqs. (65), (67)-(69) for one interface and one field from the six stencil nodes i-2..i+3 (index 0..5): returns
 // f^hi_L + f^hi_R (twice the unlimited F^) and queues the reconstructions that need the limiter (slots 2s, 2s+1).
+// WENO: `alpha` carries weno_eps; the weights are not homogeneous in F, so the 1/2 of Eq. (65) is applied before the reconstruction
+// and the sum is doubled again (exact) to keep the caller's 1/(2h).
+template <bool WENO>
 __device__ __forceinline__ double flux_hat2(LimQueue& q, const double f[6], const double u[6], double lam, double alpha, bool active,
                                             int s, int lane, unsigned& mask) {
   double p[5], m[5];
+  if (WENO) {
+#pragma unroll
+    for (int n = 0; n < 5; ++n) { p[n] = 0.5 * fma(lam, u[n], f[n]); m[n] = 0.5 * fma(-lam, u[n + 1], f[n + 1]); }
+    return 2.0 * (weno5(p[0], p[1], p[2], p[3], p[4], alpha) + weno5(m[4], m[3], m[2], m[1], m[0], alpha));
+  }
 #pragma unroll
   for (int n = 0; n < 5; ++n) { p[n] = fma(lam, u[n], f[n]); m[n] = fma(-lam, u[n + 1], f[n + 1]); }
   bool nl, nr;
@@ -219,7 +244,7 @@ namespace {
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int RW = 4;    // warps per CTA of the reconstruction kernels
 
-template <int DIR, int SEG, bool FUSED>
+template <int DIR, int SEG, bool FUSED, bool WENO>
 __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
                                                             const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk,
                                                             const __grid_constant__ Fuse fz) {
@@ -273,10 +298,10 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     for (int m = 1; m <= SEG; ++m) pre[m - 1] = (FUSED && active && c0 + m - 1 < nline) ? fused_fetch(fz, DBAR + a, (size_t)(base + (long long)(g0 + m + 2) * ls)) : 0.0;
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
-      acc[m] = flux_hat2(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
-      q_flush(q, lane, alpha);
+      acc[m] = flux_hat2<WENO>(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
+      if (!WENO) q_flush(q, lane, alpha);
     }
-    q_drain(q, lane, alpha);
+    if (!WENO) q_drain(q, lane, alpha);
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
       if (mask & (1u << (2 * m))) acc[m] += q.corr[(2 * m) * 32 + lane];
@@ -295,6 +320,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
 // ---------------------------------------------------------------------------------------------------------------
 // x: one thread per interface; a warp covers 32 interfaces = 31 zones (lane 31 only supplies F^ to lane 30).
 // ---------------------------------------------------------------------------------------------------------------
+template <bool WENO>
 __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
                                                         const double* __restrict__ Wk, size_t sw, double* __restrict__ K, size_t sk) {
   __shared__ double q_v[RW][5 * QCAP];
@@ -334,14 +360,14 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
 #pragma unroll
       for (int n = 0; n < 6; ++n) { fn[n] = __ldg(f + node(n)); un[n] = __ldg(u + node(n)); }
     }
-    acc[a] = flux_hat2(q, fw, uw, lam, alpha, active, a, lane, mask);   // twice F^ at zone - 1/2
-    q_flush(q, lane, alpha);
+    acc[a] = flux_hat2<WENO>(q, fw, uw, lam, alpha, active, a, lane, mask);   // twice F^ at zone - 1/2
+    if (!WENO) q_flush(q, lane, alpha);
     if (a < 9) {
 #pragma unroll
       for (int n = 0; n < 6; ++n) { fw[n] = fn[n]; uw[n] = un[n]; }
     }
   }
-  q_drain(q, lane, alpha);
+  if (!WENO) q_drain(q, lane, alpha);
 #pragma unroll
   for (int a = 0; a < 10; ++a) {
     double fl = acc[a];
@@ -354,28 +380,32 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
 
 }  // namespace
 
-template <int SEG>
+template <int SEG, bool WENO>
 static void launch_march(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
+  const double a = WENO ? par.weno_eps : par.mp5_alpha;
   if (dir == 1) {
     dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.nz, (d.ny + SEG - 1) / SEG);
-    k_recon_march<1, SEG, false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
+    k_recon_march<1, SEG, false, WENO><<<grid, 32 * RW, 0, s>>>(d, a, U, su, Wk, sw, K, sk, fz);
   } else {                                                                    // z is the last pass over the fluid K: the RK combine rides on it
     dim3 grid((d.nx + 32 * RW - 1) / (32 * RW), d.ny, (d.nz + SEG - 1) / SEG);
-    if (fz.Uout) k_recon_march<2, SEG, true><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
-    else k_recon_march<2, SEG, false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk, fz);
+    if (fz.Uout) k_recon_march<2, SEG, true, WENO><<<grid, 32 * RW, 0, s>>>(d, a, U, su, Wk, sw, K, sk, fz);
+    else k_recon_march<2, SEG, false, WENO><<<grid, 32 * RW, 0, s>>>(d, a, U, su, Wk, sw, K, sk, fz);
   }
 }
 
 cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U, size_t su, const double* Wk, size_t sw, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
   static int seg = 0;
   if (seg == 0) { const char* v = getenv("MHD_RECON_SEG"); seg = v ? atoi(v) : 6; }
+  const bool weno = par.recon_kind == 1;
   if (dir == 0) {
     dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
-    k_recon_x<<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
-  } else if (seg == 4) launch_march<4>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
-  else if (seg == 6) launch_march<6>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
-  else if (seg == 12) launch_march<12>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
-  else launch_march<8>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+    if (weno) k_recon_x<true><<<grid, 32 * RW, 0, s>>>(d, par.weno_eps, U, su, Wk, sw, K, sk);
+    else k_recon_x<false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
+  } else if (weno) launch_march<6, true>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else if (seg == 4) launch_march<4, false>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else if (seg == 6) launch_march<6, false>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else if (seg == 12) launch_march<12, false>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
+  else launch_march<8, false>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
   return cudaGetLastError();
 }
 

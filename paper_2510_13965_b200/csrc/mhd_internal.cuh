@@ -39,6 +39,8 @@ struct Par {
   double m1_kappa0, m1_rho0, m1_species_scale[3], m1_efloor, m1_tol, m1_mb;
   int m1_maxit, m1_odd_even;
   double m1_arad, m1_oe_guard;
+  int recon_kind;
+  double weno_eps, les_C_M;
 };
 
 struct Slot {

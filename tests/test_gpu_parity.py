@@ -686,3 +686,51 @@ def test_fused_and_separate_combine_agree(oracle_mod, rk):
             assert np.array_equal(Fg, Fo)
             assert np.all(_rel(Ug, Uo, interior=False)[0] < 1e-9) and np.all(_rel(Pg, Po, interior=False)[0] < 1e-9)
         assert np.all(_rel(res[0][0], res[1][0], interior=False)[0] < 1e-11)
+
+
+# ---- WENO5 as the second reconstruction ------------------------------------------
+def test_weno5_one_stage_parity(oracle_mod):
+    """recon_kind = 1 on config 1 (all terms live) and on ragged sizes with outflow: the same 1e-11 bar as MP5."""
+    cfg = synth.config1(n=32, gauge_perturbation=True)
+    cfg["params"].update(recon_kind=1)
+    _one_stage(oracle_mod, cfg)
+    cfg = synth.config1(n=32, gauge_perturbation=True)
+    cfg["params"].update(recon_kind=1, weno_eps=1e-12)      # a tiny epsilon: the non-linear weights are fully live
+    nx, ny, nz = 37, 19, 13
+    cfg["U"] = np.ascontiguousarray(np.tile(cfg["U"], (1, 1, 1, 2))[:, :nz + 6, :ny + 6, :nx + 6])
+    cfg["P"] = np.ascontiguousarray(np.tile(cfg["P"], (1, 1, 1, 2))[:, :nz + 6, :ny + 6, :nx + 6])
+    cfg["n"] = (nx, ny, nz)
+    cfg["bc"] = [1, 1, 0, 1, 1, 0]
+    _one_stage(oracle_mod, cfg, rhs_tol=1e-11)
+
+
+def test_weno5_ten_steps_and_star_surface(oracle_mod):
+    """10 RK4 steps of config 1 with WENO5 (<= 1e-9), and one stage across the surface of the TOV star of config 3, where the
+    weights switch stencils."""
+    cfg = synth.config1(n=16, gauge_perturbation=True)
+    cfg["params"].update(recon_kind=1)
+    o, patch, U, P = _setup(oracle_mod, cfg)
+    a, w = synth.tableau("rk4")
+    from paper_2510_13965_b200 import binding
+    dt = 0.25 * cfg["dx"]
+    patch.upload(U=U)
+    patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, 10)
+    Uo = U.copy()
+    _, Fo = o.evolve(Uo, cfg["bc"], a, w, dt, 10)
+    r, _ = _rel(patch.U.cpu().numpy(), Uo, interior=False)
+    assert np.all(r < 1e-9), r
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    patch.close()
+    cfg = synth.config3(n=32)
+    cfg["params"].update(recon_kind=1)
+    _one_stage(oracle_mod, cfg)
+
+
+def test_recon_kind_argument_check():
+    from paper_2510_13965_b200 import binding
+    par = synth.default_params(recon_kind=2)
+    with pytest.raises(binding.MhdError):
+        binding.mhd_patch_create(binding.make_desc(par, 8, 8, 8, 3, 0.1))
+    par = synth.default_params(recon_kind=1, weno_eps=0.0)
+    with pytest.raises(binding.MhdError):
+        binding.mhd_patch_create(binding.make_desc(par, 8, 8, 8, 3, 0.1))
