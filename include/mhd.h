@@ -203,6 +203,28 @@ int mhd_m1_gravity(mhd_patch *p, int slot_V, int slot_K, void *cuda_stream);
  * M1 explicit part -> rhs + back-reaction + radiation in the CCZ4 sources. */
 int mhd_advance_imex(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
 
+/* ---- AMR transfer operators on a patch pair (Sec. IV B l.608-626; refinement ratio 2, vertex-centred grids so that every
+ * coarse point is also a fine point, l.620). `origin[3]` (x, y, z) is the coarse INTERIOR index of the coarse point under fine
+ * interior point (0, 0, 0); fine interior index a (negative / >= n in the ghosts) sits at coarse position origin + a / 2.
+ * Both patches live on the same device; the two slots must hold the same number of fields (any slot but FLAGS).
+ *
+ * mhd_prolong: sets every fine grid point of the box lo[d] <= index < hi[d] (GHOSTED fine array indices, x, y, z) of slot_f from slot_c:
+ * a coincident point is a copy, a midpoint is the fifth-order Lagrange formula of Eq. (80) (l.616), applied along x, then y, then z
+ * (tensor product). Serves both the filling of a new fine patch (box = whole array) and the fine ghost zones at a coarse-fine
+ * boundary (one box per face). MHD_E_ARG if a coarse stencil point (offsets -2..+3) falls outside the coarse array. */
+int mhd_prolong(mhd_patch *coarse, int slot_c, mhd_patch *fine, int slot_f, const int origin[3], const int lo[3], const int hi[3],
+                void *cuda_stream);
+/* mhd_restrict: direct copy (l.626) of the fine INTERIOR points with even indices onto the coarse points they coincide with. */
+int mhd_restrict(mhd_patch *fine, int slot_f, mhd_patch *coarse, int slot_c, const int origin[3], void *cuda_stream);
+/* Dense-output interpolator (Eqs. 56-59, l.412-434), the time interpolation of the coarse level that sub-cycling needs (l.644-649):
+ * scheme 0 = RK(4,4), Eq. (58), third order; scheme 1 = SSP-RK(3,3), Eq. (59), second order. On the interior,
+ *   deriv = 0:      slot_out <- U0 + sum_j b_j(theta) dt K_j                         (Eq. 56; theta = (t - t^n)/dt)
+ *   deriv = 1..3:   slot_out <- dt^-deriv sum_j d^deriv b_j / dtheta^deriv dt K_j    (Eq. 57: time derivatives at t^n + theta dt)
+ * U0 (slot MHD_SLOT_U0) and K_j (MHD_SLOT_K1 + j - 1) must hold U^n and F(U^(j)) of the step, as the mhd_rk_stage sequence leaves
+ * them. slot_out: any state slot but U0 and the K_j used. mhd_dense_weights returns the number of stages and b_j (host, no device work). */
+int mhd_dense_weights(int scheme, double theta, int deriv, double b[4]);
+int mhd_dense_output(mhd_patch *p, int scheme, double theta, double dt, int deriv, int slot_out, void *cuda_stream);
+
 /* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */
 int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_stream);
 

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SOURCES = ["orc_stencil.cpp", "orc_eos.cpp", "orc_c2p.cpp", "orc_ccz4.cpp", "orc_grmhd.cpp",
-            "orc_rk.cpp", "orc_m1.cpp", "orc_m1_patch.cpp", "orc_capi.cpp"]
+            "orc_rk.cpp", "orc_m1.cpp", "orc_m1_patch.cpp", "orc_amr.cpp", "orc_capi.cpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 NSTATE, NPRIM = 32, 10
@@ -148,6 +148,13 @@ def _load(counting):
         L.orc_m1_backreaction.argtypes = [vp, vp, vp, vp, vp]
         L.orc_m1_gravity.argtypes = [vp, vp, vp, vp, vp]
         L.orc_evolve_imex.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, f64, i32]
+        L.orc_prolong.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp]
+        L.orc_restrict.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp]
+        L.orc_dense_weights.argtypes = [i32, f64, i32, vp]
+        L.orc_dense_weights.restype = i32
+        L.orc_dense_output.argtypes = [vp, i32, vp, vp, i32, vp, f64, f64, i32]
+        L.orc_prolong_mid.argtypes = [vp, ctypes.c_long]
+        L.orc_prolong_mid.restype = f64
     return _libs[counting]
 
 
@@ -338,3 +345,44 @@ Oracle.m1_implicit = _m1_implicit
 Oracle.m1_backreaction = _m1_backreaction
 Oracle.m1_gravity = _m1_gravity
 Oracle.evolve_imex = _evolve_imex
+
+
+# ---- AMR transfer operators on a patch pair -----------------------------------------------------
+def _i3(v):
+    return np.asarray(v, dtype=np.int32)
+
+
+def prolong(Uc, ngc, Uf, ngf, origin, lo, hi):
+    """Fill the index box [lo, hi) (x, y, z; ghosted fine array indices) of the fine array Uf (fields, MZ, MY, MX) from the coarse array
+    Uc by Eq. (80) / copy; origin = coarse interior index (x, y, z) of the coarse point under fine interior point (0, 0, 0)."""
+    nc = _i3([Uc.shape[3] - 2 * ngc, Uc.shape[2] - 2 * ngc, Uc.shape[1] - 2 * ngc])
+    nf = _i3([Uf.shape[3] - 2 * ngf, Uf.shape[2] - 2 * ngf, Uf.shape[1] - 2 * ngf])
+    o, l, h = _i3(origin), _i3(lo), _i3(hi)
+    lib().orc_prolong(_ptr(nc), ngc, _ptr(Uc), _ptr(nf), ngf, _ptr(Uf), Uc.shape[0], _ptr(o), _ptr(l), _ptr(h))
+    return Uf
+
+
+def restrict(Uf, ngf, Uc, ngc, origin):
+    """Copy the even fine interior points onto the coarse points they coincide with (l.626)."""
+    nc = _i3([Uc.shape[3] - 2 * ngc, Uc.shape[2] - 2 * ngc, Uc.shape[1] - 2 * ngc])
+    nf = _i3([Uf.shape[3] - 2 * ngf, Uf.shape[2] - 2 * ngf, Uf.shape[1] - 2 * ngf])
+    o = _i3(origin)
+    lib().orc_restrict(_ptr(nf), ngf, _ptr(Uf), _ptr(nc), ngc, _ptr(Uc), Uc.shape[0], _ptr(o))
+    return Uc
+
+
+def dense_weights(scheme, theta, deriv=0):
+    """b_j(theta) of Eq. (58) (scheme 0, RK4) / Eq. (59) (scheme 1, SSP-RK3) or their deriv-th theta-derivative (Eq. 57)"""
+    b = np.zeros(4)
+    s = lib().orc_dense_weights(int(scheme), float(theta), int(deriv), _ptr(b))
+    return b[:s].copy()
+
+
+def _dense_output(self, U0, Ks, scheme, theta, dt, deriv=0):
+    out = U0.copy()
+    ptrs = (ctypes.c_void_p * len(Ks))(*[k.ctypes.data for k in Ks])
+    lib().orc_dense_output(self.h, U0.shape[0], _ptr(out), _ptr(U0), int(scheme), ptrs, float(theta), float(dt), int(deriv))
+    return out
+
+
+Oracle.dense_output = _dense_output

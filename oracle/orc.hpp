@@ -157,4 +157,11 @@ void m1_gravity(const Params& par, const Grid& g, const double* U, const double*
 void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double* P, uint8_t* flags, const int bc[6], int stages,
                  const double* a_expl, const double* w_expl, const double* a_impl, const double* w_impl, double dt, int n_steps);
 
+// ---- AMR transfer operators on a patch pair (Sec. IV B l.608-626, Eqs. 56-59, 79-80); orc_amr.cpp
+double prolong_mid(const double* u, long s);                                              // Eq. (80)
+void prolong(const Grid& gc, const double* Uc, const Grid& gf, double* Uf, int nfields, const int origin[3], const int lo[3], const int hi[3]);
+void restrict_copy(const Grid& gf, const double* Uf, const Grid& gc, double* Uc, int nfields, const int origin[3]);
+int dense_weights(int scheme, double theta, int deriv, double b[4]);                      // Eqs. (58), (59), (57)
+void dense_output(const Grid& g, int nfields, double* Uout, const double* U0, int scheme, const double* const* K, double theta, double dt, int deriv);
+
 }  // namespace orc

@@ -124,6 +124,20 @@ void orc_evolve_imex(void* hh, double* U, double* V, double* P, uint8_t* flags, 
   evolve_imex(h->par, h->grid, U, V, P, flags, bc, stages, ae, we, ai, wi, dt, n_steps);
 }
 
+// ---- AMR transfer operators (grids passed explicitly: n[3], ng)
+static Grid mkgrid(const int* n, int ng) { return Grid{n[0], n[1], n[2], ng, 1.0, 1.0, 1.0}; }
+void orc_prolong(const int* nc, int ngc, const double* Uc, const int* nf, int ngf, double* Uf, int nfields, const int* origin, const int* lo, const int* hi) {
+  prolong(mkgrid(nc, ngc), Uc, mkgrid(nf, ngf), Uf, nfields, origin, lo, hi);
+}
+void orc_restrict(const int* nf, int ngf, const double* Uf, const int* nc, int ngc, double* Uc, int nfields, const int* origin) {
+  restrict_copy(mkgrid(nf, ngf), Uf, mkgrid(nc, ngc), Uc, nfields, origin);
+}
+int orc_dense_weights(int scheme, double theta, int deriv, double* b4) { return dense_weights(scheme, theta, deriv, b4); }
+void orc_dense_output(void* hh, int nfields, double* Uout, const double* U0, int scheme, const double* const* K, double theta, double dt, int deriv) {
+  dense_output(((Handle*)hh)->grid, nfields, Uout, U0, scheme, K, theta, dt, deriv);
+}
+double orc_prolong_mid(const double* u, long s) { return prolong_mid(u, s); }
+
 // ---- pointwise helpers for the pins
 double orc_d1(const double* u, long s, double h) { return d1(u, s, h); }
 double orc_d2(const double* u, long s, double h) { return d2(u, s, h); }

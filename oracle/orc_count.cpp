@@ -70,6 +70,7 @@ using orc_cnt::Cnt;
 #include "orc_rk.cpp"
 #include "orc_m1.cpp"
 #include "orc_m1_patch.cpp"
+#include "orc_amr.cpp"
 #include "orc_capi.cpp"
 #undef double
 

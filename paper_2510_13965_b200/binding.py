@@ -58,7 +58,8 @@ class mhd_status(ctypes.Structure):
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
-           "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex"]
+           "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex",
+           "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output"]
 NKERNELS = 12
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
                   "m1_point", "m1_div", "m1_implicit"]
@@ -97,6 +98,10 @@ def lib():
         L.mhd_m1_gravity.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
+        L.mhd_prolong.argtypes = [_p, _i, _p, _i, ctypes.POINTER(_i), ctypes.POINTER(_i), ctypes.POINTER(_i), _p]
+        L.mhd_restrict.argtypes = [_p, _i, _p, _i, ctypes.POINTER(_i), _p]
+        L.mhd_dense_weights.argtypes = [_i, _d, _i, ctypes.POINTER(_d)]
+        L.mhd_dense_output.argtypes = [_p, _i, _d, _d, _i, _i, _p]
         if L.mhd_desc_sizeof() != ctypes.sizeof(mhd_patch_desc):
             raise RuntimeError("mhd_patch_desc layout mismatch between include/mhd.h and binding.py")
         _lib = L
@@ -219,6 +224,30 @@ def mhd_m1_gravity(h, slot_V, slot_K, stream=None):
 
 def mhd_advance_imex(h, tableau, bc, dt, n_steps, stream=None):
     _check(lib().mhd_advance_imex(h, ctypes.byref(tableau), _bc(bc), dt, n_steps, stream))
+
+
+def _i3(v):
+    return (_i * 3)(*[int(x) for x in v])
+
+
+def mhd_prolong(h_coarse, slot_c, h_fine, slot_f, origin, lo, hi, stream=None):
+    _check(lib().mhd_prolong(h_coarse, slot_c, h_fine, slot_f, _i3(origin), _i3(lo), _i3(hi), stream))
+
+
+def mhd_restrict(h_fine, slot_f, h_coarse, slot_c, origin, stream=None):
+    _check(lib().mhd_restrict(h_fine, slot_f, h_coarse, slot_c, _i3(origin), stream))
+
+
+def mhd_dense_weights(scheme, theta, deriv=0):
+    b = (_d * 4)()
+    s = lib().mhd_dense_weights(scheme, theta, deriv, b)
+    if s < 0:
+        _check(s)
+    return [b[j] for j in range(s)]
+
+
+def mhd_dense_output(h, scheme, theta, dt, deriv, slot_out, stream=None):
+    _check(lib().mhd_dense_output(h, scheme, theta, dt, deriv, slot_out, stream))
 
 
 def mhd_patch_status(h, slot_flags=SLOT_FLAGS, stream=None):

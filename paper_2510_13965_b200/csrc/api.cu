@@ -402,6 +402,75 @@ int mhd_advance_imex(mhd_patch* p, const mhd_tableau* t, const int bc[6], double
 #undef CK
 }
 
+// ---- AMR transfer operators on a patch pair
+int mhd_prolong(mhd_patch* coarse, int slot_c, mhd_patch* fine, int slot_f, const int origin[3], const int lo[3], const int hi[3], void* stream) {
+  if (!coarse || !fine || !origin || !lo || !hi || coarse == fine) return MHD_E_ARG;
+  if (slot_c < 0 || slot_c >= MHD_NSLOTS || slot_f < 0 || slot_f >= MHD_NSLOTS || slot_c == MHD_SLOT_FLAGS || slot_f == MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (slot_fields(slot_c) != slot_fields(slot_f)) return MHD_E_ARG;
+  if (!slot_ok(coarse, slot_c) || !slot_ok(fine, slot_f)) return MHD_E_UNBOUND;
+  const Dims &dc = coarse->dims, &df = fine->dims;
+  const int mf[3] = {df.mx, df.my, df.mz}, mc[3] = {dc.mx, dc.my, dc.mz};
+  for (int a = 0; a < 3; ++a) {
+    if (lo[a] < 0 || hi[a] > mf[a] || hi[a] < lo[a]) return MHD_E_ARG;
+    if (hi[a] == lo[a]) return MHD_OK;
+    // every coarse point the box needs (offsets -2..3 around a midpoint, the point itself under a coincident point) must exist
+    for (int e = 0; e < 2; ++e) {
+      const int af = (e == 0 ? lo[a] : hi[a] - 1) - df.ng;
+      const int hfl = af >= 0 ? af / 2 : -((-af + 1) / 2);
+      const int c = origin[a] + hfl + dc.ng, odd = af - 2 * hfl;
+      // a box of more than one point holds both parities: test the wider stencil unless the box is a single point
+      const bool wide = odd || hi[a] - lo[a] > 1;
+      if (c - (wide ? 2 : 0) < 0 || c + (wide ? 3 : 0) >= mc[a]) return MHD_E_ARG;
+    }
+  }
+  return launch_prolong(dc, dptr(coarse, slot_c), coarse->slot[slot_c].stride, df, dptr(fine, slot_f), fine->slot[slot_f].stride, slot_fields(slot_c),
+                        origin, lo, hi, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_restrict(mhd_patch* fine, int slot_f, mhd_patch* coarse, int slot_c, const int origin[3], void* stream) {
+  if (!coarse || !fine || !origin || coarse == fine) return MHD_E_ARG;
+  if (slot_c < 0 || slot_c >= MHD_NSLOTS || slot_f < 0 || slot_f >= MHD_NSLOTS || slot_c == MHD_SLOT_FLAGS || slot_f == MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (slot_fields(slot_c) != slot_fields(slot_f)) return MHD_E_ARG;
+  if (!slot_ok(coarse, slot_c) || !slot_ok(fine, slot_f)) return MHD_E_UNBOUND;
+  const Dims &dc = coarse->dims, &df = fine->dims;
+  const int nf[3] = {df.nx, df.ny, df.nz}, mc[3] = {dc.mx, dc.my, dc.mz};
+  for (int a = 0; a < 3; ++a)
+    if (origin[a] + dc.ng < 0 || origin[a] + (nf[a] - 1) / 2 + dc.ng >= mc[a]) return MHD_E_ARG;
+  return launch_restrict(df, dptr(fine, slot_f), fine->slot[slot_f].stride, dc, dptr(coarse, slot_c), coarse->slot[slot_c].stride, slot_fields(slot_c),
+                         origin, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
+int mhd_dense_weights(int scheme, double theta, int deriv, double b[4]) {
+  if (!b || (scheme != 0 && scheme != 1) || deriv < 0 || deriv > 3) return MHD_E_ARG;
+  // coefficients of theta^1, theta^2, theta^3 of b_j(theta): Eq. (58) RK(4,4), Eq. (59) SSP-RK(3,3)
+  static const double rk4[4][3] = {{1.0, -1.5, 2.0 / 3.0}, {0.0, 1.0, -2.0 / 3.0}, {0.0, 1.0, -2.0 / 3.0}, {0.0, -0.5, 2.0 / 3.0}};
+  static const double ssp3[4][3] = {{1.0, -5.0 / 6.0, 0.0}, {0.0, 1.0 / 6.0, 0.0}, {0.0, 4.0 / 6.0, 0.0}, {0.0, 0.0, 0.0}};
+  const double (*p)[3] = scheme == 0 ? rk4 : ssp3;
+  const double t = theta;
+  for (int j = 0; j < 4; ++j) {
+    const double c1 = p[j][0], c2 = p[j][1], c3 = p[j][2];
+    b[j] = deriv == 0 ? t * (c1 + t * (c2 + t * c3)) : deriv == 1 ? c1 + t * (2.0 * c2 + 3.0 * t * c3) : deriv == 2 ? 2.0 * c2 + 6.0 * t * c3 : 6.0 * c3;
+  }
+  return scheme == 0 ? 4 : 3;
+}
+
+int mhd_dense_output(mhd_patch* p, int scheme, double theta, double dt, int deriv, int slot_out, void* stream) {
+  double b[4];
+  const int s = mhd_dense_weights(scheme, theta, deriv, b);
+  if (!p || s < 0 || !(dt > 0.0) || !is_state_slot(slot_out) || slot_out == MHD_SLOT_U0) return MHD_E_ARG;
+  if (!slot_ok(p, slot_out) || !slot_ok(p, MHD_SLOT_U0)) return MHD_E_UNBOUND;
+  const double* K[4]; size_t sk[4]; double c[4];
+  for (int j = 0; j < s; ++j) {
+    if (slot_out == MHD_SLOT_K1 + j) return MHD_E_ARG;
+    if (!slot_ok(p, MHD_SLOT_K1 + j)) return MHD_E_UNBOUND;
+    K[j] = dptr(p, MHD_SLOT_K1 + j); sk[j] = p->slot[MHD_SLOT_K1 + j].stride;
+    c[j] = b[j] * dt / pow(dt, deriv);                     // k_j = dt K_j; Eq. (57): dt^-m
+  }
+  Timed tm(p, 6, (cudaStream_t)stream);
+  return launch_dense(p->dims, MHD_NSTATE, dptr(p, slot_out), p->slot[slot_out].stride, dptr(p, MHD_SLOT_U0), p->slot[MHD_SLOT_U0].stride, s, K, sk, c,
+                      deriv == 0, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
 int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream) {
   if (!p || !out || slot_flags != MHD_SLOT_FLAGS) return MHD_E_ARG;
   if (!slot_ok(p, slot_flags)) return MHD_E_UNBOUND;

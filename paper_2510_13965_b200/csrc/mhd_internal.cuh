@@ -112,5 +112,10 @@ cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, s
                                double* R, size_t sr, double adt, uint8_t* flags, cudaStream_t s);
 cudaError_t launch_m1_gravity(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
                               double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_prolong(const Dims& dc, const double* Uc, size_t sc, const Dims& df, double* Uf, size_t sf, int nfields,
+                           const int origin[3], const int lo[3], const int hi[3], cudaStream_t s);
+cudaError_t launch_restrict(const Dims& df, const double* Uf, size_t sf, const Dims& dc, double* Uc, size_t sc, int nfields, const int origin[3], cudaStream_t s);
+cudaError_t launch_dense(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0, int nk, const double* const* K,
+                         const size_t* sk, const double* c, int with_u0, cudaStream_t s);
 cudaError_t launch_m1_backreact(const Dims& d, const Par& par, const double* R, size_t sr, double* K, size_t sk, cudaStream_t s);
 }  // namespace mhd
