@@ -130,6 +130,7 @@ typedef struct {
 
 typedef struct {
   unsigned long long n_points, n_atmo, n_eps_lo, n_eps_hi, n_vmax, n_ye, n_fatal, n_noconv, n_m1fix;
+  unsigned long long halo_timeout;   /* non-zero: a wait on a neighbour patch (fused halo fill) expired; the state is not valid */
 } mhd_status;
 
 typedef struct mhd_patch mhd_patch;   /* opaque */
@@ -144,8 +145,32 @@ void mhd_patch_destroy(mhd_patch *p);
 int mhd_patch_bind(mhd_patch *p, int slot, void *dev_ptr, size_t field_stride);
 
 /* a1 — ghost fill: bc[6] = {x-,x+,y-,y+,z-,z+}, 0 periodic wrap, 1 outflow (copy of the nearest
- * interior value). Fills all ng ghost layers incl. edges and corners of every field of the slot, in place. */
+ * interior value), 2 neighbour patch (below). Fills all ng ghost layers incl. edges and corners of every field of the slot, in
+ * place. MHD_E_ARG if a periodic or neighbour axis has fewer interior points than ghost layers. */
 int mhd_fill_ghosts(mhd_patch *p, int slot_state, const int bc[6], void *cuda_stream);
+
+/* ---- Domain decomposition: halo exchange fused with the ghost fill ("spatial decomposition") ----
+ * The patch is one brick of a regular decomposition; all bricks have the same nx, ny, nz, ng. A face with bc = 2 has a neighbour
+ * brick behind it: its ghost layers are read by the ghost-fill kernel directly from the neighbour's interior, i.e. from the SAME SLOT
+ * of the neighbour patch, whose device pointer is registered here — a pointer on this GPU, or a peer-GPU mapping (cudaIpcOpenMemHandle
+ * / peer access) read over NVLink: no pack, send or unpack. dir[3] in {-1,0,1}^3 \ {0} names the neighbour: faces, and the edge /
+ * corner neighbours wherever two / three neighbour faces meet (a domain-periodic axis split over several bricks is a neighbour
+ * axis too; an axis with a single brick keeps bc 0 / 1). Register every state slot mhd_advance rotates (U, U0, and U1 if bound):
+ * the entries travel with the buffers. MHD_E_UNBOUND from mhd_fill_ghosts if a needed neighbour is missing. */
+int mhd_patch_set_neighbor(mhd_patch *p, int slot, const int dir[3], const void *peer_dev_ptr, size_t peer_field_stride);
+/* Ordering between patches driven from different streams / processes / GPUs. Each patch owns 27 epoch words in device memory
+ * (mhd_patch_halo_words; export with mhd_ipc_export). After mhd_patch_set_neighbor_word(p, dir, <halo words of the neighbour in
+ * direction dir>) every ghost fill with neighbour faces runs   signal "my interior is final" -> wait for the neighbours' signal ->
+ * fill -> signal "I have read" -> wait   as stream-ordered kernels (system-scope release / acquire on the words; no host
+ * synchronisation, no collective library). All bricks must issue the same sequence of ghost fills. A wait that expires (~4 s) sets
+ * mhd_status.halo_timeout instead of hanging the device. Patches driven from ONE stream need no words. */
+void *mhd_patch_halo_words(mhd_patch *p);
+int mhd_patch_set_neighbor_word(mhd_patch *p, const int dir[3], void *peer_halo_words);
+/* CUDA IPC helpers (one process per GPU): export = handle of the allocation that holds dev_ptr + offset of dev_ptr in it; import
+ * maps it into this process and returns the usable device pointer; close unmaps it. */
+int mhd_ipc_export(const void *dev_ptr, unsigned char handle[64], size_t *offset);
+int mhd_ipc_import(const unsigned char handle[64], size_t offset, void **dev_ptr);
+int mhd_ipc_close(void *dev_ptr, size_t offset);
 
 /* a2 — conserved -> primitive at every grid point incl. ghosts (App. D, Eqs. D1-D15, error policy
  * l.1157-1162). Writes the 10 primitives and the flag byte; where a rule changed a primitive the fluid conserved

@@ -52,14 +52,15 @@ class mhd_tableau(ctypes.Structure):
 
 class mhd_status(ctypes.Structure):
     _fields_ = [(n, ctypes.c_ulonglong) for n in
-                ("n_points", "n_atmo", "n_eps_lo", "n_eps_hi", "n_vmax", "n_ye", "n_fatal", "n_noconv", "n_m1fix")]
+                ("n_points", "n_atmo", "n_eps_lo", "n_eps_hi", "n_vmax", "n_ye", "n_fatal", "n_noconv", "n_m1fix", "halo_timeout")]
 
 
 EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patch_bind", "mhd_fill_ghosts", "mhd_con2prim",
            "mhd_prim2con", "mhd_rhs", "mhd_rk_stage", "mhd_advance", "mhd_advance_host", "mhd_patch_status",
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
            "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex",
-           "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output"]
+           "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output",
+           "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
 NKERNELS = 12
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
                   "m1_point", "m1_div", "m1_implicit"]
@@ -98,6 +99,13 @@ def lib():
         L.mhd_m1_gravity.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
+        L.mhd_patch_set_neighbor.argtypes = [_p, _i, ctypes.POINTER(_i), _p, ctypes.c_size_t]
+        L.mhd_patch_halo_words.argtypes = [_p]
+        L.mhd_patch_halo_words.restype = _p
+        L.mhd_patch_set_neighbor_word.argtypes = [_p, ctypes.POINTER(_i), _p]
+        L.mhd_ipc_export.argtypes = [_p, ctypes.c_char_p, ctypes.POINTER(ctypes.c_size_t)]
+        L.mhd_ipc_import.argtypes = [ctypes.c_char_p, ctypes.c_size_t, ctypes.POINTER(_p)]
+        L.mhd_ipc_close.argtypes = [_p, ctypes.c_size_t]
         L.mhd_prolong.argtypes = [_p, _i, _p, _i, ctypes.POINTER(_i), ctypes.POINTER(_i), ctypes.POINTER(_i), _p]
         L.mhd_restrict.argtypes = [_p, _i, _p, _i, ctypes.POINTER(_i), _p]
         L.mhd_dense_weights.argtypes = [_i, _d, _i, ctypes.POINTER(_d)]
@@ -228,6 +236,36 @@ def mhd_advance_imex(h, tableau, bc, dt, n_steps, stream=None):
 
 def _i3(v):
     return (_i * 3)(*[int(x) for x in v])
+
+
+def mhd_patch_set_neighbor(h, slot, direction, peer_dev_ptr, peer_field_stride):
+    _check(lib().mhd_patch_set_neighbor(h, slot, _i3(direction), peer_dev_ptr, peer_field_stride))
+
+
+def mhd_patch_halo_words(h):
+    return lib().mhd_patch_halo_words(h)
+
+
+def mhd_patch_set_neighbor_word(h, direction, peer_halo_words):
+    _check(lib().mhd_patch_set_neighbor_word(h, _i3(direction), peer_halo_words))
+
+
+def mhd_ipc_export(dev_ptr):
+    """(64-byte handle, offset) of a device pointer, to be sent to the process that owns the neighbouring GPU"""
+    buf = ctypes.create_string_buffer(64)
+    off = ctypes.c_size_t(0)
+    _check(lib().mhd_ipc_export(dev_ptr, buf, ctypes.byref(off)))
+    return buf.raw, int(off.value)
+
+
+def mhd_ipc_import(handle, offset):
+    out = _p()
+    _check(lib().mhd_ipc_import(handle, offset, ctypes.byref(out)))
+    return out.value
+
+
+def mhd_ipc_close(dev_ptr, offset):
+    _check(lib().mhd_ipc_close(dev_ptr, offset))
 
 
 def mhd_prolong(h_coarse, slot_c, h_fine, slot_f, origin, lo, hi, stream=None):

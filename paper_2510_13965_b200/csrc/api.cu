@@ -194,7 +194,8 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.m1_odd_even = desc->m1_odd_even; q.m1_arad = desc->m1_arad; q.m1_oe_guard = desc->m1_oe_guard;
   q.recon_kind = desc->recon_kind; q.weno_eps = desc->weno_eps; q.les_C_M = desc->les_C_M;
   p->d_counts = nullptr;
-  if (cudaMalloc(&p->d_counts, 16 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
+  if (cudaMalloc(&p->d_counts, 48 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
+  if (cudaMemset(p->d_counts, 0, 48 * sizeof(unsigned long long)) != cudaSuccess) { cudaFree(p->d_counts); delete p; return MHD_E_CUDA; }
   *out = p;
   return MHD_OK;
 }
@@ -217,11 +218,108 @@ int mhd_patch_bind(mhd_patch* p, int slot, void* dev_ptr, size_t field_stride) {
 
 int mhd_fill_ghosts(mhd_patch* p, int slot_state, const int bc[6], void* stream) {
   if (!p || !bc) return MHD_E_ARG;
-  for (int a = 0; a < 6; ++a) if (bc[a] != 0 && bc[a] != 1) return MHD_E_ARG;
+  const int n[3] = {p->dims.nx, p->dims.ny, p->dims.nz};
+  bool halo = false;
+  for (int a = 0; a < 6; ++a) {
+    if (bc[a] < 0 || bc[a] > 2) return MHD_E_ARG;
+    if (bc[a] != 1 && n[a / 2] < p->dims.ng) return MHD_E_ARG;      // a wrap by n must land on an interior point
+    halo = halo || bc[a] == 2;
+  }
   if (slot_state < 0 || slot_state >= MHD_NSLOTS || slot_state == MHD_SLOT_FLAGS) return MHD_E_ARG;
   if (!slot_ok(p, slot_state)) return MHD_E_UNBOUND;
-  Timed tm(p, 0, (cudaStream_t)stream);
-  return launch_fill_ghosts(p->dims, dptr(p, slot_state), p->slot[slot_state].stride, slot_fields(slot_state), bc, (cudaStream_t)stream) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  const Slot& sl = p->slot[slot_state];
+  unsigned long long *mine[27], *theirs[27];
+  int nw = 0;
+  if (halo) {
+    // every direction whose non-zero components all cross a neighbour face needs the neighbour's array (faces, and the edges and
+    // corners shared by two or three neighbour faces)
+    for (int q = 0; q < 27; ++q) {
+      const int dd[3] = {q % 3 - 1, (q / 3) % 3 - 1, q / 9 - 1};
+      bool need = q != 13;
+      for (int a = 0; a < 3; ++a) if (dd[a] != 0 && bc[2 * a + (dd[a] > 0)] != 2) need = false;
+      if (!need) continue;
+      if (!sl.peer[q]) return MHD_E_UNBOUND;
+      if (p->peer_word[q]) { theirs[nw] = p->peer_word[q]; mine[nw] = p->d_counts + 16 + q; ++nw; }
+    }
+  }
+  Timed tm(p, 0, s);
+  // two-phase ordering against the neighbours (only when epoch words were registered: patches driven from one stream need none):
+  // "my interior is final" -> all neighbours say so -> fill (reads their interiors) -> "I have read" -> all neighbours have read
+  if (nw) {
+    const unsigned long long e = ++p->halo_epoch;
+    if (launch_halo_signal(theirs, nw, e, s) != cudaSuccess || launch_halo_wait(mine, nw, e, p->d_counts + 43, s) != cudaSuccess) return MHD_E_CUDA;
+  }
+  if (launch_fill_ghosts(p->dims, dptr(p, slot_state), sl.stride, slot_fields(slot_state), bc, halo ? &sl : nullptr, s) != cudaSuccess) return MHD_E_CUDA;
+  if (nw) {
+    const unsigned long long e = ++p->halo_epoch;
+    if (launch_halo_signal(theirs, nw, e, s) != cudaSuccess || launch_halo_wait(mine, nw, e, p->d_counts + 43, s) != cudaSuccess) return MHD_E_CUDA;
+  }
+  return MHD_OK;
+}
+
+static int dir_index(const int dir[3]) {
+  if (!dir) return -1;
+  for (int a = 0; a < 3; ++a) if (dir[a] < -1 || dir[a] > 1) return -1;
+  const int q = (dir[0] + 1) + 3 * (dir[1] + 1) + 9 * (dir[2] + 1);
+  return q == 13 ? -1 : q;
+}
+
+int mhd_patch_set_neighbor(mhd_patch* p, int slot, const int dir[3], const void* peer_dev_ptr, size_t peer_field_stride) {
+  const int q = dir_index(dir);
+  if (!p || q < 0 || slot < 0 || slot >= MHD_NSLOTS || slot == MHD_SLOT_FLAGS) return MHD_E_ARG;
+  if (peer_dev_ptr && peer_field_stride < (size_t)p->dims.npts) return MHD_E_ARG;
+  p->slot[slot].peer[q] = (const double*)peer_dev_ptr;          // NULL clears the entry
+  p->slot[slot].peer_stride[q] = peer_field_stride;
+  return MHD_OK;
+}
+
+void* mhd_patch_halo_words(mhd_patch* p) { return p ? (void*)(p->d_counts + 16) : nullptr; }
+
+int mhd_patch_set_neighbor_word(mhd_patch* p, const int dir[3], void* peer_words) {
+  const int q = dir_index(dir);
+  if (!p || q < 0) return MHD_E_ARG;
+  // the neighbour in direction q sees this patch in direction 26 - q: that is the word of its array this patch signals
+  p->peer_word[q] = peer_words ? (unsigned long long*)peer_words + (26 - q) : nullptr;
+  return MHD_OK;
+}
+
+// ---- CUDA IPC helpers for one process per GPU: a device pointer inside any allocation (e.g. a torch tensor of the caching allocator)
+// is exported as the allocation's handle plus the pointer's offset in it
+int mhd_ipc_export(const void* dev_ptr, unsigned char handle[64], size_t* offset) {
+  if (!dev_ptr || !handle || !offset) return MHD_E_ARG;
+  typedef int (*RangeFn)(unsigned long long*, size_t*, unsigned long long);
+  static RangeFn range = nullptr;
+  if (!range) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess) return MHD_E_CUDA;
+    range = (RangeFn)fn;
+  }
+  unsigned long long base = 0;
+  size_t size = 0;
+  if (range(&base, &size, (unsigned long long)(uintptr_t)dev_ptr) != 0) return MHD_E_CUDA;
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+  cudaIpcMemHandle_t h;
+  if (cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base) != cudaSuccess) { cudaGetLastError(); return MHD_E_CUDA; }
+  memcpy(handle, &h, 64);
+  *offset = (size_t)((unsigned long long)(uintptr_t)dev_ptr - base);
+  return MHD_OK;
+}
+
+int mhd_ipc_import(const unsigned char handle[64], size_t offset, void** dev_ptr) {
+  if (!handle || !dev_ptr) return MHD_E_ARG;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle, 64);
+  void* base = nullptr;
+  if (cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return MHD_E_CUDA; }
+  *dev_ptr = (char*)base + offset;
+  return MHD_OK;
+}
+
+int mhd_ipc_close(void* dev_ptr, size_t offset) {
+  if (!dev_ptr) return MHD_E_ARG;
+  return cudaIpcCloseMemHandle((char*)dev_ptr - offset) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
 }
 
 int mhd_con2prim(mhd_patch* p, int slot_state, int slot_prim, int slot_flags, void* stream) {
@@ -476,12 +574,14 @@ int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream
   if (!slot_ok(p, slot_flags)) return MHD_E_UNBOUND;
   cudaStream_t s = (cudaStream_t)stream;
   if (launch_count_flags(p->dims, (const uint8_t*)p->slot[slot_flags].ptr, p->d_counts, s) != cudaSuccess) return MHD_E_CUDA;
-  unsigned long long h[8];
+  unsigned long long h[8], hto = 0;
   if (cudaMemcpyAsync(h, p->d_counts, sizeof(h), cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  if (cudaMemcpyAsync(&hto, p->d_counts + 43, sizeof(hto), cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
   if (cudaStreamSynchronize(s) != cudaSuccess) return MHD_E_CUDA;
   out->n_points = (unsigned long long)p->dims.npts;
   out->n_atmo = h[0]; out->n_eps_lo = h[1]; out->n_eps_hi = h[2]; out->n_vmax = h[3];
   out->n_ye = h[4]; out->n_fatal = h[5]; out->n_noconv = h[6]; out->n_m1fix = h[7];
+  out->halo_timeout = hto;
   return MHD_OK;
 }
 

@@ -5,19 +5,29 @@
 namespace mhd {
 
 // ---------------------------------------------------------------------------------------------
-// Ghost fill. The sequential x,y,z fill of the textbook algorithm equals one direct map per axis
-// (wrap or clamp to the interior), so every ghost cell is written exactly once from an interior cell.
+// Ghost fill, fused with the halo exchange between neighbouring patches.
+// The sequential x,y,z fill of the textbook algorithm equals one direct map per axis (wrap, clamp to the interior, or
+// "the same wrap, but in the neighbour's array"), so every ghost cell is written exactly once from an interior cell — of this
+// patch, or of the neighbour patch in direction (dx, dy, dz), read straight from its memory (a peer GPU's HBM over NVLink when the
+// pointer is a peer mapping): there is no pack / send / unpack. Bricks of one decomposition have equal extents, so the index map
+// along a neighbour axis is the periodic one.
 // Ghost cells are enumerated slab by slab: 2 z-slabs (full MX x MY), 2 y-slabs (interior z), 2 x-slabs.
 // ---------------------------------------------------------------------------------------------
-struct GhostMap { int bc[6]; };
+struct GhostMap {
+  int bc[6];
+  const double* peer[27];     // source array per direction (dx+1) + 3 (dy+1) + 9 (dz+1); [13] = this patch
+  size_t pstride[27];
+};
 
-__device__ __forceinline__ int ghost_src(int i, int n, int ng, int bc_lo, int bc_hi) {
-  if (i < ng) return bc_lo == 0 ? i + n : ng;
-  if (i >= ng + n) return bc_hi == 0 ? i - n : ng + n - 1;
+// bc: 0 periodic, 1 outflow, 2 neighbour; dir receives -1 / 0 / +1
+__device__ __forceinline__ int ghost_src(int i, int n, int ng, int bc_lo, int bc_hi, int& dir) {
+  dir = 0;
+  if (i < ng) { dir = bc_lo == 2 ? -1 : 0; return bc_lo == 1 ? ng : i + n; }
+  if (i >= ng + n) { dir = bc_hi == 2 ? 1 : 0; return bc_hi == 1 ? ng + n - 1 : i - n; }
   return i;
 }
 
-__global__ void __launch_bounds__(256) k_fill_ghosts(Dims d, double* __restrict__ U, size_t stride, GhostMap m) {
+__global__ void __launch_bounds__(256) k_fill_ghosts(Dims d, double* __restrict__ U, size_t stride, const __grid_constant__ GhostMap m) {
   const long long nzs = 2LL * d.ng * d.my * d.mx;          // z-slabs
   const long long nys = 2LL * d.ng * d.nz * d.mx;          // y-slabs (interior k)
   const long long nxs = 2LL * d.ng * d.nz * d.ny;          // x-slabs (interior j,k)
@@ -42,19 +52,67 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Dims d, double* __restrict_
     k = d.ng + (int)(r / ((long long)2 * d.ng * d.ny));
     i = q < d.ng ? q : d.nx + q;
   }
-  const int si = ghost_src(i, d.nx, d.ng, m.bc[0], m.bc[1]);
-  const int sj = ghost_src(j, d.ny, d.ng, m.bc[2], m.bc[3]);
-  const int sk = ghost_src(k, d.nz, d.ng, m.bc[4], m.bc[5]);
-  double* u = U + (size_t)blockIdx.y * stride;
-  u[k * d.sz + j * d.sy + i] = u[sk * d.sz + sj * d.sy + si];
+  int dx, dy, dz;
+  const int si = ghost_src(i, d.nx, d.ng, m.bc[0], m.bc[1], dx);
+  const int sj = ghost_src(j, d.ny, d.ng, m.bc[2], m.bc[3], dy);
+  const int sk = ghost_src(k, d.nz, d.ng, m.bc[4], m.bc[5], dz);
+  const int dir = (dx + 1) + 3 * (dy + 1) + 9 * (dz + 1);
+  const double* src = m.peer[dir] + (size_t)blockIdx.y * m.pstride[dir];
+  U[(size_t)blockIdx.y * stride + k * d.sz + j * d.sy + i] = src[sk * d.sz + sj * d.sy + si];
 }
 
-cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], cudaStream_t s) {
+cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], const Slot* peers, cudaStream_t s) {
   GhostMap m;
   for (int a = 0; a < 6; ++a) m.bc[a] = bc[a];
+  for (int q = 0; q < 27; ++q) {
+    const bool has = peers && peers->peer[q];
+    m.peer[q] = has ? peers->peer[q] : U;
+    m.pstride[q] = has ? peers->peer_stride[q] : stride;
+  }
+  m.peer[13] = U; m.pstride[13] = stride;
   const long long n = 2LL * d.ng * ((long long)d.my * d.mx + (long long)d.nz * d.mx + (long long)d.nz * d.ny);
   dim3 grid((unsigned)((n + 255) / 256), nfields);
   k_fill_ghosts<<<grid, 256, 0, s>>>(d, U, stride, m);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Cross-patch ordering for the fused halo fill: every patch owns 27 epoch words (one per neighbour direction). "signal" stores the
+// epoch into the word the neighbour in direction q watches (a peer-memory store, released at system scope after this stream's
+// earlier kernels); "wait" spins until the words of this patch's own neighbours have reached the epoch. A bounded spin (~4 s) so
+// that a lost peer cannot hang the device: on expiry a flag is raised in the patch's scratch and the kernel returns.
+// ---------------------------------------------------------------------------------------------
+struct HaloSync { unsigned long long* word[27]; int n; };
+
+__global__ void k_halo_signal(const __grid_constant__ HaloSync h, unsigned long long epoch) {
+  if (threadIdx.x >= h.n) return;
+  __threadfence_system();
+  asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(h.word[threadIdx.x]), "l"(epoch) : "memory");
+}
+
+__global__ void k_halo_wait(const __grid_constant__ HaloSync h, unsigned long long epoch, unsigned long long* timeout_flag) {
+  if (threadIdx.x >= h.n) return;
+  const long long t0 = clock64();
+  unsigned long long v;
+  do {
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(h.word[threadIdx.x]) : "memory");
+    if (v >= epoch) return;
+  } while (clock64() - t0 < 8000000000LL);
+  *timeout_flag = 1ULL;
+}
+
+cudaError_t launch_halo_signal(unsigned long long* const* words, int n, unsigned long long epoch, cudaStream_t s) {
+  HaloSync h;
+  h.n = n;
+  for (int q = 0; q < 27; ++q) h.word[q] = q < n ? words[q] : nullptr;
+  k_halo_signal<<<1, 32, 0, s>>>(h, epoch);
+  return cudaGetLastError();
+}
+cudaError_t launch_halo_wait(unsigned long long* const* words, int n, unsigned long long epoch, unsigned long long* timeout_flag, cudaStream_t s) {
+  HaloSync h;
+  h.n = n;
+  for (int q = 0; q < 27; ++q) h.word[q] = q < n ? words[q] : nullptr;
+  k_halo_wait<<<1, 32, 0, s>>>(h, epoch, timeout_flag);
   return cudaGetLastError();
 }
 

@@ -46,6 +46,11 @@ struct Par {
 struct Slot {
   void* ptr = nullptr;
   size_t stride = 0;
+  // halo exchange fused with the ghost fill: the same slot of the neighbouring patch in direction (dx+1) + 3 (dy+1) + 9 (dz+1)
+  // (device pointers, possibly peer-GPU mappings). They travel with the slot when mhd_advance swaps state buffers: every patch of a
+  // decomposition performs the same swaps.
+  const double* peer[27] = {};
+  size_t peer_stride[27] = {};
 };
 
 // Explicit RK combine (Eq. 53) fused into the last kernel that touches a field of K_i (k_adv_ko for the 22 spacetime fields,
@@ -82,7 +87,10 @@ struct mhd_patch {
   mhd::Dims dims;
   mhd::Par par;
   mhd::Slot slot[MHD_NSLOTS];
-  unsigned long long* d_counts;   // device scratch: 8 counters for mhd_patch_status, then 8 doubles (EoS part of the atmosphere state)
+  unsigned long long* d_counts;   // device scratch: 8 counters for mhd_patch_status, then 8 doubles (EoS part of the atmosphere state),
+                                  // then [16..42] the 27 halo epoch words of this patch, [43] the halo time-out flag
+  unsigned long long* peer_word[27] = {};   // where to signal the neighbour in direction q (its epoch word for direction 26 - q)
+  unsigned long long halo_epoch = 0;
   // optional per-kernel timing (mhd_patch_profile)
   bool profiling = false;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -92,7 +100,9 @@ struct mhd_patch {
 
 namespace mhd {
 // kernel launchers (one per translation unit); all return cudaGetLastError()
-cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], cudaStream_t s);
+cudaError_t launch_fill_ghosts(const Dims& d, double* U, size_t stride, int nfields, const int bc[6], const Slot* peers, cudaStream_t s);
+cudaError_t launch_halo_signal(unsigned long long* const* words, int n, unsigned long long epoch, cudaStream_t s);
+cudaError_t launch_halo_wait(unsigned long long* const* words, int n, unsigned long long epoch, unsigned long long* timeout_flag, cudaStream_t s);
 cudaError_t launch_con2prim(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, uint8_t* flags, double* atmo, cudaStream_t s);
 cudaError_t launch_prim2con(const Dims& d, const Par& par, double* U, size_t su, double* P, size_t sp, cudaStream_t s);
 cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* K, size_t sk, cudaStream_t s);
