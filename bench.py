@@ -93,10 +93,24 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_leg(cfg_name, n_sample, steps):
-    """The oracle as it stands, single thread, on a bounded sample of the workload; returns (value, seconds, zone_stages)."""
+def cpu_info():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count() or 1, "cpu_model": model}
+
+
+def oracle_leg(cfg_name, n_sample, steps, threads=1):
+    """The oracle as it stands on a bounded sample of the workload: threads = 1 is the plain single-threaded build, threads > 1 the
+    -fopenmp build of the same sources (outermost grid loops only, arithmetic unchanged); returns (value, seconds, zone_stages, threads)."""
     import oracle
     from paper_2510_13965_b200 import synth
+    threads = oracle.use_threads(threads)
     cfg = workload_inputs(cfg_name, n_sample)
     n = cfg["n"]
     o = oracle.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"], table=cfg.get("table"))
@@ -114,7 +128,27 @@ def oracle_leg(cfg_name, n_sample, steps):
         nst = len(w)
     sec = time.perf_counter() - t0
     zs = float(n[0] * n[1] * n[2] * nst * steps)
-    return zs / sec, sec, zs
+    oracle.use_threads(1)
+    return zs / sec, sec, zs, threads
+
+
+def falg_nonredundant(workload, eos_kind, nonatmo, pts_per_zone, nstages, m1):
+    """Algorithmic FP64 flops per zone and LAUNCH of each kernel class, every quantity counted once (FMA = 2): the itemised count of
+    SURVEY 8(d) (DESIGN.md section 6 lists the items). Nothing the kernels recompute for their own convenience is in here."""
+    d_first, d_second, d_mixed, d_adv, d_ko = 4.0, 7.0, 20.0, 9.0, 8.0          # flops of one stencil application (Eqs. 60-62, l.454-460)
+    deriv_centred = 48 * d_first + 33 * d_second + 33 * d_mixed                 # 16 fields x 3, 11 fields x (3 + 3)
+    ccz4_pointwise = 2750.0                                                     # Eqs. (13)-(26): Christoffels, Ricci (the Gamma~ Gamma~ sum alone ~1 k), D_i D_j alpha, RHS
+    grmhd_sources = 300.0                                                       # right-hand sides of Eq. (32) from the same derivatives
+    mp5 = 60.0 * 20.0                                                           # 60 reconstructions x Eq. (70) + the test of Eq. (72); the limiter (up to ~80 more) not claimed
+    splitting = 600.0                                                           # Eqs. (65), (69), (64) for 10 fields x 3 directions, lambda maxima
+    c2p = (2000.0 if eos_kind != 2 else 2000.0 + 10000.0) * nonatmo * pts_per_zone   # bracketed solve ~15 evaluations; table: + gathers / log10 / exp10 per evaluation
+    out = {"fill_ghosts": 0.0, "con2prim": c2p, "ccz4_algebra": deriv_centred + ccz4_pointwise + grmhd_sources,
+           "adv_ko": 66 * d_adv + 66 * d_ko, "point_flux": 500.0 * pts_per_zone,
+           "recon_x": (mp5 + splitting) / 3, "recon_y": (mp5 + splitting) / 3, "recon_z": (mp5 + splitting) / 3,
+           "rk_combine": 2.0 * 2.5 * 32,
+           # M1: closure root + fluxes ~2 k per species, implicit 4x4 Newton ~1 k per species and iteration (SURVEY: +6-8 k per zone-stage in all)
+           "m1_point": 3 * 1200.0 * pts_per_zone if m1 else 0.0, "m1_div": 3 * 500.0 if m1 else 0.0, "m1_implicit": 3 * 800.0 * pts_per_zone if m1 else 0.0}
+    return out
 
 
 def run_reference(args):
@@ -123,21 +157,23 @@ def run_reference(args):
         return
     n_s = args.ref_n
     vals = []
+    nthr = max(1, args.ref_threads)
     for _ in range(args.warmup):
-        oracle_leg(args.workload, 16, 1)
+        oracle_leg(args.workload, 16, 1, args.ref_threads)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        v, sec, zs = oracle_leg(args.workload, n_s, 1)
+        v, sec, zs, nthr = oracle_leg(args.workload, n_s, 1, args.ref_threads)
         vals.append((zs, sec))
     total = time.perf_counter() - t0
     value = sum(z for z, _ in vals) / sum(s for _, s in vals)
-    sample = "%d^3 crop-sized instance of workload %s, 1 RK4 step per bench step, single thread" % (n_s, args.workload)
+    sample = "%d^3 instance of workload %s, 1 RK step per bench step, %d thread(s)" % (n_s, args.workload, nthr)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "zone-stages/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s_%d" % (args.workload, args.n), "bounded_sample": sample},
-        "cpu_baseline": {"value": value, "unit": "zone-stages/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": dict({"value": value, "unit": "zone-stages/s", "cores": nthr, "kind": "oracle", "sample": sample,
+                              "pins": "oracle pinned except readings R1, R10, R17, R26 (unpinnable against the paper; DESIGN.md section 4)"}, **cpu_info()),
         "e2e": {"value": value, "unit": "zone-stages/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -151,6 +187,9 @@ def main():
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=40, help="sample size of the oracle legs")
+    ap.add_argument("--ref-threads", type=int, default=1, help="--impl reference: threads of the oracle (1 = the plain build)")
+    ap.add_argument("--decomp", default=None, help="e.g. 1x1x2: ONE patch split into bricks over the ranks, halo exchange fused with the ghost fill "
+                                                   "(strong scaling; needs world = product, or world 1 for the self-neighbour check); default: replicas")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -175,10 +214,29 @@ def main():
 
     cfg = workload_inputs(args.workload, args.n)
     n, ng = cfg["n"], cfg["ng"]
-    zones = n[0] * n[1] * n[2]
     m1 = "V" in cfg
     nstages = 3 if m1 else STAGES
+    grid = None
+    if args.decomp:                       # ONE patch of the workload's size split over the ranks (strong scaling)
+        from paper_2510_13965_b200 import decomp
+        grid = decomp.brick_grid(world, [int(x) for x in args.decomp.lower().split("x")])
+        box = decomp.local_box(rank, grid, n)
+        n_glob, n = n, tuple(hi - lo for lo, hi in box)
+        for key in ("U", "P", "V"):
+            if key in cfg:
+                cfg[key] = decomp.cut_local(cfg[key], rank, grid, n_glob, ng)
+    zones = n[0] * n[1] * n[2]
     patch = binding.Patch(cfg["params"], n, ng, cfg["dx"], stages=nstages, table=cfg.get("table"), device="cuda:%d" % local, m1=m1)
+    halo_imports = []
+    if grid is not None:
+        if world == 1:                    # one GPU: the brick is its own neighbour across z, with the epoch words of the multi-GPU protocol
+            for d in ((0, 0, 1), (0, 0, -1)):
+                for name, (slot, t) in decomp.state_slots(patch).items():
+                    binding.mhd_patch_set_neighbor(patch.h, slot, d, t.data_ptr(), patch.npts)
+                binding.mhd_patch_set_neighbor_word(patch.h, d, binding.mhd_patch_halo_words(patch.h))
+            cfg["bc"] = list(cfg["bc"][:4]) + [2, 2] if cfg["bc"][4] == 0 and cfg["bc"][5] == 0 else cfg["bc"]
+        else:
+            cfg["bc"], halo_imports = decomp.connect_distributed(patch, rank, grid, cfg["bc"])
     if m1:                              # config 5: IMEX(3,3,2) pair (R1), 3 stages per step
         tab = binding.make_tableau(*synth.imex_tableau())
         patch.V.copy_(torch.as_tensor(cfg["V"]))
@@ -227,23 +285,33 @@ def main():
 
     # ---- end to end through the host-buffer entry point (H2D of the state, advance, D2H of state + flags) ------
     e2e = None
-    if not args.no_e2e and not m1:
+    if not args.no_e2e:
         hostU = U_init.cpu().pin_memory()
+        hostV = V_init.cpu().pin_memory() if m1 else None
         hostF = torch.zeros(patch.flags.shape[1:], dtype=torch.uint8).pin_memory()
-        src = hostU.clone()
+        src, srcV = hostU.clone(), (hostV.clone() if m1 else None)
         e_steps = max(1, min(args.steps, 3))
-        patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)     # warm-up
+
+        def host_step():
+            if m1:
+                patch.advance_imex_host(tab, cfg["bc"], dt, 1, hostU, hostV, hostF)
+            else:
+                patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)
+        host_step()                                                  # warm-up
         hostU.copy_(src)
+        if m1:
+            hostV.copy_(srcV)
         barrier()
         t0 = time.perf_counter()
         for _ in range(e_steps):
-            patch.advance_host(tab, cfg["bc"], dt, 1, hostU, hostF)
+            host_step()
         torch.cuda.synchronize()
         sec = time.perf_counter() - t0
         sec = max_over_ranks(sec, device="cuda")
-        nbytes = hostU.numel() * 8
-        e2e = {"value": world * zones * STAGES * e_steps / sec, "unit": "zone-stages/s", "h2d_bytes_per_step": nbytes,
-               "d2h_bytes_per_step": nbytes + hostF.numel(), "steps": e_steps}
+        nbytes = hostU.numel() * 8 + (hostV.numel() * 8 if m1 else 0)
+        e2e = {"value": world * zones * nstages * e_steps / sec, "unit": "zone-stages/s", "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes + hostF.numel(), "steps": e_steps,
+               "entry_point": "mhd_advance_imex_host" if m1 else "mhd_advance_host"}
 
     if rank != 0:
         if world > 1:
@@ -251,10 +319,12 @@ def main():
         return
 
     # ---- roofline of the dominant kernel -----------------------------------------------
-    # The path is bound by the plain FP64 pipe ("alu"): F_alg = 21.6 kflop per zone-stage (operation-counting build of
-    # the oracle, tests/golden/op_counts.json) against 1.28 kB of algorithmic HBM traffic is 17 flop/B, the ridge of this
-    # GPU is 34 TFLOP/s / 6.5 TB/s = 5.2 flop/B. Peak = FP64 FMA throughput measured by the library's own register-
-    # resident DFMA probe (nominal 148 SMs x 64 lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s).
+    # The path is bound by the plain FP64 pipe ("alu"): ~11-13 kflop per zone-stage against 1.28 kB of algorithmic HBM traffic is ~9 flop/B,
+    # the ridge of this GPU is 34 TFLOP/s / 6.5 TB/s = 5.2 flop/B. Peak = FP64 FMA throughput measured by the library's own register-resident
+    # DFMA probe (nominal 148 SMs x 64 lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s).
+    # Numerator = ALGORITHMIC flops, every derivative, flux and symmetric component counted once (falg_nonredundant below, the itemised count of
+    # SURVEY 8(d) / DESIGN.md section 6), never more than what the kernel executed (ncu: DADD + DMUL + 2 DFMA thread instructions of the tracked
+    # capture profiles/r2_ncu_c4_128.json). The oracle's operation count (tests/golden/op_counts.json) is NOT used: the oracle recomputes on purpose.
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -262,61 +332,75 @@ def main():
         pass
     hbm_peak, hbm_src = (peaks["hbm_gbs"], "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
     fp64_peak = binding.mhd_probe_fp64_flops(patch.stream()) / 1e12
-    oc = json.load(open(os.path.join(ROOT, "tests", "golden", "op_counts.json")))[args.workload[:2]]
     pts_per_zone = patch.npts / zones
-    # algorithmic flops per zone and launch of each kernel class (the oracle's count of the step(s) the kernel performs)
-    alg_flops = {"fill_ghosts": 0.0, "con2prim": oc["con2prim_per_point"]["flops"] * pts_per_zone,
-                 "ccz4_algebra": oc["ccz4_per_zone"]["flops"] - oc["adv_ko_per_zone"]["flops"] + oc["grmhd_src_per_zone"]["flops"],
-                 "adv_ko": oc["adv_ko_per_zone"]["flops"], "point_flux": 0.0,
-                 "recon_x": oc["grmhd_flux_per_zone"]["flops"] / 3, "recon_y": oc["grmhd_flux_per_zone"]["flops"] / 3,
-                 "recon_z": oc["grmhd_flux_per_zone"]["flops"] / 3, "rk_combine": 2.5 * oc["rk_combine_per_zone_per_term"]["flops"],
-                 # M1: not claimed. The oracle re-solves the closure by plain bisection (~60 evaluations) at every node of every
-                 # line and direction, so its count (tests/golden/op_counts.json, c5) says nothing about the work needed
-                 "m1_point": 0.0, "m1_div": 0.0, "m1_implicit": 0.0}
+    nonatmo = 1.0 - status["n_atmo"] / status["n_points"]
+    alg_flops = falg_nonredundant(args.workload, cfg["params"]["eos_kind"], nonatmo, pts_per_zone, nstages, m1)
     # algorithmic doubles moved per zone and launch (reads + writes at the minimum)
     alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "ccz4_algebra": 22 + 10 + 5 + 32, "adv_ko": 22 * 3, "recon_x": 21 + 20,
                    "recon_y": 21 + 20, "recon_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33,
                    "m1_point": 21 + 15 + 75, "m1_div": 15 + 75 + 22 + 15, "m1_implicit": 21 + 15 + 30}
-    # measured DRAM traffic per zone and launch, bytes: dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture
-    # profiles/r1g_ncu_full_c4_128.md (128^3; per-zone figures carry over to 256^3, the tiles are the same)
-    ncu_traffic = {"ccz4_algebra": 592.9, "adv_ko": 634.2, "point_flux": 546.8, "recon_x": 332.2, "recon_y": 355.3, "recon_z": 359.7,
-                   "rk_combine": 802.8, "con2prim": 259.7, "fill_ghosts": 79.3}
-    # FP64 pipe utilisation of each kernel in the same capture (sm__inst_executed_pipe_fp64, % of peak): the executed-instruction
-    # view beside the algorithmic-flop view (the oracle's count includes work a fused kernel shares, so "frac" reads high)
-    ncu_fp64_busy = {"ccz4_algebra": 0.38, "adv_ko": 0.36, "point_flux": 0.28, "recon_x": 0.18, "recon_y": 0.31, "recon_z": 0.31,
-                     "rk_combine": 0.03, "con2prim": 0.26, "fill_ghosts": 0.0}
+    # ncu figures of the tracked capture (written by `python -m paper_2510_13965_b200.ncu_summary`; per-zone figures carry over to this size, the
+    # tiles are the same); null when the capture is of another workload class
+    cap, cap_meta = {}, None
+    try:
+        capj = json.load(open(os.path.join(ROOT, "profiles", "r2_ncu_c4_128.json")))
+        cap_meta = capj["meta"]
+        if not m1:
+            cap = capj["kernels"]
+    except Exception:
+        pass
     total_kernel_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_launches = prof[dom]
     sec_per_launch = dom_ms / max(dom_launches, 1) * 1e-3
-    achieved = alg_flops[dom] * zones / sec_per_launch / 1e12
-    F_alg = oc["per_zone_stage_flops"]
-    if m1:                              # conservative: the M1 steps add time but no claimed flops
-        F_alg -= oc["m1_implicit_per_point"]["flops"] * pts_per_zone + oc["m1_rhs_per_zone"]["flops"]
+    exe = {k: (cap[k]["executed_fp64_flops_per_zone"] if k in cap else None) for k in prof}
+    if not args.workload.startswith("c4"):
+        exe["con2prim"] = None               # the capture is of workload c4: its con2prim count (table EoS, 42 % star) does not carry over
+
+    def claimed(k):                         # algorithmic flops of class k per zone, capped by what the kernel executed
+        return min(alg_flops[k], exe[k]) if exe.get(k) is not None else alg_flops[k]
+    achieved = claimed(dom) * zones / sec_per_launch / 1e12
+    F_alg = sum(claimed(k) * (prof[k][1] / max(args.steps * nstages, 1)) for k in prof if prof[k][1] > 0)    # per zone-stage, launches per stage counted
+    F_exe = sum((exe[k] or 0.0) * (prof[k][1] / max(args.steps * nstages, 1)) for k in prof if prof[k][1] > 0) if cap else None
     step_tflops = F_alg * value / world / 1e12
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
                 "peak_source": "measured: FP64 DFMA probe of the library (mhd_probe_fp64_flops); nominal 37.2",
-                "traffic": ncu_traffic[dom] * zones if dom in ncu_traffic else None,
-                "traffic_source": "bytes per launch = ncu dram bytes per zone (profiles/r1g, 128^3 capture) x zones of this run",
-                "alg_bytes": alg_doubles[dom] * 8.0 * zones, "fp64_pipe_busy_ncu": ncu_fp64_busy.get(dom),
+                "numerator": "algorithmic flops, each derivative / flux / symmetric component once (bench.falg_nonredundant), capped by the executed DADD+DMUL+2*DFMA of the ncu capture",
+                "traffic": cap[dom]["dram_bytes_per_zone"] * zones if dom in cap else None,
+                "traffic_source": ("dram__bytes_read.sum + dram__bytes_write.sum per zone of the ncu --set full capture profiles/r2_ncu_c4_128.json (commit %s) x zones of this run"
+                                   % cap_meta["commit"]) if dom in cap else None,
+                "alg_bytes": alg_doubles[dom] * 8.0 * zones,
+                "fp64_pipe_busy_ncu": cap[dom]["fp64_pipe_pct"] / 100.0 if dom in cap and cap[dom]["fp64_pipe_pct"] is not None else None,
+                "executed_flops_per_zone_ncu": exe.get(dom),
                 "kernel_ms_per_launch": dom_ms / max(dom_launches, 1),
                 "share_of_step": dom_ms / total_kernel_ms if total_kernel_ms else None,
                 "alg_flops_per_zone": alg_flops[dom],
                 "hbm": {"achieved_gbs": alg_doubles[dom] * 8.0 * zones / sec_per_launch / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src},
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
-                "kernel_frac_of_fp64_peak": {k: (alg_flops[k] * zones / (v[0] / max(v[1], 1) * 1e-3) / 1e12 / fp64_peak if v[0] > 0 else None)
+                "kernel_frac_of_fp64_peak": {k: (claimed(k) * zones / (v[0] / max(v[1], 1) * 1e-3) / 1e12 / fp64_peak if v[0] > 0 else None)
                                              for k, v in prof.items()},
                 # whole step against the binding roof: T_bound = max(B_alg / BW, F_alg / P_fp64) per zone-stage
-                "step": {"alg_flops_per_zone_stage": F_alg, "alg_bytes_per_zone_stage": 1280, "achieved_tflops": step_tflops,
-                         "frac_of_fp64_peak": step_tflops / fp64_peak, "frac_of_hbm_peak": 1280.0 * value / world / 1e9 / hbm_peak,
-                         "binding": "alu"}}
+                "step": {"alg_flops_per_zone_stage": F_alg, "executed_flops_per_zone_stage_ncu": F_exe, "alg_bytes_per_zone_stage": 1280 if not m1 else 1880,
+                         "achieved_tflops": step_tflops, "frac_of_fp64_peak": step_tflops / fp64_peak,
+                         "frac_of_hbm_peak": (1280.0 if not m1 else 1880.0) * value / world / 1e9 / hbm_peak,
+                         "dram_bytes_per_zone_stage_ncu": sum(cap[k]["dram_bytes_per_zone"] for k in cap) if cap else None,
+                         "binding": "alu", "target": 0.5}}
 
     cpu = None
     if not args.no_cpu_baseline:
-        v, sec, zs = oracle_leg(args.workload, args.ref_n, 1)
-        cpu = {"value": v, "unit": "zone-stages/s", "cores": 1, "kind": "oracle",
-               "sample": "%d^3 instance of workload %s, 1 RK4 step (%.1f s), single thread" % (args.ref_n, args.workload, sec)}
+        v, sec, zs, _ = oracle_leg(args.workload, args.ref_n, 1)
+        nall = os.cpu_count() or 1
+        va, seca, _, nthr = oracle_leg(args.workload, args.ref_n, 1, threads=nall) if nall > 1 else (v, sec, zs, 1)
+        cpu = dict({"value": v, "unit": "zone-stages/s", "cores": 1, "kind": "oracle",
+                    "sample": "%d^3 instance of workload %s, 1 RK step (%.1f s), single thread" % (args.ref_n, args.workload, sec),
+                    "all_cores": {"value": va, "cores": nthr, "seconds": seca, "build": "-fopenmp on the outermost grid loops, arithmetic unchanged"},
+                    "pins": "oracle pinned except readings R1, R10, R17, R26 (unpinnable against the paper; DESIGN.md section 4)"}, **cpu_info())
 
+    bad = []
+    if status["n_fatal"] or status["n_noconv"]:
+        bad.append("n_fatal=%d n_noconv=%d after the timed region: the state left the method's domain of validity" % (status["n_fatal"], status["n_noconv"]))
+    if status.get("halo_timeout"):
+        bad.append("a halo wait expired")
     out = {
         "metric": METRIC, "value": value, "unit": "zone-stages/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -327,7 +411,16 @@ def main():
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(v[1] for v in prof.values())),
         "roofline": roofline, "cpu_baseline": cpu, "flags": {k: v for k, v in status.items() if k != "n_points"},
     }
+    if grid is not None:
+        out["scaling"] = "strong"
+        out["config"]["parallelism"] = "bricks %s, halo exchange fused with the ghost fill%s" % (
+            "x".join(str(g) for g in grid), " (one GPU: the brick is its own neighbour across z)" if world == 1 else "")
+    if bad:
+        out["invalid"] = "; ".join(bad)
     print(json.dumps(out))
+    if bad:
+        sys.stderr.write("bench.py: INVALID RUN: %s\n" % "; ".join(bad))
+        sys.exit(1)
     if world > 1:
         dist.destroy_process_group()
 

@@ -78,7 +78,7 @@ enum {
   MHD_E_ARG = -1,        /* null pointer / out-of-range argument            */
   MHD_E_UNBOUND = -2,    /* a slot needed by the call has not been bound    */
   MHD_E_CUDA = -3,       /* CUDA runtime error (launch, copy, allocation)   */
-  MHD_E_UNSUPPORTED = -4 /* feature not built (e.g. n_species != 0)         */
+  MHD_E_UNSUPPORTED = -4 /* not supported: n_species other than 0 or 3, an M1 call on a patch without species */
 };
 
 /* Plain data, copied at create time. Pointers inside are DEVICE pointers that must outlive the patch. */
@@ -249,6 +249,11 @@ int mhd_restrict(mhd_patch *fine, int slot_f, mhd_patch *coarse, int slot_c, con
  * them. slot_out: any state slot but U0 and the K_j used. mhd_dense_weights returns the number of stages and b_j (host, no device work). */
 int mhd_dense_weights(int scheme, double theta, int deriv, double b[4]);
 int mhd_dense_output(mhd_patch *p, int scheme, double theta, double dt, int deriv, int slot_out, void *cuda_stream);
+
+/* Same, end to end with HOST buffers (packed, field_stride = MX*MY*MZ): host_U (MHD_NSTATE fields) and host_V (MHD_NM1 fields) are
+ * copied to slots U and V, advanced, copied back together with the flags (host_flags may be NULL); synchronises the stream. */
+int mhd_advance_imex_host(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, double *host_U, double *host_V,
+                          uint8_t *host_flags, void *cuda_stream);
 
 /* Counts flag bits over all grid points of slot_flags. Synchronises the stream. */
 int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_stream);

@@ -60,7 +60,7 @@ EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patc
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
            "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex",
            "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output",
-           "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
+           "mhd_advance_imex_host", "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
 NKERNELS = 12
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
                   "m1_point", "m1_div", "m1_implicit"]
@@ -99,6 +99,7 @@ def lib():
         L.mhd_m1_gravity.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
+        L.mhd_advance_imex_host.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p, _p, _p, _p]
         L.mhd_patch_set_neighbor.argtypes = [_p, _i, ctypes.POINTER(_i), _p, ctypes.c_size_t]
         L.mhd_patch_halo_words.argtypes = [_p]
         L.mhd_patch_halo_words.restype = _p
@@ -288,6 +289,10 @@ def mhd_dense_output(h, scheme, theta, dt, deriv, slot_out, stream=None):
     _check(lib().mhd_dense_output(h, scheme, theta, dt, deriv, slot_out, stream))
 
 
+def mhd_advance_imex_host(h, tableau, bc, dt, n_steps, host_U_ptr, host_V_ptr, host_flags_ptr=None, stream=None):
+    _check(lib().mhd_advance_imex_host(h, ctypes.byref(tableau), _bc(bc), dt, n_steps, host_U_ptr, host_V_ptr, host_flags_ptr, stream))
+
+
 def mhd_patch_status(h, slot_flags=SLOT_FLAGS, stream=None):
     st = mhd_status()
     _check(lib().mhd_patch_status(h, slot_flags, ctypes.byref(st), stream))
@@ -415,6 +420,10 @@ class Patch:
         """host_U: pinned CPU float64 tensor (NSTATE, MZ, MY, MX), updated in place; host_flags: uint8 tensor or None."""
         mhd_advance_host(self.h, tableau, bc, dt, n_steps, host_U.data_ptr(),
                          None if host_flags is None else host_flags.data_ptr(), self.stream())
+
+    def advance_imex_host(self, tableau, bc, dt, n_steps, host_U, host_V, host_flags=None):
+        mhd_advance_imex_host(self.h, tableau, bc, dt, n_steps, host_U.data_ptr(), host_V.data_ptr(),
+                              None if host_flags is None else host_flags.data_ptr(), self.stream())
 
     def profile(self, enable):
         mhd_patch_profile(self.h, enable)

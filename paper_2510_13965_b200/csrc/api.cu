@@ -146,6 +146,8 @@ int stage_sequence(mhd_patch* p, const mhd_tableau* t, const int bc[6], double d
 
 extern "C" {
 
+int mhd_advance_imex(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, void* stream);
+
 size_t mhd_desc_sizeof(void) { return sizeof(mhd_patch_desc); }
 
 int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
@@ -372,6 +374,31 @@ int mhd_advance(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, 
   return stage_sequence(p, t, bc, dt, n_steps, (cudaStream_t)stream);
 }
 
+// packed host array <-> slot (field stride of the slot may exceed the packed one)
+static bool copy_fields(double* dst, size_t sd, const double* src, size_t ss, int nfields, size_t n, cudaMemcpyKind kind, cudaStream_t s) {
+  if (sd == n && ss == n) return cudaMemcpyAsync(dst, src, n * nfields * sizeof(double), kind, s) == cudaSuccess;
+  for (int f = 0; f < nfields; ++f)
+    if (cudaMemcpyAsync(dst + f * sd, src + f * ss, n * sizeof(double), kind, s) != cudaSuccess) return false;
+  return true;
+}
+
+int mhd_advance_imex_host(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, double* host_U, double* host_V,
+                          uint8_t* host_flags, void* stream) {
+  if (!p || !t || !bc || !host_U || !host_V || n_steps < 0) return MHD_E_ARG;
+  if (p->desc.n_species != 3) return MHD_E_UNSUPPORTED;
+  if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_V) || !slot_ok(p, MHD_SLOT_FLAGS)) return MHD_E_UNBOUND;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n = (size_t)p->dims.npts;
+  if (!copy_fields(dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, host_U, n, MHD_NSTATE, n, cudaMemcpyHostToDevice, s)) return MHD_E_CUDA;
+  if (!copy_fields(dptr(p, MHD_SLOT_V), p->slot[MHD_SLOT_V].stride, host_V, n, MHD_NM1, n, cudaMemcpyHostToDevice, s)) return MHD_E_CUDA;
+  const int rc = mhd_advance_imex(p, t, bc, dt, n_steps, stream);
+  if (rc != MHD_OK) return rc;
+  if (!copy_fields(host_U, n, dptr(p, MHD_SLOT_U), p->slot[MHD_SLOT_U].stride, MHD_NSTATE, n, cudaMemcpyDeviceToHost, s)) return MHD_E_CUDA;
+  if (!copy_fields(host_V, n, dptr(p, MHD_SLOT_V), p->slot[MHD_SLOT_V].stride, MHD_NM1, n, cudaMemcpyDeviceToHost, s)) return MHD_E_CUDA;
+  if (host_flags && cudaMemcpyAsync(host_flags, p->slot[MHD_SLOT_FLAGS].ptr, n, cudaMemcpyDeviceToHost, s) != cudaSuccess) return MHD_E_CUDA;
+  return cudaStreamSynchronize(s) == cudaSuccess ? MHD_OK : MHD_E_CUDA;
+}
+
 int mhd_advance_host(mhd_patch* p, const mhd_tableau* t, const int bc[6], double dt, int n_steps, double* host_U, uint8_t* host_flags, void* stream) {
   if (!p || !t || !bc || !host_U || n_steps < 0) return MHD_E_ARG;
   if (!slot_ok(p, MHD_SLOT_U) || !slot_ok(p, MHD_SLOT_FLAGS)) return MHD_E_UNBOUND;
@@ -588,6 +615,13 @@ int mhd_patch_status(mhd_patch* p, int slot_flags, mhd_status* out, void* stream
 int mhd_patch_profile(mhd_patch* p, int enable) {
   if (!p) return MHD_E_ARG;
   p->profiling = enable != 0;
+  // events are created here, outside any timed region: enough pairs for a few RK steps of the longest stage sequence
+  while (enable && p->pool.size() < 256) {
+    mhd_patch::Ev ev;
+    if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess) return MHD_E_CUDA;
+    ev.cls = 0;
+    p->pool.push_back(ev);
+  }
   return MHD_OK;
 }
 
