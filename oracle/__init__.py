@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SOURCES = ["orc_stencil.cpp", "orc_eos.cpp", "orc_c2p.cpp", "orc_ccz4.cpp", "orc_grmhd.cpp",
-            "orc_rk.cpp", "orc_m1.cpp", "orc_m1_patch.cpp", "orc_amr.cpp", "orc_capi.cpp"]
+            "orc_rk.cpp", "orc_m1.cpp", "orc_m1_patch.cpp", "orc_amr.cpp", "orc_les.cpp", "orc_capi.cpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 NSTATE, NPRIM = 32, 10
@@ -148,6 +148,9 @@ def _load(counting):
         L.orc_m1_backreaction.argtypes = [vp, vp, vp, vp, vp]
         L.orc_m1_gravity.argtypes = [vp, vp, vp, vp, vp]
         L.orc_evolve_imex.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, f64, i32]
+        L.orc_les_flux.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_les_HM_point.argtypes = [vp, vp, vp, f64, vp]
+        L.orc_les_aux_point.argtypes = [vp, vp, f64, vp, vp, vp]
         L.orc_prolong.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp]
         L.orc_restrict.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp]
         L.orc_dense_weights.argtypes = [i32, f64, i32, vp]
@@ -386,3 +389,34 @@ def _dense_output(self, U0, Ks, scheme, theta, dt, deriv=0):
 
 
 Oracle.dense_output = _dense_output
+
+
+# ---- LES gradient SGS term of the induction equation (App. A) ------------------------------------------
+LES_NAUX = 26
+LES_NAMES = ["Bu0", "Bu1", "Bu2", "vu0", "vu1", "vu2", "vl0", "vl1", "vl2", "Bl0", "Bl1", "Bl2", "El0", "El1", "El2", "Eu0", "Eu1", "Eu2",
+             "vB", "Theta", "Wm2", "rho", "eps", "h", "dpdrho", "dpdeps"]
+
+
+def les_HM_point(a, da, gu, p):
+    """H_M^{ki} (first index = flux direction) from the 26 auxiliary fields a, their partial derivatives da[m][f], gamma^{ij}, pressure"""
+    out = np.zeros(9)
+    lib().orc_les_HM_point(_ptr(_f64(a)), _ptr(_f64(da)), _ptr(_f64(gu)), float(p), _ptr(out))
+    return out.reshape(3, 3)
+
+
+def _les_aux_point(self, gl, sqrtg, Bu, prim):
+    out = np.zeros(LES_NAUX)
+    lib().orc_les_aux_point(self.h, _ptr(_f64(gl)), float(sqrtg), _ptr(_f64(Bu)), _ptr(_f64(prim)), _ptr(out))
+    return out
+
+
+def _les_flux(self, U, P):
+    """(L, A): L[3 k + i] = -alpha G_B^{ki}, the SGS part of the k-flux of Bbar^i (zero within 2 points of the array edge); A = auxiliary fields"""
+    L = np.zeros((9,) + self.shape)
+    A = np.zeros((LES_NAUX,) + self.shape)
+    lib().orc_les_flux(self.h, _ptr(U), _ptr(P), _ptr(L), _ptr(A))
+    return L, A
+
+
+Oracle.les_aux_point = _les_aux_point
+Oracle.les_flux = _les_flux

@@ -124,6 +124,15 @@ void orc_evolve_imex(void* hh, double* U, double* V, double* P, uint8_t* flags, 
   evolve_imex(h->par, h->grid, U, V, P, flags, bc, stages, ae, we, ai, wi, dt, n_steps);
 }
 
+// ---- LES (App. A)
+void orc_les_flux(void* hh, const double* U, const double* P, double* L9, double* A26) { Handle* h = (Handle*)hh; les_flux(h->par, h->grid, U, P, L9, A26); }
+void orc_les_HM_point(const double* a26, const double* da3x26, const double* gu9, double p, double* HM9) {
+  les_HM_point(a26, (const double (*)[LES_NAUX])da3x26, (const double (*)[3])gu9, p, (double (*)[3])HM9);
+}
+void orc_les_aux_point(void* hh, const double* gl9, double sqrtg, const double* Bu, const double* prim, double* a26) {
+  les_aux_point(((Handle*)hh)->par, (const double (*)[3])gl9, sqrtg, Bu, prim, a26);
+}
+
 // ---- AMR transfer operators (grids passed explicitly: n[3], ng)
 static Grid mkgrid(const int* n, int ng) { return Grid{n[0], n[1], n[2], ng, 1.0, 1.0, 1.0}; }
 void orc_prolong(const int* nc, int ngc, const double* Uc, const int* nf, int ngf, double* Uf, int nfields, const int* origin, const int* lo, const int* hi) {

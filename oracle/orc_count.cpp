@@ -71,6 +71,9 @@ using orc_cnt::Cnt;
 #include "orc_m1.cpp"
 #include "orc_m1_patch.cpp"
 #include "orc_amr.cpp"
+#define SYM SYM_les_unit
+#include "orc_les.cpp"
+#undef SYM
 #include "orc_capi.cpp"
 #undef double
 

@@ -89,6 +89,23 @@ static TabPos tab_T_from_loge(const Params& par, TabPos r, TabPos y, double le) 
   return {it, (le - e_lo) / (e_hi - e_lo)};
 }
 
+// dp/drho at fixed eps and dp/deps at fixed rho (App. A, l.882: "analytically for hybrid EoSs, but only numerically for the tabulated ones")
+void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps) {
+  if (par.eos_kind == 0) { dpdrho = (par.eos_gamma - 1.0) * eps; dpdeps = (par.eos_gamma - 1.0) * rho; return; }
+  if (par.eos_kind == 1) {
+    // p = p_cold + (Gamma_th - 1) rho (eps - eps_cold) (Eq. 30), d p_cold / d rho = Gamma_i p_cold / rho, d eps_cold / d rho = p_cold / rho^2
+    double pc, ec, G;
+    pp_cold(par, rho, pc, ec, G);
+    const double gth = par.eos_gamma_th - 1.0;
+    dpdrho = G * pc / rho + gth * (eps - ec) - gth * pc / rho;
+    dpdeps = gth * rho;
+    return;
+  }
+  const double hr = 1e-4 * rho, he = 1e-4 * (std::fabs(eps) + 1e-10);
+  dpdrho = (eos_from_rho_eps(par, rho + hr, eps, ye).p - eos_from_rho_eps(par, rho - hr, eps, ye).p) / (2.0 * hr);
+  dpdeps = (eos_from_rho_eps(par, rho, eps + he, ye).p - eos_from_rho_eps(par, rho, eps - he, ye).p) / (2.0 * he);
+}
+
 EosOut eos_from_rho_eps(const Params& par, double rho, double eps, double ye) {
   EosOut o;
   if (par.eos_kind == 0) {

@@ -110,6 +110,12 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
   for (int kk = ng; kk < G.nz + ng; ++kk) for (int jj = ng; jj < G.ny + ng; ++jj) for (int ii = ng; ii < G.nx + ng; ++ii)
     for (int a = 0; a < 10; ++a) K[(size_t)(DBAR + a) * n + G.idx(ii, jj, kk)] = 0.0;
 
+  // ---- LES: the sub-grid-scale tensor of the induction equation is part of the flux bracket of Eq. (32) (App. A; orc_les.cpp)
+  std::vector<double> Lsgs, Laux;
+  if (par.les_C_M != 0.0 && (parts & 1)) {
+    Lsgs.resize(9 * n); Laux.resize((size_t)LES_NAUX * n);
+    les_flux(par, G, U, P, Lsgs.data(), Laux.data());
+  }
   // ---- flux divergence, direction by direction, line by line (Eqs. 64-69)
   for (int d = 0; d < 3 && (parts & 1); ++d) {
     const int d1_ = (d + 1) % 3, d2_ = (d + 2) % 3;
@@ -125,6 +131,7 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
         load_point(G, U, P, base + (size_t)i * st[d], q);
         double F[10];
         flux_point(par, q, d, F, sp[i]);
+        if (!Lsgs.empty()) for (int c3 = 0; c3 < 3; ++c3) F[6 + c3] += Lsgs[(size_t)(3 * d + c3) * n + base + (size_t)i * st[d]];   // - alpha G_B^{d c3}
         for (int f = 0; f < 10; ++f) { Fp[f * Md + i] = F[f]; Uc[f * Md + i] = q.uc[f]; }
       }
       // interfaces i+1/2 for i = ng-1 .. ng+N-1

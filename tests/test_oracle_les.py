@@ -1,0 +1,243 @@
+"""Pins of the oracle's LES gradient sub-grid-scale term (App. A, Eqs. A11-A17).
+
+The appendix states the model itself: tau_F^k = -xi grad(dF^k/dC)|_C . grad C (l.822), i.e. the SGS tensor of the induction equation
+is  H^{ki} = sum_ab  d2 F^{ki} / dC_a dC_b  (grad C_a . grad C_b)  with F^{ki}(C) = B^i v^k(C) - B^k v^i(C) and C the conserved
+fields. The first pin evaluates that definition directly — the Hessian of the flux through an independent multi-precision
+conserved-to-primitive solve (mpmath) — and requires the oracle's transcription of the closed forms (A12)-(A16) to equal it. That
+fixes every reading of the appendix's undefined symbols (Theta, calE, E, h), every sign and factor of (A12)-(A16) and the index order
+of H_M^{ki}. Further pins: covariance under a constant rescaling of the metric (index placement, sqrt(gamma) in E), the factors
+alpha C_M xi sqrt(gamma) of (A11), fourth-order convergence of the grid routine, xi ~ Delta^2, and the place of the term in Eq. (32)."""
+import math
+import random
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+from paper_2510_13965_b200 import synth
+
+
+# ------------------------------------------------------------------ the definition, in multi-precision (independent of oracle/)
+def _cons(P, eos):
+    rho, eps, v, B = P[0], P[1], P[2:5], P[5:8]
+    p = eos(rho, eps)
+    v2 = sum(x * x for x in v); B2 = sum(x * x for x in B); vB = sum(a * b for a, b in zip(v, B))
+    W2 = 1 / (1 - v2)
+    h = rho * (1 + eps) + p                                                   # enthalpy density, l.232
+    D = rho * mp.sqrt(W2)
+    S = [(h * W2 + B2) * v[i] - vB * B[i] for i in range(3)]                   # Eq. (29)
+    tau = h * W2 - p + B2 - (vB ** 2 + B2 / W2) / 2 - D
+    return [D] + S + [tau] + list(B)
+
+
+def _flux(C, guess, eos):
+    B = C[5:8]
+
+    def f(rho, eps, v1, v2, v3):
+        c = _cons([rho, eps, v1, v2, v3] + list(B), eos)
+        return [c[i] - C[i] for i in range(5)]
+    sol = mp.findroot(f, guess[:5], tol=mp.mpf(10) ** -32, maxsteps=60)
+    v = [sol[2], sol[3], sol[4]]
+    return [[B[i] * v[k] - B[k] * v[i] for i in range(3)] for k in range(3)]    # F[k][i]: k-flux of B^i
+
+
+def _hessian_contraction(P0, gradP, eos):
+    mp.mp.dps = 36
+    P0 = [mp.mpf(x) for x in P0]
+    gradP = [[mp.mpf(x) for x in row] for row in gradP]
+    d = mp.mpf(10) ** -12
+    J = [[None] * 8 for _ in range(8)]
+    for q in range(8):
+        Pp, Pm = list(P0), list(P0)
+        Pp[q] += d; Pm[q] -= d
+        cp, cm = _cons(Pp, eos), _cons(Pm, eos)
+        for a in range(8):
+            J[a][q] = (cp[a] - cm[a]) / (2 * d)
+    gradC = [[sum(J[a][q] * gradP[m][q] for q in range(8)) for a in range(8)] for m in range(3)]
+    dotC = [[sum(gradC[m][a] * gradC[m][b] for m in range(3)) for b in range(8)] for a in range(8)]
+    C0 = _cons(P0, eos)
+    dd = mp.mpf(10) ** -8
+    cache = {}
+
+    def at(sa, a, sb, b):
+        key = (sa, a, sb, b) if (a, sa) <= (b, sb) else (sb, b, sa, a)
+        if key not in cache:
+            C = list(C0)
+            C[a] += sa * dd; C[b] += sb * dd
+            cache[key] = _flux(C, P0, eos)
+        return cache[key]
+    H = np.zeros((3, 3))
+    for a in range(8):
+        for b in range(8):
+            pp, pm, mp_, mm = at(1, a, 1, b), at(1, a, -1, b), at(-1, a, 1, b), at(-1, a, -1, b)
+            for k in range(3):
+                for i in range(3):
+                    H[k, i] += float((pp[k][i] - pm[k][i] - mp_[k][i] + mm[k][i]) / (4 * dd * dd) * dotC[a][b])
+    return H
+
+
+def _aux_and_gradients(o, par, P0, gradP, gl, sqrtg):
+    """oracle auxiliary fields at P0 = (rho, eps, v^i, B^i) and their gradients by the chain rule (central differences of the oracle's
+    own les_aux_point in the primitives)"""
+    def aux(P):
+        rho, eps, v, B = P[0], P[1], P[2:5], P[5:8]
+        vl = gl @ np.array(v)
+        W = 1.0 / math.sqrt(1.0 - float(vl @ np.array(v)))
+        prim = np.zeros(10)
+        prim[0], prim[1], prim[2], prim[4:7], prim[7] = rho, 0.3, eps, v, W
+        prim[3] = o.eos(rho, eps)[0]
+        return o.les_aux_point(gl, sqrtg, B, prim), prim[3]
+    a0, p0 = aux(P0)
+    da = np.zeros((3, 26))
+    for q in range(8):
+        h = 1e-6 * max(1.0, abs(P0[q]))
+        Pp, Pm = list(P0), list(P0)
+        Pp[q] += h; Pm[q] -= h
+        der = (aux(Pp)[0] - aux(Pm)[0]) / (2 * h)
+        for m in range(3):
+            da[m] += der * gradP[m][q]
+    return a0, da, p0
+
+
+@pytest.mark.parametrize("seed,kind", [(1, 0), (2, 0), (3, 0), (4, 1), (5, 1)])
+def test_HM_equals_the_gradient_model_it_is_derived_from(oracle_mod, seed, kind):
+    """(A12)-(A16) as transcribed == sum_ab d2F^{ki}/dC_a dC_b grad C_a . grad C_b (flat space; ideal gas and hybrid EoS).
+    Mutations this catches: any wrong sign / factor / index in (A12)-(A16), Theta or calE or E or h read differently, enthalpy
+    taken as specific, H_M^{ik} instead of H_M^{ki}, dp/drho and dp/deps swapped."""
+    rnd = random.Random(seed)
+    P0 = [rnd.uniform(0.5, 1.5), rnd.uniform(0.1, 1.0)] + [rnd.uniform(-0.4, 0.4) for _ in range(3)] + [rnd.uniform(-0.8, 0.8) for _ in range(3)]
+    gradP = [[rnd.uniform(-1, 1) for _ in range(8)] for _ in range(3)]
+    if kind == 0:
+        gam = 2.0 if seed != 3 else 5.0 / 3.0
+        par = synth.default_params(eos_kind=0, eos_gamma=gam)
+        eos = lambda rho, eps: (mp.mpf(gam) - 1) * rho * eps
+    else:
+        K, G, gth = 0.7, 2.5, 1.6
+        par = synth.default_params(eos_kind=1, eos_gamma_th=gth, n_pieces=1, pp_K=[K], pp_Gamma=[G], pp_rho=[1e300])
+        eos = lambda rho, eps: K * rho ** mp.mpf(G) + (mp.mpf(gth) - 1) * rho * (eps - K * rho ** (mp.mpf(G) - 1) / (mp.mpf(G) - 1))
+    o = oracle_mod.Oracle(par, 4, 4, 4, 3, 0.1)
+    want = _hessian_contraction(P0, gradP, eos)
+    a0, da, p0 = _aux_and_gradients(o, par, P0, gradP, np.eye(3), 1.0)
+    got = oracle_mod.les_HM_point(a0, da, np.eye(3), p0)
+    assert np.abs(got - want).max() < 2e-6 * np.abs(want).max(), (got, want)
+    assert np.abs(got + got.T).max() < 1e-12 * np.abs(got).max()              # antisymmetric
+
+
+def test_HM_is_covariant_under_a_constant_rescaling_of_the_metric(oracle_mod):
+    """gamma_ij = a^2 delta_ij is flat space in coordinates x' = a x: components v^k = v'^k / a, v_k = a v'_k, d_m = a d'_m, and a tensor
+    with two upper indices obeys H^{ki} = H'^{ki} / a^2. Catches a missing / misplaced metric factor: gamma^{mn} in the dot products,
+    an upper component where a lower one belongs (and vice versa) in (A12), sqrt(gamma) in E^i = -eps^{ijk} v_j B_k."""
+    rnd = random.Random(11)
+    par = synth.default_params(eos_kind=0, eos_gamma=2.0)
+    o = oracle_mod.Oracle(par, 4, 4, 4, 3, 0.1)
+    P0 = [rnd.uniform(0.5, 1.5), rnd.uniform(0.1, 1.0)] + [rnd.uniform(-0.4, 0.4) for _ in range(3)] + [rnd.uniform(-0.8, 0.8) for _ in range(3)]
+    gradP = [[rnd.uniform(-1, 1) for _ in range(8)] for _ in range(3)]
+    a0, da, p0 = _aux_and_gradients(o, par, P0, gradP, np.eye(3), 1.0)
+    flat = oracle_mod.les_HM_point(a0, da, np.eye(3), p0)
+    a = 1.7
+    # the same physical state in the coordinates with gamma_ij = a^2 delta_ij: upper components / a, d_m = a d'_m
+    Pc = list(P0)
+    for q in range(2, 8):
+        Pc[q] = P0[q] / a
+    gradPc = [[gradP[m][q] * a / (a if q >= 2 else 1.0) for q in range(8)] for m in range(3)]
+    ac, dac, pc = _aux_and_gradients(o, par, Pc, gradPc, a * a * np.eye(3), a ** 3)
+    curved = oracle_mod.les_HM_point(ac, dac, np.eye(3) / a ** 2, pc)
+    assert np.abs(curved - flat / a ** 2).max() < 1e-7 * np.abs(flat).max() / a ** 2
+
+
+def _smooth_state(n, ng, L=1.0, chi0=1.0, alpha0=1.0):
+    """flat conformal metric with constant chi and lapse; analytic smooth primitives on a periodic box"""
+    dx = L / n
+    X, Y, Z = synth.mesh(n, n, n, ng, dx)
+    k = 2 * math.pi / L
+    U = np.zeros((32,) + X.shape)
+    U[0] = U[3] = U[5] = 1.0
+    U[12] = chi0
+    U[18] = alpha0
+    prim = lambda x, y, z: np.array([1.0 + 0.2 * np.sin(k * x) * np.cos(k * y), 0.5 + 0.1 * np.cos(k * z + 0.3), 0.2 * np.sin(k * y + 0.1), 0.15 * np.cos(k * (x + z)),
+                                     -0.1 * np.sin(k * (x - y)), 0.5 + 0.2 * np.cos(k * y), 0.3 * np.sin(k * z + 0.7), 0.4 + 0.1 * np.sin(k * (x + y + z))])
+    Pv = prim(X, Y, Z)
+    P = np.zeros((10,) + X.shape)
+    P[0], P[1], P[2] = Pv[0], 0.3, Pv[1]
+    P[4:7] = Pv[2:5]
+    sg = chi0 ** -1.5
+    for i in range(3):
+        U[28 + i] = sg * Pv[5 + i]
+    return U, P, dx, prim, k
+
+
+def test_grid_routine_factors_convergence_and_delta_squared(oracle_mod):
+    """les_flux on a periodic grid against les_HM_point fed with ANALYTIC gradients, in a metric gamma_ij = delta_ij / chi0 with lapse
+    alpha0: L^{ki} -> alpha0 C_M (Delta^2 / (24 chi0)) chi0^(-3/2) H_M^{ki} at fourth order (Eq. 60), which also pins (A11)'s
+    alpha, C_M, xi = gamma^{1/3} Delta^2 / 24 and sqrt(gamma); the same fields on a grid twice as fine give a term four times smaller
+    ("vanishing SGS terms for an infinite resolution", l.863); L is antisymmetric, linear in C_M and zero for a uniform state."""
+    chi0, al0, CM = 0.8, 0.9, 8.0
+    par = synth.default_params(eos_kind=0, eos_gamma=2.0, les_C_M=CM)
+    errs, mags = [], []
+    for n in (16, 32):
+        ng = 5
+        U, P, dx, prim, k = _smooth_state(n, ng, chi0=chi0, alpha0=al0)
+        o = oracle_mod.Oracle(par, n, n, n, ng, dx)
+        o.prim2con(U, P)
+        L, A = o.les_flux(U, P)
+        assert np.abs(L + L.reshape(3, 3, *L.shape[1:]).transpose(1, 0, 2, 3, 4).reshape(L.shape)).max() < 1e-13 * np.abs(L).max()
+        # one probe point (interior index (3, 5, 2) of the coarse grid, the same physical point on the fine grid)
+        f = n // 16
+        ii, jj, kk = 3 * f + ng, 5 * f + ng, 2 * f + ng
+        x, y, z = (ii - ng) * dx, (jj - ng) * dx, (kk - ng) * dx
+        h = 1e-5
+        P0 = prim(x, y, z)
+        gradP = [(prim(x + h * (m == 0), y + h * (m == 1), z + h * (m == 2)) - prim(x - h * (m == 0), y - h * (m == 1), z - h * (m == 2))) / (2 * h) for m in range(3)]
+        gl = np.eye(3) / chi0
+        a0, da, p0 = _aux_and_gradients(o, par, list(P0), gradP, gl, chi0 ** -1.5)
+        HM = oracle_mod.les_HM_point(a0, da, chi0 * np.eye(3), p0)
+        want = al0 * CM * dx * dx / (24.0 * chi0) * chi0 ** -1.5 * HM
+        got = L[:, kk, jj, ii].reshape(3, 3)
+        errs.append(np.abs(got / dx ** 2 - want / dx ** 2).max())
+        mags.append(np.abs(got).max())
+        assert np.abs(A[:, kk, jj, ii] - a0).max() < 1e-13
+        # within 2 points of the array edge the stencil does not fit: zero there
+        assert np.all(L[:, :2] == 0) and np.all(L[:, :, :, -2:] == 0) and np.any(L[:, 2] != 0)
+    assert errs[1] < errs[0] / 12.0 and errs[1] < 1e-3 * mags[1] / (1.0 / 32) ** 2, errs        # fourth order
+    assert 3.5 < mags[0] / mags[1] < 4.5, mags                                                    # ~ Delta^2
+    # linear in C_M, zero for a uniform state
+    n, ng = 8, 5
+    U, P, dx, prim, k = _smooth_state(n, ng)
+    o1 = oracle_mod.Oracle(dict(par, les_C_M=1.0), n, n, n, ng, dx)
+    o8 = oracle_mod.Oracle(par, n, n, n, ng, dx)
+    o1.prim2con(U, P)
+    L1, _ = o1.les_flux(U, P)
+    L8, _ = o8.les_flux(U, P)
+    assert np.allclose(8.0 * L1, L8, rtol=1e-14, atol=0)
+    for f in (0, 2, 4, 5, 6):
+        P[f] = P[f, 0, 0, 0]
+    for f in range(28, 31):
+        U[f] = U[f, 0, 0, 0]
+    o8.prim2con(U, P)
+    L0, _ = o8.les_flux(U, P)
+    assert np.abs(L0).max() == 0.0
+
+
+def test_the_term_sits_inside_the_flux_bracket_of_eq32(oracle_mod):
+    """rhs(C_M) - rhs(0) for Bbar^i = -d_k (-alpha G_B^{ki}) up to the truncation error of the flux-split reconstruction on smooth data;
+    no other field changes. Catches: the term added to the wrong field / direction, with the wrong sign, or after the divergence."""
+    n, ng = 24, 5
+    par = synth.default_params(eos_kind=0, eos_gamma=2.0, les_C_M=8.0, grav_G=0.0)
+    U, P, dx, prim, k = _smooth_state(n, ng)
+    o8 = oracle_mod.Oracle(par, n, n, n, ng, dx)
+    o0 = oracle_mod.Oracle(dict(par, les_C_M=0.0), n, n, n, ng, dx)
+    o8.prim2con(U, P)
+    o8.fill_ghosts(U, [0] * 6)
+    Pq, _ = o8.con2prim(U)
+    K8, K0 = o8.rhs(U, Pq, part="grmhd_flux"), o0.rhs(U, Pq, part="grmhd_flux")
+    L, _ = o8.les_flux(U, Pq)
+    dK = K8 - K0
+    assert np.abs(dK[:28]).max() == 0.0 and np.abs(dK[31]).max() == 0.0
+    inner = (slice(ng, -ng),) * 3
+    for i in range(3):
+        div = np.zeros_like(L[0])
+        for kdir, ax in ((0, 2), (1, 1), (2, 0)):
+            F = L[3 * kdir + i]
+            div += (8.0 * (np.roll(F, -1, ax) - np.roll(F, 1, ax)) - (np.roll(F, -2, ax) - np.roll(F, 2, ax))) / (12.0 * dx)
+        got, want = dK[28 + i][inner], -div[inner]
+        assert np.abs(got - want).max() < 0.02 * np.abs(want).max(), (i, np.abs(got - want).max(), np.abs(want).max())
