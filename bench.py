@@ -147,6 +147,7 @@ def falg_nonredundant(workload, eos_kind, nonatmo, pts_per_zone, nstages, m1):
            "recon_x": (mp5 + splitting) / 3, "recon_y": (mp5 + splitting) / 3, "recon_z": (mp5 + splitting) / 3,
            "rk_combine": 2.0 * 2.5 * 32,
            # M1: closure root + fluxes ~2 k per species, implicit 4x4 Newton ~1 k per species and iteration (SURVEY: +6-8 k per zone-stage in all)
+           "les": (26 * 3 * 4 + 36 * 5 + 300 + 150) * pts_per_zone,              # 78 gradients, 36 contracted products, (A12)-(A16), auxiliary fields
            "m1_point": 3 * 1200.0 * pts_per_zone if m1 else 0.0, "m1_div": 3 * 500.0 if m1 else 0.0, "m1_implicit": 3 * 800.0 * pts_per_zone if m1 else 0.0}
     return out
 
@@ -338,7 +339,7 @@ def main():
     # algorithmic doubles moved per zone and launch (reads + writes at the minimum)
     alg_doubles = {"fill_ghosts": 0.0, "con2prim": 18 + 16, "ccz4_algebra": 22 + 10 + 5 + 32, "adv_ko": 22 * 3, "recon_x": 21 + 20,
                    "recon_y": 21 + 20, "recon_z": 21 + 20, "rk_combine": 3.75 * 32, "point_flux": 29 + 33,
-                   "m1_point": 21 + 15 + 75, "m1_div": 15 + 75 + 22 + 15, "m1_implicit": 21 + 15 + 30}
+                   "m1_point": 21 + 15 + 75, "m1_div": 15 + 75 + 22 + 15, "m1_implicit": 21 + 15 + 30, "les": 17 + 26 + 26 + 12}
     # ncu figures of the tracked capture (written by `python -m paper_2510_13965_b200.ncu_summary`; per-zone figures carry over to this size, the
     # tiles are the same); null when the capture is of another workload class
     cap, cap_meta = {}, None

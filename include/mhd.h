@@ -38,6 +38,7 @@ extern "C" {
 #define MHD_NWORK 33        /* 3 directions x (10 flux brackets of Eq. 32 + 1 speed bound of App. B) */
 #define MHD_NM1 15          /* (Nbar, Ebar, Fbar_i) x 3 neutrino species, field 5 s + {0..4} */
 #define MHD_NM1WORK 75      /* per species: 3 directions x (5 flux brackets + speed), kappa_a + kappa_s, P_ij */
+#define MHD_NLESWORK 26     /* auxiliary fields of the LES sub-grid-scale term (App. A): B^k, v^k, v_k, B_k, E_k, E^k, v.B, Theta, W^-2, rho, eps, h, dp/drho, dp/deps */
 #define MHD_MAX_STAGES 8
 #define MHD_MAX_PIECES 8
 
@@ -58,7 +59,8 @@ enum {
   MHD_SLOT_U1 = MHD_SLOT_R1 + MHD_MAX_STAGES,    /* optional third state buffer (MHD_NSTATE fields): lets mhd_advance fuse the RK combine
                                                     into the right-hand-side kernels (the new stage state cannot overwrite the one
                                                     whose stencils are being read); unbound = separate combine kernel */
-  MHD_NSLOTS = MHD_SLOT_U1 + 1
+  MHD_SLOT_LESWORK = MHD_SLOT_U1 + 1,            /* scratch of the LES term (MHD_NLESWORK fields); needed when les_C_M != 0 */
+  MHD_NSLOTS = MHD_SLOT_LESWORK + 1
 };
 
 /* flag bits: error policy of PAPER.md:1157-1162 */
@@ -119,7 +121,9 @@ typedef struct {
                                       ref. [63]: linear weights 1/10, 6/10, 3/10, exponent 2) */
   double weno_eps;                 /* recon_kind 1: the epsilon added to the smoothness indicators (ref. [63]: 1e-6); must be > 0 */
   double les_C_M;                  /* App. A, Eq. (A11): coefficient C_M of the sub-grid-scale tensor of the induction equation (the paper's
-                                      production value is 8); 0 = LES terms off */
+                                      production value is 8); 0 = LES terms off. When non-zero: ng >= 5 (the gradients of the
+                                      auxiliary fields are needed at every node the reconstruction reads), eos_kind 0 or 1 (analytic dp/drho,
+                                      dp/deps, l.882), MHD_SLOT_LESWORK bound; otherwise mhd_patch_create / mhd_rhs refuse */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */
@@ -189,6 +193,13 @@ int mhd_prim2con(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream)
  * (overwritten: pointwise F^d(U,P) and speeds at every grid point, computed once and read by the three 1-D
  * reconstruction passes). */
 int mhd_rhs(mhd_patch *p, int slot_state, int slot_prim, int slot_rhs, void *cuda_stream);
+
+/* LES (App. A Eqs. A11-A17): the sub-grid-scale tensor of the induction equation. Computes the auxiliary
+ * fields of App. A at every grid point into MHD_SLOT_LESWORK and ADDS -alpha G_B^{ki} = alpha C_M xi sqrt(gamma) H_M^{ki}
+ * (xi = gamma^{1/3} Delta^2 / 24, Delta = (dx dy dz)^{1/3}) to the pointwise flux of Bbar^i in direction k held in MHD_SLOT_WORK
+ * (field 11 k + 6 + i), at every point at least 2 points inside the array. mhd_rhs calls it between the pointwise fluxes and the
+ * reconstruction when les_C_M != 0; exposed for tests and for callers that sequence the right-hand side themselves. */
+int mhd_les_flux(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream);
 
 /* a9 — explicit RK combine on the interior (Eq. 53).
  *   stage = 0          : U0 <- U  (start of a step)
@@ -263,8 +274,8 @@ int mhd_patch_status(mhd_patch *p, int slot_flags, mhd_status *out, void *cuda_s
  * the elapsed milliseconds and launch counts per kernel class since the last read, and resets them.
  * Classes: 0 ghost fill, 1 con2prim, 2 ccz4 algebra (+ fluid sources), 3 reconstruction x, 4 y, 5 z, 6 rk combine / copy,
  * 7 pointwise fluxes, 8 advection + Kreiss-Oliger, 9 M1 closure + pointwise fluxes, 10 M1 flux divergence + sources,
- * 11 M1 implicit solve + back-reaction. */
-#define MHD_NKERNELS 12
+ * 11 M1 implicit solve + back-reaction, 12 LES sub-grid-scale term. */
+#define MHD_NKERNELS 13
 int mhd_patch_profile(mhd_patch *p, int enable);
 int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long long launches[MHD_NKERNELS], void *cuda_stream);
 

@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
 SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
 NM1, NM1WORK = 15, 75
-SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1, SLOT_U1 = 13, 14, 15, 16, 24, 32
+SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1, SLOT_U1, SLOT_LESWORK = 13, 14, 15, 16, 24, 32, 33
+NLESWORK = 26
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p
@@ -60,10 +61,10 @@ EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patc
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
            "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex",
            "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output",
-           "mhd_advance_imex_host", "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
-NKERNELS = 12
+           "mhd_advance_imex_host", "mhd_les_flux", "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
+NKERNELS = 13
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
-                  "m1_point", "m1_div", "m1_implicit"]
+                  "m1_point", "m1_div", "m1_implicit", "les"]
 
 _lib = None
 
@@ -99,6 +100,7 @@ def lib():
         L.mhd_m1_gravity.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p]
         L.mhd_strerror.restype = ctypes.c_char_p
+        L.mhd_les_flux.argtypes = [_p, _i, _i, _p]
         L.mhd_advance_imex_host.argtypes = [_p, ctypes.POINTER(mhd_tableau), ctypes.POINTER(_i), _d, _i, _p, _p, _p, _p]
         L.mhd_patch_set_neighbor.argtypes = [_p, _i, ctypes.POINTER(_i), _p, ctypes.c_size_t]
         L.mhd_patch_halo_words.argtypes = [_p]
@@ -201,6 +203,10 @@ def mhd_prim2con(h, slot_state=SLOT_U, slot_prim=SLOT_P, stream=None):
 
 def mhd_rhs(h, slot_state, slot_prim, slot_rhs, stream=None):
     _check(lib().mhd_rhs(h, slot_state, slot_prim, slot_rhs, stream))
+
+
+def mhd_les_flux(h, slot_state=SLOT_U, slot_prim=SLOT_P, stream=None):
+    _check(lib().mhd_les_flux(h, slot_state, slot_prim, stream))
 
 
 def mhd_rk_stage(h, tableau, stage, dt, stream=None):
@@ -344,6 +350,10 @@ class Patch:
         for slot, t in [(SLOT_U, self.U), (SLOT_U0, self.U0), (SLOT_P, self.P), (SLOT_FLAGS, self.flags), (SLOT_WORK, self.work)] + \
                        [(SLOT_K1 + j, k) for j, k in enumerate(self.K)]:
             mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
+        self.leswork = None
+        if float(params.get("les_C_M", 0.0)) != 0.0:             # LES sub-grid-scale term: scratch for the auxiliary fields of App. A
+            self.leswork = z(NLESWORK)
+            mhd_patch_bind(self.h, SLOT_LESWORK, self.leswork.data_ptr(), self.npts)
         self.U1 = None
         if fused and not m1:                                # third state buffer: mhd_advance then fuses the RK combine into the RHS kernels (measured slower on B200
                                                             # with the present latency-bound k_adv_ko / k_recon_march: 111.9 vs 107.5 ms per step at c4_256; off by default)

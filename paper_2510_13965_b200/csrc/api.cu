@@ -13,12 +13,14 @@ int slot_fields(int slot) {
   if (slot == MHD_SLOT_FLAGS) return 1;
   if (slot == MHD_SLOT_WORK) return MHD_NWORK;
   if (slot == MHD_SLOT_M1WORK) return MHD_NM1WORK;
+  if (slot == MHD_SLOT_LESWORK) return MHD_NLESWORK;
   if (slot >= MHD_SLOT_V) return MHD_NM1;
   return MHD_NSTATE;
 }
 bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLOTS && p->slot[slot].ptr != nullptr; }
 bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || slot == MHD_SLOT_U1 || (slot >= MHD_SLOT_K1 && slot < MHD_SLOT_K1 + MHD_MAX_STAGES); }
 bool is_m1_slot(int slot) { return slot >= MHD_SLOT_V && slot < MHD_SLOT_U1 && slot != MHD_SLOT_M1WORK; }
+int les_impl(mhd_patch* p, int slot_state, int slot_prim, cudaStream_t s);
 double* dptr(const mhd_patch* p, int slot) { return (double*)p->slot[slot].ptr; }
 
 // piecewise-polytrope continuity constants: K_i, a_i for i > 0
@@ -60,6 +62,7 @@ int rhs_impl(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, const Fu
   { Timed tm(p, 2, s); if (launch_ccz4_algebra(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
   { Timed tm(p, 8, s); if (launch_adv_ko(p->dims, p->par, U, su, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA; }
   { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
+  if (p->par.les_C_M != 0.0) { const int rc = les_impl(p, slot_state, slot_prim, s); if (rc != MHD_OK) return rc; }
   for (int dir = 0; dir < 3; ++dir) {
     Timed tm(p, 3 + dir, s);
     if (launch_recon(dir, p->dims, p->par, U, su, Wk, sw, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA;
@@ -67,6 +70,14 @@ int rhs_impl(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, const Fu
   return MHD_OK;
 }
 
+
+int les_impl(mhd_patch* p, int slot_state, int slot_prim, cudaStream_t s) {
+  if (!slot_ok(p, MHD_SLOT_LESWORK) || !slot_ok(p, MHD_SLOT_WORK)) return MHD_E_UNBOUND;
+  Timed tm(p, 12, s);
+  return launch_les(p->dims, p->par, dptr(p, slot_state), p->slot[slot_state].stride, dptr(p, slot_prim), p->slot[slot_prim].stride,
+                    dptr(p, MHD_SLOT_LESWORK), p->slot[MHD_SLOT_LESWORK].stride, dptr(p, MHD_SLOT_WORK), p->slot[MHD_SLOT_WORK].stride, s) == cudaSuccess
+             ? MHD_OK : MHD_E_CUDA;
+}
 
 // n_steps full RK steps, the combine of Eq. (53) fused into the right-hand-side kernels (needs the third state buffer MHD_SLOT_U1).
 // Three buffers rotate: one holds U^n for the whole step, each stage differentiates `cur` and writes the next stage state into the
@@ -156,6 +167,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
   if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
+  if (desc->les_C_M != 0.0 && (desc->ng < 5 || desc->eos_kind == 2)) return MHD_E_UNSUPPORTED;
   if (desc->recon_kind < 0 || desc->recon_kind > 1 || (desc->recon_kind == 1 && !(desc->weno_eps > 0.0))) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
   if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2 ||
@@ -343,6 +355,13 @@ int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* str
   if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P || !is_state_slot(slot_rhs) || slot_rhs == slot_state) return MHD_E_ARG;
   if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim) || !slot_ok(p, slot_rhs) || !slot_ok(p, MHD_SLOT_WORK)) return MHD_E_UNBOUND;
   return rhs_impl(p, slot_state, slot_prim, slot_rhs, Fuse(), (cudaStream_t)stream);
+}
+
+int mhd_les_flux(mhd_patch* p, int slot_state, int slot_prim, void* stream) {
+  if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P) return MHD_E_ARG;
+  if (p->par.les_C_M == 0.0) return MHD_E_ARG;
+  if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim)) return MHD_E_UNBOUND;
+  return les_impl(p, slot_state, slot_prim, (cudaStream_t)stream);
 }
 
 int mhd_rk_stage(mhd_patch* p, const mhd_tableau* t, int stage, double dt, void* stream) {

@@ -122,6 +122,8 @@ cudaError_t launch_m1_implicit(const Dims& d, const Par& par, const double* U, s
                                double* R, size_t sr, double adt, uint8_t* flags, cudaStream_t s);
 cudaError_t launch_m1_gravity(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
                               double* K, size_t sk, cudaStream_t s);
+cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
+                       double* Wk, size_t sw, cudaStream_t s);
 cudaError_t launch_prolong(const Dims& dc, const double* Uc, size_t sc, const Dims& df, double* Uf, size_t sf, int nfields,
                            const int origin[3], const int lo[3], const int hi[3], cudaStream_t s);
 cudaError_t launch_restrict(const Dims& df, const double* Uf, size_t sf, const Dims& dc, double* Uc, size_t sc, int nfields, const int origin[3], cudaStream_t s);

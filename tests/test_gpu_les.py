@@ -1,0 +1,118 @@
+"""GPU parity of the LES sub-grid-scale term of the induction equation (App. A, C_M = 8) against the oracle, through
+the C ABI. Ghost width 5 (the gradients of the auxiliary fields are needed at every node the reconstruction reads).
+Tolerances: auxiliary fields 1e-13, the SGS flux 1e-11 of its own magnitude, RHS 1e-11 per component (north_star), 10 steps 1e-9."""
+import numpy as np
+import pytest
+
+from paper_2510_13965_b200 import synth
+
+pytestmark = pytest.mark.gpu
+NG = 5
+
+
+def _boost_B(cfg, factor=30.0):
+    """config 1 has B^2/rho ~ 1e-3: scale the magnetic field up so that the SGS tensor is not negligible beside the resolved flux"""
+    cfg["U"][28:31] *= factor
+    return cfg
+
+
+def _setup(oracle_mod, cfg):
+    from paper_2510_13965_b200 import binding
+    n = cfg["n"]
+    o = oracle_mod.Oracle(cfg["params"], n[0], n[1], n[2], NG, cfg["dx"])
+    U, P = cfg["U"].copy(), cfg["P"].copy()
+    o.prim2con(U, P)
+    patch = binding.Patch(cfg["params"], n, NG, cfg["dx"], stages=4)
+    return binding, o, patch, U, P
+
+
+def _rel(a, b):
+    s = (slice(None), slice(NG, -NG), slice(NG, -NG), slice(NG, -NG))
+    num = np.abs(a[s] - b[s]).reshape(a.shape[0], -1).max(axis=1)
+    den = np.abs(b[s]).reshape(b.shape[0], -1).max(axis=1)
+    return num / np.where(den > 0, den, 1.0), den
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_les_flux_and_one_stage_parity(oracle_mod, kind):
+    cfg = _boost_B(synth.config1(n=20, gauge_perturbation=True, ng=NG))
+    cfg["params"].update(les_C_M=8.0)
+    if kind == 1:
+        cfg["params"].update(eos_kind=1, eos_gamma_th=1.8, n_pieces=3, pp_K=[30.0, 0.0, 0.0], pp_Gamma=[1.9, 2.4, 2.9], pp_rho=[1.0e-3, 5.0e-3, 1e300])
+        cfg["P"][synth.EPS] = 0.25
+    binding, o, patch, U, P = _setup(oracle_mod, cfg)
+    Uo = U.copy()
+    o.fill_ghosts(Uo, cfg["bc"])
+    Po, Fo = o.con2prim(Uo)
+    Lo, Ao = o.les_flux(Uo, Po)
+    Ko = o.rhs(Uo, Po)
+    K0 = oracle_mod.Oracle(dict(cfg["params"], les_C_M=0.0), *cfg["n"], NG, cfg["dx"]).rhs(Uo, Po)
+    patch.upload(U=U)
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    patch.work.zero_()
+    binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
+    Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
+    ra = np.abs(Ag - Ao).reshape(26, -1).max(axis=1) / np.abs(Ao).reshape(26, -1).max(axis=1)
+    assert np.all(ra < 1e-13), ra
+    scale = np.abs(Lo).max()
+    assert scale > 0
+    for k in range(3):
+        for i in range(3):
+            assert np.abs(Wg[11 * k + 6 + i] - Lo[3 * k + i]).max() <= 1e-11 * scale, (k, i)
+    used = {11 * k + 6 + i for k in range(3) for i in range(3) if i != k}
+    assert all(np.all(Wg[f] == 0) for f in range(33) if f not in used)              # nothing else is touched
+    Kg = patch.rhs(1).cpu().numpy()
+    rk, den = _rel(Kg, Ko)
+    assert np.all(rk[den > 0] < 1e-11), rk
+    # the term is live: it changes the induction equation by more than the parity tolerance
+    d, _ = _rel(Ko[28:31], K0[28:31])
+    assert np.all(d > 1e-6), d
+    patch.close()
+
+
+def test_les_ten_steps(oracle_mod):
+    cfg = _boost_B(synth.config1(n=12, gauge_perturbation=True, ng=NG))
+    cfg["params"].update(les_C_M=8.0)
+    binding, o, patch, U, P = _setup(oracle_mod, cfg)
+    a, w = synth.tableau("rk4")
+    dt = 0.25 * cfg["dx"]
+    patch.upload(U=U)
+    patch.advance(binding.make_tableau(a, w), cfg["bc"], dt, 10)
+    Uo = U.copy()
+    _, Fo = o.evolve(Uo, cfg["bc"], a, w, dt, 10)
+    Ug = patch.U.cpu().numpy()
+    num = np.abs(Ug - Uo).reshape(32, -1).max(axis=1)
+    den = np.abs(Uo).reshape(32, -1).max(axis=1)
+    assert np.all(num <= 1e-9 * np.where(den > 0, den, 1.0)), num / np.where(den > 0, den, 1.0)
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    patch.close()
+
+
+def test_les_ragged_outflow_and_refusals(oracle_mod):
+    from paper_2510_13965_b200 import binding
+    cfg = _boost_B(synth.config1(n=20, gauge_perturbation=True, ng=NG))
+    cfg["params"].update(les_C_M=8.0)
+    nx, ny, nz = 23, 13, 9
+    cfg["U"] = np.ascontiguousarray(np.tile(cfg["U"], (1, 1, 1, 2))[:, :nz + 2 * NG, :ny + 2 * NG, :nx + 2 * NG])
+    cfg["P"] = np.ascontiguousarray(np.tile(cfg["P"], (1, 1, 1, 2))[:, :nz + 2 * NG, :ny + 2 * NG, :nx + 2 * NG])
+    cfg["n"] = (nx, ny, nz)
+    cfg["bc"] = [1, 1, 0, 1, 1, 0]
+    binding, o, patch, U, P = _setup(oracle_mod, cfg)
+    Uo = U.copy()
+    o.fill_ghosts(Uo, cfg["bc"])
+    Po, Fo = o.con2prim(Uo)
+    Ko = o.rhs(Uo, Po)
+    patch.upload(U=U)
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    Kg = patch.rhs(1).cpu().numpy()
+    rk, den = _rel(Kg, Ko)
+    assert np.all(rk[den > 0] < 1e-11), rk
+    patch.close()
+    # ghost width 3, and the tabulated EoS, are refused at create time
+    with pytest.raises(binding.MhdError):
+        binding.mhd_patch_create(binding.make_desc(synth.default_params(les_C_M=8.0), 8, 8, 8, 3, 0.1))
+    with pytest.raises(binding.MhdError):
+        binding.mhd_patch_create(binding.make_desc(synth.default_params(les_C_M=8.0, eos_kind=2), 8, 8, 8, 5, 0.1))
