@@ -205,7 +205,8 @@ int mhd_les_flux(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream)
  *   stage = 0          : U0 <- U  (start of a step)
  *   1 <= stage < s     : U <- U0 + dt * sum_{j<=stage} a_expl[stage][j-1] K_j      (= U^(stage+1))
  *   stage = s          : U <- U0 + dt * sum_j w_expl[j-1] K_j                      (= U^{n+1})
- * K_j is slot MHD_SLOT_K1 + j - 1; zero coefficients are skipped (their slots need not be bound). */
+ * K_j is slot MHD_SLOT_K1 + j - 1; zero coefficients are skipped (their slots need not be bound). Ghost points of U carry no
+ * meaning afterwards (large patches are combined as whole flat arrays): mhd_fill_ghosts refills them before anything reads them. */
 int mhd_rk_stage(mhd_patch *p, const mhd_tableau *t, int stage, double dt, void *cuda_stream);
 
 /* n_steps full RK steps, device resident: per stage fill -> con2prim -> rhs(K_stage) -> rk_stage; the state is

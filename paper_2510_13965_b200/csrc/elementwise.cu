@@ -141,11 +141,43 @@ __global__ void __launch_bounds__(128) k_rk_combine(Dims d, int nfields, double*
   }
 }
 
+// The same combine over whole fields as flat arrays of double2 (ghost points included: they hold U0's ghosts plus whatever K's never-written
+// ghosts hold, and are refilled before anything reads them). Used when the ghost shell is a small fraction of the patch and every field
+// is 16-byte aligned: perfectly linear 128-bit accesses instead of rows that start 24 bytes into a 128-byte line.
+template <int NK>
+__global__ void __launch_bounds__(256) k_rk_combine_flat(long long n2, double2* __restrict__ Uout, size_t so, const double2* __restrict__ U0, size_t s0, RkArgs a) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n2) return;
+  const size_t f = blockIdx.y;
+  double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+  for (int m = 0; m < NK; ++m) {
+    const double2 k = __ldg((const double2*)(a.K[m] + f * a.sk[m]) + t);
+    acc.x = fma(a.c[m], k.x, acc.x); acc.y = fma(a.c[m], k.y, acc.y);
+  }
+  const double2 u = __ldg(U0 + f * (s0 / 2) + t);
+  Uout[f * (so / 2) + t] = make_double2(u.x + acc.x, u.y + acc.y);
+}
+
 cudaError_t launch_rk_combine(const Dims& d, int nfields, double* Uout, size_t so, const double* U0, size_t s0,
                               int nk, const double* const* K, const size_t* sk, const double* coef, double dt, cudaStream_t s) {
   RkArgs a;
   a.nk = nk;
   for (int m = 0; m < nk; ++m) { a.K[m] = K[m]; a.sk[m] = sk[m]; a.c[m] = dt * coef[m]; }
+  bool flat = (d.npts % 2 == 0) && (so % 2 == 0) && (s0 % 2 == 0) && !((uintptr_t)Uout & 15) && !((uintptr_t)U0 & 15) &&
+              (double)d.npts <= 1.10 * (double)d.nx * d.ny * d.nz;
+  for (int m = 0; m < nk; ++m) flat = flat && (sk[m] % 2 == 0) && !((uintptr_t)K[m] & 15);
+  if (flat) {
+    const long long n2 = d.npts / 2;
+    dim3 fgrid((unsigned)((n2 + 255) / 256), nfields);
+    switch (nk) {
+#define CASE(N) case N: k_rk_combine_flat<N><<<fgrid, 256, 0, s>>>(n2, (double2*)Uout, so, (const double2*)U0, s0, a); break;
+      CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+      default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+  }
   dim3 grid((d.nx + 127) / 128, d.ny, d.nz), block(128);
   switch (nk) {
 #define CASE(N) case N: k_rk_combine<N><<<grid, block, 0, s>>>(d, nfields, Uout, so, U0, s0, a); break;

@@ -734,3 +734,31 @@ def test_recon_kind_argument_check():
     par = synth.default_params(recon_kind=1, weno_eps=0.0)
     with pytest.raises(binding.MhdError):
         binding.mhd_patch_create(binding.make_desc(par, 8, 8, 8, 3, 0.1))
+
+
+def test_rk_combine_full_size_flat_path(oracle_mod):
+    """At bench size the combine runs over whole fields as flat double2 arrays (ghosts included). 200^3: every interior point against
+    U0 + dt (a1 K1 + a2 K2) evaluated by the oracle's rk_combine on sampled boxes and by an FP64 torch expression everywhere (1e-15:
+    FMA contraction only)."""
+    import torch
+    from paper_2510_13965_b200 import binding
+    n = (200, 200, 200)
+    patch = binding.Patch(synth.default_params(), n, NG, 0.1, stages=2)
+    g = torch.Generator(device="cuda").manual_seed(7)
+    for t in (patch.U0, patch.K[0], patch.K[1]):
+        t.copy_(torch.rand(t.shape, generator=g, device="cuda", dtype=torch.float64) - 0.5)
+    a = np.array([[0.0, 0.0], [0.3, 0.7]])
+    w = np.array([0.25, 0.75])
+    dt = 0.013
+    patch.rk_stage(binding.make_tableau(a, w), 2, dt)                       # U <- U0 + dt (w1 K1 + w2 K2)
+    want = patch.U0 + dt * (w[0] * patch.K[0] + w[1] * patch.K[1])
+    inner = (slice(None), slice(NG, -NG), slice(NG, -NG), slice(NG, -NG))
+    assert ((patch.U - want)[inner].abs().max() <= 1e-15).item()
+    o = oracle_mod.Oracle(synth.default_params(), 12, 12, 12, NG, 0.1)
+    for lo in ((0, 0, 0), (188, 91, 40), (100, 188, 188)):
+        sl = (slice(None), slice(lo[2], lo[2] + 18), slice(lo[1], lo[1] + 18), slice(lo[0], lo[0] + 18))
+        U0, K1, K2 = [np.ascontiguousarray(t[sl].cpu().numpy()) for t in (patch.U0, patch.K[0], patch.K[1])]
+        wo = o.rk_combine(U0, [K1, K2], w, dt)
+        got = patch.U[sl].cpu().numpy()
+        assert np.abs(got - wo)[inner].max() <= 1e-15
+    patch.close()
