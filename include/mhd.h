@@ -180,7 +180,9 @@ int mhd_ipc_close(void *dev_ptr, size_t offset);
  * l.1157-1162). Writes the 10 primitives and the flag byte; where a rule changed a primitive the fluid conserved
  * fields of slot_state are reset from the corrected primitives (Bbar, phibar untouched). slot_prim is also READ: if it holds
  * valid primitives (e.g. of the previous stage) they give the starting bracket of the root solve (warm start); the result is
- * the same root to solver tolerance whatever slot_prim held, zeros and NaNs included. */
+ * the same root to solver tolerance whatever slot_prim held, zeros and NaNs included.
+ * A patch has ONE primitive slot and ONE flag slot: slot_prim must be MHD_SLOT_P and slot_flags MHD_SLOT_FLAGS (MHD_E_ARG otherwise; the
+ * arguments keep the call in the form of the problem statement and leave room for more slots); slot_state is any state slot (U, U0, U1, K_j). */
 int mhd_con2prim(mhd_patch *p, int slot_state, int slot_prim, int slot_flags, void *cuda_stream);
 
 /* inverse of a2 for initial data (Eq. 29): slot_prim holds rho, Ye, eps, v^i; fills p, W, T, cs2 there and

@@ -6,18 +6,19 @@
 // (the flux kernels of flux.cu subtract the flux divergence afterwards).
 //
 // Two kernels:
-//   k_ccz4_algebra  everything that needs the radius-2 centred derivatives (Eqs. 60-62). A CTA of 256 threads owns a
-//                   16x4x4 tile, one point per thread. The 16 fields that are differentiated are staged one at a time
-//                   through a 3-deep shared-memory ring of 22x8x8 tiles (tile + halo) filled by the copy engine (TMA), so
-//                   every stencil operand is an LDS with a compile-time offset and the copy of field f+2 overlaps the
-//                   arithmetic on field f. Phase 1 turns each tile into derivatives, contracts second derivatives at
-//                   once (gamma~^mn d_m d_n gamma~_ab, gamma~^jk d_j d_k beta^c, d_j d_k beta^k) and parks the 72
-//                   surviving numbers per point in a per-thread shared-memory scratch column; phase 2 is the
-//                   pointwise algebra of Eqs. (13)-(26) and the sources of Eq. (32) reading that scratch. Registers
-//                   then hold only the working set of the phase, not 130 derivatives at once.
+//   k_ccz4_algebra  everything that needs the radius-2 centred derivatives (Eqs. 60-62). A CTA owns a 16 x TY x TZ tile, one
+//                   point per thread (default 16x4x2 = 128 threads, two CTAs per SM: the derivative phase of one CTA, bound by
+//                   shared-memory loads, overlaps the pointwise algebra of the other, bound by the FP64 pipe). The 16 fields
+//                   that are differentiated are staged one at a time through a 3-deep shared-memory ring of 22 x (TY+4) x (TZ+4)
+//                   tiles (tile + halo) filled by the copy engine (TMA), so every stencil operand is an LDS with a compile-time
+//                   offset and the copy of field f+2 overlaps the arithmetic on field f. Phase 1 turns each tile into
+//                   derivatives, folds second derivatives, d Gamma^, d K^, d Theta into register accumulators at once
+//                   (gamma~^mn d_m d_n gamma~_ab, gamma~^jk d_j d_k beta^c, d_j d_k beta^k, ...) and parks the 33 first
+//                   derivatives the algebra needs more than once (NSCR) per point in a per-thread shared-memory scratch column;
+//                   phase 2 is the pointwise algebra of Eqs. (13)-(26) and the sources of Eq. (32) reading that scratch.
 //   k_adv_ko        beta^k d_k u with the one-sided stencils plus the KO term, radius 3, 1-D along each axis, added to
 //                   K for the 22 spacetime fields (and KO alone for the matter fields when sigma_ko_matter != 0).
-//                   A thread marches 8 zones along z with a 7-value register window; x / y neighbours come from L1.
+//                   A thread marches AZ = 4 zones along z with a register window; x / y neighbours come from L1.
 //
 // All stencils are evaluated on differences (note N1 of DESIGN.md): algebraically identical to the printed
 // coefficients, exact zeros in flat space, no cancellation noise.
