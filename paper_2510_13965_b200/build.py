@@ -21,7 +21,7 @@ def _newer(target, deps):
 
 
 def build(force=False, verbose=False):
-    headers = [os.path.join(CSRC, "mhd_internal.cuh"), os.path.join(CSRC, "rootfind.cuh"), os.path.join(HERE, "..", "include", "mhd.h"), os.path.abspath(__file__)]
+    headers = [os.path.join(CSRC, "mhd_internal.cuh"), os.path.join(CSRC, "rootfind.cuh"), os.path.join(CSRC, "tma.cuh"), os.path.join(HERE, "..", "include", "mhd.h"), os.path.abspath(__file__)]
     objs, jobs = [], []
     for src, extra in SOURCES.items():
         s = os.path.join(CSRC, src)

@@ -27,6 +27,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include "mhd_internal.cuh"
+#include "tma.cuh"
 
 namespace mhd {
 
@@ -62,30 +63,8 @@ __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_grou
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// ---- TMA: one cp.async.bulk.tensor per field and tile (a 22 x 8 x (TZ+4) box of the 4-D tensor (x, y, z, field); coordinates past
-// the end of the array are zero-filled by the copy engine: those points belong to ragged tiles and are masked), completion on an mbarrier
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_4d(double* smem, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3) {
-  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];\n"
-               ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"((uint64_t)map), "r"((unsigned)__cvta_generic_to_shared(bar)),
-                 "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
-}
+// ---- TMA: one cp.async.bulk.tensor per field and tile (a 22 x (TY+4) x (TZ+4) box of the 4-D tensor (x, y, z, field); coordinates past the end of
+// the array are zero-filled by the copy engine: those points belong to ragged tiles and are masked), completion on an mbarrier: tma.cuh
 
 // unscaled Eq. (60): 12 h D u
 template <int O>
@@ -154,7 +133,7 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
     if (tid == 0) {
 #pragma unroll
       for (int b = 0; b < NBUF; ++b) mbar_init(full + b, 1);
-      asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+      mbar_fence_init();
     }
     __syncthreads();
   }
@@ -618,29 +597,13 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
 }
 }  // namespace
 
-// Tensor map of a state slot as a 4-D tensor (x, y, z, field) of doubles with a 22 x 8 x (TZ+4) x 1 box. Legal when the row pitch and the
-// field stride are multiples of 16 bytes (MX even, stride even), the base is 16-byte aligned and the box origin i0 - XL + ng is even
-// (ng odd); otherwise the cp.async path is used.
+// Tensor map of the state slot with the algebra kernel's box: legal for even MX / stride and an even box origin i0 - XL + ng (ng odd);
+// otherwise the cp.async path is used. MHD_CCZ4_TMA=0 forces the cp.async path.
 static bool make_tensor_map(const Dims& d, const double* U, size_t su, int ty, int tz, CUtensorMap* out) {
-  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                               const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn encode = nullptr;
-  static bool tried = false;
-  if (!tried) {
-    tried = true;
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) encode = (EncodeFn)fn;
-    const char* v = getenv("MHD_CCZ4_TMA");
-    if (v && atoi(v) == 0) encode = nullptr;
-  }
-  if (!encode || (d.mx & 1) || (su & 1) || ((uintptr_t)U & 15) || ((d.ng - XL) & 1)) return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)d.mx, (cuuint64_t)d.my, (cuuint64_t)d.mz, (cuuint64_t)MHD_NSTATE};
-  const cuuint64_t strides[3] = {(cuuint64_t)d.mx * 8, (cuuint64_t)d.sz * 8, (cuuint64_t)su * 8};
-  const cuuint32_t box[4] = {(cuuint32_t)SX, (cuuint32_t)(ty + 2 * RH), (cuuint32_t)(tz + 2 * RH), 1};
-  const cuuint32_t estr[4] = {1, 1, 1, 1};
-  return encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  static int off = -1;
+  if (off < 0) { const char* v = getenv("MHD_CCZ4_TMA"); off = v && atoi(v) == 0; }
+  if (off || ((d.ng - XL) & 1)) return false;
+  return make_tensor_map_4d(d, U, su, MHD_NSTATE, SX, ty + 2 * RH, tz + 2 * RH, out);
 }
 
 template <int TY, int TZ>

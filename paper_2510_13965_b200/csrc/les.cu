@@ -12,6 +12,7 @@
 //                (26 fields x 12 neighbours per point).
 // EoS derivatives: analytic for the ideal gas and the hybrid piecewise polytrope (l.882); the tabulated EoS is not supported here.
 #include "mhd_internal.cuh"
+#include "tma.cuh"
 
 namespace mhd {
 
@@ -58,61 +59,17 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   a[A_RHO * sa] = rho; a[A_EPS * sa] = eps; a[A_H * sa] = h; a[A_DPR * sa] = dpr; a[A_DPE * sa] = dpe;
 }
 
-__global__ void __launch_bounds__(128) k_les_flux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
-                                                  const double* __restrict__ P, size_t sp, const double* __restrict__ A, size_t sa,
-                                                  double* __restrict__ Wk, size_t sw) {
-  const int i = 2 + blockIdx.x * blockDim.x + threadIdx.x, j = 2 + blockIdx.y, k = 2 + blockIdx.z;
-  if (i >= d.mx - 2) return;
-  const size_t pt = (size_t)k * d.sz + (size_t)j * d.sy + i;
-  // inverse physical metric gamma^{mn} = chi gamma~^{mn}
-  double gu[6];
-  const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
-  {
-    double g[6];
-#pragma unroll
-    for (int c = 0; c < 6; ++c) g[c] = __ldg(U + (size_t)(GXX + c) * su + pt);
-    const double s = chi / (g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]));
-    gu[0] = (g[3] * g[5] - g[4] * g[4]) * s; gu[1] = (g[2] * g[4] - g[1] * g[5]) * s; gu[2] = (g[1] * g[4] - g[2] * g[3]) * s;
-    gu[3] = (g[0] * g[5] - g[2] * g[2]) * s; gu[4] = (g[1] * g[2] - g[0] * g[4]) * s; gu[5] = (g[0] * g[3] - g[1] * g[1]) * s;
-  }
-  // point values and gradients: dl = d_m f (Eq. 60), du = gamma^{mn} d_n f, so that grad f . grad g = sum_m dl_f[m] du_g[m]
-  double a[NAUX], dl[NAUX][3], du[NAUX][3];
-  const double c12[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
-  const long long st[3] = {1, d.sy, d.sz};
-#pragma unroll
-  for (int f = 0; f < NAUX; ++f) {
-    const double* s = A + (size_t)f * sa + pt;
-    a[f] = __ldg(s);
-#pragma unroll
-    for (int m = 0; m < 3; ++m) dl[f][m] = (8.0 * (__ldg(s + st[m]) - __ldg(s - st[m])) - (__ldg(s + 2 * st[m]) - __ldg(s - 2 * st[m]))) * c12[m];
-    du[f][0] = gu[0] * dl[f][0] + gu[1] * dl[f][1] + gu[2] * dl[f][2];
-    du[f][1] = gu[1] * dl[f][0] + gu[3] * dl[f][1] + gu[4] * dl[f][2];
-    du[f][2] = gu[2] * dl[f][0] + gu[4] * dl[f][1] + gu[5] * dl[f][2];
-  }
-  auto dot = [&](int f, int g) { return dl[f][0] * du[g][0] + dl[f][1] * du[g][1] + dl[f][2] * du[g][2]; };
-  const double p = __ldg(P + (size_t)PRESS * sp + pt);
+// The closed forms (A12)-(A16) from the point values a[] and the contracted gradient products, and the update of the work slot
+struct LesDots { double dVB_B[3], dTH_v[3], dBv[3][3], sBv, sBBvB, sBvTh, sBB, sEE, svv, dWW, dWR, dWH, dPR_R, dPE_E, dRE; };
+
+__device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, const double a[NAUX], const LesDots& D, double p, double chi, double al,
+                                                 double* __restrict__ Wk, size_t sw, size_t pt) {
+  const double (&dVB_B)[3] = D.dVB_B; const double (&dTH_v)[3] = D.dTH_v; const double (&dBv)[3][3] = D.dBv;
+  const double sBv = D.sBv, sBBvB = D.sBBvB, sBvTh = D.sBvTh, sBB = D.sBB, sEE = D.sEE, svv = D.svv;
+  const double dWW = D.dWW, dWR = D.dWR, dWH = D.dWH, dPR_R = D.dPR_R, dPE_E = D.dPE_E, dRE = D.dRE;
   const double vB = a[A_VB], Th = a[A_TH], W2 = 1.0 / a[A_WM2], rho = a[A_RHO], h = a[A_H], dpr = a[A_DPR], dpe = a[A_DPE];
   const double calE = h * W2, iTh = 1.0 / Th, icalE = 1.0 / calE;
   const double E2 = a[A_EL] * a[A_EU] + a[A_EL + 1] * a[A_EU + 1] + a[A_EL + 2] * a[A_EU + 2];
-  // products shared between (A12)-(A16)
-  double dVB_B[3], dTH_v[3], dBv[3][3];        // grad(v.B).grad B^k, grad Theta.grad v^k, grad B^i.grad v^k
-#pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    dVB_B[c] = dot(A_VB, A_BU + c);
-    dTH_v[c] = dot(A_TH, A_VU + c);
-#pragma unroll
-    for (int e = 0; e < 3; ++e) dBv[c][e] = dot(A_BU + c, A_VU + e);
-  }
-  double sBv = 0.0, sBBvB = 0.0, sBvTh = 0.0, sBB = 0.0, sEE = 0.0, svv = 0.0;
-#pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    sBv += dot(A_BU + c, A_VL + c);
-    sBBvB += a[A_BL + c] * dVB_B[c];
-    sBvTh += a[A_BU + c] * dot(A_VL + c, A_TH);
-    sBB += dot(A_BL + c, A_BU + c);
-    sEE += dot(A_EL + c, A_EU + c);
-    svv += dot(A_VL + c, A_VU + c);
-  }
   double Psi_v[3], vPsi = 0.0;
   const double brk = (Th * sBv + sBBvB - sBvTh) * icalE;
 #pragma unroll
@@ -131,11 +88,10 @@ __global__ void __launch_bounds__(128) k_les_flux(const __grid_constant__ Dims d
   const double TmE = Th - E2;
   const double Psi_Th = Th / TmE * (sBB - sEE - BvPsi);
   const double Psi_A = W2 * (p * dpe + rho * rho * dpr);
-  const double dWW = dot(A_WM2, A_WM2);
   const double pref = calE * W2 * TmE / ((rho * calE - Psi_A) * TmE * W2 + Psi_A * Th);
-  const double brace = rho * (dot(A_DPR, A_RHO) + dot(A_DPE, A_EPS)) - 2.0 * dpe * dot(A_RHO, A_EPS)
-                       - (calE * dpe - Psi_A) * (0.25 * W2 * dWW + dot(A_WM2, A_RHO) / rho)
-                       - 2.0 * a[A_WM2] * dpe * (sBB - W2 * W2 * dot(A_WM2, A_H))
+  const double brace = rho * (dPR_R + dPE_E) - 2.0 * dpe * dRE
+                       - (calE * dpe - Psi_A) * (0.25 * W2 * dWW + dWR / rho)
+                       - 2.0 * a[A_WM2] * dpe * (sBB - W2 * W2 * dWH)
                        - (calE * dpe + Psi_A) * (vPsi + svv + W2 * dWW)
                        + Psi_Th * icalE * iTh * ((calE * dpe + Psi_A) * TmE - Psi_A * Th * a[A_WM2]);
   const double H_Th = Psi_Th + Th / TmE * (pref * brace);                                   // (A13)
@@ -156,14 +112,219 @@ __global__ void __launch_bounds__(128) k_les_flux(const __grid_constant__ Dims d
     }
 }
 
+__global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
+                                                  const double* __restrict__ P, size_t sp, const double* __restrict__ A, size_t sa,
+                                                  double* __restrict__ Wk, size_t sw) {
+  // a CTA owns a 16 x 4 x 4 block of points so that most y / z neighbours of a point are loaded by the same CTA and hit in L1
+  const int i = 2 + blockIdx.x * 16 + threadIdx.x, j = 2 + blockIdx.y * 4 + threadIdx.y, k = 2 + blockIdx.z * 4 + threadIdx.z;
+  if (i >= d.mx - 2 || j >= d.my - 2 || k >= d.mz - 2) return;
+  const size_t pt = (size_t)k * d.sz + (size_t)j * d.sy + i;
+  // inverse physical metric gamma^{mn} = chi gamma~^{mn}
+  double gu[6];
+  const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
+  {
+    double g[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) g[c] = __ldg(U + (size_t)(GXX + c) * su + pt);
+    const double s = chi / (g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]));
+    gu[0] = (g[3] * g[5] - g[4] * g[4]) * s; gu[1] = (g[2] * g[4] - g[1] * g[5]) * s; gu[2] = (g[1] * g[4] - g[2] * g[3]) * s;
+    gu[3] = (g[0] * g[5] - g[2] * g[2]) * s; gu[4] = (g[1] * g[2] - g[0] * g[4]) * s; gu[5] = (g[0] * g[3] - g[1] * g[1]) * s;
+  }
+  // Gradients are streamed field by field (Eq. 60) and contracted at once: only the raised gradients gamma^{mn} d_n f of a few anchor
+  // fields (B^c, Theta, then W^-2, rho, eps) stay in registers, so that grad f . grad g = sum_m d_m f (gamma^{mn} d_n g) costs three FMAs and the
+  // kernel holds ~60 doubles instead of the 180 that all 26 gradients in both index positions would take.
+  const double c12[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
+  const long long st[3] = {1, d.sy, d.sz};
+  auto val = [&](int f) { return __ldg(A + (size_t)f * sa + pt); };
+  auto grad = [&](int f, double g[3]) {
+    const double* s = A + (size_t)f * sa + pt;
+#pragma unroll
+    for (int m = 0; m < 3; ++m) g[m] = (8.0 * (__ldg(s + st[m]) - __ldg(s - st[m])) - (__ldg(s + 2 * st[m]) - __ldg(s - 2 * st[m]))) * c12[m];
+  };
+  auto raise = [&](const double g[3], double r[3]) {
+    r[0] = gu[0] * g[0] + gu[1] * g[1] + gu[2] * g[2];
+    r[1] = gu[1] * g[0] + gu[3] * g[1] + gu[4] * g[2];
+    r[2] = gu[2] * g[0] + gu[4] * g[1] + gu[5] * g[2];
+  };
+  auto dotp = [](const double g[3], const double r[3]) { return g[0] * r[0] + g[1] * r[1] + g[2] * r[2]; };
+  double a[NAUX];                               // point values the closed forms use (vector components; the scalars are fetched where needed)
+#pragma unroll
+  for (int f = 0; f < A_VB; ++f) a[f] = val(f);
+  double uB[3][3], uTH[3], t[3], t2[3], r[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { grad(A_BU + c, t); raise(t, uB[c]); }
+  grad(A_TH, t); raise(t, uTH);
+  double dVB_B[3], dTH_v[3], dBv[3][3];         // grad(v.B).grad B^k, grad Theta.grad v^k, grad B^i.grad v^k
+  grad(A_VB, t);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) dVB_B[c] = dotp(t, uB[c]);
+  double sBv = 0.0, sBBvB = 0.0, sBvTh = 0.0, sBB = 0.0, sEE = 0.0, svv = 0.0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    grad(A_VU + c, t);
+    dTH_v[c] = dotp(t, uTH);
+#pragma unroll
+    for (int e = 0; e < 3; ++e) dBv[e][c] = dotp(t, uB[e]);
+    raise(t, r);
+    grad(A_VL + c, t2);
+    svv += dotp(t2, r);
+    sBv += dotp(t2, uB[c]);
+    sBvTh += a[A_BU + c] * dotp(t2, uTH);
+    grad(A_BL + c, t);
+    sBB += dotp(t, uB[c]);
+    grad(A_EU + c, t); raise(t, r);
+    grad(A_EL + c, t2);
+    sEE += dotp(t2, r);
+    sBBvB += a[A_BL + c] * dVB_B[c];
+  }
+  double dWW, dWR, dWH, dPR_R, dPE_E, dRE;
+  {
+    double uW[3], uR[3], uE[3];
+    grad(A_WM2, t); raise(t, uW); dWW = dotp(t, uW);
+    grad(A_RHO, t); dWR = dotp(t, uW); raise(t, uR);
+    grad(A_H, t); dWH = dotp(t, uW);
+    grad(A_DPR, t); dPR_R = dotp(t, uR);
+    grad(A_EPS, t); dRE = dotp(t, uR); raise(t, uE);
+    grad(A_DPE, t); dPE_E = dotp(t, uE);
+  }
+  const double p = __ldg(P + (size_t)PRESS * sp + pt);
+  a[A_VB] = val(A_VB); a[A_TH] = val(A_TH); a[A_WM2] = val(A_WM2); a[A_RHO] = val(A_RHO); a[A_H] = val(A_H); a[A_DPR] = val(A_DPR); a[A_DPE] = val(A_DPE);
+  LesDots D;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { D.dVB_B[c] = dVB_B[c]; D.dTH_v[c] = dTH_v[c]; for (int e = 0; e < 3; ++e) D.dBv[c][e] = dBv[c][e]; }
+  D.sBv = sBv; D.sBBvB = sBBvB; D.sBvTh = sBvTh; D.sBB = sBB; D.sEE = sEE; D.svv = svv;
+  D.dWW = dWW; D.dWR = dWR; D.dWH = dWH; D.dPR_R = dPR_R; D.dPE_E = dPE_E; D.dRE = dRE;
+  les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// The same computation with the auxiliary fields staged by the copy engine (default whenever the LESWORK slot admits a tensor map):
+// a CTA of 256 threads owns a 16 x 4 x 4 block of points; the 26 fields pass one at a time, in the order the streaming contraction
+// needs them, in 5 groups of 5-6 fields through two shared-memory buffers of 20 x 8 x 8 tiles (block + halo 2) filled by
+// cp.async.bulk.tensor with mbarrier completion, so the 12 stencil operands of a field are shared-memory loads with compile-time
+// offsets and the copy of group g+1 overlaps the arithmetic on group g (one barrier per group: a barrier per field leaves too little work
+// between barriers, measured 32.6 vs 29.2 ms per step for the L1 version at c1_256). (k_les_flux above fetches them through L1/L2 with one exposed latency per field at 8 warps/SM.)
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int LX = 16, LY = 4, LZ = 4, LH = 2, LSX = LX + 2 * LH, LSY = LY + 2 * LH, LSZ = LZ + 2 * LH, LTILE = LSX * LSY * LSZ, LGMAX = 6;
+// the fields pass in 5 groups (one barrier and one mbarrier wait per group, not per field): {B^c, Theta, v.B}, three times {v^c, v_c, B_c, E^c, E_c}, the 6 scalars
+__device__ constexpr int LGSTART[6] = {0, 5, 10, 15, 20, 26};
+constexpr size_t LES_SMEM = (size_t)2 * LGMAX * LTILE * sizeof(double) + 64;
+// order of passage: anchors B^c, Theta; v.B; then per component c: v^c, v_c, B_c, E^c, E_c; then W^-2, rho, h, dp/drho, eps, dp/deps
+__device__ constexpr int LORDER[NAUX] = {A_BU, A_BU + 1, A_BU + 2, A_TH, A_VB,
+                                         A_VU, A_VL, A_BL, A_EU, A_EL, A_VU + 1, A_VL + 1, A_BL + 1, A_EU + 1, A_EL + 1, A_VU + 2, A_VL + 2, A_BL + 2, A_EU + 2, A_EL + 2,
+                                         A_WM2, A_RHO, A_H, A_DPR, A_EPS, A_DPE};
+
+__global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
+                                                                  const double* __restrict__ P, size_t sp, double* __restrict__ Wk, size_t sw,
+                                                                  const __grid_constant__ CUtensorMap tmap) {
+  static_assert((LTILE * sizeof(double)) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
+  extern __shared__ __align__(128) double ring[];
+  uint64_t* full = (uint64_t*)(ring + 2 * LGMAX * LTILE);
+  const int tid = threadIdx.x, tx = tid % LX, ty = (tid / LX) % LY, tz = tid / (LX * LY);
+  const int i0 = 2 + blockIdx.x * LX, j0 = 2 + blockIdx.y * LY, k0 = 2 + blockIdx.z * LZ;      // array indices of the block's first point
+  const int i = i0 + tx, j = j0 + ty, k = k0 + tz;
+  const bool inside = i < d.mx - 2 && j < d.my - 2 && k < d.mz - 2;
+  const size_t pt = (size_t)min(k, d.mz - 3) * d.sz + (size_t)min(j, d.my - 3) * d.sy + min(i, d.mx - 3);
+  if (tid == 0) {
+#pragma unroll
+    for (int b = 0; b < 2; ++b) mbar_init(full + b, 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  auto issue = [&](int g) {                       // the box origin i0 - 2 = 16 blockIdx.x is even: on a 16-byte boundary
+    if (tid == 0) {
+      const int n0 = LGSTART[g], n1 = LGSTART[g + 1];
+      mbar_expect_tx(full + g % 2, (unsigned)(n1 - n0) * LTILE * (unsigned)sizeof(double));
+      for (int n = n0; n < n1; ++n) tma_load_4d(ring + ((g % 2) * LGMAX + (n - n0)) * LTILE, &tmap, full + g % 2, i0 - LH, j0 - LH, k0 - LH, LORDER[n]);
+    }
+  };
+  issue(0);
+  double gu[6];
+  const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
+  {
+    double g[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) g[c] = __ldg(U + (size_t)(GXX + c) * su + pt);
+    const double s = chi / (g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]));
+    gu[0] = (g[3] * g[5] - g[4] * g[4]) * s; gu[1] = (g[2] * g[4] - g[1] * g[5]) * s; gu[2] = (g[1] * g[4] - g[2] * g[3]) * s;
+    gu[3] = (g[0] * g[5] - g[2] * g[2]) * s; gu[4] = (g[1] * g[2] - g[0] * g[4]) * s; gu[5] = (g[0] * g[3] - g[1] * g[1]) * s;
+  }
+  const double p = __ldg(P + (size_t)PRESS * sp + pt);
+  const double c12[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
+  auto raise = [&](const double g[3], double r[3]) {
+    r[0] = gu[0] * g[0] + gu[1] * g[1] + gu[2] * g[2];
+    r[1] = gu[1] * g[0] + gu[3] * g[1] + gu[4] * g[2];
+    r[2] = gu[2] * g[0] + gu[4] * g[1] + gu[5] * g[2];
+  };
+  auto dotp = [](const double g[3], const double r[3]) { return g[0] * r[0] + g[1] * r[1] + g[2] * r[2]; };
+  const int ctr = ((tz + LH) * LSY + (ty + LH)) * LSX + (tx + LH);
+  double a[NAUX];
+  LesDots D;
+  D.sBv = D.sBBvB = D.sBvTh = D.sBB = D.sEE = D.svv = 0.0;
+  double uB[3][3], uTH[3], uV[3], uX[3], uR[3];      // raised gradients of the anchors: B^c, Theta, the current v^c, the current E^c / W^-2 / eps, rho
+#pragma unroll
+  for (int g5 = 0; g5 < 5; ++g5) {
+    __syncthreads();                                 // everybody is done reading the buffer the next copy overwrites
+    if (g5 + 1 < 5) issue(g5 + 1);
+    mbar_wait(full + g5 % 2, (g5 / 2) & 1);
+#pragma unroll
+   for (int n = LGSTART[g5]; n < LGSTART[g5 + 1]; ++n) {
+    const double* s = ring + ((g5 % 2) * LGMAX + (n - LGSTART[g5])) * LTILE + ctr;
+    constexpr int OX = 1, OY = LSX, OZ = LSX * LSY;
+    const int f = LORDER[n];
+    a[f] = s[0];
+    double g[3];
+    g[0] = (8.0 * (s[OX] - s[-OX]) - (s[2 * OX] - s[-2 * OX])) * c12[0];
+    g[1] = (8.0 * (s[OY] - s[-OY]) - (s[2 * OY] - s[-2 * OY])) * c12[1];
+    g[2] = (8.0 * (s[OZ] - s[-OZ]) - (s[2 * OZ] - s[-2 * OZ])) * c12[2];
+    if (n < 3) raise(g, uB[n]);                                            // B^c
+    else if (n == 3) raise(g, uTH);                                        // Theta
+    else if (n == 4) {                                                     // v.B
+#pragma unroll
+      for (int c = 0; c < 3; ++c) D.dVB_B[c] = dotp(g, uB[c]);
+    } else if (n < 20) {
+      const int c = (n - 5) / 5, w = (n - 5) % 5;
+      if (w == 0) {                                                        // v^c
+        D.dTH_v[c] = dotp(g, uTH);
+#pragma unroll
+        for (int e = 0; e < 3; ++e) D.dBv[e][c] = dotp(g, uB[e]);
+        raise(g, uV);
+      } else if (w == 1) {                                                 // v_c
+        D.svv += dotp(g, uV);
+        D.sBv += dotp(g, uB[c]);
+        D.sBvTh += a[A_BU + c] * dotp(g, uTH);
+      } else if (w == 2) {                                                 // B_c
+        D.sBB += dotp(g, uB[c]);
+        D.sBBvB += a[A_BL + c] * D.dVB_B[c];
+      } else if (w == 3) raise(g, uX);                                     // E^c
+      else D.sEE += dotp(g, uX);                                           // E_c
+    } else if (n == 20) { raise(g, uX); D.dWW = dotp(g, uX); }             // W^-2
+    else if (n == 21) { D.dWR = dotp(g, uX); raise(g, uR); }               // rho
+    else if (n == 22) D.dWH = dotp(g, uX);                                 // h
+    else if (n == 23) D.dPR_R = dotp(g, uR);                               // dp/drho
+    else if (n == 24) { D.dRE = dotp(g, uR); raise(g, uX); }               // eps
+    else D.dPE_E = dotp(g, uX);                                            // dp/deps
+   }
+  }
+  if (inside) les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
+}
+
 }  // namespace
 
 cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
                        double* Wk, size_t sw, cudaStream_t s) {
   k_les_aux<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
   if (d.mx > 4 && d.my > 4 && d.mz > 4) {
-    dim3 grid((d.mx - 4 + 127) / 128, d.my - 4, d.mz - 4);
-    k_les_flux<<<grid, 128, 0, s>>>(d, par, U, su, P, sp, A, sa, Wk, sw);
+    dim3 grid((d.mx - 4 + 15) / 16, (d.my - 4 + 3) / 4, (d.mz - 4 + 3) / 4), block(16, 4, 4);
+    CUtensorMap map;
+    static int attr[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    bool tma = dev >= 0 && dev < 64 && make_tensor_map_4d(d, A, sa, NAUX, LSX, LSY, LSZ, &map);
+    if (tma && !attr[dev]) { tma = cudaFuncSetAttribute(k_les_flux_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LES_SMEM) == cudaSuccess; attr[dev] = tma; }
+    if (tma) k_les_flux_tma<<<grid, LX * LY * LZ, LES_SMEM, s>>>(d, par, U, su, P, sp, Wk, sw, map);
+    else k_les_flux<<<grid, block, 0, s>>>(d, par, U, su, P, sp, A, sa, Wk, sw);
   }
   return cudaGetLastError();
 }
