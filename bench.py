@@ -369,7 +369,9 @@ def main():
         return min(alg_flops[k], exe[k]) if exe.get(k) is not None else alg_flops[k]
     achieved = claimed(dom) * zones / sec_per_launch / 1e12
     F_alg = sum(claimed(k) * (prof[k][1] / max(args.steps * nstages, 1)) for k in prof if prof[k][1] > 0)    # per zone-stage, launches per stage counted
-    F_exe = sum((exe[k] or 0.0) * (prof[k][1] / max(args.steps * nstages, 1)) for k in prof if prof[k][1] > 0) if cap else None
+    launched = [k for k in prof if prof[k][1] > 0]
+    F_exe = (sum(exe[k] * (prof[k][1] / max(args.steps * nstages, 1)) for k in launched)
+             if cap and all(exe.get(k) is not None for k in launched) else None)       # only when the capture covers every kernel of this workload
     step_tflops = F_alg * value / world / 1e12
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
                 "peak_source": "measured: FP64 DFMA probe of the library (mhd_probe_fp64_flops); nominal 37.2",
