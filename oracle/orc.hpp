@@ -2,7 +2,7 @@
 //
 // Plain, slow, single-threaded FP64 C++ restatement of the per-stage hot path of
 // MHDuet (arXiv 2510.13965): ghost fill, con2prim, CCZ4+GRMHD right-hand side and
-// the explicit Runge-Kutta combine, written step by step from PAPER.md in the
+// the explicit Runge-Kutta combine (plus M1, the LES term, WENO5 and the AMR transfer operators), written step by step from PAPER.md in the
 // paper's order and notation. It shares no code with the CUDA library under
 // paper_2510_13965_b200/csrc/. Only tests/, __graft_entry__.smoke() and the
 // cpu_baseline / --impl reference legs of bench.py may build, load or call it.
@@ -20,7 +20,10 @@
 // limits; App. C forms = Sec. II C forms; Jacobian vs finite differences; implicit-solve limits; (C11)-(C12) in a moving
 // fluid; fix-up branches; Schwarzschild beam; isotropic radiation and a null beam in wavy Minkowski = flux brackets and all
 // geometric sources of Eqs. 38-40 incl. R19 and the number flux; one hand-computed face of Eq. 77; odd-even switch as printed
-// and with the R33 guard).
+// and with the R33 guard), WENO5 (Eq. 70 at linear weights; smoothness indicators from their integral definition; order; ENO), AMR transfer
+// operators (printed coefficients of Eq. 80, polynomial exactness, Lagrange remainder, RK continuous-extension order conditions for Eqs. 58-59),
+// LES term (App. A closed forms = the Hessian contraction the appendix defines them by, through an independent multi-precision con2prim;
+// metric-rescaling covariance; factors of A11; Delta^2; place in Eq. 32), decomposed ghost fill = undecomposed ghost fill.
 // PARITY UNPINNED (readings of passages the paper leaves open; nothing in the paper or the mathematics fixes them): the values
 // of the implicit tableau (R1: Table II has no body), the error-policy parameter values (R10), the outflow boundary order
 // (R17), the choice of (log10 rho, log10 T, Ye) / (log10 p, log10 eps) as the table's interpolation variables (R26).
