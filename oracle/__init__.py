@@ -148,6 +148,7 @@ def _load(counting):
         L.orc_m1_backreaction.argtypes = [vp, vp, vp, vp, vp]
         L.orc_m1_gravity.argtypes = [vp, vp, vp, vp, vp]
         L.orc_evolve_imex.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, f64, i32]
+        L.orc_eos_dp.argtypes = [vp, f64, f64, f64, vp]
         L.orc_les_flux.argtypes = [vp, vp, vp, vp, vp]
         L.orc_les_HM_point.argtypes = [vp, vp, vp, f64, vp]
         L.orc_les_aux_point.argtypes = [vp, vp, f64, vp, vp, vp]
@@ -392,9 +393,9 @@ Oracle.dense_output = _dense_output
 
 
 # ---- LES gradient SGS term of the induction equation (App. A) ------------------------------------------
-LES_NAUX = 26
+LES_NAUX = 29
 LES_NAMES = ["Bu0", "Bu1", "Bu2", "vu0", "vu1", "vu2", "vl0", "vl1", "vl2", "Bl0", "Bl1", "Bl2", "El0", "El1", "El2", "Eu0", "Eu1", "Eu2",
-             "vB", "Theta", "Wm2", "rho", "eps", "h", "dpdrho", "dpdeps"]
+             "vB", "Theta", "Wm2", "rho", "eps", "h", "dpdrho", "dpdeps", "Ye", "dpdYe", "D"]
 
 
 def les_HM_point(a, da, gu, p):
@@ -418,5 +419,13 @@ def _les_flux(self, U, P):
     return L, A
 
 
+def _eos_dp(self, rho, eps, ye=0.3):
+    """(dp/drho at fixed eps, Ye; dp/deps at fixed rho, Ye; dp/dYe at fixed rho, eps)"""
+    out = np.zeros(3)
+    lib().orc_eos_dp(self.h, float(rho), float(eps), float(ye), _ptr(out))
+    return out
+
+
+Oracle.eos_dp = _eos_dp
 Oracle.les_aux_point = _les_aux_point
 Oracle.les_flux = _les_flux

@@ -162,8 +162,8 @@ void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double*
 
 // ---- LES gradient sub-grid-scale term of the induction equation (App. A Eqs. A11-A17); orc_les.cpp
 enum { LES_BU = 0, LES_VU = 3, LES_VL = 6, LES_BL = 9, LES_EL = 12, LES_EU = 15, LES_VB = 18, LES_TH = 19, LES_WM2 = 20, LES_RHO = 21, LES_EPS = 22,
-       LES_H = 23, LES_DPDRHO = 24, LES_DPDEPS = 25, LES_NAUX = 26 };
-void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps);
+       LES_H = 23, LES_DPDRHO = 24, LES_DPDEPS = 25, LES_YE = 26, LES_DPDYE = 27, LES_D = 28, LES_NAUX = 29 };
+void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps, double& dpdye);
 void les_aux_point(const Params& par, const double gl[3][3], double sqrtg, const double Bu[3], const double prim[NPRIM], double a[LES_NAUX]);
 void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], double p, double HM[3][3]);   // (A16)
 void les_flux(const Params& par, const Grid& G, const double* U, const double* P, double* L, double* A);                       // -alpha G_B^{ki}

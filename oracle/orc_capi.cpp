@@ -133,6 +133,8 @@ void orc_les_aux_point(void* hh, const double* gl9, double sqrtg, const double* 
   les_aux_point(((Handle*)hh)->par, (const double (*)[3])gl9, sqrtg, Bu, prim, a26);
 }
 
+void orc_eos_dp(void* hh, double rho, double eps, double ye, double* out3) { eos_dp(((Handle*)hh)->par, rho, eps, ye, out3[0], out3[1], out3[2]); }
+
 // ---- AMR transfer operators (grids passed explicitly: n[3], ng)
 static Grid mkgrid(const int* n, int ng) { return Grid{n[0], n[1], n[2], ng, 1.0, 1.0, 1.0}; }
 void orc_prolong(const int* nc, int ngc, const double* Uc, const int* nf, int ngf, double* Uf, int nfields, const int* origin, const int* lo, const int* hi) {

@@ -89,8 +89,28 @@ static TabPos tab_T_from_loge(const Params& par, TabPos r, TabPos y, double le) 
   return {it, (le - e_lo) / (e_hi - e_lo)};
 }
 
-// dp/drho at fixed eps and dp/deps at fixed rho (App. A, l.882: "analytically for hybrid EoSs, but only numerically for the tabulated ones")
-void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps) {
+// slope of the trilinear interpolant of table q along one axis (0: log10 rho, 1: log10 T, 2: Ye) inside the cell (r, t, y): the difference of the
+// two faces of the cell across that axis, each face bilinear in the other two variables, over the node spacing
+static double tab_slope(const Params& par, const double* q, TabPos r, TabPos t, TabPos y, int axis) {
+  double sum = 0.0;
+  for (int c1 = 0; c1 < 2; ++c1)
+    for (int c2 = 0; c2 < 2; ++c2) {
+      double w, hi, lo;
+      if (axis == 0) { w = (c1 ? t.w : 1.0 - t.w) * (c2 ? y.w : 1.0 - y.w); hi = tab_node(par, q, r.i + 1, t.i + c1, y.i + c2); lo = tab_node(par, q, r.i, t.i + c1, y.i + c2); }
+      else if (axis == 1) { w = (c1 ? r.w : 1.0 - r.w) * (c2 ? y.w : 1.0 - y.w); hi = tab_node(par, q, r.i + c1, t.i + 1, y.i + c2); lo = tab_node(par, q, r.i + c1, t.i, y.i + c2); }
+      else { w = (c1 ? r.w : 1.0 - r.w) * (c2 ? t.w : 1.0 - t.w); hi = tab_node(par, q, r.i + c1, t.i + c2, y.i + 1); lo = tab_node(par, q, r.i + c1, t.i + c2, y.i); }
+      sum += w * (hi - lo);
+    }
+  return sum / (axis == 0 ? par.dlr : axis == 1 ? par.dlT : par.dye);
+}
+
+// dp/drho at fixed (eps, Ye), dp/deps at fixed (rho, Ye), dp/dYe at fixed (rho, eps) (App. A, l.882: "analytically for hybrid EoSs, but only
+// numerically for the tabulated ones"). Table (reading R42): the derivatives of the interpolant itself inside the cell that holds (rho, T, Ye) —
+// with lp = log10 p, le = log10(eps + shift) trilinear in (lr, lT, Ye):  d lp/d lr at fixed le = lp_r - lp_T le_r / le_T,  d lp/d le at fixed lr =
+// lp_T / le_T,  d lp/d Ye at fixed (lr, le) = lp_Y - lp_T le_Y / le_T;  then dp/drho = (p/rho) d lp/d lr, dp/deps = p/(eps + shift) d lp/d le,
+// dp/dYe = p ln 10 d lp/d Ye.
+void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps, double& dpdye) {
+  dpdye = 0.0;
   if (par.eos_kind == 0) { dpdrho = (par.eos_gamma - 1.0) * eps; dpdeps = (par.eos_gamma - 1.0) * rho; return; }
   if (par.eos_kind == 1) {
     // p = p_cold + (Gamma_th - 1) rho (eps - eps_cold) (Eq. 30), d p_cold / d rho = Gamma_i p_cold / rho, d eps_cold / d rho = p_cold / rho^2
@@ -101,9 +121,15 @@ void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho
     dpdeps = gth * rho;
     return;
   }
-  const double hr = 1e-4 * rho, he = 1e-4 * (std::fabs(eps) + 1e-10);
-  dpdrho = (eos_from_rho_eps(par, rho + hr, eps, ye).p - eos_from_rho_eps(par, rho - hr, eps, ye).p) / (2.0 * hr);
-  dpdeps = (eos_from_rho_eps(par, rho, eps + he, ye).p - eos_from_rho_eps(par, rho, eps - he, ye).p) / (2.0 * he);
+  const TabPos r = tab_locate(std::log10(rho), par.lr0, par.dlr, par.n_rho);
+  const TabPos y = tab_locate(ye, par.ye0, par.dye, par.n_ye);
+  const TabPos t = tab_T_from_loge(par, r, y, std::log10(eps + par.tab_eps_shift));
+  const double p = std::pow(10.0, tab_interp(par, par.tab_logp, r, t, y));
+  const double lp_r = tab_slope(par, par.tab_logp, r, t, y, 0), lp_T = tab_slope(par, par.tab_logp, r, t, y, 1), lp_Y = tab_slope(par, par.tab_logp, r, t, y, 2);
+  const double le_r = tab_slope(par, par.tab_loge, r, t, y, 0), le_T = tab_slope(par, par.tab_loge, r, t, y, 1), le_Y = tab_slope(par, par.tab_loge, r, t, y, 2);
+  dpdrho = p / rho * (lp_r - lp_T * le_r / le_T);
+  dpdeps = p / (eps + par.tab_eps_shift) * (lp_T / le_T);
+  dpdye = p * std::log(10.0) * (lp_Y - lp_T * le_Y / le_T);
 }
 
 EosOut eos_from_rho_eps(const Params& par, double rho, double eps, double ye) {

@@ -23,7 +23,7 @@ namespace orc {
 
 static const int SYM[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
 
-// the 26 auxiliary fields whose gradients App. A needs, at one point
+// the 29 auxiliary fields whose gradients App. A needs, at one point
 void les_aux_point(const Params& par, const double gl[3][3], double sqrtg, const double Bu[3], const double prim[NPRIM], double a[LES_NAUX]) {
   const double rho = prim[RHO], eps = prim[EPS], p = prim[PRESS], W = prim[WLOR];
   double vu[3] = {prim[VX], prim[VY], prim[VZ]}, vl[3], Bl[3];
@@ -48,7 +48,9 @@ void les_aux_point(const Params& par, const double gl[3][3], double sqrtg, const
   a[LES_TH] = h * W * W + B2;
   a[LES_WM2] = 1.0 / (W * W);
   a[LES_RHO] = rho; a[LES_EPS] = eps; a[LES_H] = h;
-  eos_dp(par, rho, eps, prim[YE], a[LES_DPDRHO], a[LES_DPDEPS]);
+  eos_dp(par, rho, eps, prim[YE], a[LES_DPDRHO], a[LES_DPDEPS], a[LES_DPDYE]);
+  a[LES_YE] = prim[YE];
+  a[LES_D] = rho * W;
 }
 
 // H_M^{ki} of Eq. (A16) at one point: a = auxiliary fields, da[m] = their partial derivatives d_m, gu = gamma^{ij}, p = pressure
@@ -93,7 +95,9 @@ void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const 
   for (int i = 0; i < 3; ++i) for (int k = 0; k < 3; ++k) BvPsi += 0.5 * (Bl[i] * vl[k] - Bl[k] * vl[i]) * Psi_M[k][i];   // B_[i v_k] Psi_M^{ki}
   const double Psi_Th = Th / (Th - E2) * (sBB - sEE - BvPsi);
   const double Psi_A = W2 * (p * dpdeps + rho * rho * dpdrho);
-  // ---- H_p (A12); dp/dYe = 0 for the EoS kinds with analytic derivatives, its two terms are not built (kind 2: numerical, R39)
+  // ---- H_p (A12). The two Y_e terms are printed after the closing brace; the definition the appendix states (tau = -xi grad(dF/dC).grad C, checked
+  // numerically with a Y_e-dependent EoS) puts them INSIDE the braces with the factor rho of the first term (reading R42): rho [grad(dp/dYe).grad Ye -
+  // (2/D) dp/dYe grad Ye.grad D]
   double vPsi = 0.0;
   for (int j = 0; j < 3; ++j) vPsi += vl[j] * Psi_v[j];
   const double dWW = dot(LES_WM2, LES_WM2);
@@ -103,7 +107,8 @@ void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const 
       - (calE * dpdeps - Psi_A) * (0.25 * W2 * dWW + dot(LES_WM2, LES_RHO) / rho)
       - 2.0 / W2 * dpdeps * (sBB - W2 * W2 * dot(LES_WM2, LES_H))
       - (calE * dpdeps + Psi_A) * (vPsi + svv + W2 * dWW)
-      + Psi_Th / (calE * Th) * ((calE * dpdeps + Psi_A) * (Th - E2) - Psi_A * Th / W2);
+      + Psi_Th / (calE * Th) * ((calE * dpdeps + Psi_A) * (Th - E2) - Psi_A * Th / W2)
+      + rho * (dot(LES_DPDYE, LES_YE) - 2.0 / a[LES_D] * a[LES_DPDYE] * dot(LES_YE, LES_D));
   const double H_p = pref * brace;
   const double H_Th = Psi_Th + Th / (Th - E2) * H_p;                                        // (A13)
   double H_v[3];
