@@ -38,7 +38,8 @@ extern "C" {
 #define MHD_NWORK 33        /* 3 directions x (10 flux brackets of Eq. 32 + 1 speed bound of App. B) */
 #define MHD_NM1 15          /* (Nbar, Ebar, Fbar_i) x 3 neutrino species, field 5 s + {0..4} */
 #define MHD_NM1WORK 75      /* per species: 3 directions x (5 flux brackets + speed), kappa_a + kappa_s, P_ij */
-#define MHD_NLESWORK 26     /* auxiliary fields of the LES sub-grid-scale term (App. A): B^k, v^k, v_k, B_k, E_k, E^k, v.B, Theta, W^-2, rho, eps, h, dp/drho, dp/deps */
+#define MHD_NLESWORK 29     /* auxiliary fields of the LES sub-grid-scale term (App. A): B^k, v^k, v_k, B_k, E_k, E^k, v.B, Theta, W^-2, rho, eps, h, dp/drho, dp/deps,
+                               and (tabulated EoS only) Ye, dp/dYe, D */
 #define MHD_MAX_STAGES 8
 #define MHD_MAX_PIECES 8
 
@@ -122,8 +123,9 @@ typedef struct {
   double weno_eps;                 /* recon_kind 1: the epsilon added to the smoothness indicators (ref. [63]: 1e-6); must be > 0 */
   double les_C_M;                  /* App. A, Eq. (A11): coefficient C_M of the sub-grid-scale tensor of the induction equation (the paper's
                                       production value is 8); 0 = LES terms off. When non-zero: ng >= 5 (the gradients of the
-                                      auxiliary fields are needed at every node the reconstruction reads), eos_kind 0 or 1 (analytic dp/drho,
-                                      dp/deps, l.882), MHD_SLOT_LESWORK bound; otherwise mhd_patch_create / mhd_rhs refuse */
+                                      auxiliary fields are needed at every node the reconstruction reads) and MHD_SLOT_LESWORK bound; otherwise
+                                      mhd_patch_create / mhd_rhs refuse. dp/drho, dp/deps, dp/dYe: analytic for eos_kind 0 / 1, derivatives of the
+                                      interpolant inside the table cell for eos_kind 2 (l.882) */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */

@@ -17,7 +17,7 @@ NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
 SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
 NM1, NM1WORK = 15, 75
 SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1, SLOT_U1, SLOT_LESWORK = 13, 14, 15, 16, 24, 32, 33
-NLESWORK = 26
+NLESWORK = 29
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p

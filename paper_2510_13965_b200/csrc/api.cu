@@ -167,7 +167,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
   if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
-  if (desc->les_C_M != 0.0 && (desc->ng < 5 || desc->eos_kind == 2)) return MHD_E_UNSUPPORTED;
+  if (desc->les_C_M != 0.0 && desc->ng < 5) return MHD_E_UNSUPPORTED;
   if (desc->recon_kind < 0 || desc->recon_kind > 1 || (desc->recon_kind == 1 && !(desc->weno_eps > 0.0))) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
   if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2 ||

@@ -19,7 +19,74 @@ namespace mhd {
 namespace {
 
 enum { A_BU = 0, A_VU = 3, A_VL = 6, A_BL = 9, A_EL = 12, A_EU = 15, A_VB = 18, A_TH = 19, A_WM2 = 20, A_RHO = 21, A_EPS = 22, A_H = 23,
-       A_DPR = 24, A_DPE = 25, NAUX = MHD_NLESWORK };
+       A_DPR = 24, A_DPE = 25, A_YE = 26, A_DPY = 27, A_D = 28, NAUX = MHD_NLESWORK, NAUX_NOYE = 26 };   // the last three only with the tabulated EoS
+
+// ---- tabulated EoS: derivatives of the trilinear interpolant inside the cell that holds (rho, T, Ye) (reading R42)
+struct TabCell { int ir, it, iy; double wr, wt, wy; };
+__device__ __forceinline__ void tab_pos(double x, double x0, double idx, int n, int& i, double& w) {
+  double s = fmin(fmax((x - x0) * idx, 0.0), (double)(n - 1));
+  i = min((int)s, n - 2);
+  w = s - (double)i;
+}
+// value of table t at T node `it`, bilinear in (log10 rho, Ye)
+__device__ __forceinline__ double tab_column(const Par& q, const double* __restrict__ t, const TabCell& c, int it) {
+  const size_t b0 = ((size_t)c.iy * q.n_T + it) * q.n_rho + c.ir, b1 = b0 + (size_t)q.n_T * q.n_rho;
+  const double lo = __ldg(t + b0) + c.wr * (__ldg(t + b0 + 1) - __ldg(t + b0)), hi = __ldg(t + b1) + c.wr * (__ldg(t + b1 + 1) - __ldg(t + b1));
+  return lo + c.wy * (hi - lo);
+}
+__device__ __noinline__ void table_dp(const Par& q, double rho, double eps, double ye, double& dpr, double& dpe, double& dpy) {
+  TabCell c;
+  tab_pos(log10(rho), q.lr0, q.idlr, q.n_rho, c.ir, c.wr);
+  tab_pos(ye, q.ye0, q.idye, q.n_ye, c.iy, c.wy);
+  const double le = log10(eps + q.tab_eps_shift);
+  {                                                          // T by inversion of the interpolant along the monotone log T axis, clamped
+    int lo = 0, hi = q.n_T - 1;
+    double e_lo = tab_column(q, q.tab_loge, c, lo), e_hi = tab_column(q, q.tab_loge, c, hi);
+    if (le <= e_lo) { c.it = 0; c.wt = 0.0; }
+    else if (le >= e_hi) { c.it = q.n_T - 2; c.wt = 1.0; }
+    else {
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        const double em = tab_column(q, q.tab_loge, c, mid);
+        if (le >= em) { lo = mid; e_lo = em; } else { hi = mid; e_hi = em; }
+      }
+      c.it = lo; c.wt = (le - e_lo) / (e_hi - e_lo);
+    }
+  }
+  // the 8 corners of both tables; slope along an axis = difference of the two faces across it (each bilinear in the other two) / spacing
+  double sl[2][3], val = 0.0;
+#pragma unroll
+  for (int tb = 0; tb < 2; ++tb) {
+    const double* __restrict__ t = tb == 0 ? q.tab_logp : q.tab_loge;
+    double v[2][2][2];                                       // [rho][T][Ye]
+#pragma unroll
+    for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+      for (int ct = 0; ct < 2; ++ct) {
+        const size_t b = ((size_t)(c.iy + cy) * q.n_T + (c.it + ct)) * q.n_rho + c.ir;
+        v[0][ct][cy] = __ldg(t + b); v[1][ct][cy] = __ldg(t + b + 1);
+      }
+    const double wr[2] = {1.0 - c.wr, c.wr}, wt[2] = {1.0 - c.wt, c.wt}, wy[2] = {1.0 - c.wy, c.wy};
+    double sr = 0.0, st = 0.0, sy = 0.0, s0 = 0.0;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        sr += wt[a] * wy[b] * (v[1][a][b] - v[0][a][b]);
+        st += wr[a] * wy[b] * (v[a][1][b] - v[a][0][b]);
+        sy += wr[a] * wt[b] * (v[a][b][1] - v[a][b][0]);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) s0 += wr[a] * wt[b] * wy[e] * v[a][b][e];
+      }
+    sl[tb][0] = sr * q.idlr; sl[tb][1] = st * q.idlT; sl[tb][2] = sy * q.idye;
+    if (tb == 0) val = s0;
+  }
+  const double p = exp10(val);
+  dpr = p / rho * (sl[0][0] - sl[0][1] * sl[1][0] / sl[1][1]);
+  dpe = p / (eps + q.tab_eps_shift) * (sl[0][1] / sl[1][1]);
+  dpy = p * 2.302585092994045684 * (sl[0][2] - sl[0][1] * sl[1][2] / sl[1][1]);
+}
+
 
 __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                  const double* __restrict__ P, size_t sp, double* __restrict__ A, size_t sa) {
@@ -38,8 +105,9 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   const double Eu[3] = {-(vl[1] * Bl[2] - vl[2] * Bl[1]) * isg, -(vl[2] * Bl[0] - vl[0] * Bl[2]) * isg, -(vl[0] * Bl[1] - vl[1] * Bl[0]) * isg};
   const double El[3] = {g[0] * Eu[0] + g[1] * Eu[1] + g[2] * Eu[2], g[1] * Eu[0] + g[3] * Eu[1] + g[4] * Eu[2], g[2] * Eu[0] + g[4] * Eu[1] + g[5] * Eu[2]};
   const double h = rho * (1.0 + eps) + p;
-  double dpr, dpe;
+  double dpr, dpe, dpy = 0.0;
   if (par.eos_kind == 0) { dpr = (par.eos_gamma - 1.0) * eps; dpe = (par.eos_gamma - 1.0) * rho; }
+  else if (par.eos_kind == 2) table_dp(par, rho, eps, pr(YE), dpr, dpe, dpy);
   else {                                                       // hybrid: p = K rho^G + (Gth - 1) rho (eps - a - K rho^(G-1) / (G-1)) in the piece of rho
     int i = 0;
     while (i < par.n_pieces - 1 && rho >= par.pp_rho[i]) ++i;
@@ -57,10 +125,11 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   a[A_TH * sa] = h * W * W + (Bl[0] * Bu[0] + Bl[1] * Bu[1] + Bl[2] * Bu[2]);
   a[A_WM2 * sa] = 1.0 / (W * W);
   a[A_RHO * sa] = rho; a[A_EPS * sa] = eps; a[A_H * sa] = h; a[A_DPR * sa] = dpr; a[A_DPE * sa] = dpe;
+  if (par.eos_kind == 2) { a[A_YE * sa] = pr(YE); a[A_DPY * sa] = dpy; a[A_D * sa] = rho * W; }
 }
 
 // The closed forms (A12)-(A16) from the point values a[] and the contracted gradient products, and the update of the work slot
-struct LesDots { double dVB_B[3], dTH_v[3], dBv[3][3], sBv, sBBvB, sBvTh, sBB, sEE, svv, dWW, dWR, dWH, dPR_R, dPE_E, dRE; };
+struct LesDots { double dVB_B[3], dTH_v[3], dBv[3][3], sBv, sBBvB, sBvTh, sBB, sEE, svv, dWW, dWR, dWH, dPR_R, dPE_E, dRE, yterm; };   // yterm = grad(dp/dYe).grad Ye - (2/D) dp/dYe grad Ye.grad D
 
 __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, const double a[NAUX], const LesDots& D, double p, double chi, double al,
                                                  double* __restrict__ Wk, size_t sw, size_t pt) {
@@ -93,7 +162,8 @@ __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, 
                        - (calE * dpe - Psi_A) * (0.25 * W2 * dWW + dWR / rho)
                        - 2.0 * a[A_WM2] * dpe * (sBB - W2 * W2 * dWH)
                        - (calE * dpe + Psi_A) * (vPsi + svv + W2 * dWW)
-                       + Psi_Th * icalE * iTh * ((calE * dpe + Psi_A) * TmE - Psi_A * Th * a[A_WM2]);
+                       + Psi_Th * icalE * iTh * ((calE * dpe + Psi_A) * TmE - Psi_A * Th * a[A_WM2])
+                       + rho * D.yterm;                     // the Y_e terms of (A12), inside the braces (reading R42); zero unless the EoS is tabulated
   const double H_Th = Psi_Th + Th / TmE * (pref * brace);                                   // (A13)
   double H_v[3];
 #pragma unroll
@@ -194,6 +264,14 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
   for (int c = 0; c < 3; ++c) { D.dVB_B[c] = dVB_B[c]; D.dTH_v[c] = dTH_v[c]; for (int e = 0; e < 3; ++e) D.dBv[c][e] = dBv[c][e]; }
   D.sBv = sBv; D.sBBvB = sBBvB; D.sBvTh = sBvTh; D.sBB = sBB; D.sEE = sEE; D.svv = svv;
   D.dWW = dWW; D.dWR = dWR; D.dWH = dWH; D.dPR_R = dPR_R; D.dPE_E = dPE_E; D.dRE = dRE;
+  D.yterm = 0.0;
+  if (par.eos_kind == 2) {
+    double uY[3];
+    grad(A_YE, t); raise(t, uY);
+    grad(A_DPY, t2); const double dPY_Y = dotp(t2, uY);
+    grad(A_D, t2);
+    D.yterm = dPY_Y - 2.0 / val(A_D) * val(A_DPY) * dotp(t2, uY);
+  }
   les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
 }
 
@@ -208,12 +286,12 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int LX = 16, LY = 4, LZ = 4, LH = 2, LSX = LX + 2 * LH, LSY = LY + 2 * LH, LSZ = LZ + 2 * LH, LTILE = LSX * LSY * LSZ, LGMAX = 6;
 // the fields pass in 5 groups (one barrier and one mbarrier wait per group, not per field): {B^c, Theta, v.B}, three times {v^c, v_c, B_c, E^c, E_c}, the 6 scalars
-__device__ constexpr int LGSTART[6] = {0, 5, 10, 15, 20, 26};
+__device__ constexpr int LGSTART[7] = {0, 5, 10, 15, 20, 26, 29};   // the sixth group {Ye, dp/dYe, D} only with the tabulated EoS
 constexpr size_t LES_SMEM = (size_t)2 * LGMAX * LTILE * sizeof(double) + 64;
 // order of passage: anchors B^c, Theta; v.B; then per component c: v^c, v_c, B_c, E^c, E_c; then W^-2, rho, h, dp/drho, eps, dp/deps
 __device__ constexpr int LORDER[NAUX] = {A_BU, A_BU + 1, A_BU + 2, A_TH, A_VB,
                                          A_VU, A_VL, A_BL, A_EU, A_EL, A_VU + 1, A_VL + 1, A_BL + 1, A_EU + 1, A_EL + 1, A_VU + 2, A_VL + 2, A_BL + 2, A_EU + 2, A_EL + 2,
-                                         A_WM2, A_RHO, A_H, A_DPR, A_EPS, A_DPE};
+                                         A_WM2, A_RHO, A_H, A_DPR, A_EPS, A_DPE, A_YE, A_DPY, A_D};
 
 __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                                   const double* __restrict__ P, size_t sp, double* __restrict__ Wk, size_t sw,
@@ -262,11 +340,14 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   double a[NAUX];
   LesDots D;
   D.sBv = D.sBBvB = D.sBvTh = D.sBB = D.sEE = D.svv = 0.0;
+  D.yterm = 0.0;
+  const int ngroups = par.eos_kind == 2 ? 6 : 5;
   double uB[3][3], uTH[3], uV[3], uX[3], uR[3];      // raised gradients of the anchors: B^c, Theta, the current v^c, the current E^c / W^-2 / eps, rho
 #pragma unroll
-  for (int g5 = 0; g5 < 5; ++g5) {
+  for (int g5 = 0; g5 < 6; ++g5) {
+    if (g5 >= ngroups) break;                        // uniform over the grid
     __syncthreads();                                 // everybody is done reading the buffer the next copy overwrites
-    if (g5 + 1 < 5) issue(g5 + 1);
+    if (g5 + 1 < ngroups) issue(g5 + 1);
     mbar_wait(full + g5 % 2, (g5 / 2) & 1);
 #pragma unroll
    for (int n = LGSTART[g5]; n < LGSTART[g5 + 1]; ++n) {
@@ -304,7 +385,10 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
     else if (n == 22) D.dWH = dotp(g, uX);                                 // h
     else if (n == 23) D.dPR_R = dotp(g, uR);                               // dp/drho
     else if (n == 24) { D.dRE = dotp(g, uR); raise(g, uX); }               // eps
-    else D.dPE_E = dotp(g, uX);                                            // dp/deps
+    else if (n == 25) D.dPE_E = dotp(g, uX);                               // dp/deps
+    else if (n == 26) raise(g, uX);                                        // Ye
+    else if (n == 27) D.yterm = dotp(g, uX);                               // dp/dYe
+    else D.yterm -= 2.0 / a[A_D] * a[A_DPY] * dotp(g, uX);                 // D
    }
   }
   if (inside) les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
@@ -321,7 +405,7 @@ cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su
     static int attr[64] = {};
     int dev = 0;
     cudaGetDevice(&dev);
-    bool tma = dev >= 0 && dev < 64 && make_tensor_map_4d(d, A, sa, NAUX, LSX, LSY, LSZ, &map);
+    bool tma = dev >= 0 && dev < 64 && make_tensor_map_4d(d, A, sa, par.eos_kind == 2 ? NAUX : NAUX_NOYE, LSX, LSY, LSZ, &map);
     if (tma && !attr[dev]) { tma = cudaFuncSetAttribute(k_les_flux_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LES_SMEM) == cudaSuccess; attr[dev] = tma; }
     if (tma) k_les_flux_tma<<<grid, LX * LY * LZ, LES_SMEM, s>>>(d, par, U, su, P, sp, Wk, sw, map);
     else k_les_flux<<<grid, block, 0, s>>>(d, par, U, su, P, sp, A, sa, Wk, sw);

@@ -54,6 +54,7 @@ def test_les_flux_and_one_stage_parity(oracle_mod, kind):
     patch.work.zero_()
     binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
     Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
+    Ag, Ao = Ag[:26], Ao[:26]                                  # Ye, dp/dYe, D are staged only for the tabulated EoS (dp/dYe = 0 otherwise)
     den = np.abs(Ao).reshape(Ao.shape[0], -1).max(axis=1)
     ra = np.abs(Ag - Ao).reshape(Ao.shape[0], -1).max(axis=1) / np.where(den > 0, den, 1.0)
     assert np.all(ra < 1e-13), ra
@@ -115,5 +116,44 @@ def test_les_ragged_outflow_and_refusals(oracle_mod):
     # ghost width 3, and the tabulated EoS, are refused at create time
     with pytest.raises(binding.MhdError):
         binding.mhd_patch_create(binding.make_desc(synth.default_params(les_C_M=8.0), 8, 8, 8, 3, 0.1))
-    with pytest.raises(binding.MhdError):
-        binding.mhd_patch_create(binding.make_desc(synth.default_params(les_C_M=8.0, eos_kind=2), 8, 8, 8, 5, 0.1))
+
+
+def test_les_with_the_tabulated_eos(oracle_mod):
+    """config 4 (hot star, table EoS) with C_M = 8: the EoS derivatives are those of the interpolant inside the table cell (R42) and the
+    Y_e terms of (A12) are live (auxiliary fields Ye, dp/dYe, D). Auxiliary fields, SGS flux and one-stage RHS against the oracle."""
+    cfg = synth.config4(n=24, ng=NG)
+    cfg["params"].update(les_C_M=8.0)
+    cfg["U"][28:31] *= 300.0                                   # B^2 / p ~ 1e-3 in the core: the SGS tensor is not negligible
+    from paper_2510_13965_b200 import binding
+    n = cfg["n"]
+    o = oracle_mod.Oracle(cfg["params"], n[0], n[1], n[2], NG, cfg["dx"], table=cfg["table"])
+    U, P = cfg["U"].copy(), cfg["P"].copy()
+    o.prim2con(U, P)
+    patch = binding.Patch(cfg["params"], n, NG, cfg["dx"], stages=4, table=cfg["table"])
+    Uo = U.copy()
+    o.fill_ghosts(Uo, cfg["bc"])
+    Po, Fo = o.con2prim(Uo)
+    Lo, Ao = o.les_flux(Uo, Po)
+    Ko = o.rhs(Uo, Po)
+    patch.upload(U=U)
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    patch.work.zero_()
+    binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
+    Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
+    den = np.abs(Ao).reshape(Ao.shape[0], -1).max(axis=1)
+    for g0 in range(0, 18, 3):                                 # components of a vector share the vector's norm (v^z = 0 for rotation about z)
+        den[g0:g0 + 3] = den[g0:g0 + 3].max()
+    den[18] = den[3] * den[9]                                  # v.B vanishes analytically (azimuthal v, poloidal B): its scale is |v| |B|
+    ra = np.abs(Ag - Ao).reshape(Ao.shape[0], -1).max(axis=1) / np.where(den > 0, den, 1.0)
+    assert np.all(ra < 1e-11), [(int(f), float(ra[f])) for f in np.nonzero(ra >= 1e-11)[0]]     # primitives through the table's T inversion: 1e-11 (N3)
+    assert den[26] > 0 and den[27] > 0 and den[28] > 0         # Ye, dp/dYe, D are live
+    scale = np.abs(Lo).max()
+    for k in range(3):
+        for i in range(3):
+            assert np.abs(Wg[11 * k + 6 + i] - Lo[3 * k + i]).max() <= 1e-9 * scale, (k, i, np.abs(Wg[11 * k + 6 + i] - Lo[3 * k + i]).max() / scale)
+    Kg = patch.rhs(1).cpu().numpy()
+    rk, dn = _rel(Kg, Ko)
+    assert np.all(rk[dn > 0] < 1e-11), rk
+    patch.close()
