@@ -152,3 +152,21 @@ def test_dense_output_parity(oracle_mod, scheme, name):
     with pytest.raises(binding.MhdError):
         binding.mhd_dense_output(patch.h, scheme, 0.5, dt, 0, binding.SLOT_U0, patch.stream())
     patch.close()
+
+
+def test_prolong_tiled_path_ragged_boxes(oracle_mod):
+    """Boxes of at least 32 x 8 x 8 fine points take the separable shared-memory kernel: whole array and boxes that start on odd indices and end
+    inside a block, against the oracle; points outside the box keep their content."""
+    binding, pc, pf, Uc, Uf = _pair(30, (40, 12, 10), seed=5)
+    org = (5, 9, 10)
+    M = pf.U.shape[1:][::-1]
+    for lo, hi in (((0, 0, 0), M), ((1, 3, 2), (45, 17, 15)), ((7, 0, 5), (40, 9, 14))):
+        pf.upload(U=Uf)
+        binding.mhd_prolong(pc.h, binding.SLOT_U, pf.h, binding.SLOT_U, org, lo, hi, pf.stream())
+        want = oracle_mod.prolong(Uc, NG, Uf.copy(), NG, org, lo, hi)
+        got = pf.U.cpu().numpy()
+        assert np.abs(got - want).max() <= 1e-14 * np.abs(want).max(), (lo, hi)
+        mask = np.ones(got.shape[1:], bool)
+        mask[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]] = False
+        assert np.array_equal(got[:, mask], Uf[:, mask])
+    pc.close(); pf.close()
