@@ -88,6 +88,7 @@ __device__ __noinline__ void table_dp(const Par& q, double rho, double eps, doub
 }
 
 
+template <bool TABLE>
 __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                  const double* __restrict__ P, size_t sp, double* __restrict__ A, size_t sa) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -106,8 +107,8 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   const double El[3] = {g[0] * Eu[0] + g[1] * Eu[1] + g[2] * Eu[2], g[1] * Eu[0] + g[3] * Eu[1] + g[4] * Eu[2], g[2] * Eu[0] + g[4] * Eu[1] + g[5] * Eu[2]};
   const double h = rho * (1.0 + eps) + p;
   double dpr, dpe, dpy = 0.0;
-  if (par.eos_kind == 0) { dpr = (par.eos_gamma - 1.0) * eps; dpe = (par.eos_gamma - 1.0) * rho; }
-  else if (par.eos_kind == 2) table_dp(par, rho, eps, pr(YE), dpr, dpe, dpy);
+  if (TABLE) table_dp(par, rho, eps, pr(YE), dpr, dpe, dpy);
+  else if (par.eos_kind == 0) { dpr = (par.eos_gamma - 1.0) * eps; dpe = (par.eos_gamma - 1.0) * rho; }
   else {                                                       // hybrid: p = K rho^G + (Gth - 1) rho (eps - a - K rho^(G-1) / (G-1)) in the piece of rho
     int i = 0;
     while (i < par.n_pieces - 1 && rho >= par.pp_rho[i]) ++i;
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   a[A_TH * sa] = h * W * W + (Bl[0] * Bu[0] + Bl[1] * Bu[1] + Bl[2] * Bu[2]);
   a[A_WM2 * sa] = 1.0 / (W * W);
   a[A_RHO * sa] = rho; a[A_EPS * sa] = eps; a[A_H * sa] = h; a[A_DPR * sa] = dpr; a[A_DPE * sa] = dpe;
-  if (par.eos_kind == 2) { a[A_YE * sa] = pr(YE); a[A_DPY * sa] = dpy; a[A_D * sa] = rho * W; }
+  if (TABLE) { a[A_YE * sa] = pr(YE); a[A_DPY * sa] = dpy; a[A_D * sa] = rho * W; }
 }
 
 // The closed forms (A12)-(A16) from the point values a[] and the contracted gradient products, and the update of the work slot
@@ -398,7 +399,8 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
 
 cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
                        double* Wk, size_t sw, cudaStream_t s) {
-  k_les_aux<<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
+  if (par.eos_kind == 2) k_les_aux<true><<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
+  else k_les_aux<false><<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
   if (d.mx > 4 && d.my > 4 && d.mz > 4) {
     dim3 grid((d.mx - 4 + 15) / 16, (d.my - 4 + 3) / 4, (d.mz - 4 + 3) / 4), block(16, 4, 4);
     CUtensorMap map;

@@ -199,9 +199,10 @@ __device__ __forceinline__ double d1c(const double* __restrict__ u, long long s,
 __global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims d, double oe, const double* __restrict__ U, size_t su,
                                                 const double* __restrict__ V, size_t sv, const double* __restrict__ Wk, size_t sw,
                                                 double* __restrict__ KV, size_t sk) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= d.nx) return;
-  const size_t pt = (size_t)(blockIdx.z + d.ng) * d.sz + (size_t)(blockIdx.y + d.ng) * d.sy + (i + d.ng);
+  // a CTA owns a 16 x 4 x 2 block of zones: the y / z neighbours of the metric derivatives below are then mostly loaded by the same CTA (L1 hits)
+  const int i = blockIdx.x * 16 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z * 2 + threadIdx.z;
+  if (i >= d.nx || j >= d.ny || k >= d.nz) return;
+  const size_t pt = (size_t)(k + d.ng) * d.sz + (size_t)(j + d.ng) * d.sy + (i + d.ng);
   const long long st[3] = {1, d.sy, d.sz};
   const double h[3] = {d.dx, d.dy, d.dz};
 #pragma unroll 1
@@ -542,9 +543,8 @@ cudaError_t launch_m1_point(const Dims& d, const Par& par, const double* U, size
 }
 cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
                           double* KV, size_t sk, cudaStream_t s) {
-  dim3 grid((d.nx + 127) / 128, d.ny, d.nz);
   const double oe = par.m1_odd_even != 0 ? par.m1_oe_guard : -1.0;
-  k_m1_div<<<grid, 128, 0, s>>>(d, oe, U, su, V, sv, Wk, sw, KV, sk);
+  k_m1_div<<<dim3((d.nx + 15) / 16, (d.ny + 3) / 4, (d.nz + 1) / 2), dim3(16, 4, 2), 0, s>>>(d, oe, U, su, V, sv, Wk, sw, KV, sk);
   constexpr int SEG = 6;
   k_m1_march<1, SEG><<<dim3((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG), 128, 0, s>>>(d, oe, V, sv, Wk, sw, KV, sk);
   k_m1_march<2, SEG><<<dim3((d.nx + 127) / 128, d.ny, (d.nz + SEG - 1) / SEG), 128, 0, s>>>(d, oe, V, sv, Wk, sw, KV, sk);
