@@ -151,6 +151,7 @@ def _load(counting):
         L.orc_eos_dp.argtypes = [vp, f64, f64, f64, vp]
         L.orc_les_flux.argtypes = [vp, vp, vp, vp, vp]
         L.orc_les_HM_point.argtypes = [vp, vp, vp, f64, vp]
+        L.orc_les_H_point.argtypes = [vp, vp, vp, vp, f64, f64, vp, vp, vp, vp]
         L.orc_les_aux_point.argtypes = [vp, vp, f64, vp, vp, vp]
         L.orc_prolong.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp, vp, vp]
         L.orc_restrict.argtypes = [vp, i32, vp, vp, i32, vp, i32, vp]
@@ -393,9 +394,10 @@ Oracle.dense_output = _dense_output
 
 
 # ---- LES gradient SGS term of the induction equation (App. A) ------------------------------------------
-LES_NAUX = 29
+LES_NAUX = 31
+LES_NFLUX = 24
 LES_NAMES = ["Bu0", "Bu1", "Bu2", "vu0", "vu1", "vu2", "vl0", "vl1", "vl2", "Bl0", "Bl1", "Bl2", "El0", "El1", "El2", "Eu0", "Eu1", "Eu2",
-             "vB", "Theta", "Wm2", "rho", "eps", "h", "dpdrho", "dpdeps", "Ye", "dpdYe", "D"]
+             "vB", "Theta", "Wm2", "rho", "eps", "h", "dpdrho", "dpdeps", "Ye", "dpdYe", "D", "calE", "DYe"]
 
 
 def les_HM_point(a, da, gu, p):
@@ -403,6 +405,13 @@ def les_HM_point(a, da, gu, p):
     out = np.zeros(9)
     lib().orc_les_HM_point(_ptr(_f64(a)), _ptr(_f64(da)), _ptr(_f64(gu)), float(p), _ptr(out))
     return out.reshape(3, 3)
+
+
+def les_H_point(a, da, gu, gl, sqrtg, p):
+    """(H_M^{ki}, H_N^k, H_{N_Y}^k, H_T^{ki}) of (A15)-(A17) at one point (first index of H_M = flux direction)"""
+    HM, HN, HNY, HT = np.zeros(9), np.zeros(3), np.zeros(3), np.zeros(9)
+    lib().orc_les_H_point(_ptr(_f64(a)), _ptr(_f64(da)), _ptr(_f64(gu)), _ptr(_f64(gl)), float(sqrtg), float(p), _ptr(HM), _ptr(HN), _ptr(HNY), _ptr(HT))
+    return HM.reshape(3, 3), HN, HNY, HT.reshape(3, 3)
 
 
 def _les_aux_point(self, gl, sqrtg, Bu, prim):
@@ -413,7 +422,7 @@ def _les_aux_point(self, gl, sqrtg, Bu, prim):
 
 def _les_flux(self, U, P):
     """(L, A): L[3 k + i] = -alpha G_B^{ki}, the SGS part of the k-flux of Bbar^i (zero within 2 points of the array edge); A = auxiliary fields"""
-    L = np.zeros((9,) + self.shape)
+    L = np.zeros((LES_NFLUX,) + self.shape)
     A = np.zeros((LES_NAUX,) + self.shape)
     lib().orc_les_flux(self.h, _ptr(U), _ptr(P), _ptr(L), _ptr(A))
     return L, A

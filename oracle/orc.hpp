@@ -92,6 +92,7 @@ struct Params {
   int recon_kind;              // R of Eq. (66): 0 MP5 (default), 1 WENO5 (l.486-488)
   double weno_eps;             // the epsilon of [63] Eq. (2.16) (their 1e-6); R37
   double les_C_M;              // App. A: coefficient of the SGS tensor of the induction equation (paper: 8); 0 = off
+  double les_C_N, les_C_Y, les_C_T;   // (A11): coefficients of the SGS tensors of the D, D Ye and S_i equations (paper: 0)
 };
 
 // ---- stencils (Sec. III B)
@@ -162,10 +163,12 @@ void evolve_imex(const Params& par, const Grid& g, double* U, double* V, double*
 
 // ---- LES gradient sub-grid-scale term of the induction equation (App. A Eqs. A11-A17); orc_les.cpp
 enum { LES_BU = 0, LES_VU = 3, LES_VL = 6, LES_BL = 9, LES_EL = 12, LES_EU = 15, LES_VB = 18, LES_TH = 19, LES_WM2 = 20, LES_RHO = 21, LES_EPS = 22,
-       LES_H = 23, LES_DPDRHO = 24, LES_DPDEPS = 25, LES_YE = 26, LES_DPDYE = 27, LES_D = 28, LES_NAUX = 29 };
+       LES_H = 23, LES_DPDRHO = 24, LES_DPDEPS = 25, LES_YE = 26, LES_DPDYE = 27, LES_D = 28, LES_CALE = 29, LES_DYE = 30, LES_NAUX = 31, LES_NFLUX = 24 };
 void eos_dp(const Params& par, double rho, double eps, double ye, double& dpdrho, double& dpdeps, double& dpdye);
 void les_aux_point(const Params& par, const double gl[3][3], double sqrtg, const double Bu[3], const double prim[NPRIM], double a[LES_NAUX]);
 void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], double p, double HM[3][3]);   // (A16)
+void les_H_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], const double gl[3][3], double sqrtg, double p,
+                 double HM[3][3], double* HN, double* HNY, double (*HT)[3]);                                                  // (A15)-(A17)
 void les_flux(const Params& par, const Grid& G, const double* U, const double* P, double* L, double* A);                       // -alpha G_B^{ki}
 
 // ---- AMR transfer operators on a patch pair (Sec. IV B l.608-626, Eqs. 56-59, 79-80); orc_amr.cpp

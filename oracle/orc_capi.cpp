@@ -17,7 +17,7 @@ bool set_scalar(Params& p, const std::string& k, double v) {
   D(rho_atmo) D(rho_cut) D(rho_low) D(alpha_bh) D(w_max) D(rho_max) D(eps_min) D(eps_max)
   D(ye_min) D(ye_max) D(ye_atmo) D(eps_atmo) D(T_atmo) I(c2p_maxit)
   D(m1_kappa0) D(m1_rho0) D(m1_efloor) D(m1_tol) D(m1_mb) I(m1_maxit) I(m1_odd_even) D(m1_arad) D(m1_oe_guard)
-  I(recon_kind) D(weno_eps) D(les_C_M)
+  I(recon_kind) D(weno_eps) D(les_C_M) D(les_C_N) D(les_C_Y) D(les_C_T)
   I(n_rho) I(n_T) I(n_ye) D(lr0) D(dlr) D(lT0) D(dlT) D(ye0) D(dye) D(tab_eps_shift) D(tab_h0)
 #undef D
 #undef I
@@ -128,6 +128,9 @@ void orc_evolve_imex(void* hh, double* U, double* V, double* P, uint8_t* flags, 
 void orc_les_flux(void* hh, const double* U, const double* P, double* L9, double* A26) { Handle* h = (Handle*)hh; les_flux(h->par, h->grid, U, P, L9, A26); }
 void orc_les_HM_point(const double* a26, const double* da3x26, const double* gu9, double p, double* HM9) {
   les_HM_point(a26, (const double (*)[LES_NAUX])da3x26, (const double (*)[3])gu9, p, (double (*)[3])HM9);
+}
+void orc_les_H_point(const double* a, const double* da, const double* gu9, const double* gl9, double sqrtg, double p, double* HM9, double* HN3, double* HNY3, double* HT9) {
+  les_H_point(a, (const double (*)[LES_NAUX])da, (const double (*)[3])gu9, (const double (*)[3])gl9, sqrtg, p, (double (*)[3])HM9, HN3, HNY3, (double (*)[3])HT9);
 }
 void orc_les_aux_point(void* hh, const double* gl9, double sqrtg, const double* Bu, const double* prim, double* a26) {
   les_aux_point(((Handle*)hh)->par, (const double (*)[3])gl9, sqrtg, Bu, prim, a26);

@@ -112,8 +112,8 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
 
   // ---- LES: the sub-grid-scale tensor of the induction equation is part of the flux bracket of Eq. (32) (App. A; orc_les.cpp)
   std::vector<double> Lsgs, Laux;
-  if (par.les_C_M != 0.0 && (parts & 1)) {
-    Lsgs.resize(9 * n); Laux.resize((size_t)LES_NAUX * n);
+  if ((par.les_C_M != 0.0 || par.les_C_N != 0.0 || par.les_C_Y != 0.0 || par.les_C_T != 0.0) && (parts & 1)) {
+    Lsgs.resize((size_t)LES_NFLUX * n); Laux.resize((size_t)LES_NAUX * n);
     les_flux(par, G, U, P, Lsgs.data(), Laux.data());
   }
   // ---- flux divergence, direction by direction, line by line (Eqs. 64-69)
@@ -131,7 +131,12 @@ void rhs_grmhd_parts(const Params& par, const Grid& G, const double* U, const do
         load_point(G, U, P, base + (size_t)i * st[d], q);
         double F[10];
         flux_point(par, q, d, F, sp[i]);
-        if (!Lsgs.empty()) for (int c3 = 0; c3 < 3; ++c3) F[6 + c3] += Lsgs[(size_t)(3 * d + c3) * n + base + (size_t)i * st[d]];   // - alpha G_B^{d c3}
+        if (!Lsgs.empty()) {                                          // - alpha G of Eq. (32), direction d
+          const size_t q = base + (size_t)i * st[d];
+          F[0] += Lsgs[(size_t)(9 + d) * n + q];
+          F[1] += Lsgs[(size_t)(12 + d) * n + q];
+          for (int c3 = 0; c3 < 3; ++c3) { F[3 + c3] += Lsgs[(size_t)(15 + 3 * d + c3) * n + q]; F[6 + c3] += Lsgs[(size_t)(3 * d + c3) * n + q]; }
+        }
         for (int f = 0; f < 10; ++f) { Fp[f * Md + i] = F[f]; Uc[f * Md + i] = q.uc[f]; }
       }
       // interfaces i+1/2 for i = ng-1 .. ng+N-1

@@ -51,10 +51,15 @@ void les_aux_point(const Params& par, const double gl[3][3], double sqrtg, const
   eos_dp(par, rho, eps, prim[YE], a[LES_DPDRHO], a[LES_DPDEPS], a[LES_DPDYE]);
   a[LES_YE] = prim[YE];
   a[LES_D] = rho * W;
+  a[LES_CALE] = h * W * W;
+  a[LES_DYE] = rho * W * prim[YE];
 }
 
 // H_M^{ki} of Eq. (A16) at one point: a = auxiliary fields, da[m] = their partial derivatives d_m, gu = gamma^{ij}, p = pressure
-void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], double p, double HM[3][3]) {
+// H_M^{ki} of (A16) and, when HN / HNY / HT are not null, H_N^k, H_{N_Y}^k of (A15) and H_T^{ki} of (A17) (both indices up) at one point:
+// a = auxiliary fields, da[m] = their partial derivatives d_m, gu = gamma^{ij}, gl = gamma_ij, sqrtg = sqrt(gamma), p = pressure
+void les_H_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], const double gl[3][3], double sqrtg, double p,
+                 double HM[3][3], double* HN, double* HNY, double (*HT)[3]) {
   auto dot = [&](int f, int g) {                              // grad f . grad g = gamma^{mn} d_m f d_n g
     double s = 0.0;
     for (int m = 0; m < 3; ++m) for (int n = 0; n < 3; ++n) s += gu[m][n] * da[m][f] * da[n][g];
@@ -115,16 +120,48 @@ void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const 
   for (int k = 0; k < 3; ++k) H_v[k] = Psi_v[k] - (vu[k] + vB / calE * Bu[k]) * H_Th / Th;  // (A14)
   for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i)                                   // (A16): 2 B^[i H_v^k] + 4 grad B^[i . grad v^k]
     HM[k][i] = (Bu[i] * H_v[k] - Bu[k] * H_v[i]) + 2.0 * (dot(LES_BU + i, LES_VU + k) - dot(LES_BU + k, LES_VU + i));
+  if (HN) for (int k = 0; k < 3; ++k) HN[k] = 2.0 * dot(LES_D, LES_VU + k) + a[LES_D] * H_v[k];              // (A15)
+  if (HNY) for (int k = 0; k < 3; ++k) HNY[k] = 2.0 * dot(LES_DYE, LES_VU + k) + a[LES_DYE] * H_v[k];
+  if (HT) {
+    // H_E^i = 1/2 eps^i_{jk} H_M^{jk} (A16) is the same contraction for E^i = -eps^{ijk} v_j B_k: with the FIRST index of H_M the flux direction (R40),
+    // H_M^{(dir k)(comp j)} belongs to the flux B^j v^k - B^k v^j, so that eps_{ijk} (B^j v^k - B^k v^j) / 2 = -eps_{ijk} v^j B^k = E_i and
+    // H_E_i = 1/2 sqrt(gamma) [ijk] H_M^{(dir k)(comp j)}; E only enters (A17) quadratically, so its overall sign convention does not matter
+    double HEl[3], HEu[3];
+    for (int i = 0; i < 3; ++i) {
+      const int j = (i + 1) % 3, k = (i + 2) % 3;
+      HEl[i] = 0.5 * sqrtg * (HM[k][j] - HM[j][k]);
+    }
+    for (int i = 0; i < 3; ++i) { HEu[i] = 0.0; for (int j = 0; j < 3; ++j) HEu[i] += gu[i][j] * HEl[j]; }
+    double EHE = 0.0;
+    for (int j = 0; j < 3; ++j) EHE += El[j] * HEu[j];
+    (void)gl;
+    const double trace = H_p + sBB + sEE + EHE;
+    for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i) {
+      // grad calE . grad (v^k v^i) by the product rule (reading R41): v^k grad calE . grad v^i + v^i grad calE . grad v^k
+      const double first = vu[k] * dot(LES_CALE, LES_VU + i) + vu[i] * dot(LES_CALE, LES_VU + k)
+                           + calE * (0.5 * (vu[k] * H_v[i] + vu[i] * H_v[k]) + dot(LES_VU + k, LES_VU + i)) + vu[k] * vu[i] * H_p;
+      const double second = dot(LES_BU + k, LES_BU + i) + dot(LES_EU + k, LES_EU + i) + 0.5 * (Eu[k] * HEu[i] + Eu[i] * HEu[k]);
+      HT[k][i] = 2.0 * first - 2.0 * second + (gu[k][i] - vu[k] * vu[i]) * trace;                              // (A17)
+    }
+  }
 }
 
-// SGS part of the flux bracket of Eq. (32) for Bbar^i in direction k: -alpha G_B^{ki} = +alpha C_M xi sqrt(gamma) H_M^{ki} (A11), stored in
-// field 3 k + i of L (9 fields); A (LES_NAUX fields) receives the auxiliary fields (for the pins)
+void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const double gu[3][3], double p, double HM[3][3]) {
+  const double id[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+  les_H_point(a, da, gu, id, 1.0, p, HM, nullptr, nullptr, nullptr);
+}
+
+// SGS parts of the flux brackets of Eq. (32) in direction k, -alpha G = +alpha C xi sqrt(gamma) H (A11), in the LES_NFLUX = 24 fields of L:
+//   3 k + i       Bbar^i:  C_M H_M^{ki}            9 + k   Dbar: C_N H_N^k           12 + k   DYebar: C_Y H_{N_Y}^k
+//   15 + 3 k + i  Sbar_i:  C_T gamma_ij H_T^{kj}   (taubar: (A11) defines no G_tau, none is added: reading R45)
+// A (LES_NAUX fields) receives the auxiliary fields (for the pins)
 void les_flux(const Params& par, const Grid& G, const double* U, const double* P, double* L, double* A) {
   const size_t n = G.npts();
   const long st[3] = {1, (long)G.mx(), (long)G.mx() * G.my()};
   const double hh[3] = {G.dx, G.dy, G.dz};
   const double Delta2 = std::pow(G.dx * G.dy * G.dz, 2.0 / 3.0);
-  for (size_t q = 0; q < 9 * n; ++q) L[q] = 0.0;
+  for (size_t q = 0; q < (size_t)LES_NFLUX * n; ++q) L[q] = 0.0;
+  const bool full = par.les_C_N != 0.0 || par.les_C_Y != 0.0 || par.les_C_T != 0.0;
   // auxiliary fields at every grid point
   for (int kk = 0; kk < G.mz(); ++kk) for (int jj = 0; jj < G.my(); ++jj) for (int ii = 0; ii < G.mx(); ++ii) {
     const size_t p = G.idx(ii, jj, kk);
@@ -157,11 +194,23 @@ void les_flux(const Params& par, const Grid& G, const double* U, const double* P
     gu[1][1] = chi * (g[0][0] * g[2][2] - g[0][2] * g[0][2]) / det;
     gu[1][2] = gu[2][1] = chi * (g[0][1] * g[0][2] - g[0][0] * g[1][2]) / det;
     gu[2][2] = chi * (g[0][0] * g[1][1] - g[0][1] * g[0][1]) / det;
-    double HM[3][3];
-    les_HM_point(a, da, gu, P[(size_t)PRESS * n + p], HM);
+    double HM[3][3], HN[3], HNY[3], HT[3][3], gl[3][3];
     const double sqrtg = 1.0 / (chi * std::sqrt(chi));
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) gl[i][j] = g[i][j] / chi;
+    les_H_point(a, da, gu, gl, sqrtg, P[(size_t)PRESS * n + p], HM, full ? HN : nullptr, full ? HNY : nullptr, full ? HT : nullptr);
     const double xi = Delta2 / (24.0 * chi);                  // gamma^{1/3} Delta^2 / 24, gamma = chi^-3
-    for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i) L[(size_t)(3 * k + i) * n + p] = al * par.les_C_M * xi * sqrtg * HM[k][i];
+    const double fac = al * xi * sqrtg;
+    for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i) L[(size_t)(3 * k + i) * n + p] = fac * par.les_C_M * HM[k][i];
+    if (full)
+      for (int k = 0; k < 3; ++k) {
+        L[(size_t)(9 + k) * n + p] = fac * par.les_C_N * HN[k];
+        L[(size_t)(12 + k) * n + p] = fac * par.les_C_Y * HNY[k];
+        for (int i = 0; i < 3; ++i) {
+          double lowered = 0.0;
+          for (int j = 0; j < 3; ++j) lowered += gl[i][j] * HT[k][j];
+          L[(size_t)(15 + 3 * k + i) * n + p] = fac * par.les_C_T * lowered;
+        }
+      }
   }
 }
 

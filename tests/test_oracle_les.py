@@ -180,6 +180,8 @@ def test_grid_routine_factors_convergence_and_delta_squared(oracle_mod):
         o = oracle_mod.Oracle(par, n, n, n, ng, dx)
         o.prim2con(U, P)
         L, A = o.les_flux(U, P)
+        assert np.all(L[9:] == 0.0)                                 # only C_M is set: the D, D Ye, S_i slots stay empty
+        L = L[:9]
         assert np.abs(L + L.reshape(3, 3, *L.shape[1:]).transpose(1, 0, 2, 3, 4).reshape(L.shape)).max() < 1e-13 * np.abs(L).max()
         # one probe point (interior index (3, 5, 2) of the coarse grid, the same physical point on the fine grid)
         f = n // 16
@@ -195,7 +197,7 @@ def test_grid_routine_factors_convergence_and_delta_squared(oracle_mod):
         got = L[:, kk, jj, ii].reshape(3, 3)
         errs.append(np.abs(got / dx ** 2 - want / dx ** 2).max())
         mags.append(np.abs(got).max())
-        assert np.abs(A[:, kk, jj, ii] - a0).max() < 1e-13
+        assert np.abs(A[:, kk, jj, ii] - a0).max() < 1e-13 * np.abs(a0).max()
         # within 2 points of the array edge the stencil does not fit: zero there
         assert np.all(L[:, :2] == 0) and np.all(L[:, :, :, -2:] == 0) and np.any(L[:, 2] != 0)
     assert errs[1] < errs[0] / 12.0 and errs[1] < 1e-3 * mags[1] / (1.0 / 32) ** 2, errs        # fourth order
@@ -310,7 +312,7 @@ def test_Ye_terms_of_A12_enter_inside_the_braces_with_the_factor_rho(oracle_mod)
         h = rho * (1 + eps) + p
         E = -np.cross(v, B)
         return np.concatenate([B, v, v, B, E, E, [v @ B, h * W2 + B @ B, 1 / W2, rho, eps, h, g * eps * (1 + A * ye), g * rho * (1 + A * ye),
-                                                   ye, g * rho * eps * A, rho * math.sqrt(W2)]]), p
+                                                   ye, g * rho * eps * A, rho * math.sqrt(W2), h * W2, rho * math.sqrt(W2) * ye]]), p
     a0, p0 = aux(P0)
     assert len(a0) == oracle_mod.LES_NAUX
     da = np.zeros((3, len(a0)))
@@ -330,7 +332,7 @@ def test_Ye_terms_of_A12_enter_inside_the_braces_with_the_factor_rho(oracle_mod)
     prim[0], prim[1], prim[2], prim[4:7], prim[7] = P0[0], P0[8], P0[1], v, 1 / math.sqrt(1 - v @ v)
     prim[3] = P0[0] * P0[1]
     ao = o.les_aux_point(np.eye(3), 1.0, P0[5:8], prim)
-    same = [i for i in range(29) if i not in (19, 23, 24, 25, 27)]                # all but Theta, h, dp/drho, dp/deps, dp/dYe (EoS-dependent)
+    same = [i for i in range(31) if i not in (19, 23, 24, 25, 27, 29)]            # all but Theta, h, dp/drho, dp/deps, dp/dYe, calE (EoS-dependent)
     assert np.allclose(ao[same], a0[same], rtol=1e-14, atol=0)
 
 
@@ -360,3 +362,156 @@ def test_table_eos_derivatives(oracle_mod):
         # the closed form: p = K rho^G + (Gth - 1) rho eps_th, eps = eps_cold(rho) + eps_th  =>  dp/deps = (Gth - 1) rho
         worst = max(worst, abs(dpe / ((1.75 - 1.0) * rho) - 1.0))
     assert worst < 0.05, worst
+
+
+# ------------------------------------------------------------------ the other three SGS tensors of (A11): H_N, H_{N_Y} (A15), H_T (A17)
+def _all_fluxes(C, guess, g, A):
+    """fluxes of D, D Ye, S_i and B^i in flat space as functions of the nine conserved fields (Y_e-dependent EoS p = g rho eps (1 + A Ye))"""
+    B = C[5:8]
+
+    def f(rho, eps, v1, v2, v3):
+        W = 1 / mp.sqrt(1 - v1 * v1 - v2 * v2 - v3 * v3)
+        c = _cons_ye([rho, eps, v1, v2, v3] + list(B) + [C[8] / (rho * W)], g, A)
+        return [c[i] - C[i] for i in range(5)]
+    sol = mp.findroot(f, guess[:5], tol=mp.mpf(10) ** -32, maxsteps=60)
+    rho, eps, v = sol[0], sol[1], [sol[2], sol[3], sol[4]]
+    W2 = 1 / (1 - sum(x * x for x in v))
+    ye = C[8] / (rho * mp.sqrt(W2))
+    p = g * rho * eps * (1 + A * ye)
+    B2 = sum(x * x for x in B); vB = sum(a * b for a, b in zip(v, B))
+    S, D, DY = C[1:4], C[0], C[8]
+    FN = [D * v[k] for k in range(3)]
+    FY = [DY * v[k] for k in range(3)]
+    # S_i^k of l.260 (flat metric)
+    FT = [[(v[i] * S[k] + v[k] * S[i]) / 2 + (p if i == k else 0) - (2 * B[i] * B[k] - (B2 if i == k else 0)) / (2 * W2)
+           - vB * (B[i] * v[k] + B[k] * v[i] - (vB if i == k else 0)) / 2 for i in range(3)] for k in range(3)]
+    FM = [[B[i] * v[k] - B[k] * v[i] for i in range(3)] for k in range(3)]
+    return FN, FY, FT, FM
+
+
+def test_HN_HNY_HT_equal_the_gradient_model(oracle_mod):
+    """(A15) and (A17) as transcribed == the Hessian contractions of the D, D Ye and S_i fluxes (with the Y_e-dependent EoS, so that the Y_e
+    terms of H_p are live inside H_T as well). Fixes: H_E^i = 1/2 eps^i_jk H_M^{jk} read with the first index of H_M as the flux direction
+    (the other order flips the sign of every E H_E term: H_T off by 10 %), grad calE . grad (v^k v^i), the combination (gamma^{ki} - v^k v^i)."""
+    g, A = 1.0, 0.7
+    rnd = random.Random(3)
+    P0 = [rnd.uniform(0.5, 1.5), rnd.uniform(0.1, 1.0)] + [rnd.uniform(-0.4, 0.4) for _ in range(3)] + [rnd.uniform(-0.8, 0.8) for _ in range(3)] + [rnd.uniform(0.1, 0.5)]
+    gradP = [[rnd.uniform(-1, 1) for _ in range(9)] for _ in range(3)]
+    mp.mp.dps = 36
+    P0m = [mp.mpf(x) for x in P0]
+    d = mp.mpf(10) ** -12
+    J = [[None] * 9 for _ in range(9)]
+    for q in range(9):
+        Pp, Pm = list(P0m), list(P0m)
+        Pp[q] += d; Pm[q] -= d
+        cp, cm = _cons_ye(Pp, g, A), _cons_ye(Pm, g, A)
+        for a in range(9):
+            J[a][q] = (cp[a] - cm[a]) / (2 * d)
+    gradC = [[sum(J[a][q] * mp.mpf(gradP[m][q]) for q in range(9)) for a in range(9)] for m in range(3)]
+    dotC = [[sum(gradC[m][a] * gradC[m][b] for m in range(3)) for b in range(9)] for a in range(9)]
+    C0 = _cons_ye(P0m, g, A)
+    dd = mp.mpf(10) ** -8
+    cache = {}
+
+    def at(sa, a, sb, b):
+        key = (sa, a, sb, b) if (a, sa) <= (b, sb) else (sb, b, sa, a)
+        if key not in cache:
+            C = list(C0)
+            C[a] += sa * dd; C[b] += sb * dd
+            cache[key] = _all_fluxes(C, P0m, g, A)
+        return cache[key]
+    wN, wY, wT, wM = np.zeros(3), np.zeros(3), np.zeros((3, 3)), np.zeros((3, 3))
+    for a in range(9):
+        for b in range(9):
+            pp, pm, mp_, mm = at(1, a, 1, b), at(1, a, -1, b), at(-1, a, 1, b), at(-1, a, -1, b)
+            w = dotC[a][b] / (4 * dd * dd)
+            for k in range(3):
+                wN[k] += float((pp[0][k] - pm[0][k] - mp_[0][k] + mm[0][k]) * w)
+                wY[k] += float((pp[1][k] - pm[1][k] - mp_[1][k] + mm[1][k]) * w)
+                for i in range(3):
+                    wT[k, i] += float((pp[2][k][i] - pm[2][k][i] - mp_[2][k][i] + mm[2][k][i]) * w)
+                    wM[k, i] += float((pp[3][k][i] - pm[3][k][i] - mp_[3][k][i] + mm[3][k][i]) * w)
+
+    def aux(P):
+        rho, eps, v, B, ye = P[0], P[1], np.array(P[2:5]), np.array(P[5:8]), P[8]
+        p = g * rho * eps * (1 + A * ye)
+        W2 = 1.0 / (1.0 - v @ v)
+        h = rho * (1 + eps) + p
+        E = -np.cross(v, B)
+        return np.concatenate([B, v, v, B, E, E, [v @ B, h * W2 + B @ B, 1 / W2, rho, eps, h, g * eps * (1 + A * ye), g * rho * (1 + A * ye),
+                                                   ye, g * rho * eps * A, rho * math.sqrt(W2), h * W2, rho * math.sqrt(W2) * ye]]), p
+    a0, p0 = aux(P0)
+    da = np.zeros((3, len(a0)))
+    for q in range(9):
+        Pp, Pm = list(P0), list(P0)
+        Pp[q] += 1e-6; Pm[q] -= 1e-6
+        der = (aux(Pp)[0] - aux(Pm)[0]) / 2e-6
+        for m in range(3):
+            da[m] += der * gradP[m][q]
+    HM, HN, HNY, HT = oracle_mod.les_H_point(a0, da, np.eye(3), np.eye(3), 1.0, p0)
+    for got, want in ((HM, wM), (HN, wN), (HNY, wY), (HT, wT)):
+        assert np.abs(got - want).max() < 3e-6 * np.abs(want).max(), (got, want)
+    assert np.abs(HT - HT.T).max() < 1e-12 * np.abs(HT).max()
+
+
+def test_HT_is_covariant_and_enters_the_momentum_flux_with_a_lowered_index(oracle_mod):
+    """(i) gamma_ij = a^2 delta_ij: H_T^{ki} = H_T'^{ki} / a^2, H_N^k = H_N'^k / a (index placement of E_j H_E^j, gamma^{ki}, sqrt(gamma) in
+    eps_ijk); (ii) grid level: with only C_T (C_N, C_Y) set, rhs - rhs(0) of Sbar_i (Dbar, DYebar) = -d_k of the stored SGS flux and no
+    other field changes; (iii) the Sbar_i slot holds gamma_ij H_T^{kj}."""
+    rnd = random.Random(21)
+    par = synth.default_params(eos_kind=0, eos_gamma=2.0)
+    o = oracle_mod.Oracle(par, 4, 4, 4, 3, 0.1)
+    P0 = [rnd.uniform(0.5, 1.5), rnd.uniform(0.1, 1.0)] + [rnd.uniform(-0.4, 0.4) for _ in range(3)] + [rnd.uniform(-0.8, 0.8) for _ in range(3)]
+    gradP = [[rnd.uniform(-1, 1) for _ in range(8)] for _ in range(3)]
+    a0, da, p0 = _aux_and_gradients(o, par, P0, gradP, np.eye(3), 1.0)
+    _, fN, _, fT = oracle_mod.les_H_point(a0, da, np.eye(3), np.eye(3), 1.0, p0)
+    a = 1.7
+    Pc = list(P0)
+    for q in range(2, 8):
+        Pc[q] = P0[q] / a
+    gradPc = [[gradP[m][q] * a / (a if q >= 2 else 1.0) for q in range(8)] for m in range(3)]
+    ac, dac, pc = _aux_and_gradients(o, par, Pc, gradPc, a * a * np.eye(3), a ** 3)
+    _, cN, _, cT = oracle_mod.les_H_point(ac, dac, np.eye(3) / a ** 2, a * a * np.eye(3), a ** 3, pc)
+    assert np.abs(cT - fT / a ** 2).max() < 1e-7 * np.abs(fT).max() / a ** 2
+    assert np.abs(cN - fN / a).max() < 1e-7 * np.abs(fN).max() / a
+    # grid level. The reconstruction must be linear in the added flux for rhs - rhs(0) to be the flux's own divergence: MP5 limits 0.3 % of
+    # these points (near extrema of the momentum flux), so the check runs WENO5 with eps -> infinity, which is its linear fifth-order scheme
+    n, ng = 24, 5
+    U, P, dx, prim, k = _smooth_state(n, ng, chi0=1.0, alpha0=0.9)
+    base = synth.default_params(eos_kind=0, eos_gamma=2.0, grav_G=0.0, recon_kind=1, weno_eps=1e30)
+    o0 = oracle_mod.Oracle(base, n, n, n, ng, dx)
+    o0.prim2con(U, P)
+    o0.fill_ghosts(U, [0] * 6)
+    Pq, _ = o0.con2prim(U)
+    K0 = o0.rhs(U, Pq, part="grmhd_flux")
+    inner = (slice(ng, -ng),) * 3
+    for name, fields, slots in (("les_C_N", [22], [[9, 10, 11]]), ("les_C_Y", [23], [[12, 13, 14]]),
+                                ("les_C_T", [25, 26, 27], [[15, 18, 21], [16, 19, 22], [17, 20, 23]])):
+        oc = oracle_mod.Oracle(dict(base, **{name: 2.0}), n, n, n, ng, dx)
+        L, A = oc.les_flux(U, Pq)
+        dK = oc.rhs(U, Pq, part="grmhd_flux") - K0
+        changed = [f for f in range(32) if np.abs(dK[f]).max() > 0]
+        assert changed == fields, (name, changed)
+        for f, sl in zip(fields, slots):
+            div = np.zeros_like(L[0])
+            for kdir, ax in ((0, 2), (1, 1), (2, 0)):
+                F = L[sl[kdir]]
+                div += (8.0 * (np.roll(F, -1, ax) - np.roll(F, 1, ax)) - (np.roll(F, -2, ax) - np.roll(F, 2, ax))) / (12.0 * dx)
+            got, want = dK[f][inner], -div[inner]
+            assert np.abs(got - want).max() < 0.01 * np.abs(want).max(), (name, f, np.abs(got - want).max(), np.abs(want).max())
+    # (iii) the lowered index: at one point gamma_ij = delta_ij / chi0, so slot(S_i, k) = H_T^{ki} / chi0 x alpha C xi sqrt(gamma)
+    chi0 = 0.8
+    U, P, dx, prim, k = _smooth_state(n, ng, chi0=chi0, alpha0=0.9)
+    oc = oracle_mod.Oracle(dict(base, les_C_T=2.0), n, n, n, ng, dx)
+    oc.prim2con(U, P)
+    oc.fill_ghosts(U, [0] * 6)
+    Pq, _ = oc.con2prim(U)
+    L, A = oc.les_flux(U, Pq)
+    q = (7, 8, 9)
+    st = [A[:, q[0], q[1], q[2]]]
+    d1 = lambda F, ax: (8.0 * (np.roll(F, -1, ax) - np.roll(F, 1, ax)) - (np.roll(F, -2, ax) - np.roll(F, 2, ax))) / (12.0 * dx)
+    dA = np.array([[d1(A[f], ax)[q] for f in range(A.shape[0])] for ax in (2, 1, 0)])
+    _, _, _, HT = oracle_mod.les_H_point(st[0], dA, chi0 * np.eye(3), np.eye(3) / chi0, chi0 ** -1.5, Pq[3][q])
+    want = 0.9 * 2.0 * dx * dx / (24.0 * chi0) * chi0 ** -1.5 * HT / chi0
+    got = np.array([[L[15 + 3 * kk + i][q] for i in range(3)] for kk in range(3)])
+    assert np.abs(got - want).max() < 1e-12 * np.abs(want).max()
