@@ -28,16 +28,16 @@ METRIC = "zone-stage updates/s"
 STAGES = 4
 
 
-def workload_inputs(name, n, les_cm=0.0):
+def workload_inputs(name, n, les_cm=0.0, les_other=0.0):
     """Seeded synthetic inputs (paper_2510_13965_b200.synth); returns cfg dict with U (metric, Bbar), P (rho, Ye, eps, v)."""
     from paper_2510_13965_b200 import synth
     if name == "c1" and les_cm != 0.0:      # LES sub-grid-scale term on (App. A, C_M): ghost width 5, ideal gas
         cfg = synth.config1_tiled(n, ng=5)
-        cfg["params"].update(les_C_M=les_cm)
+        cfg["params"].update(les_C_M=les_cm, les_C_N=les_other, les_C_Y=les_other, les_C_T=les_other)
         return cfg
     if name == "c4" and les_cm != 0.0:      # the paper's production setting: tabulated EoS + C_M = 8
         cfg = synth.config4(n=n, ng=5)
-        cfg["params"].update(les_C_M=les_cm)
+        cfg["params"].update(les_C_M=les_cm, les_C_N=les_other, les_C_Y=les_other, les_C_T=les_other)
         return cfg
     if les_cm != 0.0:
         raise ValueError("--les-cm is available for the workloads c1 and c4")
@@ -115,13 +115,13 @@ def cpu_info():
     return {"nproc": os.cpu_count() or 1, "cpu_model": model}
 
 
-def oracle_leg(cfg_name, n_sample, steps, threads=1, les_cm=0.0):
+def oracle_leg(cfg_name, n_sample, steps, threads=1, les_cm=0.0, les_other=0.0):
     """The oracle as it stands on a bounded sample of the workload: threads = 1 is the plain single-threaded build, threads > 1 the
     -fopenmp build of the same sources (outermost grid loops only, arithmetic unchanged); returns (value, seconds, zone_stages, threads)."""
     import oracle
     from paper_2510_13965_b200 import synth
     threads = oracle.use_threads(threads)
-    cfg = workload_inputs(cfg_name, n_sample, les_cm)
+    cfg = workload_inputs(cfg_name, n_sample, les_cm, les_other)
     n = cfg["n"]
     o = oracle.Oracle(cfg["params"], n[0], n[1], n[2], cfg["ng"], cfg["dx"], table=cfg.get("table"))
     U, P = cfg["U"].copy(), cfg["P"].copy()
@@ -170,10 +170,10 @@ def run_reference(args):
     vals = []
     nthr = max(1, args.ref_threads)
     for _ in range(args.warmup):
-        oracle_leg(args.workload, 16, 1, args.ref_threads, args.les_cm)
+        oracle_leg(args.workload, 16, 1, args.ref_threads, args.les_cm, args.les_other)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        v, sec, zs, nthr = oracle_leg(args.workload, n_s, 1, args.ref_threads, args.les_cm)
+        v, sec, zs, nthr = oracle_leg(args.workload, n_s, 1, args.ref_threads, args.les_cm, args.les_other)
         vals.append((zs, sec))
     total = time.perf_counter() - t0
     value = sum(z for z, _ in vals) / sum(s for _, s in vals)
@@ -201,6 +201,7 @@ def main():
     ap.add_argument("--ref-threads", type=int, default=1, help="--impl reference: threads of the oracle (1 = the plain build)")
     ap.add_argument("--decomp", default=None, help="e.g. 1x1x2: ONE patch split into bricks over the ranks, halo exchange fused with the ghost fill "
                                                    "(strong scaling; needs world = product, or world 1 for the self-neighbour check); default: replicas")
+    ap.add_argument("--les-other", type=float, default=0.0, help="with --les-cm: the other three SGS coefficients C_N = C_Y = C_T of App. A (the paper's runs: 0)")
     ap.add_argument("--les-cm", type=float, default=0.0, help="workloads c1 / c4 with the LES sub-grid-scale term of the induction equation, C_M (paper: 8); ghost width 5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -224,7 +225,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    cfg = workload_inputs(args.workload, args.n, args.les_cm)
+    cfg = workload_inputs(args.workload, args.n, args.les_cm, args.les_other)
     n, ng = cfg["n"], cfg["ng"]
     m1 = "V" in cfg
     nstages = 3 if m1 else STAGES
@@ -402,9 +403,9 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        v, sec, zs, _ = oracle_leg(args.workload, args.ref_n, 1, les_cm=args.les_cm)
+        v, sec, zs, _ = oracle_leg(args.workload, args.ref_n, 1, les_cm=args.les_cm, les_other=args.les_other)
         nall = os.cpu_count() or 1
-        va, seca, _, nthr = oracle_leg(args.workload, args.ref_n, 1, threads=nall, les_cm=args.les_cm) if nall > 1 else (v, sec, zs, 1)
+        va, seca, _, nthr = oracle_leg(args.workload, args.ref_n, 1, threads=nall, les_cm=args.les_cm, les_other=args.les_other) if nall > 1 else (v, sec, zs, 1)
         cpu = dict({"value": v, "unit": "zone-stages/s", "cores": 1, "kind": "oracle",
                     "sample": "%d^3 instance of workload %s, 1 RK step (%.1f s), single thread" % (args.ref_n, args.workload, sec),
                     "all_cores": {"value": va, "cores": nthr, "seconds": seca, "build": "-fopenmp on the outermost grid loops, arithmetic unchanged"},
@@ -419,7 +420,7 @@ def main():
         "metric": METRIC, "value": value, "unit": "zone-stages/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": "%s_%d%s" % (args.workload, args.n, "_les%g" % args.les_cm if args.les_cm else ""), "grid": list(n), "ghosts": ng, "rk": "rk4", "eos_kind": cfg["params"]["eos_kind"],
+        "config": {"workload": "%s_%d%s" % (args.workload, args.n, ("_les%g" % args.les_cm + ("_nyt%g" % args.les_other if args.les_other else "")) if args.les_cm else ""), "grid": list(n), "ghosts": ng, "rk": "rk4", "eos_kind": cfg["params"]["eos_kind"],
                    "l2": "inputs (32 fields x %.0f MB) far larger than L2; no flush needed" % (patch.npts * 8 / 1e6),
                    "non_atmosphere_fraction": 1.0 - status["n_atmo"] / status["n_points"], "parallelism": "replicas" if world > 1 else "single"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(v[1] for v in prof.values())),

@@ -38,8 +38,8 @@ extern "C" {
 #define MHD_NWORK 33        /* 3 directions x (10 flux brackets of Eq. 32 + 1 speed bound of App. B) */
 #define MHD_NM1 15          /* (Nbar, Ebar, Fbar_i) x 3 neutrino species, field 5 s + {0..4} */
 #define MHD_NM1WORK 75      /* per species: 3 directions x (5 flux brackets + speed), kappa_a + kappa_s, P_ij */
-#define MHD_NLESWORK 29     /* auxiliary fields of the LES sub-grid-scale term (App. A): B^k, v^k, v_k, B_k, E_k, E^k, v.B, Theta, W^-2, rho, eps, h, dp/drho, dp/deps,
-                               and (tabulated EoS only) Ye, dp/dYe, D */
+#define MHD_NLESWORK 31     /* auxiliary fields of the LES sub-grid-scale terms (App. A): B^k, v^k, v_k, B_k, E_k, E^k, v.B, Theta, W^-2, rho, eps, h, dp/drho, dp/deps,
+                               (tabulated EoS only) Ye, dp/dYe, (that or any of C_N, C_Y, C_T) D, (any of C_N, C_Y, C_T) calE = h W^2, D Ye */
 #define MHD_MAX_STAGES 8
 #define MHD_MAX_PIECES 8
 
@@ -60,7 +60,7 @@ enum {
   MHD_SLOT_U1 = MHD_SLOT_R1 + MHD_MAX_STAGES,    /* optional third state buffer (MHD_NSTATE fields): lets mhd_advance fuse the RK combine
                                                     into the right-hand-side kernels (the new stage state cannot overwrite the one
                                                     whose stencils are being read); unbound = separate combine kernel */
-  MHD_SLOT_LESWORK = MHD_SLOT_U1 + 1,            /* scratch of the LES term (MHD_NLESWORK fields); needed when les_C_M != 0 */
+  MHD_SLOT_LESWORK = MHD_SLOT_U1 + 1,            /* scratch of the LES term (MHD_NLESWORK fields); needed when any LES coefficient != 0 */
   MHD_NSLOTS = MHD_SLOT_LESWORK + 1
 };
 
@@ -126,6 +126,9 @@ typedef struct {
                                       auxiliary fields are needed at every node the reconstruction reads) and MHD_SLOT_LESWORK bound; otherwise
                                       mhd_patch_create / mhd_rhs refuse. dp/drho, dp/deps, dp/dYe: analytic for eos_kind 0 / 1, derivatives of the
                                       interpolant inside the table cell for eos_kind 2 (l.882) */
+  double les_C_N, les_C_Y, les_C_T; /* App. A, Eqs. (A11), (A15), (A17): coefficients of the sub-grid-scale tensors H_N^k (flux of Dbar), H_{N_Y}^k (flux of
+                                      DYebar) and gamma_ij H_T^{kj} (flux of Sbar_i; H_E from the curl of H_M, R44); the paper's runs leave them 0
+                                      (PAPER.md:863). taubar receives no SGS flux ((A11) defines none, R45). Same requirements as les_C_M when any is non-zero */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */
@@ -201,8 +204,9 @@ int mhd_rhs(mhd_patch *p, int slot_state, int slot_prim, int slot_rhs, void *cud
 /* LES (App. A Eqs. A11-A17): the sub-grid-scale tensor of the induction equation. Computes the auxiliary
  * fields of App. A at every grid point into MHD_SLOT_LESWORK and ADDS -alpha G_B^{ki} = alpha C_M xi sqrt(gamma) H_M^{ki}
  * (xi = gamma^{1/3} Delta^2 / 24, Delta = (dx dy dz)^{1/3}) to the pointwise flux of Bbar^i in direction k held in MHD_SLOT_WORK
- * (field 11 k + 6 + i), at every point at least 2 points inside the array. mhd_rhs calls it between the pointwise fluxes and the
- * reconstruction when les_C_M != 0; exposed for tests and for callers that sequence the right-hand side themselves. */
+ * (field 11 k + 6 + i), at every point at least 2 points inside the array; with les_C_N / les_C_Y / les_C_T set also alpha C xi sqrt(gamma) x
+ * H_N^k (field 11 k), H_{N_Y}^k (field 11 k + 1), gamma_ij H_T^{kj} (field 11 k + 3 + i). mhd_rhs calls it between the pointwise fluxes and the
+ * reconstruction when any LES coefficient != 0; exposed for tests and for callers that sequence the right-hand side themselves. */
 int mhd_les_flux(mhd_patch *p, int slot_state, int slot_prim, void *cuda_stream);
 
 /* a9 — explicit RK combine on the interior (Eq. 53).

@@ -17,7 +17,7 @@ NSTATE, NPRIM, NWORK, MAX_STAGES, MAX_PIECES = 32, 10, 33, 8, 8
 SLOT_U, SLOT_U0, SLOT_P, SLOT_FLAGS, SLOT_WORK, SLOT_K1 = 0, 1, 2, 3, 4, 5
 NM1, NM1WORK = 15, 75
 SLOT_V, SLOT_V0, SLOT_M1WORK, SLOT_KV1, SLOT_R1, SLOT_U1, SLOT_LESWORK = 13, 14, 15, 16, 24, 32, 33
-NLESWORK = 29
+NLESWORK = 31
 OK = 0
 
 _d, _i, _p = ctypes.c_double, ctypes.c_int, ctypes.c_void_p
@@ -43,7 +43,7 @@ class mhd_patch_desc(ctypes.Structure):
         ("m1_kappa0", _d), ("m1_rho0", _d), ("m1_species_scale", _d * 3), ("m1_efloor", _d), ("m1_tol", _d), ("m1_mb", _d),
         ("m1_maxit", _i), ("m1_odd_even", _i),
         ("m1_arad", _d), ("m1_oe_guard", _d),
-        ("recon_kind", _i), ("weno_eps", _d), ("les_C_M", _d),
+        ("recon_kind", _i), ("weno_eps", _d), ("les_C_M", _d), ("les_C_N", _d), ("les_C_Y", _d), ("les_C_T", _d),
     ]
 
 
@@ -351,7 +351,7 @@ class Patch:
                        [(SLOT_K1 + j, k) for j, k in enumerate(self.K)]:
             mhd_patch_bind(self.h, slot, t.data_ptr(), self.npts)
         self.leswork = None
-        if float(params.get("les_C_M", 0.0)) != 0.0:             # LES sub-grid-scale term: scratch for the auxiliary fields of App. A
+        if any(float(params.get(c, 0.0)) != 0.0 for c in ("les_C_M", "les_C_N", "les_C_Y", "les_C_T")):             # LES sub-grid-scale term: scratch for the auxiliary fields of App. A
             self.leswork = z(NLESWORK)
             mhd_patch_bind(self.h, SLOT_LESWORK, self.leswork.data_ptr(), self.npts)
         self.U1 = None

@@ -21,6 +21,7 @@ bool slot_ok(const mhd_patch* p, int slot) { return slot >= 0 && slot < MHD_NSLO
 bool is_state_slot(int slot) { return slot == MHD_SLOT_U || slot == MHD_SLOT_U0 || slot == MHD_SLOT_U1 || (slot >= MHD_SLOT_K1 && slot < MHD_SLOT_K1 + MHD_MAX_STAGES); }
 bool is_m1_slot(int slot) { return slot >= MHD_SLOT_V && slot < MHD_SLOT_U1 && slot != MHD_SLOT_M1WORK; }
 int les_impl(mhd_patch* p, int slot_state, int slot_prim, cudaStream_t s);
+bool les_on(const Par& q) { return q.les_C_M != 0.0 || q.les_C_N != 0.0 || q.les_C_Y != 0.0 || q.les_C_T != 0.0; }
 double* dptr(const mhd_patch* p, int slot) { return (double*)p->slot[slot].ptr; }
 
 // piecewise-polytrope continuity constants: K_i, a_i for i > 0
@@ -62,7 +63,7 @@ int rhs_impl(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, const Fu
   { Timed tm(p, 2, s); if (launch_ccz4_algebra(p->dims, p->par, U, su, P, sp, K, sk, s) != cudaSuccess) return MHD_E_CUDA; }
   { Timed tm(p, 8, s); if (launch_adv_ko(p->dims, p->par, U, su, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA; }
   { Timed tm(p, 7, s); if (launch_point_flux(p->dims, p->par, U, su, P, sp, Wk, sw, s) != cudaSuccess) return MHD_E_CUDA; }
-  if (p->par.les_C_M != 0.0) { const int rc = les_impl(p, slot_state, slot_prim, s); if (rc != MHD_OK) return rc; }
+  if (les_on(p->par)) { const int rc = les_impl(p, slot_state, slot_prim, s); if (rc != MHD_OK) return rc; }
   for (int dir = 0; dir < 3; ++dir) {
     Timed tm(p, 3 + dir, s);
     if (launch_recon(dir, p->dims, p->par, U, su, Wk, sw, K, sk, fz, s) != cudaSuccess) return MHD_E_CUDA;
@@ -167,7 +168,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   if (!(desc->dx > 0.0 && desc->dy > 0.0 && desc->dz > 0.0)) return MHD_E_ARG;
   if (desc->n_species != 0 && desc->n_species != 3) return MHD_E_UNSUPPORTED;
   if (desc->eos_kind < 0 || desc->eos_kind > 2) return MHD_E_ARG;
-  if (desc->les_C_M != 0.0 && desc->ng < 5) return MHD_E_UNSUPPORTED;
+  if ((desc->les_C_M != 0.0 || desc->les_C_N != 0.0 || desc->les_C_Y != 0.0 || desc->les_C_T != 0.0) && desc->ng < 5) return MHD_E_UNSUPPORTED;
   if (desc->recon_kind < 0 || desc->recon_kind > 1 || (desc->recon_kind == 1 && !(desc->weno_eps > 0.0))) return MHD_E_ARG;
   if (desc->eos_kind == 1 && (desc->n_pieces < 1 || desc->n_pieces > MHD_MAX_PIECES)) return MHD_E_ARG;
   if (desc->eos_kind == 2 && (!desc->tab_logp || !desc->tab_loge || !desc->tab_cs2 || desc->n_rho < 2 || desc->n_T < 2 || desc->n_ye < 2 ||
@@ -206,7 +207,7 @@ int mhd_patch_create(const mhd_patch_desc* desc, mhd_patch** out) {
   q.m1_tol = desc->m1_tol > 0.0 ? desc->m1_tol : 1e-13; q.m1_mb = desc->m1_mb; q.m1_maxit = desc->m1_maxit > 0 ? desc->m1_maxit : 30;
   for (int i = 0; i < 3; ++i) q.m1_species_scale[i] = desc->m1_species_scale[i];
   q.m1_odd_even = desc->m1_odd_even; q.m1_arad = desc->m1_arad; q.m1_oe_guard = desc->m1_oe_guard;
-  q.recon_kind = desc->recon_kind; q.weno_eps = desc->weno_eps; q.les_C_M = desc->les_C_M;
+  q.recon_kind = desc->recon_kind; q.weno_eps = desc->weno_eps; q.les_C_M = desc->les_C_M; q.les_C_N = desc->les_C_N; q.les_C_Y = desc->les_C_Y; q.les_C_T = desc->les_C_T;
   p->d_counts = nullptr;
   if (cudaMalloc(&p->d_counts, 48 * sizeof(unsigned long long)) != cudaSuccess) { delete p; return MHD_E_CUDA; }
   if (cudaMemset(p->d_counts, 0, 48 * sizeof(unsigned long long)) != cudaSuccess) { cudaFree(p->d_counts); delete p; return MHD_E_CUDA; }
@@ -359,7 +360,7 @@ int mhd_rhs(mhd_patch* p, int slot_state, int slot_prim, int slot_rhs, void* str
 
 int mhd_les_flux(mhd_patch* p, int slot_state, int slot_prim, void* stream) {
   if (!p || !is_state_slot(slot_state) || slot_prim != MHD_SLOT_P) return MHD_E_ARG;
-  if (p->par.les_C_M == 0.0) return MHD_E_ARG;
+  if (!les_on(p->par)) return MHD_E_ARG;
   if (!slot_ok(p, slot_state) || !slot_ok(p, slot_prim)) return MHD_E_UNBOUND;
   return les_impl(p, slot_state, slot_prim, (cudaStream_t)stream);
 }

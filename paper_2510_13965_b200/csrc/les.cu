@@ -13,13 +13,17 @@
 // EoS derivatives: analytic for the ideal gas and the hybrid piecewise polytrope (l.882); the tabulated EoS is not supported here.
 #include "mhd_internal.cuh"
 #include "tma.cuh"
+#include <utility>
 
 namespace mhd {
 
 namespace {
 
 enum { A_BU = 0, A_VU = 3, A_VL = 6, A_BL = 9, A_EL = 12, A_EU = 15, A_VB = 18, A_TH = 19, A_WM2 = 20, A_RHO = 21, A_EPS = 22, A_H = 23,
-       A_DPR = 24, A_DPE = 25, A_YE = 26, A_DPY = 27, A_D = 28, NAUX = MHD_NLESWORK, NAUX_NOYE = 26 };   // the last three only with the tabulated EoS
+       A_DPR = 24, A_DPE = 25, A_YE = 26, A_DPY = 27, A_D = 28, A_CALE = 29, A_DYE = 30, NAUX = MHD_NLESWORK, NAUX_NOYE = 26 };
+// Ye, dp/dYe only with the tabulated EoS; D with it or with FULL; calE, D Ye only with FULL (any of C_N, C_Y, C_T set: (A15), (A17))
+static_assert(NAUX == 31, "MHD_NLESWORK and the field list disagree");
+__host__ __device__ constexpr int sym3(int i, int j) { return i == j ? (i == 0 ? 0 : i == 1 ? 3 : 5) : (i + j == 1 ? 1 : i + j == 2 ? 2 : 4); }
 
 // ---- tabulated EoS: derivatives of the trilinear interpolant inside the cell that holds (rho, T, Ye) (reading R42)
 struct TabCell { int ir, it, iy; double wr, wt, wy; };
@@ -88,7 +92,7 @@ __device__ __noinline__ void table_dp(const Par& q, double rho, double eps, doub
 }
 
 
-template <bool TABLE>
+template <bool TABLE, bool FULL>
 __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                  const double* __restrict__ P, size_t sp, double* __restrict__ A, size_t sa) {
   const long long pt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -126,13 +130,20 @@ __global__ void __launch_bounds__(128) k_les_aux(const __grid_constant__ Dims d,
   a[A_TH * sa] = h * W * W + (Bl[0] * Bu[0] + Bl[1] * Bu[1] + Bl[2] * Bu[2]);
   a[A_WM2 * sa] = 1.0 / (W * W);
   a[A_RHO * sa] = rho; a[A_EPS * sa] = eps; a[A_H * sa] = h; a[A_DPR * sa] = dpr; a[A_DPE * sa] = dpe;
-  if (TABLE) { a[A_YE * sa] = pr(YE); a[A_DPY * sa] = dpy; a[A_D * sa] = rho * W; }
+  if (TABLE) { a[A_YE * sa] = pr(YE); a[A_DPY * sa] = dpy; }
+  if (TABLE || FULL) a[A_D * sa] = rho * W;
+  if (FULL) { a[A_CALE * sa] = h * W * W; a[A_DYE * sa] = rho * W * pr(YE); }
 }
 
 // The closed forms (A12)-(A16) from the point values a[] and the contracted gradient products, and the update of the work slot
 struct LesDots { double dVB_B[3], dTH_v[3], dBv[3][3], sBv, sBBvB, sBvTh, sBB, sEE, svv, dWW, dWR, dWH, dPR_R, dPE_E, dRE, yterm; };   // yterm = grad(dp/dYe).grad Ye - (2/D) dp/dYe grad Ye.grad D
 
-__device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, const double a[NAUX], const LesDots& D, double p, double chi, double al,
+// the additional products of (A15) and (A17): grad B^k.grad B^i, grad v^k.grad v^i, grad E^k.grad E^i (symmetric, sym3 order) and grad D, grad(D Ye), grad calE . grad v^k
+struct LesFull { double dBB[6], dvv[6], dEE[6], dD_v[3], dDY_v[3], dCE_v[3]; };
+
+template <bool FULL>
+__device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, const double a[NAUX], const LesDots& D, const LesFull& X, const double gu[6],
+                                                 double p, double chi, double al, const double* __restrict__ U, size_t su,
                                                  double* __restrict__ Wk, size_t sw, size_t pt) {
   const double (&dVB_B)[3] = D.dVB_B; const double (&dTH_v)[3] = D.dTH_v; const double (&dBv)[3][3] = D.dBv;
   const double sBv = D.sBv, sBBvB = D.sBBvB, sBvTh = D.sBvTh, sBB = D.sBB, sEE = D.sEE, svv = D.svv;
@@ -171,18 +182,64 @@ __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, 
   for (int c = 0; c < 3; ++c) H_v[c] = Psi_v[c] - (a[A_VU + c] + vB * icalE * a[A_BU + c]) * H_Th * iTh;   // (A14)
   // (A11): xi = gamma^{1/3} Delta^2 / 24 = Delta^2 / (24 chi), sqrt(gamma) = chi^(-3/2)
   const double Delta2 = pow(d.dx * d.dy * d.dz, 2.0 / 3.0);
-  const double fac = al * par.les_C_M * Delta2 / (24.0 * chi) / (chi * sqrt(chi));
+  const double sqrtg = 1.0 / (chi * sqrt(chi));
+  const double fac0 = al * Delta2 / (24.0 * chi) * sqrtg, fac = fac0 * par.les_C_M;
+  double HM[3][3];
 #pragma unroll
   for (int kk = 0; kk < 3; ++kk)
 #pragma unroll
     for (int ii = 0; ii < 3; ++ii) {
+      HM[kk][ii] = 0.0;
       if (ii == kk) continue;
-      const double HM = (a[A_BU + ii] * H_v[kk] - a[A_BU + kk] * H_v[ii]) + 2.0 * (dBv[ii][kk] - dBv[kk][ii]);   // (A16)
-      double* w = Wk + (size_t)(11 * kk + 6 + ii) * sw + pt;
-      *w += fac * HM;
+      HM[kk][ii] = (a[A_BU + ii] * H_v[kk] - a[A_BU + kk] * H_v[ii]) + 2.0 * (dBv[ii][kk] - dBv[kk][ii]);   // (A16)
+      if (!FULL || par.les_C_M != 0.0) {
+        double* w = Wk + (size_t)(11 * kk + 6 + ii) * sw + pt;
+        *w += fac * HM[kk][ii];
+      }
     }
+  if constexpr (FULL) {
+  // ---- (A15): H_N^k = 2 grad D . grad v^k + D H_v^k, the same with D Ye; fluxes of Dbar (field 0) and DYebar (field 1)
+#pragma unroll
+  for (int kk = 0; kk < 3; ++kk) {
+    double* w = Wk + (size_t)(11 * kk) * sw + pt;
+    if (par.les_C_N != 0.0) w[0] += fac0 * par.les_C_N * (2.0 * X.dD_v[kk] + a[A_D] * H_v[kk]);
+    if (par.les_C_Y != 0.0) w[sw] += fac0 * par.les_C_Y * (2.0 * X.dDY_v[kk] + a[A_DYE] * H_v[kk]);
+  }
+  if (par.les_C_T == 0.0) return;
+  // ---- (A17) with H_E_i = 1/2 sqrt(gamma) [ijk] H_M^{(dir k)(comp j)} (reading R44), the flux of Sbar_i is gamma_ij H_T^{kj}
+  const double H_p = pref * brace;
+  double HEl[3], HEu[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { const int j = (c + 1) % 3, k = (c + 2) % 3; HEl[c] = 0.5 * sqrtg * (HM[k][j] - HM[j][k]); }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) HEu[c] = gu[sym3(c, 0)] * HEl[0] + gu[sym3(c, 1)] * HEl[1] + gu[sym3(c, 2)] * HEl[2];
+  const double EHE = a[A_EL] * HEu[0] + a[A_EL + 1] * HEu[1] + a[A_EL + 2] * HEu[2];
+  const double trace = H_p + sBB + sEE + EHE;
+  double HT[6];
+#pragma unroll
+  for (int kk = 0; kk < 3; ++kk)
+#pragma unroll
+    for (int ii = kk; ii < 3; ++ii) {
+      const double vk = a[A_VU + kk], vi = a[A_VU + ii];
+      const double first = vk * X.dCE_v[ii] + vi * X.dCE_v[kk] + calE * (0.5 * (vk * H_v[ii] + vi * H_v[kk]) + X.dvv[sym3(kk, ii)]) + vk * vi * H_p;
+      const double second = X.dBB[sym3(kk, ii)] + X.dEE[sym3(kk, ii)] + 0.5 * (a[A_EU + kk] * HEu[ii] + a[A_EU + ii] * HEu[kk]);
+      HT[sym3(kk, ii)] = 2.0 * first - 2.0 * second + (gu[sym3(kk, ii)] - vk * vi) * trace;
+    }
+  double gl[6];
+  const double ichi = 1.0 / chi;
+#pragma unroll
+  for (int c = 0; c < 6; ++c) gl[c] = __ldg(U + (size_t)(GXX + c) * su + pt) * ichi;
+#pragma unroll
+  for (int kk = 0; kk < 3; ++kk)
+#pragma unroll
+    for (int ii = 0; ii < 3; ++ii) {
+      double* w = Wk + (size_t)(11 * kk + 3 + ii) * sw + pt;
+      *w += fac0 * par.les_C_T * (gl[sym3(ii, 0)] * HT[sym3(kk, 0)] + gl[sym3(ii, 1)] * HT[sym3(kk, 1)] + gl[sym3(ii, 2)] * HT[sym3(kk, 2)]);
+    }
+  }
 }
 
+template <bool FULL>
 __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                   const double* __restrict__ P, size_t sp, const double* __restrict__ A, size_t sa,
                                                   double* __restrict__ Wk, size_t sw) {
@@ -222,8 +279,15 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 #pragma unroll
   for (int f = 0; f < A_VB; ++f) a[f] = val(f);
   double uB[3][3], uTH[3], t[3], t2[3], r[3];
+  LesFull X;
+  double uVa[FULL ? 3 : 1][3], uEa[FULL ? 3 : 1][3];   // FULL: the raised gradients of every v^c and E^c stay for grad v^k.grad v^i, grad E^k.grad E^i
 #pragma unroll
-  for (int c = 0; c < 3; ++c) { grad(A_BU + c, t); raise(t, uB[c]); }
+  for (int c = 0; c < 3; ++c) {
+    grad(A_BU + c, t); raise(t, uB[c]);
+    if (FULL)
+#pragma unroll
+      for (int e = 0; e <= c; ++e) X.dBB[sym3(e, c)] = dotp(t, uB[e]);
+  }
   grad(A_TH, t); raise(t, uTH);
   double dVB_B[3], dTH_v[3], dBv[3][3];         // grad(v.B).grad B^k, grad Theta.grad v^k, grad B^i.grad v^k
   grad(A_VB, t);
@@ -237,6 +301,12 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 #pragma unroll
     for (int e = 0; e < 3; ++e) dBv[e][c] = dotp(t, uB[e]);
     raise(t, r);
+    if (FULL) {
+#pragma unroll
+      for (int m = 0; m < 3; ++m) uVa[FULL ? c : 0][m] = r[m];
+#pragma unroll
+      for (int e = 0; e <= c; ++e) X.dvv[sym3(e, c)] = dotp(t, uVa[FULL ? e : 0]);
+    }
     grad(A_VL + c, t2);
     svv += dotp(t2, r);
     sBv += dotp(t2, uB[c]);
@@ -244,6 +314,12 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
     grad(A_BL + c, t);
     sBB += dotp(t, uB[c]);
     grad(A_EU + c, t); raise(t, r);
+    if (FULL) {
+#pragma unroll
+      for (int m = 0; m < 3; ++m) uEa[FULL ? c : 0][m] = r[m];
+#pragma unroll
+      for (int e = 0; e <= c; ++e) X.dEE[sym3(e, c)] = dotp(t, uEa[FULL ? e : 0]);
+    }
     grad(A_EL + c, t2);
     sEE += dotp(t2, r);
     sBBvB += a[A_BL + c] * dVB_B[c];
@@ -273,7 +349,19 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
     grad(A_D, t2);
     D.yterm = dPY_Y - 2.0 / val(A_D) * val(A_DPY) * dotp(t2, uY);
   }
-  les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
+  if (FULL) {
+    a[A_D] = val(A_D); a[A_DYE] = val(A_DYE);
+    grad(A_D, t);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) X.dD_v[c] = dotp(t, uVa[FULL ? c : 0]);
+    grad(A_DYE, t);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) X.dDY_v[c] = dotp(t, uVa[FULL ? c : 0]);
+    grad(A_CALE, t);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) X.dCE_v[c] = dotp(t, uVa[FULL ? c : 0]);
+  }
+  les_closed_forms<FULL>(d, par, a, D, X, gu, p, chi, al, U, su, Wk, sw, pt);
 }
 
 
@@ -287,17 +375,25 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int LX = 16, LY = 4, LZ = 4, LH = 2, LSX = LX + 2 * LH, LSY = LY + 2 * LH, LSZ = LZ + 2 * LH, LTILE = LSX * LSY * LSZ, LGMAX = 6;
 // the fields pass in 5 groups (one barrier and one mbarrier wait per group, not per field): {B^c, Theta, v.B}, three times {v^c, v_c, B_c, E^c, E_c}, the 6 scalars
-__device__ constexpr int LGSTART[7] = {0, 5, 10, 15, 20, 26, 29};   // the sixth group {Ye, dp/dYe, D} only with the tabulated EoS
+// then, in the order of LORDER: {Ye, dp/dYe, D} with the tabulated EoS only, {calE, D Ye} with FULL only (without the table: one group {D, calE, D Ye})
+template <int... Is, class F> __device__ __forceinline__ void static_for(std::integer_sequence<int, Is...>, F&& f) { (f(std::integral_constant<int, Is>{}), ...); }
+template <bool TABLE, bool FULL> struct LGroups {
+  static constexpr int N = 5 + (TABLE ? 1 : 0) + (FULL ? 1 : 0);
+  __host__ __device__ static constexpr int start(int g) { return g < 5 ? 5 * g : g == 5 ? (TABLE ? 26 : 28) : 29; }
+  __host__ __device__ static constexpr int end(int g) { return g < 4 ? 5 * (g + 1) : g == 4 ? 26 : g == 5 ? (TABLE ? 29 : 31) : 31; }
+};
 constexpr size_t LES_SMEM = (size_t)2 * LGMAX * LTILE * sizeof(double) + 64;
 // order of passage: anchors B^c, Theta; v.B; then per component c: v^c, v_c, B_c, E^c, E_c; then W^-2, rho, h, dp/drho, eps, dp/deps
 __device__ constexpr int LORDER[NAUX] = {A_BU, A_BU + 1, A_BU + 2, A_TH, A_VB,
                                          A_VU, A_VL, A_BL, A_EU, A_EL, A_VU + 1, A_VL + 1, A_BL + 1, A_EU + 1, A_EL + 1, A_VU + 2, A_VL + 2, A_BL + 2, A_EU + 2, A_EL + 2,
-                                         A_WM2, A_RHO, A_H, A_DPR, A_EPS, A_DPE, A_YE, A_DPY, A_D};
+                                         A_WM2, A_RHO, A_H, A_DPR, A_EPS, A_DPE, A_YE, A_DPY, A_D, A_CALE, A_DYE};
 
+template <bool TABLE, bool FULL>
 __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_constant__ Dims d, const __grid_constant__ Par par, const double* __restrict__ U, size_t su,
                                                                   const double* __restrict__ P, size_t sp, double* __restrict__ Wk, size_t sw,
                                                                   const __grid_constant__ CUtensorMap tmap) {
   static_assert((LTILE * sizeof(double)) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
+  using LG = LGroups<TABLE, FULL>;
   extern __shared__ __align__(128) double ring[];
   uint64_t* full = (uint64_t*)(ring + 2 * LGMAX * LTILE);
   const int tid = threadIdx.x, tx = tid % LX, ty = (tid / LX) % LY, tz = tid / (LX * LY);
@@ -313,7 +409,7 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   __syncthreads();
   auto issue = [&](int g) {                       // the box origin i0 - 2 = 16 blockIdx.x is even: on a 16-byte boundary
     if (tid == 0) {
-      const int n0 = LGSTART[g], n1 = LGSTART[g + 1];
+      const int n0 = LG::start(g), n1 = LG::end(g);
       mbar_expect_tx(full + g % 2, (unsigned)(n1 - n0) * LTILE * (unsigned)sizeof(double));
       for (int n = n0; n < n1; ++n) tma_load_4d(ring + ((g % 2) * LGMAX + (n - n0)) * LTILE, &tmap, full + g % 2, i0 - LH, j0 - LH, k0 - LH, LORDER[n]);
     }
@@ -342,17 +438,18 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   LesDots D;
   D.sBv = D.sBBvB = D.sBvTh = D.sBB = D.sEE = D.svv = 0.0;
   D.yterm = 0.0;
-  const int ngroups = par.eos_kind == 2 ? 6 : 5;
-  double uB[3][3], uTH[3], uV[3], uX[3], uR[3];      // raised gradients of the anchors: B^c, Theta, the current v^c, the current E^c / W^-2 / eps, rho
-#pragma unroll
-  for (int g5 = 0; g5 < 6; ++g5) {
-    if (g5 >= ngroups) break;                        // uniform over the grid
+  LesFull X;
+  // raised gradients of the anchors: B^c, Theta, v^c and E^c (FULL: every component stays, for (A17)), the current W^-2 / eps / Ye, rho
+  double uB[3][3], uTH[3], uV[FULL ? 3 : 1][3], uE[FULL ? 3 : 1][3], uX[3], uR[3];
+  // the groups are expanded at compile time (a fold over their indices: `#pragma unroll` gives up on the seven groups of <TABLE, FULL> and leaves a[], D, X in local memory)
+  auto group = [&](auto G) {
+    constexpr int g5 = decltype(G)::value;
     __syncthreads();                                 // everybody is done reading the buffer the next copy overwrites
-    if (g5 + 1 < ngroups) issue(g5 + 1);
+    if (g5 + 1 < LG::N) issue(g5 + 1);
     mbar_wait(full + g5 % 2, (g5 / 2) & 1);
 #pragma unroll
-   for (int n = LGSTART[g5]; n < LGSTART[g5 + 1]; ++n) {
-    const double* s = ring + ((g5 % 2) * LGMAX + (n - LGSTART[g5])) * LTILE + ctr;
+   for (int n = LG::start(g5); n < LG::end(g5); ++n) {
+    const double* s = ring + ((g5 % 2) * LGMAX + (n - LG::start(g5))) * LTILE + ctr;
     constexpr int OX = 1, OY = LSX, OZ = LSX * LSY;
     const int f = LORDER[n];
     a[f] = s[0];
@@ -360,7 +457,12 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
     g[0] = (8.0 * (s[OX] - s[-OX]) - (s[2 * OX] - s[-2 * OX])) * c12[0];
     g[1] = (8.0 * (s[OY] - s[-OY]) - (s[2 * OY] - s[-2 * OY])) * c12[1];
     g[2] = (8.0 * (s[OZ] - s[-OZ]) - (s[2 * OZ] - s[-2 * OZ])) * c12[2];
-    if (n < 3) raise(g, uB[n]);                                            // B^c
+    if (n < 3) {                                                           // B^c
+      raise(g, uB[n]);
+      if (FULL)
+#pragma unroll
+        for (int e = 0; e <= n; ++e) X.dBB[sym3(e, n)] = dotp(g, uB[e]);
+    }
     else if (n == 3) raise(g, uTH);                                        // Theta
     else if (n == 4) {                                                     // v.B
 #pragma unroll
@@ -371,16 +473,23 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
         D.dTH_v[c] = dotp(g, uTH);
 #pragma unroll
         for (int e = 0; e < 3; ++e) D.dBv[e][c] = dotp(g, uB[e]);
-        raise(g, uV);
+        raise(g, uV[FULL ? c : 0]);
+        if (FULL)
+#pragma unroll
+          for (int e = 0; e <= c; ++e) X.dvv[sym3(e, c)] = dotp(g, uV[FULL ? e : 0]);
       } else if (w == 1) {                                                 // v_c
-        D.svv += dotp(g, uV);
+        D.svv += dotp(g, uV[FULL ? c : 0]);
         D.sBv += dotp(g, uB[c]);
         D.sBvTh += a[A_BU + c] * dotp(g, uTH);
       } else if (w == 2) {                                                 // B_c
         D.sBB += dotp(g, uB[c]);
         D.sBBvB += a[A_BL + c] * D.dVB_B[c];
-      } else if (w == 3) raise(g, uX);                                     // E^c
-      else D.sEE += dotp(g, uX);                                           // E_c
+      } else if (w == 3) {                                                 // E^c
+        raise(g, uE[FULL ? c : 0]);
+        if (FULL)
+#pragma unroll
+          for (int e = 0; e <= c; ++e) X.dEE[sym3(e, c)] = dotp(g, uE[FULL ? e : 0]);
+      } else D.sEE += dotp(g, uE[FULL ? c : 0]);                           // E_c
     } else if (n == 20) { raise(g, uX); D.dWW = dotp(g, uX); }             // W^-2
     else if (n == 21) { D.dWR = dotp(g, uX); raise(g, uR); }               // rho
     else if (n == 22) D.dWH = dotp(g, uX);                                 // h
@@ -389,30 +498,52 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
     else if (n == 25) D.dPE_E = dotp(g, uX);                               // dp/deps
     else if (n == 26) raise(g, uX);                                        // Ye
     else if (n == 27) D.yterm = dotp(g, uX);                               // dp/dYe
-    else D.yterm -= 2.0 / a[A_D] * a[A_DPY] * dotp(g, uX);                 // D
+    else if (n == 28) {                                                    // D
+      if (TABLE) D.yterm -= 2.0 / a[A_D] * a[A_DPY] * dotp(g, uX);
+      if (FULL)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) X.dD_v[c] = dotp(g, uV[FULL ? c : 0]);
+    } else if (n == 29) {                                                  // calE
+#pragma unroll
+      for (int c = 0; c < 3; ++c) X.dCE_v[c] = dotp(g, uV[FULL ? c : 0]);
+    } else {                                                               // D Ye
+#pragma unroll
+      for (int c = 0; c < 3; ++c) X.dDY_v[c] = dotp(g, uV[FULL ? c : 0]);
+    }
    }
-  }
-  if (inside) les_closed_forms(d, par, a, D, p, chi, al, Wk, sw, pt);
+  };
+  static_for(std::make_integer_sequence<int, LG::N>{}, group);
+  if (inside) les_closed_forms<FULL>(d, par, a, D, X, gu, p, chi, al, U, su, Wk, sw, pt);
 }
 
 }  // namespace
 
-cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
-                       double* Wk, size_t sw, cudaStream_t s) {
-  if (par.eos_kind == 2) k_les_aux<true><<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
-  else k_les_aux<false><<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
+template <bool TABLE, bool FULL>
+static cudaError_t launch_les_t(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
+                                double* Wk, size_t sw, cudaStream_t s) {
+  k_les_aux<TABLE, FULL><<<(unsigned)((d.npts + 127) / 128), 128, 0, s>>>(d, par, U, su, P, sp, A, sa);
   if (d.mx > 4 && d.my > 4 && d.mz > 4) {
     dim3 grid((d.mx - 4 + 15) / 16, (d.my - 4 + 3) / 4, (d.mz - 4 + 3) / 4), block(16, 4, 4);
     CUtensorMap map;
-    static int attr[64] = {};
+    static int attr[64] = {};                                  // one per instantiation
     int dev = 0;
     cudaGetDevice(&dev);
-    bool tma = dev >= 0 && dev < 64 && make_tensor_map_4d(d, A, sa, par.eos_kind == 2 ? NAUX : NAUX_NOYE, LSX, LSY, LSZ, &map);
-    if (tma && !attr[dev]) { tma = cudaFuncSetAttribute(k_les_flux_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LES_SMEM) == cudaSuccess; attr[dev] = tma; }
-    if (tma) k_les_flux_tma<<<grid, LX * LY * LZ, LES_SMEM, s>>>(d, par, U, su, P, sp, Wk, sw, map);
-    else k_les_flux<<<grid, block, 0, s>>>(d, par, U, su, P, sp, A, sa, Wk, sw);
+    bool tma = dev >= 0 && dev < 64 && make_tensor_map_4d(d, A, sa, FULL ? NAUX : TABLE ? A_D + 1 : NAUX_NOYE, LSX, LSY, LSZ, &map);
+    if (tma && !attr[dev]) {
+      tma = cudaFuncSetAttribute(k_les_flux_tma<TABLE, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LES_SMEM) == cudaSuccess;
+      attr[dev] = tma;
+    }
+    if (tma) k_les_flux_tma<TABLE, FULL><<<grid, LX * LY * LZ, LES_SMEM, s>>>(d, par, U, su, P, sp, Wk, sw, map);
+    else k_les_flux<FULL><<<grid, block, 0, s>>>(d, par, U, su, P, sp, A, sa, Wk, sw);
   }
   return cudaGetLastError();
+}
+
+cudaError_t launch_les(const Dims& d, const Par& par, const double* U, size_t su, const double* P, size_t sp, double* A, size_t sa,
+                       double* Wk, size_t sw, cudaStream_t s) {
+  const bool full = par.les_C_N != 0.0 || par.les_C_Y != 0.0 || par.les_C_T != 0.0, table = par.eos_kind == 2;
+  if (table) return full ? launch_les_t<true, true>(d, par, U, su, P, sp, A, sa, Wk, sw, s) : launch_les_t<true, false>(d, par, U, su, P, sp, A, sa, Wk, sw, s);
+  return full ? launch_les_t<false, true>(d, par, U, su, P, sp, A, sa, Wk, sw, s) : launch_les_t<false, false>(d, par, U, su, P, sp, A, sa, Wk, sw, s);
 }
 
 }  // namespace mhd

@@ -40,7 +40,7 @@ struct Par {
   int m1_maxit, m1_odd_even;
   double m1_arad, m1_oe_guard;
   int recon_kind;
-  double weno_eps, les_C_M;
+  double weno_eps, les_C_M, les_C_N, les_C_Y, les_C_T;
 };
 
 struct Slot {

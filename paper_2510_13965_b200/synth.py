@@ -100,7 +100,7 @@ def default_params(**over):
         eps_min=0.0, eps_max=1e3, ye_min=0.0, ye_max=1.0, ye_atmo=0.3, eps_atmo=1e-8, T_atmo=0.1,
         c2p_maxit=100,
         m1_kappa0=1e-6, m1_rho0=1e-3, m1_species_scale=[1.0, 0.8, 0.5], m1_efloor=1e-30, m1_tol=1e-13, m1_mb=1.0, m1_maxit=30, m1_odd_even=1, m1_arad=1.0, m1_oe_guard=1e-10,
-        recon_kind=0, weno_eps=1e-6, les_C_M=0.0,
+        recon_kind=0, weno_eps=1e-6, les_C_M=0.0, les_C_N=0.0, les_C_Y=0.0, les_C_T=0.0,
     )
     p.update(over)
     return p

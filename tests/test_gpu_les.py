@@ -54,7 +54,7 @@ def test_les_flux_and_one_stage_parity(oracle_mod, kind):
     patch.work.zero_()
     binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
     Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
-    Ag, Ao = Ag[:26], Ao[:26]                                  # Ye, dp/dYe, D are staged only for the tabulated EoS (dp/dYe = 0 otherwise)
+    Ag, Ao = Ag[:26], Ao[:26]                                  # Ye, dp/dYe, D are staged only for the tabulated EoS, calE and D Ye only with C_N / C_Y / C_T
     den = np.abs(Ao).reshape(Ao.shape[0], -1).max(axis=1)
     ra = np.abs(Ag - Ao).reshape(Ao.shape[0], -1).max(axis=1) / np.where(den > 0, den, 1.0)
     assert np.all(ra < 1e-13), ra
@@ -142,7 +142,7 @@ def test_les_with_the_tabulated_eos(oracle_mod):
     patch.work.zero_()
     binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
     Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
-    Ao = Ao[:Ag.shape[0]]                                      # the oracle stages two more fields for the C_N / C_Y / C_T tensors
+    Ag, Ao = Ag[:29], Ao[:29]                                  # calE and D Ye are staged only with C_N / C_Y / C_T
     den = np.abs(Ao).reshape(Ao.shape[0], -1).max(axis=1)
     for g0 in range(0, 18, 3):                                 # components of a vector share the vector's norm (v^z = 0 for rotation about z)
         den[g0:g0 + 3] = den[g0:g0 + 3].max()
@@ -154,6 +154,93 @@ def test_les_with_the_tabulated_eos(oracle_mod):
     for k in range(3):
         for i in range(3):
             assert np.abs(Wg[11 * k + 6 + i] - Lo[3 * k + i]).max() <= 1e-9 * scale, (k, i, np.abs(Wg[11 * k + 6 + i] - Lo[3 * k + i]).max() / scale)
+    Kg = patch.rhs(1).cpu().numpy()
+    rk, dn = _rel(Kg, Ko)
+    assert np.all(rk[dn > 0] < 1e-11), rk
+    patch.close()
+
+
+FULL = dict(les_C_M=8.0, les_C_N=2.0, les_C_Y=1.5, les_C_T=0.75)
+
+
+def _check_all_fluxes(Wg, Lo, tol):
+    """work slot (field 11 k + f of direction k: 0 Dbar, 1 DYebar, 3 + i Sbar_i, 6 + i Bbar^i) against the oracle's 24 SGS flux fields, each tensor on
+    its own scale"""
+    for k in range(3):
+        for name, wf, lf in (("N", [0], [9 + k]), ("NY", [1], [12 + k]), ("T", [3, 4, 5], [15 + 3 * k + i for i in range(3)]),
+                             ("M", [6, 7, 8], [3 * k + i for i in range(3)])):
+            scale = {"N": np.abs(Lo[9:12]).max(), "NY": np.abs(Lo[12:15]).max(), "T": np.abs(Lo[15:24]).max(), "M": np.abs(Lo[0:9]).max()}[name]
+            assert scale > 0, name
+            for a, b in zip(wf, lf):
+                err = np.abs(Wg[11 * k + a] - Lo[b]).max()
+                assert err <= tol * scale, (name, k, a, err / scale)
+        assert np.all(Wg[11 * k + 2] == 0) and np.all(Wg[11 * k + 9] == 0) and np.all(Wg[11 * k + 10] == 0)    # taubar (R45), phibar, speed: untouched
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_les_all_four_tensors(oracle_mod, kind):
+    """C_M, C_N, C_Y, C_T all set ((A15)-(A17) beside (A16)): SGS fluxes of Dbar, DYebar, Sbar_i, Bbar^i and the one-stage RHS against the oracle;
+    once on a block-aligned patch (TMA kernel) and once on a ragged one with an odd row length (no tensor map: the L1 kernel)."""
+    for shape in (None, (23, 13, 9)):
+        cfg = _boost_B(synth.config1(n=20, gauge_perturbation=True, ng=NG))
+        cfg["params"].update(FULL)
+        if kind == 1:
+            cfg["params"].update(eos_kind=1, eos_gamma_th=1.8, n_pieces=3, pp_K=[30.0, 0.0, 0.0], pp_Gamma=[1.9, 2.4, 2.9], pp_rho=[1.0e-3, 5.0e-3, 1e300])
+            cfg["P"][synth.EPS] = 0.25
+        if shape is not None:
+            nx, ny, nz = shape
+            cfg["U"] = np.ascontiguousarray(np.tile(cfg["U"], (1, 1, 1, 2))[:, :nz + 2 * NG, :ny + 2 * NG, :nx + 2 * NG])
+            cfg["P"] = np.ascontiguousarray(np.tile(cfg["P"], (1, 1, 1, 2))[:, :nz + 2 * NG, :ny + 2 * NG, :nx + 2 * NG])
+            cfg["n"] = shape
+            cfg["bc"] = [1, 1, 0, 1, 1, 0]
+        binding, o, patch, U, P = _setup(oracle_mod, cfg)
+        Uo = U.copy()
+        o.fill_ghosts(Uo, cfg["bc"])
+        Po, Fo = o.con2prim(Uo)
+        Lo, Ao = o.les_flux(Uo, Po)
+        Ko = o.rhs(Uo, Po)
+        K0 = oracle_mod.Oracle(dict(cfg["params"], les_C_N=0.0, les_C_Y=0.0, les_C_T=0.0), *cfg["n"], NG, cfg["dx"]).rhs(Uo, Po)
+        patch.upload(U=U)
+        patch.fill_ghosts(cfg["bc"])
+        patch.con2prim()
+        assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+        patch.work.zero_()
+        binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
+        Ag, Wg = patch.leswork.cpu().numpy(), patch.work.cpu().numpy()
+        for f in (28, 29, 30):                                 # D, calE, D Ye are staged now
+            assert np.abs(Ag[f] - Ao[f]).max() <= 1e-13 * np.abs(Ao[f]).max(), f
+        _check_all_fluxes(Wg, Lo, 1e-11)
+        Kg = patch.rhs(1).cpu().numpy()
+        rk, den = _rel(Kg, Ko)
+        assert np.all(rk[den > 0] < 1e-11), (shape, rk)
+        d, _ = _rel(Ko[22:28], K0[22:28])                      # the three new tensors are live in Dbar, DYebar, Sbar_i (taubar has none)
+        assert np.all(d[[0, 1, 3, 4, 5]] > 1e-6) and d[2] == 0, d
+        patch.close()
+
+
+def test_les_all_four_tensors_tabulated_eos(oracle_mod):
+    cfg = synth.config4(n=24, ng=NG)
+    cfg["params"].update(FULL)
+    cfg["U"][28:31] *= 300.0
+    from paper_2510_13965_b200 import binding
+    n = cfg["n"]
+    o = oracle_mod.Oracle(cfg["params"], n[0], n[1], n[2], NG, cfg["dx"], table=cfg["table"])
+    U, P = cfg["U"].copy(), cfg["P"].copy()
+    o.prim2con(U, P)
+    patch = binding.Patch(cfg["params"], n, NG, cfg["dx"], stages=4, table=cfg["table"])
+    Uo = U.copy()
+    o.fill_ghosts(Uo, cfg["bc"])
+    Po, Fo = o.con2prim(Uo)
+    Lo, Ao = o.les_flux(Uo, Po)
+    Ko = o.rhs(Uo, Po)
+    patch.upload(U=U)
+    patch.fill_ghosts(cfg["bc"])
+    patch.con2prim()
+    assert np.array_equal(patch.flags.cpu().numpy()[0], Fo)
+    patch.work.zero_()
+    binding.mhd_les_flux(patch.h, binding.SLOT_U, binding.SLOT_P, patch.stream())
+    Wg = patch.work.cpu().numpy()
+    _check_all_fluxes(Wg, Lo, 1e-9)                            # EoS derivatives through the table's T inversion (N3), as in the C_M-only test
     Kg = patch.rhs(1).cpu().numpy()
     rk, dn = _rel(Kg, Ko)
     assert np.all(rk[dn > 0] < 1e-11), rk
