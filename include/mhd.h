@@ -127,8 +127,8 @@ typedef struct {
                                       mhd_patch_create / mhd_rhs refuse. dp/drho, dp/deps, dp/dYe: analytic for eos_kind 0 / 1, derivatives of the
                                       interpolant inside the table cell for eos_kind 2 (l.882) */
   double les_C_N, les_C_Y, les_C_T; /* App. A, Eqs. (A11), (A15), (A17): coefficients of the sub-grid-scale tensors H_N^k (flux of Dbar), H_{N_Y}^k (flux of
-                                      DYebar) and gamma_ij H_T^{kj} (flux of Sbar_i; H_E from the curl of H_M, R44); the paper's runs leave them 0
-                                      (PAPER.md:863). taubar receives no SGS flux ((A11) defines none, R45). Same requirements as les_C_M when any is non-zero */
+                                      DYebar) and gamma_ij H_T^{kj} (flux of Sbar_i; H_E from the curl of H_M, R45, R46); the paper's runs leave them 0
+                                      (PAPER.md:863). taubar receives no SGS flux ((A11) defines none, R47). Same requirements as les_C_M when any is non-zero */
 } mhd_patch_desc;
 
 /* Butcher tableaux (Eq. 54), HOST pointers, row-major stages x stages; a_impl/w_impl may be NULL */

@@ -1,8 +1,8 @@
-// ORACLE (test infrastructure) — Large-Eddy-Simulation gradient sub-grid-scale term of the induction equation,
-// PAPER.md Sec. II B l.252-256 and App. A, Eqs. (A11)-(A17) l.855-882, with C_M = par.les_C_M (the paper's production value is 8,
-// l.863; the other three coefficients are zero there and are not built). Followed term by term in the paper's notation.
+// ORACLE (test infrastructure) — Large-Eddy-Simulation gradient sub-grid-scale terms: the tensor of the induction
+// equation, C_M = par.les_C_M (the paper's production value is 8, l.863), and the other three of (A11), C_N, C_Y, C_T (zero in the paper's
+// runs). PAPER.md Sec. II B l.252-256 and App. A, Eqs. (A11)-(A17) l.855-882, followed term by term in the paper's notation.
 //
-// Readings (R39-R44; the appendix uses symbols the paper does not define — they are fixed by the requirement that the
+// Readings (R39-R47; the appendix uses symbols the paper does not define — they are fixed by the requirement that the
 // printed chain (A12)-(A16) equals the gradient model the appendix itself states, tau_F^k = -xi grad(dF^k/dC) . grad C, which the
 // pins check numerically: tests/test_oracle_les.py):
 //   calE = h W^2 with h = rho (1 + eps) + p the enthalpy density (l.232);  Theta = calE + B^2 (so S_i = Theta v_i - (v.B) B_i, Eq. 29);
@@ -123,7 +123,7 @@ void les_H_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const d
   if (HN) for (int k = 0; k < 3; ++k) HN[k] = 2.0 * dot(LES_D, LES_VU + k) + a[LES_D] * H_v[k];              // (A15)
   if (HNY) for (int k = 0; k < 3; ++k) HNY[k] = 2.0 * dot(LES_DYE, LES_VU + k) + a[LES_DYE] * H_v[k];
   if (HT) {
-    // H_E^i = 1/2 eps^i_{jk} H_M^{jk} (A16) is the same contraction for E^i = -eps^{ijk} v_j B_k: with the FIRST index of H_M the flux direction (R40),
+    // H_E^i = 1/2 eps^i_{jk} H_M^{jk} (A16) is the same contraction for E^i = -eps^{ijk} v_j B_k: with the FIRST index of H_M the flux direction (R40, R45),
     // H_M^{(dir k)(comp j)} belongs to the flux B^j v^k - B^k v^j, so that eps_{ijk} (B^j v^k - B^k v^j) / 2 = -eps_{ijk} v^j B^k = E_i and
     // H_E_i = 1/2 sqrt(gamma) [ijk] H_M^{(dir k)(comp j)}; E only enters (A17) quadratically, so its overall sign convention does not matter
     double HEl[3], HEu[3];
@@ -137,7 +137,7 @@ void les_H_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const d
     (void)gl;
     const double trace = H_p + sBB + sEE + EHE;
     for (int k = 0; k < 3; ++k) for (int i = 0; i < 3; ++i) {
-      // grad calE . grad (v^k v^i) by the product rule (reading R41): v^k grad calE . grad v^i + v^i grad calE . grad v^k
+      // grad calE . grad (v^k v^i) by the product rule (reading R46): v^k grad calE . grad v^i + v^i grad calE . grad v^k
       const double first = vu[k] * dot(LES_CALE, LES_VU + i) + vu[i] * dot(LES_CALE, LES_VU + k)
                            + calE * (0.5 * (vu[k] * H_v[i] + vu[i] * H_v[k]) + dot(LES_VU + k, LES_VU + i)) + vu[k] * vu[i] * H_p;
       const double second = dot(LES_BU + k, LES_BU + i) + dot(LES_EU + k, LES_EU + i) + 0.5 * (Eu[k] * HEu[i] + Eu[i] * HEu[k]);
@@ -153,7 +153,7 @@ void les_HM_point(const double a[LES_NAUX], const double da[3][LES_NAUX], const 
 
 // SGS parts of the flux brackets of Eq. (32) in direction k, -alpha G = +alpha C xi sqrt(gamma) H (A11), in the LES_NFLUX = 24 fields of L:
 //   3 k + i       Bbar^i:  C_M H_M^{ki}            9 + k   Dbar: C_N H_N^k           12 + k   DYebar: C_Y H_{N_Y}^k
-//   15 + 3 k + i  Sbar_i:  C_T gamma_ij H_T^{kj}   (taubar: (A11) defines no G_tau, none is added: reading R45)
+//   15 + 3 k + i  Sbar_i:  C_T gamma_ij H_T^{kj}   (taubar: (A11) defines no G_tau, none is added: reading R47)
 // A (LES_NAUX fields) receives the auxiliary fields (for the pins)
 void les_flux(const Params& par, const Grid& G, const double* U, const double* P, double* L, double* A) {
   const size_t n = G.npts();

@@ -1,5 +1,6 @@
-// LES gradient sub-grid-scale tensor of the induction equation: PAPER.md Sec. II B l.252-256 and App. A,
-// Eqs. (A11)-(A17) l.855-882, coefficient C_M (the paper's production setting: C_M = 8, the other coefficients 0, l.863).
+// LES gradient sub-grid-scale tensors: PAPER.md Sec. II B l.252-256 and App. A, Eqs. (A11)-(A17) l.855-882.
+// The induction equation's, coefficient C_M (the paper's production setting: C_M = 8, the other coefficients 0, l.863), is the default
+// instantiation; with any of C_N, C_Y, C_T set the FULL instantiations add H_N^k, H_{N_Y}^k (A15) and H_T^{ki} (A17) to the fluxes of Dbar, DYebar, Sbar_i.
 //   -alpha G_B^{ki} = +alpha C_M xi sqrt(gamma) H_M^{ki},   xi = gamma^{1/3} Delta^2 / 24,
 // is part of the flux bracket of Bbar^i in direction k (Eq. 32): it is ADDED to the pointwise fluxes of the work slot after
 // k_point_flux and before the flux-splitting reconstruction. Readings of the appendix's undefined symbols: DESIGN.md R39-R44
@@ -10,7 +11,7 @@
 //   k_les_flux   every grid point at least 2 points inside the array: fourth-order centred gradients (Eq. 60) of those fields, the 36
 //                products grad f . grad g = gamma^{mn} d_m f d_n g that (A12)-(A16) need, then the closed forms; bound by L1/L2 loads
 //                (26 fields x 12 neighbours per point).
-// EoS derivatives: analytic for the ideal gas and the hybrid piecewise polytrope (l.882); the tabulated EoS is not supported here.
+// EoS derivatives: analytic for the ideal gas and the hybrid piecewise polytrope (l.882); derivatives of the interpolant in the cell for the table (R42).
 #include "mhd_internal.cuh"
 #include "tma.cuh"
 #include <utility>
@@ -206,7 +207,7 @@ __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, 
     if (par.les_C_Y != 0.0) w[sw] += fac0 * par.les_C_Y * (2.0 * X.dDY_v[kk] + a[A_DYE] * H_v[kk]);
   }
   if (par.les_C_T == 0.0) return;
-  // ---- (A17) with H_E_i = 1/2 sqrt(gamma) [ijk] H_M^{(dir k)(comp j)} (reading R44), the flux of Sbar_i is gamma_ij H_T^{kj}
+  // ---- (A17) with H_E_i = 1/2 sqrt(gamma) [ijk] H_M^{(dir k)(comp j)} (reading R45), the flux of Sbar_i is gamma_ij H_T^{kj}
   const double H_p = pref * brace;
   double HEl[3], HEu[3];
 #pragma unroll

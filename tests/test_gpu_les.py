@@ -174,7 +174,7 @@ def _check_all_fluxes(Wg, Lo, tol):
             for a, b in zip(wf, lf):
                 err = np.abs(Wg[11 * k + a] - Lo[b]).max()
                 assert err <= tol * scale, (name, k, a, err / scale)
-        assert np.all(Wg[11 * k + 2] == 0) and np.all(Wg[11 * k + 9] == 0) and np.all(Wg[11 * k + 10] == 0)    # taubar (R45), phibar, speed: untouched
+        assert np.all(Wg[11 * k + 2] == 0) and np.all(Wg[11 * k + 9] == 0) and np.all(Wg[11 * k + 10] == 0)    # taubar (R47), phibar, speed: untouched
 
 
 @pytest.mark.parametrize("kind", [0, 1])
