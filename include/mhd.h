@@ -220,7 +220,11 @@ int mhd_rk_stage(mhd_patch *p, const mhd_tableau *t, int stage, double dt, void 
 /* n_steps full RK steps, device resident: per stage fill -> con2prim -> rhs(K_stage) -> rk_stage; the state is
  * left with ghosts filled and primitives/flags consistent. Asynchronous. With MHD_SLOT_U1 bound the combine of Eq. (53) is
  * computed by the last right-hand-side kernel that touches each field (same arithmetic, one pass less over K and U per
- * stage; K_s of the last stage is then not stored); the buffers bound to U, U0, U1 are all overwritten, the result is in U. */
+ * stage; K_s of the last stage is then not stored); the buffers bound to U, U0, U1 are all overwritten, the result is in U.
+ * The call only enqueues kernels and memsets on cuda_stream (no synchronisation, allocation or host read; the opt-ins to large shared memory
+ * happen at the first call on a device), so after one ordinary call it may be captured into a CUDA graph and replayed (small patches are
+ * launch-bound: about 50 launches per RK4 step); a replay reproduces the direct call bit for bit when U and the primitives (the warm start of
+ * con2prim) hold the same values. Without halo neighbours only: the epoch of the halo protocol advances on the host. */
 int mhd_advance(mhd_patch *p, const mhd_tableau *t, const int bc[6], double dt, int n_steps, void *cuda_stream);
 
 /* Same, end to end with HOST buffers: copies host_U (MHD_NSTATE fields, packed, field_stride = MX*MY*MZ) to
