@@ -264,17 +264,21 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
   const int other = blockIdx.y + d.ng;
   const long long base = (DIR == 1 ? (long long)other * d.sz : (long long)other * d.sy) + (i + d.ng);
   const int g0 = c0 + d.ng - 3;
-  auto node = [&](int n) { return base + (long long)min(g0 + n, mline - 1) * ls; };   // clamped: the ragged tail never reads past the field
+  // element offset of node n of the segment inside a field, clamped (the ragged tail never reads past the field), in 32-bit arithmetic (a field has fewer
+  // than 2^32 points: checked at launch): min, multiply-add, IMAD.WIDE per access instead of a 64-bit multiply-add chain
+  const unsigned off0 = (unsigned)(base + (long long)g0 * ls), ls32 = (unsigned)ls;
+  const int nmax = mline - 1 - g0;
+  auto offn = [&](int n) { return off0 + (unsigned)min(n, nmax) * ls32; };
   // lambda of the SEG+1 interfaces: interface m lies between nodes m+2 and m+3 (relative to g0), stencil nodes m..m+5
   double lam[SEG + 1];
   {
     const double* s = Wk + (size_t)(11 * DIR + 10) * sw;
     double w[6];
 #pragma unroll
-    for (int n = 0; n < 5; ++n) w[n] = __ldg(s + node(n));
+    for (int n = 0; n < 5; ++n) w[n] = __ldg(s + offn(n));
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
-      w[(m + 5) % 6] = __ldg(s + node(m + 5));
+      w[(m + 5) % 6] = __ldg(s + offn(m + 5));
       lam[m] = pmax(pmax(pmax(w[0], w[1]), pmax(w[2], w[3])), pmax(w[4], w[5]));
     }
   }
@@ -289,13 +293,13 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     double fc[SEG + 6], uc[SEG + 6], acc[SEG + 1];
     unsigned mask = 0;
 #pragma unroll
-    for (int n = 0; n < SEG + 6; ++n) { fc[n] = __ldg(f + node(n)); uc[n] = __ldg(u + node(n)); }
+    for (int n = 0; n < SEG + 6; ++n) { fc[n] = __ldg(f + offn(n)); uc[n] = __ldg(u + offn(n)); }
     double kold[SEG];                                          // K is read-modify-write: fetched with the column, not after the arithmetic
 #pragma unroll
-    for (int m = 1; m <= SEG; ++m) kold[m - 1] = (active && c0 + m - 1 < nline) ? k[base + (long long)(g0 + m + 2) * ls] : 0.0;
+    for (int m = 1; m <= SEG; ++m) kold[m - 1] = (active && c0 + m - 1 < nline) ? k[offn(m + 2)] : 0.0;
     double pre[SEG];                                           // U0 + earlier stages of the fused RK combine (z pass only), fetched with the rest
 #pragma unroll
-    for (int m = 1; m <= SEG; ++m) pre[m - 1] = (FUSED && active && c0 + m - 1 < nline) ? fused_fetch(fz, DBAR + a, (size_t)(base + (long long)(g0 + m + 2) * ls)) : 0.0;
+    for (int m = 1; m <= SEG; ++m) pre[m - 1] = (FUSED && active && c0 + m - 1 < nline) ? fused_fetch(fz, DBAR + a, (size_t)offn(m + 2)) : 0.0;
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
       acc[m] = flux_hat2<WENO>(q, fc + m, uc + m, lam[m], alpha, active, m, lane, mask);
@@ -310,9 +314,9 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
 #pragma unroll
     for (int m = 1; m <= SEG; ++m)
       if (active && c0 + m - 1 < nline) {
-        const long long pt = base + (long long)(g0 + m + 2) * ls;       // zone c0 + m - 1
+        const size_t pt = offn(m + 2);                                   // zone c0 + m - 1
         const double knew = kold[m - 1] - (acc[m] - acc[m - 1]) * hih;          // Eq. (64)
-        if (FUSED) fused_store(fz, DBAR + a, (size_t)pt, pre[m - 1], knew, k + pt); else k[pt] = knew;
+        if (FUSED) fused_store(fz, DBAR + a, pt, pre[m - 1], knew, k + pt); else k[pt] = knew;
       }
   }
 }
@@ -335,7 +339,10 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   // left face of zone: between nodes zone-1 and zone -> stencil nodes zone-3 .. zone+2 ; global x index = zone + ng - 3 + n
   const long long base = (long long)(blockIdx.z + d.ng) * d.sz + (long long)(row + d.ng) * d.sy;
   const int g0 = zone + d.ng - 3;
-  auto node = [&](int n) { return base + min(g0 + n, d.mx - 1); };
+  unsigned off[6];                                          // element offsets of the six stencil nodes inside a field (clamped), computed once
+#pragma unroll
+  for (int n = 0; n < 6; ++n) off[n] = (unsigned)(base + min(g0 + n, d.mx - 1));
+  auto node = [&](int n) { return off[n]; };
   const bool active = zone <= d.nx;                          // interfaces 0 .. nx
   double lam;
   {
@@ -347,7 +354,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   double acc[10], kold[10];
   unsigned mask = 0;
 #pragma unroll
-  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + base + zone + d.ng] : 0.0;   // read-modify-write: fetched up front
+  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + off[3]] : 0.0;   // read-modify-write: fetched up front
   double fw[6], uw[6];
 #pragma unroll
   for (int n = 0; n < 6; ++n) { fw[n] = __ldg(Wk + node(n)); uw[n] = __ldg(U + (size_t)DBAR * su + node(n)); }
@@ -374,7 +381,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
     if (mask & (1u << (2 * a))) fl += q.corr[(2 * a) * 32 + lane];
     if (mask & (1u << (2 * a + 1))) fl += q.corr[(2 * a + 1) * 32 + lane];
     const double fr = __shfl_down_sync(FULL, fl, 1);           // F^ at zone + 1/2
-    if (store) K[(size_t)(DBAR + a) * sk + base + zone + d.ng] = kold[a] - (fr - fl) * hih;
+    if (store) K[(size_t)(DBAR + a) * sk + off[3]] = kold[a] - (fr - fl) * hih;
   }
 }
 
@@ -397,6 +404,7 @@ cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U
   static int seg = 0;
   if (seg == 0) { const char* v = getenv("MHD_RECON_SEG"); seg = v ? atoi(v) : 6; }
   const bool weno = par.recon_kind == 1;
+  if ((unsigned long long)d.npts >= (1ull << 32)) return cudaErrorInvalidValue;   // the kernels keep 32-bit element offsets inside a field
   if (dir == 0) {
     dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
     if (weno) k_recon_x<true><<<grid, 32 * RW, 0, s>>>(d, par.weno_eps, U, su, Wk, sw, K, sk);
