@@ -560,8 +560,8 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
   const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k0 = blockIdx.z * AZ;
   if (i >= d.nx || j >= d.ny) return;
   const int nzl = min(AZ, d.nz - k0);
-  const long long sy = d.sy, sz = d.sz;
-  const size_t base = (size_t)(k0 + d.ng) * sz + (size_t)(j + d.ng) * sy + (i + d.ng);
+  const int sy = (int)d.sy, sz = (int)d.sz;        // 32-bit strides: neighbour offsets relative to the thread's point stay far below 2^31 (checked at launch)
+  const size_t base = (size_t)(k0 + d.ng) * d.sz + (size_t)(j + d.ng) * d.sy + (i + d.ng);
   const double i24h[3] = {1.0 / (24.0 * d.dx), 1.0 / (24.0 * d.dy), 1.0 / (24.0 * d.dz)};
   const double cko[3] = {sigma / (64.0 * d.dx), sigma / (64.0 * d.dy), sigma / (64.0 * d.dz)};
   double cb[AZ][3];   // beta^a / (24 h_a) on the AZ planes
@@ -575,7 +575,7 @@ __global__ void __launch_bounds__(256, MINB) k_adv_ko(const __grid_constant__ Di
     double* ko = K + (size_t)f * sk + base;
     double w[AZ + 6];   // the z column k0-3 .. k0+AZ+2 (clamped for a ragged last block: those planes are not used)
 #pragma unroll
-    for (int n = 0; n < AZ + 6; ++n) w[n] = __ldg(u + (long long)min(n - 3, nzl + 2) * sz);
+    for (int n = 0; n < AZ + 6; ++n) w[n] = __ldg(u + min(n - 3, nzl + 2) * sz);
     double kold[AZ];    // K is read-modify-write: its loads are issued with the stencil loads, not after the arithmetic
 #pragma unroll
     for (int kk = 0; kk < AZ; ++kk) kold[kk] = kk < nzl ? ko[kk * sz] : 0.0;
@@ -649,6 +649,7 @@ cudaError_t launch_ccz4_algebra(const Dims& d, const Par& par, const double* U, 
 
 cudaError_t launch_adv_ko(const Dims& d, const Par& par, const double* U, size_t su, double* K, size_t sk, const Fuse& fz, cudaStream_t s) {
   constexpr int AZ = 4;
+  if (d.sz > (1ll << 26)) return cudaErrorInvalidValue;      // the kernel keeps neighbour offsets (up to AZ + 3 planes) in 32 bits
   dim3 ablock(32, 8), agrid((d.nx + 31) / 32, (d.ny + 7) / 8, (d.nz + AZ - 1) / AZ);
   if (fz.Uout) k_adv_ko<true, AZ, 2, true><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk, fz);   // last kernel to touch the spacetime K
   else k_adv_ko<true, AZ, 3, false><<<agrid, ablock, 0, s>>>(d, par.sigma_ko_spacetime, 0, 22, U, su, K, sk, fz);

@@ -338,11 +338,10 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   const int zone = z0 + lane;                                // lane l: interface zone-1/2 (left face of its zone)
   // left face of zone: between nodes zone-1 and zone -> stencil nodes zone-3 .. zone+2 ; global x index = zone + ng - 3 + n
   const long long base = (long long)(blockIdx.z + d.ng) * d.sz + (long long)(row + d.ng) * d.sy;
-  const int g0 = zone + d.ng - 3;
-  unsigned off[6];                                          // element offsets of the six stencil nodes inside a field (clamped), computed once
-#pragma unroll
-  for (int n = 0; n < 6; ++n) off[n] = (unsigned)(base + min(g0 + n, d.mx - 1));
-  auto node = [&](int n) { return off[n]; };
+  // lanes past the last interface (zone > nx) are clamped as a whole, so that the six nodes of every lane are contiguous and inside the row (ng >= 3): a
+  // load is [pointer + immediate], the pointer of a field one IMAD.WIDE from the 32-bit element offset of node 0 (a field has fewer than 2^32 points)
+  const unsigned off0 = (unsigned)(base + (min(zone, d.nx) + d.ng - 3));
+  auto node = [&](int n) { return (size_t)off0 + n; };
   const bool active = zone <= d.nx;                          // interfaces 0 .. nx
   double lam;
   {
@@ -354,7 +353,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   double acc[10], kold[10];
   unsigned mask = 0;
 #pragma unroll
-  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + off[3]] : 0.0;   // read-modify-write: fetched up front
+  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + off0 + 3] : 0.0;   // read-modify-write: fetched up front
   double fw[6], uw[6];
 #pragma unroll
   for (int n = 0; n < 6; ++n) { fw[n] = __ldg(Wk + node(n)); uw[n] = __ldg(U + (size_t)DBAR * su + node(n)); }
@@ -381,7 +380,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
     if (mask & (1u << (2 * a))) fl += q.corr[(2 * a) * 32 + lane];
     if (mask & (1u << (2 * a + 1))) fl += q.corr[(2 * a + 1) * 32 + lane];
     const double fr = __shfl_down_sync(FULL, fl, 1);           // F^ at zone + 1/2
-    if (store) K[(size_t)(DBAR + a) * sk + off[3]] = kold[a] - (fr - fl) * hih;
+    if (store) K[(size_t)(DBAR + a) * sk + off0 + 3] = kold[a] - (fr - fl) * hih;
   }
 }
 
