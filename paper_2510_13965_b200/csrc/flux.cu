@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constan
     for (int n = 0; n < SEG + 6; ++n) { fc[n] = __ldg(f + offn(n)); uc[n] = __ldg(u + offn(n)); }
     double kold[SEG];                                          // K is read-modify-write: fetched with the column, not after the arithmetic
 #pragma unroll
-    for (int m = 1; m <= SEG; ++m) kold[m - 1] = (active && c0 + m - 1 < nline) ? k[offn(m + 2)] : 0.0;
+    for (int m = 1; m <= SEG; ++m) kold[m - 1] = k[offn(m + 2)];   // unconditional: the offsets are clamped into the field, zones that do not exist are not stored
     double pre[SEG];                                           // U0 + earlier stages of the fused RK combine (z pass only), fetched with the rest
 #pragma unroll
     for (int m = 1; m <= SEG; ++m) pre[m - 1] = (FUSED && active && c0 + m - 1 < nline) ? fused_fetch(fz, DBAR + a, (size_t)offn(m + 2)) : 0.0;
