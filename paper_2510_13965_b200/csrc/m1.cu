@@ -182,12 +182,17 @@ __global__ void __launch_bounds__(128, 3) k_m1_point(const __grid_constant__ Dim
 // ---------------------------------------------------------------------------------------------------------------
 namespace {
 // F^_{i+1/2} of Eq. (77) from u_{i-1..i+2}, the fluxes at i, i+1, lambda_{i+1/2} and A_{i+1/2}
+// min / max as plain selects: fmin / fmax carry IEEE NaN handling that costs six instructions each on sm_100a (no FP64 min/max instruction), and the face
+// formula below is mostly min / max; the operands here are never NaN where the result is used
+__device__ __forceinline__ double tmin(double a, double b) { return b < a ? b : a; }
+__device__ __forceinline__ double tmax(double a, double b) { return a < b ? b : a; }
 __device__ __forceinline__ double m1_face(double um, double u0, double up, double upp, double F0, double F1, double lam, double A0, double oe) {
   const double dm = u0 - um, d0 = up - u0, dp = upp - up;
   const double r2 = 2.0 / d0;                                                                           // one reciprocal per face and field
-  const double Phi = d0 == 0.0 ? 1.0 : fmax(0.0, fmin(1.0, fmin(dm * r2, dp * r2)));                    // Eq. (78), R20
-  const double tiny = oe * fmax(fmax(fabs(um), fabs(u0)), fmax(fabs(up), fabs(upp)));                   // R33 (oe = 0: the printed rule; oe < 0: switch off)
-  const double A = (oe >= 0.0 && dm * d0 < 0.0 && d0 * dp < 0.0 && fmin(fmin(fabs(dm), fabs(d0)), fabs(dp)) > tiny) ? 1.0 : A0;   // l.565-570
+  const double Phi = d0 == 0.0 ? 1.0 : tmax(0.0, tmin(1.0, tmin(dm * r2, dp * r2)));                    // Eq. (78), R20
+  const double tiny = oe * tmax(tmax(fabs(um), fabs(u0)), tmax(fabs(up), fabs(upp)));                   // R33 (oe = 0: the printed rule; oe < 0: switch off)
+  // l.565-570; min(|dm|, |d0|, |dp|) > tiny as three chained compares
+  const double A = (oe >= 0.0 && dm * d0 < 0.0 && d0 * dp < 0.0 && fabs(dm) > tiny && fabs(d0) > tiny && fabs(dp) > tiny) ? 1.0 : A0;
   const double FHO = 0.5 * (F0 + F1);
   return FHO - A * (1.0 - Phi) * (0.5 * lam * d0);                                                      // F^HO - F^LO = lambda d0 / 2
 }
@@ -493,7 +498,11 @@ __global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dim
   const int other = blockIdx.y + d.ng;
   const long long base = (DIR == 1 ? (long long)other * d.sz : (long long)other * d.sy) + (i + d.ng);
   const int g0 = c0 + d.ng - 2;                              // line index of node 0 of the window (zone c0 - 2)
-  auto node = [&](int n) { return base + (long long)min(g0 + n, mline - 1) * ls; };   // clamped: a ragged tail never reads past the field
+  // element offset of window node n inside a field, clamped (a ragged tail never reads past the field), in 32-bit arithmetic (a field has fewer than 2^32
+  // points: checked at launch): min, multiply-add and one IMAD.WIDE per access instead of a 64-bit multiply-add chain
+  const unsigned off0 = (unsigned)(base + (long long)g0 * ls), ls32 = (unsigned)ls;
+  const int nmax = mline - 1 - g0;
+  auto node = [&](int n) { return off0 + (unsigned)min(n, nmax) * ls32; };
   const double h = DIR == 1 ? d.dy : d.dz, ih = 1.0 / h;
 #pragma unroll 1
   for (int s = 0; s < 3; ++s) {
@@ -507,7 +516,7 @@ __global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dim
 #pragma unroll
       for (int m = 0; m <= SEG; ++m) {
         const double ln = __ldg(wl + node(m + 2)), kn = __ldg(wkap + node(m + 2));
-        lam[m] = fmax(lp, ln);
+        lam[m] = tmax(lp, ln);
         const double kh = 0.5 * (kp + kn) * h;
         A[m] = kh > 0.05 ? tanh(1.0 / kh) : 1.0;
         lp = ln; kp = kn;
@@ -524,12 +533,12 @@ __global__ void __launch_bounds__(128, 4) k_m1_march(const __grid_constant__ Dim
 #pragma unroll
       for (int n = 0; n < SEG + 2; ++n) Fw[n] = __ldg(F + node(n + 1));
 #pragma unroll
-      for (int z = 0; z < SEG; ++z) kold[z] = c0 + z < nline ? kv[base + (long long)(g0 + z + 2) * ls] : 0.0;
+      for (int z = 0; z < SEG; ++z) kold[z] = kv[node(z + 2)];   // unconditional (clamped offsets); zones that do not exist are not stored
       double prev = m1_face(uw[0], uw[1], uw[2], uw[3], Fw[0], Fw[1], lam[0], A[0], oe);
 #pragma unroll
       for (int z = 0; z < SEG; ++z) {
         const double cur = m1_face(uw[z + 1], uw[z + 2], uw[z + 3], uw[z + 4], Fw[z + 1], Fw[z + 2], lam[z + 1], A[z + 1], oe);
-        if (c0 + z < nline) kv[base + (long long)(g0 + z + 2) * ls] = kold[z] - (cur - prev) * ih;
+        if (c0 + z < nline) kv[node(z + 2)] = kold[z] - (cur - prev) * ih;
         prev = cur;
       }
     }
@@ -544,6 +553,7 @@ cudaError_t launch_m1_point(const Dims& d, const Par& par, const double* U, size
 cudaError_t launch_m1_div(const Dims& d, const Par& par, const double* U, size_t su, const double* V, size_t sv, const double* Wk, size_t sw,
                           double* KV, size_t sk, cudaStream_t s) {
   const double oe = par.m1_odd_even != 0 ? par.m1_oe_guard : -1.0;
+  if ((unsigned long long)d.npts >= (1ull << 32)) return cudaErrorInvalidValue;   // k_m1_march keeps 32-bit element offsets inside a field
   k_m1_div<<<dim3((d.nx + 15) / 16, (d.ny + 3) / 4, (d.nz + 1) / 2), dim3(16, 4, 2), 0, s>>>(d, oe, U, su, V, sv, Wk, sw, KV, sk);
   constexpr int SEG = 6;
   k_m1_march<1, SEG><<<dim3((d.nx + 127) / 128, d.nz, (d.ny + SEG - 1) / SEG), 128, 0, s>>>(d, oe, V, sv, Wk, sw, KV, sk);
