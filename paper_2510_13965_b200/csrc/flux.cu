@@ -353,7 +353,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   double acc[10], kold[10];
   unsigned mask = 0;
 #pragma unroll
-  for (int a = 0; a < 10; ++a) kold[a] = store ? K[(size_t)(DBAR + a) * sk + off0 + 3] : 0.0;   // read-modify-write: fetched up front
+  for (int a = 0; a < 10; ++a) kold[a] = K[(size_t)(DBAR + a) * sk + off0 + 3];   // read-modify-write: fetched up front, unconditionally (the clamped node is inside the row)
   double fw[6], uw[6];
 #pragma unroll
   for (int n = 0; n < 6; ++n) { fw[n] = __ldg(Wk + node(n)); uw[n] = __ldg(U + (size_t)DBAR * su + node(n)); }
