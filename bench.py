@@ -147,7 +147,7 @@ def falg_nonredundant(workload, eos_kind, nonatmo, pts_per_zone, nstages, m1):
     SURVEY 8(d) (DESIGN.md section 6 lists the items). Nothing the kernels recompute for their own convenience is in here."""
     d_first, d_second, d_mixed, d_adv, d_ko = 4.0, 7.0, 20.0, 9.0, 8.0          # flops of one stencil application (Eqs. 60-62, l.454-460)
     deriv_centred = 48 * d_first + 33 * d_second + 33 * d_mixed                 # 16 fields x 3, 11 fields x (3 + 3)
-    ccz4_pointwise = 2750.0                                                     # Eqs. (13)-(26): Christoffels, Ricci (the Gamma~ Gamma~ sum alone ~1 k), D_i D_j alpha, RHS
+    ccz4_pointwise = 2150.0                                                     # Eqs. (13)-(26): Christoffels, Ricci (the Gamma~ Gamma~ sum ~0.5 k with the contraction over m done once), D_i D_j alpha, RHS
     grmhd_sources = 300.0                                                       # right-hand sides of Eq. (32) from the same derivatives
     mp5 = 60.0 * 20.0                                                           # 60 reconstructions x Eq. (70) + the test of Eq. (72); the limiter (up to ~80 more) not claimed
     splitting = 600.0                                                           # Eqs. (65), (69), (64) for 10 fields x 3 directions, lambda maxima
