@@ -180,6 +180,20 @@ k_ccz4_algebra(const __grid_constant__ Dims d, const __grid_constant__ Par par, 
 #define G_(i, j) g[sym(i, j)]
 #define GI(i, j) gi[sym(i, j)]
 
+  // The pointwise phase reads 21 point values that are not in the ring (A~_ij, the 10 conserved fluid fields, W, p, v^i). There are no registers to
+  // hold them through phase 1 and only two warps per scheduler to cover an HBM latency each, so the lines are pulled into L1 now
+  // and the loads of phase 2 find them there.
+  {
+    auto pf = [](const double* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); };
+#pragma unroll
+    for (int a = 0; a < 6; ++a) pf(U + (size_t)(AXX + a) * su + pt);
+#pragma unroll
+    for (int a = 0; a < 10; ++a) pf(U + (size_t)(DBAR + a) * su + pt);
+    pf(P + (size_t)WLOR * sp + pt); pf(P + (size_t)PRESS * sp + pt);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) pf(P + (size_t)(VX + a) * sp + pt);
+  }
+
   // ================================================================= phase 1: derivatives, field by field
   const int ctr = ((tz + RH) * SY + (ty + RH)) * SX + (tx + XL);
   const double chi = F(CHI), al = F(ALPHA);
