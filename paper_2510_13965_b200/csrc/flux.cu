@@ -366,6 +366,10 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
 #pragma unroll
       for (int n = 0; n < 6; ++n) { fn[n] = __ldg(f + node(n)); un[n] = __ldg(u + node(n)); }
     }
+    if (a < 8) {                                               // and the field after that is pulled into L1 (no registers to hold it)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(Wk + (size_t)(a + 2) * sw + node(2)));
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(U + (size_t)(DBAR + a + 2) * su + node(2)));
+    }
     acc[a] = flux_hat2<WENO>(q, fw, uw, lam, alpha, active, a, lane, mask);   // twice F^ at zone - 1/2
     if (!WENO) q_flush(q, lane, alpha);
     if (a < 9) {
