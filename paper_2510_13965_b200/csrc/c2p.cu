@@ -549,6 +549,20 @@ __device__ __forceinline__ void solve_point(const C2pIo& io, const Par& par, lon
   store_point(io, pt, gl, sg, B, rho, ye, eps, e, v, W, flag, changed);
 }
 
+// The inputs of a cell that is going to be solved are pulled into L1 ahead of time: the solve is hundreds of dependent instructions at four CTAs per SM,
+// nothing else covers the latency of its 20 input loads (D and chi were read by pass A)
+template <int KIND>
+__device__ __forceinline__ void prefetch_inputs(const double* U, size_t su, const double* P, size_t sp, size_t q) {
+  auto pf = [](const double* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); };
+#pragma unroll
+  for (int f = 0; f < 6; ++f) pf(U + (size_t)(GXX + f) * su + q);
+  pf(U + (size_t)ALPHA * su + q);
+#pragma unroll
+  for (int f = 0; f < 8; ++f) pf(U + (size_t)(DYEBAR + f) * su + q);   // DYe, tau, S_i, B^i
+  pf(P + (size_t)WLOR * sp + q); pf(P + (size_t)RHO * sp + q); pf(P + (size_t)EPS * sp + q); pf(P + (size_t)PRESS * sp + q);
+  if (KIND == 2) pf(P + (size_t)TEMP * sp + q);
+}
+
 template <int KIND>
 __global__ void __launch_bounds__(C2P_THREADS, 4) k_con2prim(const __grid_constant__ Dims d, const __grid_constant__ Par par,
                                                              double* __restrict__ U, size_t su, double* __restrict__ P, size_t sp,
@@ -575,12 +589,19 @@ __global__ void __launch_bounds__(C2P_THREADS, 4) k_con2prim(const __grid_consta
     int base = 0;
     if (lane == 0 && b) base = atomicAdd(&count, __popc(b));
     base = __shfl_sync(0xffffffffu, base, 0);
-    if (solve) list[base + __popc(b & ((1u << lane) - 1u))] = (int)(pt - chunk0);
+    if (solve) {
+      const int pos = base + __popc(b & ((1u << lane) - 1u));
+      list[pos] = (int)(pt - chunk0);
+      if (pos < C2P_THREADS) prefetch_inputs<KIND>(U, su, P, sp, (size_t)pt);   // the first cell of each thread of pass B
+    }
   }
   __syncthreads();
   // ---- pass B: the solve, dense
   const int n = count;
-  for (int e = tid; e < n; e += C2P_THREADS) solve_point<KIND>(io, par, chunk0 + list[e], atmo);
+  for (int e = tid; e < n; e += C2P_THREADS) {
+    if (e + C2P_THREADS < n) prefetch_inputs<KIND>(U, su, P, sp, (size_t)(chunk0 + list[e + C2P_THREADS]));   // this thread's next cell, while this one is solved
+    solve_point<KIND>(io, par, chunk0 + list[e], atmo);
+  }
 }
 
 template <int KIND>
