@@ -374,7 +374,7 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 // offsets and the copy of group g+1 overlaps the arithmetic on group g (one barrier per group: a barrier per field leaves too little work
 // between barriers, measured 32.6 vs 29.2 ms per step for the L1 version at c1_256). (k_les_flux above fetches them through L1/L2 with one exposed latency per field at 8 warps/SM.)
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int LX = 16, LY = 4, LZ = 4, LH = 2, LSX = LX + 2 * LH, LSY = LY + 2 * LH, LSZ = LZ + 2 * LH, LTILE = LSX * LSY * LSZ, LGMAX = 6;
+constexpr int LX = 16, LY = 4, LZ = 4, LH = 2, LSX = LX + 2 * LH, LSY = LY + 2 * LH, LSZ = LZ + 2 * LH, LTILE = LSX * LSY * LSZ, LGMAX = 6, LNBUF = 3;
 // the fields pass in 5 groups (one barrier and one mbarrier wait per group, not per field): {B^c, Theta, v.B}, three times {v^c, v_c, B_c, E^c, E_c}, the 6 scalars
 // then, in the order of LORDER: {Ye, dp/dYe, D} with the tabulated EoS only, {calE, D Ye} with FULL only (without the table: one group {D, calE, D Ye})
 template <int... Is, class F> __device__ __forceinline__ void static_for(std::integer_sequence<int, Is...>, F&& f) { (f(std::integral_constant<int, Is>{}), ...); }
@@ -383,7 +383,7 @@ template <bool TABLE, bool FULL> struct LGroups {
   __host__ __device__ static constexpr int start(int g) { return g < 5 ? 5 * g : g == 5 ? (TABLE ? 26 : 28) : 29; }
   __host__ __device__ static constexpr int end(int g) { return g < 4 ? 5 * (g + 1) : g == 4 ? 26 : g == 5 ? (TABLE ? 29 : 31) : 31; }
 };
-constexpr size_t LES_SMEM = (size_t)2 * LGMAX * LTILE * sizeof(double) + 64;
+constexpr size_t LES_SMEM = (size_t)LNBUF * LGMAX * LTILE * sizeof(double) + 64;   // three buffers: the copies run two groups ahead of the arithmetic
 // order of passage: anchors B^c, Theta; v.B; then per component c: v^c, v_c, B_c, E^c, E_c; then W^-2, rho, h, dp/drho, eps, dp/deps
 __device__ constexpr int LORDER[NAUX] = {A_BU, A_BU + 1, A_BU + 2, A_TH, A_VB,
                                          A_VU, A_VL, A_BL, A_EU, A_EL, A_VU + 1, A_VL + 1, A_BL + 1, A_EU + 1, A_EL + 1, A_VU + 2, A_VL + 2, A_BL + 2, A_EU + 2, A_EL + 2,
@@ -396,7 +396,7 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   static_assert((LTILE * sizeof(double)) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
   using LG = LGroups<TABLE, FULL>;
   extern __shared__ __align__(128) double ring[];
-  uint64_t* full = (uint64_t*)(ring + 2 * LGMAX * LTILE);
+  uint64_t* full = (uint64_t*)(ring + LNBUF * LGMAX * LTILE);
   const int tid = threadIdx.x, tx = tid % LX, ty = (tid / LX) % LY, tz = tid / (LX * LY);
   const int i0 = 2 + blockIdx.x * LX, j0 = 2 + blockIdx.y * LY, k0 = 2 + blockIdx.z * LZ;      // array indices of the block's first point
   const int i = i0 + tx, j = j0 + ty, k = k0 + tz;
@@ -404,18 +404,19 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   const size_t pt = (size_t)min(k, d.mz - 3) * d.sz + (size_t)min(j, d.my - 3) * d.sy + min(i, d.mx - 3);
   if (tid == 0) {
 #pragma unroll
-    for (int b = 0; b < 2; ++b) mbar_init(full + b, 1);
+    for (int b = 0; b < LNBUF; ++b) mbar_init(full + b, 1);
     mbar_fence_init();
   }
   __syncthreads();
   auto issue = [&](int g) {                       // the box origin i0 - 2 = 16 blockIdx.x is even: on a 16-byte boundary
     if (tid == 0) {
       const int n0 = LG::start(g), n1 = LG::end(g);
-      mbar_expect_tx(full + g % 2, (unsigned)(n1 - n0) * LTILE * (unsigned)sizeof(double));
-      for (int n = n0; n < n1; ++n) tma_load_4d(ring + ((g % 2) * LGMAX + (n - n0)) * LTILE, &tmap, full + g % 2, i0 - LH, j0 - LH, k0 - LH, LORDER[n]);
+      mbar_expect_tx(full + g % LNBUF, (unsigned)(n1 - n0) * LTILE * (unsigned)sizeof(double));
+      for (int n = n0; n < n1; ++n) tma_load_4d(ring + ((g % LNBUF) * LGMAX + (n - n0)) * LTILE, &tmap, full + g % LNBUF, i0 - LH, j0 - LH, k0 - LH, LORDER[n]);
     }
   };
   issue(0);
+  issue(1);
   double gu[6];
   const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
   {
@@ -446,11 +447,11 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   auto group = [&](auto G) {
     constexpr int g5 = decltype(G)::value;
     __syncthreads();                                 // everybody is done reading the buffer the next copy overwrites
-    if (g5 + 1 < LG::N) issue(g5 + 1);
-    mbar_wait(full + g5 % 2, (g5 / 2) & 1);
+    if (g5 + 2 < LG::N) issue(g5 + 2);             // into the buffer group g5 - 1 has just released
+    mbar_wait(full + g5 % LNBUF, (g5 / LNBUF) & 1);
 #pragma unroll
    for (int n = LG::start(g5); n < LG::end(g5); ++n) {
-    const double* s = ring + ((g5 % 2) * LGMAX + (n - LG::start(g5))) * LTILE + ctr;
+    const double* s = ring + ((g5 % LNBUF) * LGMAX + (n - LG::start(g5))) * LTILE + ctr;
     constexpr int OX = 1, OY = LSX, OZ = LSX * LSY;
     const int f = LORDER[n];
     a[f] = s[0];
