@@ -417,6 +417,18 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   };
   issue(0);
   issue(1);
+  // the fluxes this thread adds its SGS terms to at the very end (read-modify-write of the work slot) are pulled into L1 now: with one CTA per SM nothing
+  // else would cover that HBM round trip (it was 40 % of the kernel's stall samples)
+  if (inside) {
+    auto pf = [](const double* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); };
+#pragma unroll
+    for (int kk = 0; kk < 3; ++kk)
+#pragma unroll
+      for (int f = 0; f < 9; ++f) {
+        if (f == 2 || (!FULL && f < 6) || f == 6 + kk) continue;   // C_M only: the flux of Bbar^i in direction k != i; FULL: also Dbar, DYebar, Sbar_i (not taubar)
+        pf(Wk + (size_t)(11 * kk + f) * sw + pt);
+      }
+  }
   double gu[6];
   const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
   {
