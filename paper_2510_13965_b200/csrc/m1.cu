@@ -210,6 +210,11 @@ __global__ void __launch_bounds__(128, 3) k_m1_div(const __grid_constant__ Dims 
   const size_t pt = (size_t)(k + d.ng) * d.sz + (size_t)(j + d.ng) * d.sy + (i + d.ng);
   const long long st[3] = {1, d.sy, d.sz};
   const double h[3] = {d.dx, d.dy, d.dz};
+  // the pressure tensors the source terms of the second species loop read are pulled into L1 now (three exposed HBM round trips otherwise)
+#pragma unroll
+  for (int s = 0; s < 3; ++s)
+#pragma unroll
+    for (int a = 0; a < 6; ++a) asm volatile("prefetch.global.L1 [%0];" ::"l"(Wk + (size_t)(M1W * s + 19 + a) * sw + pt));
 #pragma unroll 1
   for (int s = 0; s < 3; ++s) {
     double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
