@@ -369,7 +369,7 @@ __global__ void __launch_bounds__(256, 1) k_les_flux(const __grid_constant__ Dim
 // ---------------------------------------------------------------------------------------------------------------
 // The same computation with the auxiliary fields staged by the copy engine (default whenever the LESWORK slot admits a tensor map):
 // a CTA of 256 threads owns a 16 x 4 x 4 block of points; the 26 fields pass one at a time, in the order the streaming contraction
-// needs them, in 5 groups of 5-6 fields through two shared-memory buffers of 20 x 8 x 8 tiles (block + halo 2) filled by
+// needs them, in 5 groups of 5-6 fields through three shared-memory buffers of 20 x 8 x 8 tiles (block + halo 2; the copies run two groups ahead) filled by
 // cp.async.bulk.tensor with mbarrier completion, so the 12 stencil operands of a field are shared-memory loads with compile-time
 // offsets and the copy of group g+1 overlaps the arithmetic on group g (one barrier per group: a barrier per field leaves too little work
 // between barriers, measured 32.6 vs 29.2 ms per step for the L1 version at c1_256). (k_les_flux above fetches them through L1/L2 with one exposed latency per field at 8 warps/SM.)
