@@ -145,7 +145,7 @@ struct LesFull { double dBB[6], dvv[6], dEE[6], dD_v[3], dDY_v[3], dCE_v[3]; };
 template <bool FULL>
 __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, const double a[NAUX], const LesDots& D, const LesFull& X, const double gu[6],
                                                  double p, double chi, double al, const double* __restrict__ U, size_t su,
-                                                 double* __restrict__ Wk, size_t sw, size_t pt) {
+                                                 double* __restrict__ Wk, size_t sw, size_t pt, const double* wold = nullptr) {
   const double (&dVB_B)[3] = D.dVB_B; const double (&dTH_v)[3] = D.dTH_v; const double (&dBv)[3][3] = D.dBv;
   const double sBv = D.sBv, sBBvB = D.sBBvB, sBvTh = D.sBvTh, sBB = D.sBB, sEE = D.sEE, svv = D.svv;
   const double dWW = D.dWW, dWR = D.dWR, dWH = D.dWH, dPR_R = D.dPR_R, dPE_E = D.dPE_E, dRE = D.dRE;
@@ -195,7 +195,7 @@ __device__ __forceinline__ void les_closed_forms(const Dims& d, const Par& par, 
       HM[kk][ii] = (a[A_BU + ii] * H_v[kk] - a[A_BU + kk] * H_v[ii]) + 2.0 * (dBv[ii][kk] - dBv[kk][ii]);   // (A16)
       if (!FULL || par.les_C_M != 0.0) {
         double* w = Wk + (size_t)(11 * kk + 6 + ii) * sw + pt;
-        *w += fac * HM[kk][ii];
+        *w = (wold ? wold[2 * kk + (ii > kk ? ii - 1 : ii)] : *w) + fac * HM[kk][ii];   // wold: the six fluxes fetched at kernel start (k_les_flux_tma)
       }
     }
   if constexpr (FULL) {
@@ -419,13 +419,20 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   issue(1);
   // the fluxes this thread adds its SGS terms to at the very end (read-modify-write of the work slot) are pulled into L1 now: with one CTA per SM nothing
   // else would cover that HBM round trip (it was 40 % of the kernel's stall samples)
-  if (inside) {
+  double wold[6];                                  // C_M only: the six fluxes of Bbar^i (direction k != i) are fetched into registers right away
+  if (!FULL) {
+#pragma unroll
+    for (int kk = 0; kk < 3; ++kk)
+#pragma unroll
+      for (int ii = 0; ii < 3; ++ii)
+        if (ii != kk) wold[2 * kk + (ii > kk ? ii - 1 : ii)] = Wk[(size_t)(11 * kk + 6 + ii) * sw + pt];
+  } else if (inside) {                             // FULL (no registers left): Dbar, DYebar, Sbar_i, Bbar^i fluxes (not taubar) as L1 prefetches
     auto pf = [](const double* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); };
 #pragma unroll
     for (int kk = 0; kk < 3; ++kk)
 #pragma unroll
       for (int f = 0; f < 9; ++f) {
-        if (f == 2 || (!FULL && f < 6) || f == 6 + kk) continue;   // C_M only: the flux of Bbar^i in direction k != i; FULL: also Dbar, DYebar, Sbar_i (not taubar)
+        if (f == 2 || f == 6 + kk) continue;
         pf(Wk + (size_t)(11 * kk + f) * sw + pt);
       }
   }
@@ -527,7 +534,7 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
    }
   };
   static_for(std::make_integer_sequence<int, LG::N>{}, group);
-  if (inside) les_closed_forms<FULL>(d, par, a, D, X, gu, p, chi, al, U, su, Wk, sw, pt);
+  if (inside) les_closed_forms<FULL>(d, par, a, D, X, gu, p, chi, al, U, su, Wk, sw, pt, FULL ? nullptr : wold);
 }
 
 }  // namespace
