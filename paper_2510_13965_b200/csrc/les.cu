@@ -438,14 +438,16 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   }
   double gu[6];
   const double chi = __ldg(U + (size_t)CHI * su + pt), al = __ldg(U + (size_t)ALPHA * su + pt);
-  {
-    double g[6];
+  // the point values of the metric are requested here and first used after the first group of fields has passed (its gradients are kept lower-index until
+  // then): with one CTA per SM nothing else would cover this HBM round trip
+  double gm[6];
 #pragma unroll
-    for (int c = 0; c < 6; ++c) g[c] = __ldg(U + (size_t)(GXX + c) * su + pt);
-    const double s = chi / (g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) + g[2] * (g[1] * g[4] - g[3] * g[2]));
-    gu[0] = (g[3] * g[5] - g[4] * g[4]) * s; gu[1] = (g[2] * g[4] - g[1] * g[5]) * s; gu[2] = (g[1] * g[4] - g[2] * g[3]) * s;
-    gu[3] = (g[0] * g[5] - g[2] * g[2]) * s; gu[4] = (g[1] * g[2] - g[0] * g[4]) * s; gu[5] = (g[0] * g[3] - g[1] * g[1]) * s;
-  }
+  for (int c = 0; c < 6; ++c) gm[c] = __ldg(U + (size_t)(GXX + c) * su + pt);
+  auto inverse_metric = [&]() {
+    const double s = chi / (gm[0] * (gm[3] * gm[5] - gm[4] * gm[4]) - gm[1] * (gm[1] * gm[5] - gm[4] * gm[2]) + gm[2] * (gm[1] * gm[4] - gm[3] * gm[2]));
+    gu[0] = (gm[3] * gm[5] - gm[4] * gm[4]) * s; gu[1] = (gm[2] * gm[4] - gm[1] * gm[5]) * s; gu[2] = (gm[1] * gm[4] - gm[2] * gm[3]) * s;
+    gu[3] = (gm[0] * gm[5] - gm[2] * gm[2]) * s; gu[4] = (gm[1] * gm[2] - gm[0] * gm[4]) * s; gu[5] = (gm[0] * gm[3] - gm[1] * gm[1]) * s;
+  };
   const double p = __ldg(P + (size_t)PRESS * sp + pt);
   const double c12[3] = {1.0 / (12.0 * d.dx), 1.0 / (12.0 * d.dy), 1.0 / (12.0 * d.dz)};
   auto raise = [&](const double g[3], double r[3]) {
@@ -461,7 +463,7 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
   D.yterm = 0.0;
   LesFull X;
   // raised gradients of the anchors: B^c, Theta, v^c and E^c (FULL: every component stays, for (A17)), the current W^-2 / eps / Ye, rho
-  double uB[3][3], uTH[3], uV[FULL ? 3 : 1][3], uE[FULL ? 3 : 1][3], uX[3], uR[3];
+  double uB[3][3], uTH[3], gVB[3], uV[FULL ? 3 : 1][3], uE[FULL ? 3 : 1][3], uX[3], uR[3];
   // the groups are expanded at compile time (a fold over their indices: `#pragma unroll` gives up on the seven groups of <TABLE, FULL> and leaves a[], D, X in local memory)
   auto group = [&](auto G) {
     constexpr int g5 = decltype(G)::value;
@@ -478,17 +480,24 @@ __global__ void __launch_bounds__(LX * LY * LZ, 1) k_les_flux_tma(const __grid_c
     g[0] = (8.0 * (s[OX] - s[-OX]) - (s[2 * OX] - s[-2 * OX])) * c12[0];
     g[1] = (8.0 * (s[OY] - s[-OY]) - (s[2 * OY] - s[-2 * OY])) * c12[1];
     g[2] = (8.0 * (s[OZ] - s[-OZ]) - (s[2 * OZ] - s[-2 * OZ])) * c12[2];
-    if (n < 3) {                                                           // B^c
-      raise(g, uB[n]);
-      if (FULL)
+    if (n == 5) {                                                          // first field after the anchors: now the inverse metric is needed
+      inverse_metric();
 #pragma unroll
-        for (int e = 0; e <= n; ++e) X.dBB[sym3(e, n)] = dotp(g, uB[e]);
+      for (int c = 0; c < 3; ++c) {                                        // raise grad B^c in place (FULL: grad B^e . grad B^c on the way)
+        const double lo[3] = {uB[c][0], uB[c][1], uB[c][2]};
+        raise(lo, uB[c]);
+        if (FULL)
+#pragma unroll
+          for (int e = 0; e <= c; ++e) X.dBB[sym3(e, c)] = dotp(lo, uB[e]);
+        D.dVB_B[c] = dotp(gVB, uB[c]);
+      }
+      const double lo[3] = {uTH[0], uTH[1], uTH[2]};
+      raise(lo, uTH);
     }
-    else if (n == 3) raise(g, uTH);                                        // Theta
-    else if (n == 4) {                                                     // v.B
-#pragma unroll
-      for (int c = 0; c < 3; ++c) D.dVB_B[c] = dotp(g, uB[c]);
-    } else if (n < 20) {
+    if (n < 3) { uB[n][0] = g[0]; uB[n][1] = g[1]; uB[n][2] = g[2]; }      // B^c: kept lower-index until n == 5
+    else if (n == 3) { uTH[0] = g[0]; uTH[1] = g[1]; uTH[2] = g[2]; }      // Theta
+    else if (n == 4) { gVB[0] = g[0]; gVB[1] = g[1]; gVB[2] = g[2]; }      // v.B
+    else if (n < 20) {
       const int c = (n - 5) / 5, w = (n - 5) % 5;
       if (w == 0) {                                                        // v^c
         D.dTH_v[c] = dotp(g, uTH);
