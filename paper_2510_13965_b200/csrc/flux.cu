@@ -243,6 +243,7 @@ namespace {
 // All 32 lanes of a warp stay alive (the limiter queue is warp-cooperative): columns past nx are clamped and masked.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int RW = 4;    // warps per CTA of the reconstruction kernels
+constexpr int RXROWS = 4;   // rows a warp of k_recon_x takes in turn
 
 template <int DIR, int SEG, bool FUSED, bool WENO>
 __global__ void __launch_bounds__(32 * RW, 4) k_recon_march(const __grid_constant__ Dims d, double alpha, const double* __restrict__ U, size_t su,
@@ -332,10 +333,14 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   __shared__ double q_corr[RW][20 * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   LimQueue q = {q_v[warp], q_tag[warp], q_corr[warp], 0};
-  const int row = blockIdx.y * RW + warp;                    // j index (interior)
-  if (row >= d.ny) return;                                   // whole warp leaves
   const int z0 = blockIdx.x * 31;                            // first zone of this warp
   const int zone = z0 + lane;                                // lane l: interface zone-1/2 (left face of its zone)
+  // a warp takes RXROWS consecutive rows (j), one after the other: while it works on one, the first lines of the next are pulled into L1, so that the round
+  // trip of a row's first loads (lambda, K, field 0) is exposed once per RXROWS rows
+#pragma unroll 1
+  for (int r = 0; r < RXROWS; ++r) {
+  const int row = (blockIdx.y * RW + warp) * RXROWS + r;     // j index (interior)
+  if (row >= d.ny) return;                                   // whole warp leaves
   // left face of zone: between nodes zone-1 and zone -> stencil nodes zone-3 .. zone+2 ; global x index = zone + ng - 3 + n
   const long long base = (long long)(blockIdx.z + d.ng) * d.sz + (long long)(row + d.ng) * d.sy;
   // lanes past the last interface (zone > nx) are clamped as a whole, so that the six nodes of every lane are contiguous and inside the row (ng >= 3): a
@@ -343,6 +348,14 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
   const unsigned off0 = (unsigned)(base + (min(zone, d.nx) + d.ng - 3));
   auto node = [&](int n) { return (size_t)off0 + n; };
   const bool active = zone <= d.nx;                          // interfaces 0 .. nx
+  if (r + 1 < RXROWS && row + 1 < d.ny) {
+    const size_t nx2 = (size_t)off0 + (size_t)d.sy + 2;      // node 2 of the next row
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(Wk + (size_t)10 * sw + nx2));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(Wk + nx2));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(U + (size_t)DBAR * su + nx2));
+#pragma unroll
+    for (int a = 0; a < 10; ++a) asm volatile("prefetch.global.L1 [%0];" ::"l"(K + (size_t)(DBAR + a) * sk + nx2 + 1));
+  }
   double lam;
   {
     const double* s = Wk + (size_t)10 * sw;
@@ -386,6 +399,7 @@ __global__ void __launch_bounds__(32 * RW, 4) k_recon_x(const __grid_constant__ 
     const double fr = __shfl_down_sync(FULL, fl, 1);           // F^ at zone + 1/2
     if (store) K[(size_t)(DBAR + a) * sk + off0 + 3] = kold[a] - (fr - fl) * hih;
   }
+  }
 }
 
 }  // namespace
@@ -409,7 +423,7 @@ cudaError_t launch_recon(int dir, const Dims& d, const Par& par, const double* U
   const bool weno = par.recon_kind == 1;
   if ((unsigned long long)d.npts >= (1ull << 32)) return cudaErrorInvalidValue;   // the kernels keep 32-bit element offsets inside a field
   if (dir == 0) {
-    dim3 grid((d.nx + 30) / 31, (d.ny + RW - 1) / RW, d.nz);
+    dim3 grid((d.nx + 30) / 31, (d.ny + RW * RXROWS - 1) / (RW * RXROWS), d.nz);
     if (weno) k_recon_x<true><<<grid, 32 * RW, 0, s>>>(d, par.weno_eps, U, su, Wk, sw, K, sk);
     else k_recon_x<false><<<grid, 32 * RW, 0, s>>>(d, par.mp5_alpha, U, su, Wk, sw, K, sk);
   } else if (weno) launch_march<6, true>(dir, d, par, U, su, Wk, sw, K, sk, fz, s);
