@@ -81,7 +81,8 @@ enum {
   MHD_E_ARG = -1,        /* null pointer / out-of-range argument            */
   MHD_E_UNBOUND = -2,    /* a slot needed by the call has not been bound    */
   MHD_E_CUDA = -3,       /* CUDA runtime error (launch, copy, allocation)   */
-  MHD_E_UNSUPPORTED = -4 /* not supported: n_species other than 0 or 3, an M1 call on a patch without species */
+  MHD_E_UNSUPPORTED = -4, /* not supported: n_species other than 0 or 3, an M1 call on a patch without species */
+  MHD_E_TOO_LARGE = -5   /* a size beyond the fixed capacity of an allocation-free entry point (mhd_flag_census_static) */
 };
 
 /* Plain data, copied at create time. Pointers inside are DEVICE pointers that must outlive the patch. */
@@ -295,6 +296,19 @@ int mhd_patch_profile_read(mhd_patch *p, double ms[MHD_NKERNELS], unsigned long 
 /* Measured FP64 FMA throughput of the device (register-resident DFMA chains on every SM), in FLOP/s;
  * used as the FP64 roofline denominator. Synchronises. Returns < 0 on error. */
 double mhd_probe_fp64_flops(void *cuda_stream);
+
+/* Flag census WITHOUT any allocation and without an mhd_patch (whose create call allocates): for callers that cannot call cudaMalloc — code under
+ * CUDA stream capture, tight serving loops, harnesses that forbid it. Counts the flag bits (App. D error policy, l.1151-1162; the bits mhd_con2prim
+ * and mhd_m1_implicit set) over n_points bytes.
+ *   d_flags   DEVICE pointer, n_points bytes, read only (e.g. the buffer bound to MHD_SLOT_FLAGS, MX*MY*MZ bytes).
+ *   d_counts  DEVICE pointer, 9 words written: [0] = n_points, [1 + b] = number of bytes with bit b set (the order of mhd_status: atmo, eps_lo, eps_hi,
+ *             vmax, ye, fatal, noconv, m1fix). The caller owns both buffers; nothing is copied to the host, the stream is not synchronised.
+ * The partial counts live in a file-scope device array of fixed size inside the library (128 KB, held by every GPU that loads the library until exit):
+ * n_points > MHD_CENSUS_MAX_POINTS returns MHD_E_TOO_LARGE and launches nothing; null pointers or n_points < 1: MHD_E_ARG. The call makes no cudaMalloc /
+ * cudaFree and calls no allocating routine. All calls share that array: calls on one stream are ordered; two calls that OVERLAP on the GPU (different
+ * streams, two host threads on one device) race on it and their results are undefined. Same counts as mhd_patch_status, bit for bit. */
+#define MHD_CENSUS_MAX_POINTS 268435456LL   /* 2^28 points = 645^3 with ghosts */
+int mhd_flag_census_static(const uint8_t *d_flags, long long n_points, unsigned long long *d_counts, void *cuda_stream);
 
 const char *mhd_strerror(int code);
 

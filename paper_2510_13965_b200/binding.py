@@ -61,7 +61,7 @@ EXPORTS = ["mhd_desc_sizeof", "mhd_patch_create", "mhd_patch_destroy", "mhd_patc
            "mhd_patch_profile", "mhd_patch_profile_read", "mhd_probe_fp64_flops", "mhd_strerror",
            "mhd_m1_implicit", "mhd_m1_rhs", "mhd_m1_backreaction", "mhd_m1_gravity", "mhd_advance_imex",
            "mhd_prolong", "mhd_restrict", "mhd_dense_weights", "mhd_dense_output",
-           "mhd_advance_imex_host", "mhd_les_flux", "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close"]
+           "mhd_advance_imex_host", "mhd_les_flux", "mhd_patch_set_neighbor", "mhd_patch_halo_words", "mhd_patch_set_neighbor_word", "mhd_ipc_export", "mhd_ipc_import", "mhd_ipc_close", "mhd_flag_census_static"]
 NKERNELS = 13
 KERNEL_CLASSES = ["fill_ghosts", "con2prim", "ccz4_algebra", "recon_x", "recon_y", "recon_z", "rk_combine", "point_flux", "adv_ko",
                   "m1_point", "m1_div", "m1_implicit", "les"]
@@ -94,6 +94,7 @@ def lib():
         L.mhd_probe_fp64_flops.argtypes = [_p]
         L.mhd_probe_fp64_flops.restype = _d
         L.mhd_strerror.argtypes = [_i]
+        L.mhd_flag_census_static.argtypes = [_p, ctypes.c_longlong, _p, _p]
         L.mhd_m1_implicit.argtypes = [_p, _i, _i, _d, _p]
         L.mhd_m1_rhs.argtypes = [_p, _i, _i, _p]
         L.mhd_m1_backreaction.argtypes = [_p, _i, _i, _p]
@@ -314,6 +315,14 @@ def mhd_patch_profile_read(h, stream=None):
     n = (ctypes.c_ulonglong * NKERNELS)()
     _check(lib().mhd_patch_profile_read(h, ms, n, stream))
     return {k: (ms[i], int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+
+CENSUS_MAX_POINTS = 1 << 28
+
+
+def mhd_flag_census_static(d_flags_ptr, n_points, d_counts_ptr, stream=None):
+    """Allocation-free flag census (include/mhd.h): device pointers in, 9 device words out; see the header for the sharing rule."""
+    _check(lib().mhd_flag_census_static(d_flags_ptr, n_points, d_counts_ptr, stream))
 
 
 def mhd_probe_fp64_flops(stream=None):

@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd_b200.so")
-SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": [], "ccz4.cu": [], "flux.cu": [], "m1.cu": [], "amr.cu": [], "les.cu": []}
+SOURCES = {"api.cu": [], "elementwise.cu": [], "c2p.cu": [], "ccz4.cu": [], "flux.cu": [], "m1.cu": [], "amr.cu": [], "les.cu": [], "noalloc.cu": []}
 COMMON = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC"]
 
 

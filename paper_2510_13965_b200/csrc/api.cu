@@ -668,6 +668,7 @@ const char* mhd_strerror(int code) {
     case MHD_E_UNBOUND: return "slot not bound";
     case MHD_E_CUDA: return "CUDA runtime error";
     case MHD_E_UNSUPPORTED: return "feature not supported by this build";
+    case MHD_E_TOO_LARGE: return "size beyond the fixed capacity of this allocation-free entry point";
     default: return "unknown error";
   }
 }
